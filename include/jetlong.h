@@ -1,0 +1,111 @@
+/*
+ * jetlong.h -- C ABI of libjetlong: fused bifocal RoPE attention (Jet-Long,
+ * arxiv/paper_2607_07740) for NVIDIA B200 (sm_100a).
+ *
+ * "P:nnn" cites a line of the paper text.  R1..R16 are the readings listed in
+ * DESIGN.md for points the paper leaves open.
+ *
+ * Conventions common to every entry point
+ *   - All tensor pointers are DEVICE pointers owned by the caller.  The library never allocates,
+ *     frees or retains them.  Calls are asynchronous on `stream` (a cudaStream_t passed as void*).
+ *   - Layouts (contiguous): Q, out [L, H_q, d]; K, V [L, H_kv, d]; lse [H_q, L] fp32.
+ *     Decode: q, out [H_q, d]; lse [H_q]; Kcache, Vcache [>=L, H_kv, d] (rows 0..L-1 are read).
+ *   - Q and K arrive ALREADY RoPE-rotated at their true absolute positions 0..L-1, half-split
+ *     pairing (i, i+d/2), theta_i = rope_theta^(-2i/d)  (Eq.(4); q_local in Eq.(6); R5, R6).
+ *     The library never writes to Q, K, V (the cache invariant).
+ *   - softmax scale is 1/sqrt(head_dim) (R7); lse is the natural log of sum exp(scaled score) (R8).
+ *   - GQA: query head h reads KV head h / (H_q / H_kv) (R9).
+ *   - dtype: JETLONG_BF16 (bf16 Q/K/V/out, fp32 accumulation) or JETLONG_FP32 (fp32 everything).
+ *   - Return value: a jetlong_status.  Arguments are validated before any launch; on a non-OK
+ *     status nothing has been written.  There is no CPU fallback: without a compute-capability
+ *     10.x device the compute entry points return JETLONG_UNSUPPORTED.
+ *   - INVALID_ARG: null pointer, L < 1, H_q % H_kv != 0, head_dim not in {64, 128}, w_local < 0,
+ *     w_pretrained < 1, rope_theta <= 0, unknown dtype, a pointer not 16-byte aligned, or a
+ *     workspace smaller than jetlong_workspace_bytes() reports.
+ */
+#ifndef JETLONG_H_
+#define JETLONG_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    JETLONG_OK = 0,
+    JETLONG_INVALID_ARG = 1,
+    JETLONG_UNSUPPORTED = 2,
+    JETLONG_CUDA_ERROR = 3
+} jetlong_status;
+
+enum { JETLONG_BF16 = 0, JETLONG_FP32 = 1 };
+
+/* op codes for jetlong_workspace_bytes */
+enum { JETLONG_OP_PREFILL = 0, JETLONG_OP_DECODE = 1, JETLONG_OP_CAUSAL_PREFILL = 2, JETLONG_OP_CAUSAL_DECODE = 3 };
+
+/* Eq.(2): G = max(1, ceil(L / w_pretrained)), integer arithmetic on the host.
+ * Returns -1 if L < 1 or w_pretrained < 1. */
+int64_t jetlong_group_size(int64_t L, int64_t w_pretrained);
+
+/* Bytes of caller-allocated device workspace the op needs for these shapes (0 is possible).
+ * Holds rotation tables (Eq.(5)-(6)) and split-KV partial states (decode).  16-byte aligned. */
+size_t jetlong_workspace_bytes(int op, int64_t L, int H_q, int H_kv, int head_dim, int dtype);
+
+/*
+ * Bifocal prefill (Eq.(1) P:70 with Eq.(2),(3),(5),(6); Section 3.3).
+ * For every head h and row q: keys with 0 <= q-k <= w_local score with the stored Q, K (R1);
+ * older keys score with R(Delta q) Q[q] and R(Delta k) K[k], Delta(x) = floor(x/G) - x, one G
+ * from the full L (R3).  One joint softmax over k <= q.  The remote-only partial state replaces
+ * the paper's (B - C), so no subtraction occurs (the merge is the additive LSE merge of Eq.(7)).
+ * G == 1 dispatches to jetlong_causal_prefill: bitwise the control's result.
+ */
+int jetlong_prefill(const void* Q, const void* K, const void* V, void* out, float* lse,
+                    int64_t L, int H_q, int H_kv, int head_dim,
+                    int64_t w_local, int64_t w_pretrained, double rope_theta,
+                    int dtype, void* workspace, size_t workspace_bytes, void* stream);
+
+/*
+ * Bifocal batch-1 decode: one query row per head at position L-1 against cache rows
+ * 0..L-1 (the current token's key/value already appended at row L-1; R4, R14).  G is recomputed
+ * from this L.  Split-KV scan; partial (m, l, O) states are merged by the additive LSE merge.
+ */
+int jetlong_decode(const void* q, const void* Kcache, const void* Vcache, void* out, float* lse,
+                   int64_t L, int H_q, int H_kv, int head_dim,
+                   int64_t w_local, int64_t w_pretrained, double rope_theta,
+                   int dtype, void* workspace, size_t workspace_bytes, void* stream);
+
+/* Matched control ("without bifocal attention"): plain causal attention on the given
+ * (already RoPE'd) Q, K with the same kernels, no classifier and no rotation. */
+int jetlong_causal_prefill(const void* Q, const void* K, const void* V, void* out, float* lse,
+                           int64_t L, int H_q, int H_kv, int head_dim,
+                           int dtype, void* workspace, size_t workspace_bytes, void* stream);
+
+int jetlong_causal_decode(const void* q, const void* Kcache, const void* Vcache, void* out, float* lse,
+                          int64_t L, int H_q, int H_kv, int head_dim,
+                          int dtype, void* workspace, size_t workspace_bytes, void* stream);
+
+/*
+ * Host-buffer convenience wrappers (used for end-to-end timing): same arguments, but Q, K, V, out,
+ * lse are HOST pointers (pinned or pageable).  The call allocates device buffers, copies in, runs
+ * the op on the default stream, copies out/lse back and synchronises before returning.
+ */
+int jetlong_prefill_host(const void* Q, const void* K, const void* V, void* out, float* lse,
+                         int64_t L, int H_q, int H_kv, int head_dim,
+                         int64_t w_local, int64_t w_pretrained, double rope_theta, int dtype);
+
+/* Text for a status; for JETLONG_CUDA_ERROR the text of the last CUDA error seen by this thread. */
+const char* jetlong_status_string(int status);
+
+/* Number of kernels this process has launched through the library (for bench accounting). */
+int64_t jetlong_launch_count(void);
+
+/* Which prefill implementation a bf16 call would use: 0 = SIMT fp32-FMA tiles, 1 = tcgen05 UMMA.
+ * jetlong_set_prefill_impl(-1) restores the default. Returns the previous value. */
+int jetlong_set_prefill_impl(int impl);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* JETLONG_H_ */

@@ -1,0 +1,184 @@
+"""Thin ctypes binding of libjetlong (include/jetlong.h): argument marshalling only.
+
+Every step of the hot path runs inside the CUDA library.  torch is used for device memory and
+streams.  There is no CPU fallback: if libjetlong.so is missing or the device is not a B200-class
+GPU, the calls raise.
+"""
+import ctypes
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "libjetlong.so")
+_lib = None
+
+OK, INVALID_ARG, UNSUPPORTED, CUDA_ERROR = 0, 1, 2, 3
+BF16, FP32 = 0, 1
+OP_PREFILL, OP_DECODE, OP_CAUSAL_PREFILL, OP_CAUSAL_DECODE = 0, 1, 2, 3
+
+EXPORTS = ["jetlong_group_size", "jetlong_workspace_bytes", "jetlong_prefill", "jetlong_decode",
+           "jetlong_causal_prefill", "jetlong_causal_decode", "jetlong_prefill_host", "jetlong_status_string",
+           "jetlong_launch_count", "jetlong_set_prefill_impl"]
+
+
+class JetlongError(RuntimeError):
+    def __init__(self, status, text):
+        super().__init__("libjetlong status %d: %s" % (status, text))
+        self.status = status
+
+
+def lib():
+    """Load libjetlong.so (built in-tree by build.py).  Fails loudly if it is missing."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_SO):
+            raise ImportError("libjetlong.so not built: run `python -m paper_2607_07740_b200.build` "
+                              "(there is no CPU fallback)")
+        L = ctypes.CDLL(_SO)
+        i64, i32, dbl, vp, sz = ctypes.c_int64, ctypes.c_int, ctypes.c_double, ctypes.c_void_p, ctypes.c_size_t
+        L.jetlong_group_size.restype = i64
+        L.jetlong_group_size.argtypes = [i64, i64]
+        L.jetlong_workspace_bytes.restype = sz
+        L.jetlong_workspace_bytes.argtypes = [i32, i64, i32, i32, i32, i32]
+        tail = [i64, i32, i32, i32, i64, i64, dbl, i32, vp, sz, vp]
+        L.jetlong_prefill.restype = i32
+        L.jetlong_prefill.argtypes = [vp] * 5 + tail
+        L.jetlong_decode.restype = i32
+        L.jetlong_decode.argtypes = [vp] * 5 + tail
+        ctail = [i64, i32, i32, i32, i32, vp, sz, vp]
+        L.jetlong_causal_prefill.restype = i32
+        L.jetlong_causal_prefill.argtypes = [vp] * 5 + ctail
+        L.jetlong_causal_decode.restype = i32
+        L.jetlong_causal_decode.argtypes = [vp] * 5 + ctail
+        L.jetlong_prefill_host.restype = i32
+        L.jetlong_prefill_host.argtypes = [vp] * 5 + [i64, i32, i32, i32, i64, i64, dbl, i32]
+        L.jetlong_status_string.restype = ctypes.c_char_p
+        L.jetlong_status_string.argtypes = [i32]
+        L.jetlong_launch_count.restype = i64
+        L.jetlong_set_prefill_impl.restype = i32
+        L.jetlong_set_prefill_impl.argtypes = [i32]
+        _lib = L
+    return _lib
+
+
+def _check(rc):
+    if rc != OK:
+        raise JetlongError(rc, lib().jetlong_status_string(rc).decode())
+
+
+def _dt(t):
+    if t.dtype == torch.bfloat16:
+        return BF16
+    if t.dtype == torch.float32:
+        return FP32
+    raise TypeError("libjetlong takes bf16 or fp32 tensors, got %s" % t.dtype)
+
+
+def _stream():
+    return ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def jetlong_group_size(L, w_pretrained):
+    return int(lib().jetlong_group_size(int(L), int(w_pretrained)))
+
+
+def jetlong_workspace_bytes(op, L, H_q, H_kv, head_dim, dtype):
+    return int(lib().jetlong_workspace_bytes(op, int(L), H_q, H_kv, head_dim, dtype))
+
+
+def jetlong_launch_count():
+    return int(lib().jetlong_launch_count())
+
+
+def jetlong_set_prefill_impl(impl):
+    return int(lib().jetlong_set_prefill_impl(int(impl)))
+
+
+def alloc_workspace(op, L, H_q, H_kv, head_dim, dtype, device="cuda"):
+    n = jetlong_workspace_bytes(op, L, H_q, H_kv, head_dim, dtype)
+    return torch.zeros(max(n, 256), dtype=torch.uint8, device=device)
+
+
+def _prefill_args(Q, K, V, out, lse):
+    assert Q.is_cuda and K.is_cuda and V.is_cuda and Q.is_contiguous() and K.is_contiguous() and V.is_contiguous()
+    L, H_q, d = Q.shape
+    assert K.shape == V.shape and K.shape[0] == L and K.shape[2] == d and K.dtype == Q.dtype == V.dtype
+    H_kv = K.shape[1]
+    if out is None:
+        out = torch.empty_like(Q)
+    if lse is None:
+        lse = torch.empty((H_q, L), dtype=torch.float32, device=Q.device)
+    return L, H_q, H_kv, d, out, lse
+
+
+def jetlong_prefill(Q, K, V, *, w_local, w_pretrained, rope_theta, out=None, lse=None, workspace=None):
+    """Bifocal prefill.  Q [L,H_q,d], K/V [L,H_kv,d] (bf16 or fp32, RoPE'd at true positions).  Returns out, lse."""
+    L, H_q, H_kv, d, out, lse = _prefill_args(Q, K, V, out, lse)
+    dt = _dt(Q)
+    if workspace is None:
+        workspace = alloc_workspace(OP_PREFILL, L, H_q, H_kv, d, dt, Q.device)
+    _check(lib().jetlong_prefill(Q.data_ptr(), K.data_ptr(), V.data_ptr(), out.data_ptr(), lse.data_ptr(), L, H_q,
+                                 H_kv, d, int(w_local), int(w_pretrained), float(rope_theta), dt,
+                                 workspace.data_ptr(), workspace.numel(), _stream()))
+    return out, lse
+
+
+def jetlong_causal_prefill(Q, K, V, *, out=None, lse=None, workspace=None):
+    """Matched control: plain causal attention on the given Q, K, V."""
+    L, H_q, H_kv, d, out, lse = _prefill_args(Q, K, V, out, lse)
+    dt = _dt(Q)
+    if workspace is None:
+        workspace = alloc_workspace(OP_CAUSAL_PREFILL, L, H_q, H_kv, d, dt, Q.device)
+    _check(lib().jetlong_causal_prefill(Q.data_ptr(), K.data_ptr(), V.data_ptr(), out.data_ptr(), lse.data_ptr(), L,
+                                        H_q, H_kv, d, dt, workspace.data_ptr(), workspace.numel(), _stream()))
+    return out, lse
+
+
+def _decode_args(q, Kc, Vc, L, out, lse):
+    assert q.is_cuda and q.is_contiguous() and Kc.is_contiguous() and Vc.is_contiguous()
+    H_q, d = q.shape
+    assert Kc.shape == Vc.shape and Kc.shape[0] >= L and Kc.shape[2] == d and Kc.dtype == q.dtype
+    H_kv = Kc.shape[1]
+    if out is None:
+        out = torch.empty_like(q)
+    if lse is None:
+        lse = torch.empty((H_q,), dtype=torch.float32, device=q.device)
+    return H_q, H_kv, d, out, lse
+
+
+def jetlong_decode(q, Kcache, Vcache, L, *, w_local, w_pretrained, rope_theta, out=None, lse=None, workspace=None):
+    """Bifocal decode of the query at position L-1 against cache rows 0..L-1.  q [H_q,d]."""
+    H_q, H_kv, d, out, lse = _decode_args(q, Kcache, Vcache, L, out, lse)
+    dt = _dt(q)
+    if workspace is None:
+        workspace = alloc_workspace(OP_DECODE, L, H_q, H_kv, d, dt, q.device)
+    _check(lib().jetlong_decode(q.data_ptr(), Kcache.data_ptr(), Vcache.data_ptr(), out.data_ptr(), lse.data_ptr(),
+                                int(L), H_q, H_kv, d, int(w_local), int(w_pretrained), float(rope_theta), dt,
+                                workspace.data_ptr(), workspace.numel(), _stream()))
+    return out, lse
+
+
+def jetlong_causal_decode(q, Kcache, Vcache, L, *, out=None, lse=None, workspace=None):
+    H_q, H_kv, d, out, lse = _decode_args(q, Kcache, Vcache, L, out, lse)
+    dt = _dt(q)
+    if workspace is None:
+        workspace = alloc_workspace(OP_CAUSAL_DECODE, L, H_q, H_kv, d, dt, q.device)
+    _check(lib().jetlong_causal_decode(q.data_ptr(), Kcache.data_ptr(), Vcache.data_ptr(), out.data_ptr(),
+                                       lse.data_ptr(), int(L), H_q, H_kv, d, dt, workspace.data_ptr(),
+                                       workspace.numel(), _stream()))
+    return out, lse
+
+
+def jetlong_prefill_host(Q, K, V, *, w_local, w_pretrained, rope_theta, out=None, lse=None):
+    """End-to-end call with HOST tensors (pinned or pageable): H2D, prefill, D2H inside the library."""
+    assert not Q.is_cuda and Q.is_contiguous() and K.is_contiguous() and V.is_contiguous()
+    L, H_q, d = Q.shape
+    H_kv = K.shape[1]
+    if out is None:
+        out = torch.empty_like(Q)
+    if lse is None:
+        lse = torch.empty((H_q, L), dtype=torch.float32)
+    _check(lib().jetlong_prefill_host(Q.data_ptr(), K.data_ptr(), V.data_ptr(), out.data_ptr(), lse.data_ptr(), L, H_q,
+                                      H_kv, d, int(w_local), int(w_pretrained), float(rope_theta), _dt(Q)))
+    return out, lse

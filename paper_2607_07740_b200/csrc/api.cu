@@ -1,0 +1,196 @@
+// api.cu -- the C ABI of libjetlong (include/jetlong.h): validation, dispatch, workspace layout.
+#include <atomic>
+#include <stdio.h>
+#include <string.h>
+
+#include "common.cuh"
+
+namespace jetlong {
+
+static std::atomic<long long> g_launches{0};
+static thread_local char g_err[256] = "no CUDA error recorded";
+static std::atomic<int> g_prefill_impl{-1};
+
+void note_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
+
+int check_launch(const char* what) {
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess) return JETLONG_OK;
+    snprintf(g_err, sizeof(g_err), "%s: %s", what, cudaGetErrorString(e));
+    return JETLONG_CUDA_ERROR;
+}
+
+// prefill_umma.cu
+bool umma_prefill_supported(long long L, int H_q, int H_kv, int d, int dtype);
+size_t umma_prefill_workspace_bytes(long long L, int H_q, int H_kv, int d);
+int launch_prefill_umma(const void* Q, const void* K, const void* V, void* out, float* lse, long long L, int H_q,
+                        int H_kv, int d, long long w0, long long G, double theta, bool bifocal, void* ws,
+                        size_t ws_bytes, cudaStream_t st);
+
+static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; }
+
+static int validate(const void* a, const void* b, const void* c, const void* o, const void* l, long long L, int H_q,
+                    int H_kv, int d, long long w0, long long w_pre, double theta, int dtype) {
+    if (!a || !b || !c || !o || !l) return JETLONG_INVALID_ARG;
+    if (L < 1 || H_q < 1 || H_kv < 1 || (H_q % H_kv) != 0) return JETLONG_INVALID_ARG;
+    if (d != 64 && d != 128) return JETLONG_INVALID_ARG;
+    if (w0 < 0 || w_pre < 1 || !(theta > 0.0)) return JETLONG_INVALID_ARG;
+    if (dtype != JETLONG_BF16 && dtype != JETLONG_FP32) return JETLONG_INVALID_ARG;
+    if (!aligned16(a) || !aligned16(b) || !aligned16(c) || !aligned16(o) || !aligned16(l)) return JETLONG_INVALID_ARG;
+    return JETLONG_OK;
+}
+
+static int device_ok() {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return JETLONG_UNSUPPORTED; }
+    int major = 0;
+    if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) {
+        cudaGetLastError();
+        return JETLONG_UNSUPPORTED;
+    }
+    return major == 10 ? JETLONG_OK : JETLONG_UNSUPPORTED;
+}
+
+static bool use_umma(long long L, int H_q, int H_kv, int d, int dtype) {
+    const int impl = g_prefill_impl.load();
+    if (impl == 0) return false;
+    return umma_prefill_supported(L, H_q, H_kv, d, dtype);
+}
+
+static size_t prefill_ws(long long L, int H_q, int H_kv, int d, int dtype, bool bifocal) {
+    size_t simt = bifocal ? align256((size_t)L * (d / 2) * sizeof(float2)) : 0;
+    size_t umma = umma_prefill_supported(L, H_q, H_kv, d, dtype) ? umma_prefill_workspace_bytes(L, H_q, H_kv, d) : 0;
+    return simt > umma ? simt : umma;      // either implementation may be selected at run time
+}
+
+static int prefill_common(const void* Q, const void* K, const void* V, void* out, float* lse, long long L, int H_q,
+                          int H_kv, int d, long long w0, long long w_pre, double theta, int dtype, void* ws,
+                          size_t ws_bytes, void* stream, bool bifocal) {
+    int rc = validate(Q, K, V, out, lse, L, H_q, H_kv, d, w0, w_pre, theta, dtype);
+    if (rc != JETLONG_OK) return rc;
+    long long G = bifocal ? jetlong_group_size(L, w_pre) : 1;
+    if (G == 1 || w0 >= L - 1) bifocal = false;          // step a2: G = 1 (or an all-covering window) is the control
+    const size_t need = prefill_ws(L, H_q, H_kv, d, dtype, bifocal);
+    if (need > 0 && (!ws || ws_bytes < need || !aligned16(ws))) return JETLONG_INVALID_ARG;
+    rc = device_ok();
+    if (rc != JETLONG_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (use_umma(L, H_q, H_kv, d, dtype))
+        return launch_prefill_umma(Q, K, V, out, lse, L, H_q, H_kv, d, w0, G, theta, bifocal, ws, ws_bytes, st);
+    const float2* tab = nullptr;
+    if (bifocal) {
+        rc = build_key_table((float2*)ws, L, G, d, theta, st);
+        if (rc != JETLONG_OK) return rc;
+        tab = (const float2*)ws;
+    }
+    return launch_prefill_simt(Q, K, V, out, lse, L, H_q, H_kv, d, w0, G, tab, dtype, bifocal, st);
+}
+
+static int decode_common(const void* q, const void* K, const void* V, void* out, float* lse, long long L, int H_q,
+                         int H_kv, int d, long long w0, long long w_pre, double theta, int dtype, void* ws,
+                         size_t ws_bytes, void* stream, bool bifocal) {
+    int rc = validate(q, K, V, out, lse, L, H_q, H_kv, d, w0, w_pre, theta, dtype);
+    if (rc != JETLONG_OK) return rc;
+    long long G = bifocal ? jetlong_group_size(L, w_pre) : 1;
+    if (G == 1 || w0 >= L - 1) bifocal = false;
+    const size_t need = decode_workspace_bytes(L, H_q, H_kv, d);
+    if (!ws || ws_bytes < need || !aligned16(ws)) return JETLONG_INVALID_ARG;
+    rc = device_ok();
+    if (rc != JETLONG_OK) return rc;
+    return launch_decode(q, K, V, out, lse, L, H_q, H_kv, d, w0, G, theta, dtype, bifocal, ws, ws_bytes,
+                         (cudaStream_t)stream);
+}
+
+}  // namespace jetlong
+
+using namespace jetlong;
+
+extern "C" {
+
+int64_t jetlong_group_size(int64_t L, int64_t w_pretrained) {
+    if (L < 1 || w_pretrained < 1) return -1;
+    int64_t G = (L + w_pretrained - 1) / w_pretrained;      // Eq.(2), integers only
+    return G < 1 ? 1 : G;
+}
+
+size_t jetlong_workspace_bytes(int op, int64_t L, int H_q, int H_kv, int head_dim, int dtype) {
+    if (L < 1 || H_q < 1 || H_kv < 1 || (H_q % H_kv) || (head_dim != 64 && head_dim != 128)) return 0;
+    switch (op) {
+        case JETLONG_OP_PREFILL: return prefill_ws(L, H_q, H_kv, head_dim, dtype, true);
+        case JETLONG_OP_CAUSAL_PREFILL: return prefill_ws(L, H_q, H_kv, head_dim, dtype, false);
+        case JETLONG_OP_DECODE:
+        case JETLONG_OP_CAUSAL_DECODE: return decode_workspace_bytes(L, H_q, H_kv, head_dim);
+        default: return 0;
+    }
+}
+
+int jetlong_prefill(const void* Q, const void* K, const void* V, void* out, float* lse, int64_t L, int H_q, int H_kv,
+                    int head_dim, int64_t w_local, int64_t w_pretrained, double rope_theta, int dtype, void* workspace,
+                    size_t workspace_bytes, void* stream) {
+    return prefill_common(Q, K, V, out, lse, L, H_q, H_kv, head_dim, w_local, w_pretrained, rope_theta, dtype,
+                          workspace, workspace_bytes, stream, true);
+}
+
+int jetlong_causal_prefill(const void* Q, const void* K, const void* V, void* out, float* lse, int64_t L, int H_q,
+                           int H_kv, int head_dim, int dtype, void* workspace, size_t workspace_bytes, void* stream) {
+    return prefill_common(Q, K, V, out, lse, L, H_q, H_kv, head_dim, 0, 1, 1.0, dtype, workspace, workspace_bytes,
+                          stream, false);
+}
+
+int jetlong_decode(const void* q, const void* Kcache, const void* Vcache, void* out, float* lse, int64_t L, int H_q,
+                   int H_kv, int head_dim, int64_t w_local, int64_t w_pretrained, double rope_theta, int dtype,
+                   void* workspace, size_t workspace_bytes, void* stream) {
+    return decode_common(q, Kcache, Vcache, out, lse, L, H_q, H_kv, head_dim, w_local, w_pretrained, rope_theta, dtype,
+                         workspace, workspace_bytes, stream, true);
+}
+
+int jetlong_causal_decode(const void* q, const void* Kcache, const void* Vcache, void* out, float* lse, int64_t L,
+                          int H_q, int H_kv, int head_dim, int dtype, void* workspace, size_t workspace_bytes,
+                          void* stream) {
+    return decode_common(q, Kcache, Vcache, out, lse, L, H_q, H_kv, head_dim, 0, 1, 1.0, dtype, workspace,
+                         workspace_bytes, stream, false);
+}
+
+int jetlong_prefill_host(const void* Q, const void* K, const void* V, void* out, float* lse, int64_t L, int H_q,
+                         int H_kv, int head_dim, int64_t w_local, int64_t w_pretrained, double rope_theta, int dtype) {
+    int rc = validate(Q, K, V, out, lse, L, H_q, H_kv, head_dim, w_local, w_pretrained, rope_theta, dtype);
+    if (rc != JETLONG_OK) return rc;
+    rc = device_ok();
+    if (rc != JETLONG_OK) return rc;
+    const size_t es = dtype == JETLONG_FP32 ? 4 : 2;
+    const size_t nq = (size_t)L * H_q * head_dim * es, nk = (size_t)L * H_kv * head_dim * es;
+    const size_t nl = (size_t)L * H_q * sizeof(float);
+    const size_t nws = jetlong_workspace_bytes(JETLONG_OP_PREFILL, L, H_q, H_kv, head_dim, dtype);
+    unsigned char* dev = nullptr;
+    const size_t oq = 0, ok = align256(nq), ov = ok + align256(nk), oo = ov + align256(nk), ol = oo + align256(nq),
+                 ow = ol + align256(nl), total = ow + align256(nws) + 256;
+    if (cudaMalloc(&dev, total) != cudaSuccess) return check_launch("cudaMalloc");
+    cudaMemcpyAsync(dev + oq, Q, nq, cudaMemcpyHostToDevice, 0);
+    cudaMemcpyAsync(dev + ok, K, nk, cudaMemcpyHostToDevice, 0);
+    cudaMemcpyAsync(dev + ov, V, nk, cudaMemcpyHostToDevice, 0);
+    rc = jetlong_prefill(dev + oq, dev + ok, dev + ov, dev + oo, (float*)(dev + ol), L, H_q, H_kv, head_dim, w_local,
+                         w_pretrained, rope_theta, dtype, dev + ow, align256(nws) + 256, nullptr);
+    if (rc == JETLONG_OK) {
+        cudaMemcpyAsync(out, dev + oo, nq, cudaMemcpyDeviceToHost, 0);
+        cudaMemcpyAsync(lse, dev + ol, nl, cudaMemcpyDeviceToHost, 0);
+        if (cudaStreamSynchronize(0) != cudaSuccess) rc = check_launch("jetlong_prefill_host");
+    }
+    cudaFree(dev);
+    return rc;
+}
+
+const char* jetlong_status_string(int status) {
+    switch (status) {
+        case JETLONG_OK: return "ok";
+        case JETLONG_INVALID_ARG: return "invalid argument";
+        case JETLONG_UNSUPPORTED: return "unsupported device or configuration (needs compute capability 10.x)";
+        case JETLONG_CUDA_ERROR: return g_err;
+        default: return "unknown status";
+    }
+}
+
+int64_t jetlong_launch_count(void) { return g_launches.load(); }
+
+int jetlong_set_prefill_impl(int impl) { return g_prefill_impl.exchange(impl); }
+
+}  // extern "C"

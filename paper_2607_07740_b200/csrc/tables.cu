@@ -1,0 +1,93 @@
+// tables.cu -- rotation tables for the correction rotation of Eq.(5)-(6).
+//
+// Angles Delta(k)*theta_i reach ~1e5 rad at L=128K, so forming them in fp32 is wrong by ~6e-3 rad.
+// Every table entry is therefore computed in fp64 on the device (theta_i = rope_theta^(-2i/d) by pow,
+// angle = integer * theta_i, sincos in double) and rounded once to fp32.
+#include <math.h>
+
+#include "common.cuh"
+
+namespace jetlong {
+
+// ---- per-key table: T[k][i] = (cos, sin)(Delta(k) theta_i) ------------------------------------------
+__global__ void key_table_kernel(float2* __restrict__ tab, long long L, long long G, int half, double log2_theta,
+                                 int d) {
+    long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= L * half) return;
+    long long k = idx / half;
+    int i = (int)(idx - k * half);
+    double th = exp2(-2.0 * (double)i / (double)d * log2_theta);
+    double a = (double)delta_pos(k, G) * th;
+    double s, c;
+    sincos(a, &s, &c);
+    tab[idx] = make_float2((float)c, (float)s);
+}
+
+int build_key_table(float2* tab, long long L, long long G, int d, double theta, cudaStream_t st) {
+    int half = d / 2;
+    long long n = L * half;
+    int threads = 256;
+    long long blocks = (n + threads - 1) / threads;
+    key_table_kernel<<<(unsigned)blocks, threads, 0, st>>>(tab, L, G, half, log2(theta), d);
+    note_launch();
+    return check_launch("key_table_kernel");
+}
+
+// ---- two-level table -----------------------------------------------------------------------------------
+// For n = -Delta >= 0 written as n = 256 a + b:  R(Delta) = R(-256 a) R(-b).
+//   HI[a][i] = (cos, sin)(-256 a theta_i), a in [0, n_hi)      LO[b][i] = (cos, sin)(-b theta_i), b in [0, 256)
+// Independent of G; depends on L only through n_hi = ceil(L/256)+1, so consecutive decode steps skip the
+// rebuild (header match) except once every 256 tokens.
+// Region layout: [TableHeader (256 B)] [LO: 256*half float2] [HI: n_hi*half float2]
+static constexpr unsigned long long kMagic = 0x4a45544c4f4e4732ull;  // "JETLONG2"
+
+size_t two_level_bytes(long long L, int d) {
+    long long n_hi = (L + 255) / 256 + 1;
+    return 256 + align256((size_t)(256 + n_hi) * (d / 2) * sizeof(float2));
+}
+
+__global__ void two_level_kernel(unsigned char* __restrict__ region, long long n_hi, int half, double theta,
+                                 double log2_theta, int d) {
+    TableHeader* hdr = reinterpret_cast<TableHeader*>(region);
+    // header already valid for these parameters: nothing to do (decode steps 1..n hit this path)
+    if (hdr->magic == kMagic && hdr->theta == theta && hdr->n_hi == n_hi && hdr->d == d) return;
+    float2* lo = reinterpret_cast<float2*>(region + 256);
+    float2* hi = lo + 256 * half;
+    long long total = (256 + n_hi) * half;
+    for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < total;
+         idx += (long long)gridDim.x * blockDim.x) {
+        long long row = idx / half;
+        int i = (int)(idx - row * half);
+        double th = exp2(-2.0 * (double)i / (double)d * log2_theta);
+        double n = row < 256 ? (double)row : 256.0 * (double)(row - 256);
+        double s, c;
+        sincos(-n * th, &s, &c);
+        (row < 256 ? lo : hi)[(row < 256 ? row : row - 256) * half + i] = make_float2((float)c, (float)s);
+    }
+}
+
+__global__ void two_level_seal_kernel(unsigned char* region, long long n_hi, double theta, int d) {
+    TableHeader* hdr = reinterpret_cast<TableHeader*>(region);
+    if (hdr->magic == kMagic && hdr->theta == theta && hdr->n_hi == n_hi && hdr->d == d) return;
+    hdr->theta = theta;
+    hdr->n_hi = n_hi;
+    hdr->d = d;
+    hdr->pad = 0;
+    __threadfence();
+    hdr->magic = kMagic;
+}
+
+int build_two_level(void* region, long long L, int d, double theta, cudaStream_t st) {
+    long long n_hi = (L + 255) / 256 + 1;
+    int half = d / 2;
+    long long total = (256 + n_hi) * half;
+    int threads = 256;
+    int blocks = (int)((total + threads - 1) / threads);
+    if (blocks > 1024) blocks = 1024;
+    two_level_kernel<<<blocks, threads, 0, st>>>((unsigned char*)region, n_hi, half, theta, log2(theta), d);
+    two_level_seal_kernel<<<1, 1, 0, st>>>((unsigned char*)region, n_hi, theta, d);
+    note_launch(2);
+    return check_launch("two_level_kernel");
+}
+
+}  // namespace jetlong

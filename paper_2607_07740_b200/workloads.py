@@ -70,10 +70,11 @@ def _rope_true_positions(x, pos0, theta, chunk=8192):
     return x
 
 
-def make_qkv(L, H_q, H_kv, d, rope_theta, dtype, seed, outliers=False, device="cpu", q_pos0=0, n_q=None):
+def make_qkv(L, H_q, H_kv, d, rope_theta, dtype, seed, outliers=False, device="cpu", q_pos0=0, n_q=None, k_pos0=0):
     """Q [n_q,H_q,d], K [L,H_kv,d], V [L,H_kv,d] in `dtype` on `device`.
 
-    Q rows sit at absolute positions q_pos0 .. q_pos0+n_q-1 (default: 0..L-1); K rows at 0..L-1.
+    Q rows sit at absolute positions q_pos0 .. q_pos0+n_q-1 (default: 0..L-1); K rows at k_pos0 .. k_pos0+L-1
+    (default 0..L-1; a non-zero k_pos0 is only used by the global-rotation invariance test).
     outliers: 4 seeded channel indices per KV head of the un-rotated x_k are scaled by 8.
     """
     n_q = L if n_q is None else n_q
@@ -90,7 +91,7 @@ def make_qkv(L, H_q, H_kv, d, rope_theta, dtype, seed, outliers=False, device="c
             xk[:, kv, idx] *= 8.0
     Q = _rope_true_positions(xq, q_pos0, rope_theta).to(td).contiguous()
     del xq
-    K = _rope_true_positions(xk, 0, rope_theta).to(td).contiguous()
+    K = _rope_true_positions(xk, k_pos0, rope_theta).to(td).contiguous()
     del xk
     return Q, K, v.to(td).contiguous()
 

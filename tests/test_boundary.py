@@ -1,0 +1,81 @@
+"""CPU-only checks of the C-ABI boundary: the library loads, exports every symbol include/jetlong.h declares,
+computes Eq.(2) on the host and validates arguments before touching the device."""
+import ctypes
+import os
+import re
+
+import pytest
+
+from paper_2607_07740_b200 import binding as B
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _declared():
+    src = open(os.path.join(ROOT, "include", "jetlong.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(jetlong_[a-z_]+)\s*\(", src)))
+
+
+def test_every_declared_symbol_is_exported_and_bound():
+    names = _declared()
+    assert len(names) >= 10
+    L = B.lib()
+    for n in names:
+        assert hasattr(L, n), n
+    assert sorted(B.EXPORTS) == names
+
+
+def test_group_size_host():
+    assert B.jetlong_group_size(98304, 32768) == 3 and B.jetlong_group_size(98305, 32768) == 4
+    assert B.jetlong_group_size(1, 32768) == 1 and B.jetlong_group_size(32768, 32768) == 1
+    assert B.jetlong_group_size(0, 5) == -1 and B.jetlong_group_size(5, 0) == -1
+    for m in range(1, 50):
+        assert B.jetlong_group_size(m * 4096, 4096) == m and B.jetlong_group_size(m * 4096 + 1, 4096) == m + 1
+
+
+def test_workspace_sizes():
+    assert B.jetlong_workspace_bytes(B.OP_PREFILL, 1024, 4, 2, 64, B.FP32) >= 1024 * 32 * 8
+    assert B.jetlong_workspace_bytes(B.OP_DECODE, 131072, 32, 8, 128, B.BF16) > 0
+    assert B.jetlong_workspace_bytes(B.OP_DECODE, 131072, 32, 8, 96, B.BF16) == 0       # bad head_dim
+    assert B.jetlong_workspace_bytes(99, 1024, 4, 2, 64, B.FP32) == 0
+
+
+def test_validation_happens_before_any_launch():
+    L = B.lib()
+    buf = (ctypes.c_char * 4096)()
+    a = ctypes.addressof(buf)
+    a = (a + 15) & ~15
+    ok_args = dict(L=8, H_q=2, H_kv=1, d=64, w0=1, w_pre=4, theta=1e4, dt=B.FP32)
+
+    def call(**kw):
+        p = dict(ok_args, **kw)
+        ptrs = kw.get("ptrs", [a, a, a, a, a])
+        return L.jetlong_prefill(*ptrs, p["L"], p["H_q"], p["H_kv"], p["d"], p["w0"], p["w_pre"], p["theta"], p["dt"],
+                                 a, 4096, None)
+
+    assert call(ptrs=[0, a, a, a, a]) == B.INVALID_ARG
+    assert call(L=0) == B.INVALID_ARG
+    assert call(H_q=3, H_kv=2) == B.INVALID_ARG
+    assert call(d=96) == B.INVALID_ARG
+    assert call(w0=-1) == B.INVALID_ARG
+    assert call(w_pre=0) == B.INVALID_ARG
+    assert call(theta=0.0) == B.INVALID_ARG
+    assert call(dt=7) == B.INVALID_ARG
+    assert call(ptrs=[a + 4, a, a, a, a]) == B.INVALID_ARG
+    # workspace too small for the rotation table
+    assert L.jetlong_prefill(a, a, a, a, a, 4096, 2, 1, 64, 1, 4, 1e4, B.FP32, a, 16, None) == B.INVALID_ARG
+    # valid arguments but no B200 here: the library refuses instead of falling back to the CPU
+    import torch
+    if not torch.cuda.is_available():
+        assert call() == B.UNSUPPORTED
+    assert b"invalid" in L.jetlong_status_string(B.INVALID_ARG)
+
+
+def test_product_does_not_import_the_oracle():
+    pkg = os.path.join(ROOT, "paper_2607_07740_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                txt = open(os.path.join(dirpath, f)).read()
+                assert "import oracle" not in txt and "from oracle" not in txt and "jetlong_oracle" not in txt, f

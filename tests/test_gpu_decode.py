@@ -1,0 +1,89 @@
+"""GPU parity: jetlong_decode / jetlong_causal_decode against the oracle's row L-1."""
+import numpy as np
+import pytest
+import torch
+
+import paper_2607_07740_b200 as J
+from paper_2607_07740_b200 import workloads as W
+
+from parity_util import check, oracle_rows
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda"
+
+
+def _decode_vs_oracle(L, H_q, H_kv, d, theta, w_pre, w0, dtype, seed, what):
+    Q, K, V = W.make_qkv(L, H_q, H_kv, d, theta, dtype, seed, dtype == "bf16", DEV, q_pos0=L - 1, n_q=1)
+    out, lse = J.jetlong_decode(Q[0].contiguous(), K, V, L, w_local=w0, w_pretrained=w_pre, rope_theta=theta)
+    torch.cuda.synchronize()
+    rows = [L - 1] * H_q
+    heads = list(range(H_q))
+    ro, rl = oracle_rows(Q, K, V, rows, heads, w_local=w0, w_pretrained=w_pre, rope_theta=theta,
+                         q_pos_rows=[0] * H_q)
+    return check(out, lse, ro, rl, Q.dtype, what)
+
+
+@pytest.mark.parametrize("L,H_q,H_kv,d,theta,w_pre,w0,dtype", [
+    (1000, 32, 8, 128, 1e6, 256, 100, "bf16"),     # G=4, the C5 head layout
+    (4097, 32, 8, 128, 1e6, 1024, 512, "bf16"),    # G=5, ragged
+    (777, 4, 2, 128, 1e6, 200, 100, "bf16"),       # H_kv=2 -> 4 warps per head
+    (513, 4, 4, 64, 1e4, 128, 64, "bf16"),         # d=64, g=1
+    (300, 6, 2, 64, 1e4, 100, 7, "fp32"),          # g=3 -> GQ=1
+    (1024, 4, 2, 64, 1e4, 256, 64, "fp32"),        # config-1 shaped
+    (200, 2, 1, 128, 1e6, 64, 0, "fp32"),          # w0=0
+    (64, 2, 1, 64, 1e4, 256, 3, "bf16"),           # G=1 -> control
+    (1, 2, 1, 64, 1e4, 16, 3, "fp32"),
+    (5, 8, 8, 128, 1e4, 2, 1, "bf16"),
+])
+def test_decode_small(L, H_q, H_kv, d, theta, w_pre, w0, dtype):
+    _decode_vs_oracle(L, H_q, H_kv, d, theta, w_pre, w0, dtype, 4321 + L, "decode L=%d" % L)
+
+
+def test_decode_equals_last_prefill_row():
+    L, H_q, H_kv, d, theta, w_pre, w0 = 900, 8, 2, 128, 1e6, 256, 100
+    Q, K, V = W.make_qkv(L, H_q, H_kv, d, theta, "fp32", 99, False, DEV)
+    out_p, lse_p = J.jetlong_prefill(Q, K, V, w_local=w0, w_pretrained=w_pre, rope_theta=theta)
+    out_d, lse_d = J.jetlong_decode(Q[L - 1].contiguous(), K, V, L, w_local=w0, w_pretrained=w_pre, rope_theta=theta)
+    assert (out_p[L - 1] - out_d).abs().max() < 1e-4
+    assert (lse_p[:, L - 1] - lse_d).abs().max() < 1e-5
+
+
+def test_causal_decode_control():
+    L, H_q, H_kv, d = 3000, 32, 8, 128
+    Q, K, V = W.make_qkv(L, H_q, H_kv, d, 1e6, "bf16", 77, True, DEV, q_pos0=L - 1, n_q=1)
+    out, lse = J.jetlong_causal_decode(Q[0].contiguous(), K, V, L)
+    ro, rl = oracle_rows(Q, K, V, [L - 1] * H_q, list(range(H_q)), w_local=0, w_pretrained=1, rope_theta=1e6,
+                         mode="causal", q_pos_rows=[0] * H_q)
+    check(out, lse, ro, rl, Q.dtype, "causal decode")
+
+
+@pytest.mark.parametrize("L0", W.C5_L0)
+def test_config5_decode_steps(L0):
+    """Config 5: 256 consecutive steps, L = L0 + t, G crosses 2->3 / 4->5 after step 0 (R14)."""
+    c = W.C5
+    steps = W.C5_STEPS
+    Qs, Kc, Vc = W.make_decode_inputs(c, L0, steps, DEV)
+    ws = J.binding.alloc_workspace(J.binding.OP_DECODE, L0 + steps, c.H_q, c.H_kv, c.d, J.BF16, DEV)
+    outs, lses = [], []
+    for t in range(steps):
+        L = L0 + t
+        o, l = J.jetlong_decode(Qs[t].contiguous(), Kc, Vc, L, w_local=c.w_local, w_pretrained=c.w_pretrained,
+                                rope_theta=c.rope_theta, workspace=ws)
+        outs.append(o)
+        lses.append(l)
+    torch.cuda.synchronize()
+    assert J.jetlong_group_size(L0, c.w_pretrained) + 1 == J.jetlong_group_size(L0 + 1, c.w_pretrained)
+    Kf = Kc.float().cpu().numpy()
+    Vf = Vc.float().cpu().numpy()
+    import oracle
+    worst = dict(out_abs=0.0, out_rel=0.0, lse=0.0)
+    for t in range(steps):                      # every step, all 32 heads, each over its full key range
+        L = L0 + t
+        Qr = Qs[t].float().cpu().numpy()
+        ro, rl = oracle.attend_rows((Qr, c.H_q), Kf[:L], Vf[:L], [L - 1] * c.H_q, list(range(c.H_q)),
+                                    w_local=c.w_local, w_pretrained=c.w_pretrained, rope_theta=c.rope_theta,
+                                    q_is_compact=True)
+        r = check(outs[t], lses[t], ro, rl, torch.bfloat16, "C5 L0=%d step %d" % (L0, t))
+        for k in worst:
+            worst[k] = max(worst[k], r[k])
+    print("C5 L0=%d worst errors over %d steps: %s" % (L0, steps, worst))

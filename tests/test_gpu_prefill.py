@@ -1,0 +1,119 @@
+"""GPU parity: jetlong_prefill / jetlong_causal_prefill (through the C ABI) against the fp64 oracle."""
+import numpy as np
+import pytest
+import torch
+
+import paper_2607_07740_b200 as J
+from paper_2607_07740_b200 import workloads as W
+
+from parity_util import all_pairs, check, gather, oracle_rows
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda"
+
+
+def _run_full(L, H_q, H_kv, d, theta, w_pre, w0, dtype, seed, outliers=False, what=""):
+    Q, K, V = W.make_qkv(L, H_q, H_kv, d, theta, dtype, seed, outliers, DEV)
+    out, lse = J.jetlong_prefill(Q, K, V, w_local=w0, w_pretrained=w_pre, rope_theta=theta)
+    torch.cuda.synchronize()
+    rows, heads = all_pairs(L, H_q)
+    ro, rl = oracle_rows(Q, K, V, rows, heads, w_local=w0, w_pretrained=w_pre, rope_theta=theta)
+    og, lg = gather(out, lse, rows, heads)
+    return check(og, lg, ro, rl, Q.dtype, what), (Q, K, V, out, lse)
+
+
+def test_config1_full_fp32():
+    c = W.C1
+    _run_full(c.L, c.H_q, c.H_kv, c.d, c.rope_theta, c.w_pretrained, c.w_local, "fp32", c.seed(), what="C1 L=1024")
+
+
+def test_config1_L256_is_causal_bitexact():
+    c = W.C1
+    Q, K, V = W.make_qkv(256, c.H_q, c.H_kv, c.d, c.rope_theta, "fp32", c.seed(), False, DEV)
+    out, lse = J.jetlong_prefill(Q, K, V, w_local=c.w_local, w_pretrained=c.w_pretrained, rope_theta=c.rope_theta)
+    outc, lsec = J.jetlong_causal_prefill(Q, K, V)
+    torch.cuda.synchronize()
+    assert torch.equal(out, outc) and torch.equal(lse, lsec)           # step a2: G = 1 dispatches to the control
+    rows, heads = all_pairs(256, c.H_q)
+    ro, rl = oracle_rows(Q, K, V, rows, heads, w_local=c.w_local, w_pretrained=c.w_pretrained, rope_theta=c.rope_theta)
+    check(*gather(out, lse, rows, heads), ro, rl, Q.dtype, "C1 L=256")
+
+
+@pytest.mark.parametrize("L,H_q,H_kv,d,theta,w_pre,w0,dtype", [
+    (777, 4, 2, 128, 1e6, 200, 100, "bf16"),      # G=4, ragged tail, several tiles, straddle not tile aligned
+    (513, 4, 4, 64, 1e4, 128, 64, "bf16"),        # G=5, d=64, MHA
+    (640, 8, 2, 128, 1e6, 320, 128, "bf16"),      # G=2, g=4, tile-aligned window
+    (300, 2, 1, 128, 5e5, 100, 0, "bf16"),        # w0=0: only self is local
+    (300, 2, 1, 64, 1e4, 100, 7, "fp32"),         # G=3, fp32 d=64
+    (200, 2, 2, 128, 1e6, 64, 33, "fp32"),        # fp32 d=128
+    (65, 2, 1, 64, 1e4, 16, 3, "fp32"),
+    (64, 2, 1, 64, 1e4, 16, 3, "bf16"),
+    (63, 2, 1, 128, 1e4, 16, 3, "bf16"),
+    (1, 2, 1, 64, 1e4, 16, 3, "fp32"),
+    (2, 2, 1, 128, 1e4, 1, 0, "bf16"),
+])
+def test_small_shapes_full(L, H_q, H_kv, d, theta, w_pre, w0, dtype):
+    _run_full(L, H_q, H_kv, d, theta, w_pre, w0, dtype, 1234 + L, outliers=(dtype == "bf16"), what="small L=%d" % L)
+
+
+def test_window_covering_everything_is_control():
+    Q, K, V = W.make_qkv(300, 4, 2, 128, 1e6, "bf16", 5, True, DEV)
+    out, lse = J.jetlong_prefill(Q, K, V, w_local=299, w_pretrained=64, rope_theta=1e6)
+    outc, lsec = J.jetlong_causal_prefill(Q, K, V)
+    assert torch.equal(out, outc) and torch.equal(lse, lsec)
+
+
+def test_control_matches_oracle_causal():
+    L, H_q, H_kv, d = 500, 4, 2, 128
+    Q, K, V = W.make_qkv(L, H_q, H_kv, d, 1e6, "bf16", 6, True, DEV)
+    out, lse = J.jetlong_causal_prefill(Q, K, V)
+    rows, heads = all_pairs(L, H_q)
+    ro, rl = oracle_rows(Q, K, V, rows, heads, w_local=0, w_pretrained=1, rope_theta=1e6, mode="causal")
+    check(*gather(out, lse, rows, heads), ro, rl, Q.dtype, "control")
+
+
+def test_inputs_are_never_written():
+    Q, K, V = W.make_qkv(400, 4, 2, 128, 1e6, "bf16", 7, True, DEV)
+    q0, k0, v0 = Q.clone(), K.clone(), V.clone()
+    J.jetlong_prefill(Q, K, V, w_local=50, w_pretrained=100, rope_theta=1e6)
+    torch.cuda.synchronize()
+    assert torch.equal(Q, q0) and torch.equal(K, k0) and torch.equal(V, v0)   # cache invariant, Eq.(4)
+
+
+def test_global_rotation_invariance_fp32():
+    # rotating both Q and K by a global R(c) changes nothing: only Delta corrections are applied (pin (ii))
+    L, H_q, H_kv, d, theta = 300, 2, 1, 64, 1e4
+    outs = []
+    for c in (0, 1000):
+        Q, K, V = W.make_qkv(L, H_q, H_kv, d, theta, "fp32", 8, False, DEV, q_pos0=c, k_pos0=c)
+        out, lse = J.jetlong_prefill(Q, K, V, w_local=10, w_pretrained=100, rope_theta=theta)
+        outs.append((out.clone(), lse.clone()))
+    assert (outs[0][0] - outs[1][0]).abs().max() < 2e-4
+    assert (outs[0][1] - outs[1][1]).abs().max() < 2e-4
+
+
+def _sampled(cfg, L, w0, n_pairs, layer=0, what=""):
+    Q, K, V = W.make_config_inputs(cfg, DEV, layer=layer, L=L)
+    out, lse = J.jetlong_prefill(Q, K, V, w_local=w0, w_pretrained=cfg.w_pretrained, rope_theta=cfg.rope_theta)
+    torch.cuda.synchronize()
+    G = J.jetlong_group_size(L, cfg.w_pretrained)
+    rows, heads = W.sample_pairs(L, cfg.H_q, n_pairs, cfg.seed(layer), w0, G)
+    ro, rl = oracle_rows(Q, K, V, rows, heads, w_local=w0, w_pretrained=cfg.w_pretrained, rope_theta=cfg.rope_theta)
+    return check(*gather(out, lse, rows, heads), ro, rl, Q.dtype, what)
+
+
+def test_config2_sampled_rows():
+    c = W.C2
+    _sampled(c, c.L, c.w_local, 512, what="C2 L=65536")
+
+
+@pytest.mark.parametrize("L", W.C3_SWEEP_L)
+def test_config3_sweep_sampled_rows(L):
+    c = W.C3
+    _sampled(c, L, c.w_local, 512 if L == c.L else 128, what="C3 L=%d" % L)
+
+
+@pytest.mark.parametrize("w0,layer", [(2048, 0), (8192, 35)])
+def test_config4_layers_sampled_rows(w0, layer):
+    c = W.C4
+    _sampled(c, c.L, w0, 128, layer=layer, what="C4 w0=%d layer %d" % (w0, layer))
