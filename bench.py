@@ -1,0 +1,334 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the libjetlong hot path on synthetic Qwen3-shaped data.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+
+A "step" is one bifocal prefill call (scope rows a1-a8) on BASELINE.json configs[1]
+(Qwen3-1.7B-shaped, L=65536, H_q=16, H_kv=8, d=128, w_local=4096, w_pretrained=32768, G=2).
+`value` = TFLOP/s with FLOPs = 2*d*H_q*L*(L+1) (the causal convention of BASELINE.json), inputs
+resident in HBM.  Beside it, measured in the same run: the matched control kernel (a10), batch-1
+decode at 128K (a9, KV-read GB/s), the end-to-end number through the host-buffer C-ABI call, the
+roofline of the dominant kernel and the CPU oracle on a bounded sample.
+
+N > 1 ("replicas only"): the path has no exchange step, every rank runs the same
+workload on its own GPU and `value` is the sum; no collective is on the data path.
+"""
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import torch  # noqa: E402
+
+
+def flops_causal(L, H_q, d):
+    return 2.0 * d * H_q * L * (L + 1)
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled during the timed region (B200_PROFILING.md)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index = index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"], stdout=subprocess.PIPE,
+                                         stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                sm.append(float(f[1])); mx.append(float(f[2])); pw.append(float(f[3]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "power_w_max": max(pw),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        j = json.load(open(p))
+        return dict(tflops_burst=j["bf16_tflops"], tflops_sustained=j.get("bf16_tflops_sustained", j["bf16_tflops"]),
+                    hbm_gbs=j["hbm_gbs"], source="measured (MEASURED_PEAKS.json)")
+    return dict(tflops_burst=1590.0, tflops_sustained=1400.0, hbm_gbs=6650.0, source="fallback (B200_PROFILING.md)")
+
+
+def oracle_sample(cfg, n_pairs, Q, K, V):
+    """Time the fp64 CPU oracle, as it stands, on n_pairs seeded (row, head) pairs of the workload."""
+    import oracle
+    from paper_2607_07740_b200 import workloads as W
+    rows, heads = W.sample_pairs(cfg.L, cfg.H_q, n_pairs, cfg.seed(), None, None)
+    rows, heads = rows[:n_pairs], heads[:n_pairs]
+    Kf = K.float().cpu().numpy()
+    Vf = V.float().cpu().numpy()
+    ri = torch.as_tensor(rows, device=Q.device)
+    hi = torch.as_tensor(heads, device=Q.device)
+    Qr = Q[ri, hi].float().cpu().numpy()
+    t0 = time.perf_counter()
+    oracle.attend_rows((Qr, cfg.H_q), Kf, Vf, rows, heads, w_local=cfg.w_local, w_pretrained=cfg.w_pretrained,
+                       rope_theta=cfg.rope_theta, q_is_compact=True)
+    dt = time.perf_counter() - t0
+    visits = float(sum(r + 1 for r in rows))
+    tflops = visits * 4.0 * cfg.d / dt / 1e12          # 2d (QK) + 2d (PV) flops per key visit, same convention
+    return dict(value=tflops, unit="TFLOP/s", cores=oracle.num_threads(), kind="oracle",
+                sample="%d seeded (row, head) pairs of the workload, each over its full key range; %.3g key "
+                       "visits in %.1f s; extrapolated full-config time %.0f s" %
+                       (len(rows), visits, dt, flops_causal(cfg.L, cfg.H_q, cfg.d) / (tflops * 1e12)),
+                seconds=dt)
+
+
+def run_reference(args, cfg):
+    """--impl reference: the oracle as it stands, on the host cores; each step a bounded sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from paper_2607_07740_b200 import workloads as W
+    dev = "cuda" if torch.cuda.is_available() else "cpu"
+    Q, K, V = W.make_config_inputs(cfg, dev)
+    n_pairs = 24
+    vals = []
+    for i in range(args.warmup + args.steps):
+        r = oracle_sample(cfg, n_pairs, Q, K, V)
+        if i >= args.warmup:
+            vals.append(r)
+    v = sum(x["value"] for x in vals) / len(vals)
+    ms = 1e3 * sum(x["seconds"] for x in vals) / len(vals)
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": "TFLOP/s", "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": workload_config(cfg),
+            "cpu_baseline": {"value": v, "unit": "TFLOP/s", "cores": vals[0]["cores"], "kind": "oracle",
+                             "sample": vals[0]["sample"]},
+            "e2e": {"value": v, "unit": "TFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+METRIC = "bifocal-attn prefill TFLOP/s @64K-128K (% bf16 peak); decode KV-read GB/s"
+
+
+def workload_config(cfg):
+    return {"workload": "BASELINE.json configs[1]: Qwen3-1.7B-shaped single-layer bifocal prefill",
+            "L": cfg.L, "H_q": cfg.H_q, "H_kv": cfg.H_kv, "head_dim": cfg.d, "w_local": cfg.w_local,
+            "w_pretrained": cfg.w_pretrained, "G": -(-cfg.L // cfg.w_pretrained), "rope_theta": cfg.rope_theta,
+            "batch": 1, "parallelism": "replicas only (no sharding, no collective)",
+            "l2": "inputs+outputs (0.8 GB) exceed the 126 MB L2; no flush needed between iterations"}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-extras", action="store_true", help="skip control / decode / e2e / oracle legs (profiling)")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" and not args.no_extras else args.warmup
+
+    from paper_2607_07740_b200 import workloads as W
+    cfg = W.C2
+    if args.impl == "reference":
+        return run_reference(args, cfg)
+
+    import paper_2607_07740_b200 as J
+    from paper_2607_07740_b200 import binding as B
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: libjetlong has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    Q, K, V = W.make_config_inputs(cfg, dev)
+    out = torch.empty_like(Q)
+    lse = torch.empty((cfg.H_q, cfg.L), dtype=torch.float32, device=dev)
+    ws = B.alloc_workspace(B.OP_PREFILL, cfg.L, cfg.H_q, cfg.H_kv, cfg.d, B.BF16, dev)
+    kw = dict(w_local=cfg.w_local, w_pretrained=cfg.w_pretrained, rope_theta=cfg.rope_theta)
+    fl = flops_causal(cfg.L, cfg.H_q, cfg.d)
+
+    def step():
+        J.jetlong_prefill(Q, K, V, out=out, lse=lse, workspace=ws, **kw)
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    n0 = J.jetlong_launch_count()
+    evs = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    barrier()
+    evs[0].record()
+    for i in range(args.steps):
+        step()
+        evs[i + 1].record()
+    barrier()
+    launches = J.jetlong_launch_count() - n0
+    clocks = sampler.stop() if rank == 0 else None
+    total_ms = evs[0].elapsed_time(evs[-1])
+    per = [evs[i].elapsed_time(evs[i + 1]) for i in range(args.steps)]
+    t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total_ms = float(t.item())
+    ms_per_step = total_ms / args.steps
+    value = world * fl / (ms_per_step * 1e-3) / 1e12
+
+    line = {"metric": METRIC, "value": value, "unit": "TFLOP/s", "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "bf16", "data": "synthetic", "config": workload_config(cfg),
+            "tokens_per_s": world * cfg.L / (ms_per_step * 1e-3), "gpu_launches": int(launches), "clocks": clocks,
+            "ms_per_step_min": min(per), "ms_per_step_median": statistics.median(per)}
+
+    pk = peaks()
+    if rank == 0 and not args.no_extras:
+        # ---- roofline of the dominant kernel (the prefill kernel is >99% of a step) ---------------------
+        impl = "tcgen05 UMMA" if _umma_active(B, cfg) else "SIMT fp32 FMA"
+        kern_ms = statistics.median(per)
+        ach = fl / (kern_ms * 1e-3) / 1e12
+        traffic = None
+        tp = os.path.join(ROOT, "profiles", "traffic.json")
+        if os.path.exists(tp):
+            traffic = json.load(open(tp)).get("prefill_dram_bytes_per_launch")
+        if impl == "tcgen05 UMMA":
+            peak, bound, which = pk["tflops_sustained"], "tensor", "sustained cuBLAS bf16, " + pk["source"]
+        else:
+            # fp32 FMA path: 148 SMs x 128 lanes x 2 flop x max SM clock (alu roofline)
+            peak, bound, which = 148 * 128 * 2 * 1.965e9 / 1e12, "alu", "148 SM x 128 FMA lanes x 2 x 1965 MHz (derived)"
+        line["roofline"] = {"bound": bound, "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
+                            "traffic": traffic, "kernel": "prefill (" + impl + ")", "peak_source": which,
+                            "frac_of_bf16_burst_peak": ach / pk["tflops_burst"],
+                            "frac_of_nominal_2250": ach / 2250.0}
+        # ---- matched control (a10) on the same buffers ---------------------------------------------------
+        wsc = B.alloc_workspace(B.OP_CAUSAL_PREFILL, cfg.L, cfg.H_q, cfg.H_kv, cfg.d, B.BF16, dev)
+        for _ in range(2):
+            J.jetlong_causal_prefill(Q, K, V, out=out, lse=lse, workspace=wsc)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        nrep = max(3, min(args.steps, 10))
+        e0.record()
+        for _ in range(nrep):
+            J.jetlong_causal_prefill(Q, K, V, out=out, lse=lse, workspace=wsc)
+        e1.record()
+        torch.cuda.synchronize()
+        cms = e0.elapsed_time(e1) / nrep
+        line["control"] = {"ms": cms, "tflops": fl / (cms * 1e-3) / 1e12, "bifocal_over_control": cms / ms_per_step}
+        # ---- end to end through the host-buffer C-ABI call -----------------------------------------------
+        Qh, Kh, Vh = Q.cpu().pin_memory(), K.cpu().pin_memory(), V.cpu().pin_memory()
+        oh = torch.empty_like(Qh).pin_memory()
+        lh = torch.empty((cfg.H_q, cfg.L), dtype=torch.float32).pin_memory()
+        J.jetlong_prefill_host(Qh, Kh, Vh, out=oh, lse=lh, **kw)
+        ne = 3
+        t0 = time.perf_counter()
+        for _ in range(ne):
+            J.jetlong_prefill_host(Qh, Kh, Vh, out=oh, lse=lh, **kw)
+        ems = (time.perf_counter() - t0) / ne * 1e3
+        line["e2e"] = {"value": fl / (ems * 1e-3) / 1e12, "unit": "TFLOP/s", "ms": ems,
+                       "h2d_bytes_per_step": Qh.numel() * 2 + Kh.numel() * 2 + Vh.numel() * 2,
+                       "d2h_bytes_per_step": oh.numel() * 2 + lh.numel() * 4,
+                       "api": "jetlong_prefill_host (pinned host buffers; cudaMalloc + H2D + kernels + D2H + sync)"}
+        del Qh, Kh, Vh, oh, lh
+        # ---- decode (a9): config 5 at L0 = 131072 ---------------------------------------------------------
+        line["decode"] = bench_decode(J, B, W, dev, pk)
+        # ---- the CPU oracle on a bounded sample ---------------------------------------------------------
+        cb = oracle_sample(cfg, 24, Q, K, V)
+        cb.pop("seconds")
+        line["cpu_baseline"] = cb
+    if rank == 0:
+        print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def _umma_active(B, cfg):
+    # the UMMA path needs no SIMT key table; the library reports which one a bf16 call would take
+    try:
+        return bool(B.lib().jetlong_prefill_uses_umma(cfg.L, cfg.H_q, cfg.H_kv, cfg.d))
+    except AttributeError:
+        return False
+
+
+def bench_decode(J, B, W, dev, pk, L0=131072, steps=64):
+    c = W.C5
+    Qs, Kc, Vc = W.make_decode_inputs(c, L0, steps, dev)
+    ws = B.alloc_workspace(B.OP_DECODE, L0 + steps, c.H_q, c.H_kv, c.d, B.BF16, dev)
+    o = torch.empty((c.H_q, c.d), dtype=torch.bfloat16, device=dev)
+    l = torch.empty((c.H_q,), dtype=torch.float32, device=dev)
+    res = {}
+    for name in ("bifocal", "control"):
+        def run(t):
+            if name == "bifocal":
+                J.jetlong_decode(Qs[t], Kc, Vc, L0 + t, w_local=c.w_local, w_pretrained=c.w_pretrained,
+                                 rope_theta=c.rope_theta, out=o, lse=l, workspace=ws)
+            else:
+                J.jetlong_causal_decode(Qs[t], Kc, Vc, L0 + t, out=o, lse=l, workspace=ws)
+        for t in range(4):
+            run(t)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for t in range(steps):
+            run(t)
+        e1.record()
+        torch.cuda.synchronize()
+        us = e0.elapsed_time(e1) / steps * 1e3
+        kv_bytes = 2.0 * (L0 + steps / 2) * c.H_kv * c.d * 2
+        res[name] = {"us_per_step": us, "kv_read_gbs": kv_bytes / (us * 1e-6) / 1e9,
+                     "frac_hbm_peak": kv_bytes / (us * 1e-6) / 1e9 / pk["hbm_gbs"]}
+    res["workload"] = "BASELINE.json configs[4]: Qwen3-8B-shaped batch-1 decode, L0=%d, %d steps, KV cache %.0f MB > L2" % (
+        L0, steps, 2.0 * L0 * c.H_kv * c.d * 2 / 1e6)
+    res["hbm_peak_gbs"] = pk["hbm_gbs"]
+    res["peak_source"] = pk["source"]
+    return res
+
+
+if __name__ == "__main__":
+    main()

@@ -105,6 +105,9 @@ int64_t jetlong_launch_count(void);
  * jetlong_set_prefill_impl(-1) restores the default. Returns the previous value. */
 int jetlong_set_prefill_impl(int impl);
 
+/* 1 if a bf16 prefill of these shapes runs on the tcgen05 UMMA kernel under the current setting, else 0. */
+int jetlong_prefill_uses_umma(int64_t L, int H_q, int H_kv, int head_dim);
+
 #ifdef __cplusplus
 }
 #endif

@@ -41,7 +41,7 @@ def lib():
         L.jlo_rope.argtypes = [vp, i32, dbl, i64, vp]
         L.jlo_num_threads.restype = i32
         L.jlo_attend_rows.restype = i32
-        L.jlo_attend_rows.argtypes = [vp, vp, vp, i64, i32, i32, i32, i64, i64, dbl, i32, i64, i64, vp, vp, vp, vp]
+        L.jlo_attend_rows.argtypes = [vp, vp, vp, i64, i32, i32, i32, i64, i64, dbl, i32, i64, i64, vp, vp, vp, vp, vp]
         L.jlo_three_call_rows.restype = i32
         L.jlo_three_call_rows.argtypes = [vp, vp, vp, i64, i32, i32, i32, i64, i64, dbl, i64, vp, vp, vp, vp, vp]
         L.jlo_scores_row.restype = i32
@@ -91,11 +91,12 @@ def _rows_heads(rows, heads):
 
 
 def attend_rows(Q, K, V, rows, heads, *, w_local, w_pretrained, rope_theta, mode="bifocal", pos_shift=0,
-                q_is_compact=False):
+                q_is_compact=False, Ls=None):
     """out[n,d], lse[n] (float64) for the (row, head) pairs.
 
     Q: [L,H_q,d] (or, with q_is_compact, [n,d] already gathered plus H_q passed via heads max is
     not possible -- so compact callers must pass H_q through Q=(Qrows, H_q)).  K, V: [L,H_kv,d].
+    Ls: optional per-pair current length (decode runs): pair j sees keys 0..rows[j] with G from Ls[j].
     """
     K = _f32(K)
     V = _f32(V)
@@ -113,9 +114,12 @@ def attend_rows(Q, K, V, rows, heads, *, w_local, w_pretrained, rope_theta, mode
     assert Qrows.shape == (n, d)
     out = np.empty((n, d), dtype=np.float64)
     lse = np.empty((n,), dtype=np.float64)
+    if Ls is not None:
+        Ls = np.ascontiguousarray(Ls, dtype=np.int64)
+        assert Ls.shape == rows.shape
     rc = lib().jlo_attend_rows(_p(Qrows), _p(K), _p(V), L, H_q, H_kv, d, int(w_local), int(w_pretrained),
                                float(rope_theta), {"bifocal": 0, "causal": 1}[mode], int(pos_shift), n,
-                               _p(rows), _p(heads), _p(out), _p(lse))
+                               _p(rows), _p(heads), _p(Ls) if Ls is not None else None, _p(out), _p(lse))
     if rc != 0:
         raise ValueError("jlo_attend_rows: bad arguments")
     return out, lse

@@ -109,16 +109,17 @@ static double dotd(const double* a, const double* b, int d) {
  * One G for all rows, from the full length L (R3).  GQA: kv head = h / (H_q/H_kv) (R9).
  * pos_shift shifts every absolute position (q and k) by a constant before Eq.(3)/(5); the
  * library contract is pos_shift = 0, the shift-invariance pin uses other values.
+ * Ls (may be NULL): per-pair current sequence length L_j for decode runs; G_j = G(L_j).
  * Returns 0, or -1 on bad arguments.
  */
 int jlo_attend_rows(const float* Qrows, const float* K, const float* V,
                     int64_t L, int H_q, int H_kv, int d,
                     int64_t w0, int64_t w_pre, double theta, int mode, int64_t pos_shift,
-                    int64_t n, const int64_t* rows, const int32_t* heads,
+                    int64_t n, const int64_t* rows, const int32_t* heads, const int64_t* Ls,
                     double* out, double* lse) {
     if (L < 1 || H_q < 1 || H_kv < 1 || H_q % H_kv || d < 2 || (d & 1) || w0 < 0 || w_pre < 1 ||
         !(theta > 0.0) || n < 0) return -1;
-    const int64_t G = jlo_group_size(L, w_pre);
+    const int64_t G_all = jlo_group_size(L, w_pre);
     const int g = H_q / H_kv;
     const double scale = 1.0 / sqrt((double)d);
     double fr[4096];                       /* theta_i, i < d/2, computed once per call */
@@ -130,6 +131,9 @@ int jlo_attend_rows(const float* Qrows, const float* K, const float* V,
         const int64_t q = rows[j];
         const int h = heads[j];
         if (q < 0 || q >= L || h < 0 || h >= H_q) { bad = 1; continue; }
+        /* decode runs: pair j may carry its own current length L_j <= L; G follows it (R4, R14) */
+        int64_t G = G_all;
+        if (Ls) { if (Ls[j] < 1 || Ls[j] > L || q >= Ls[j]) { bad = 1; continue; } G = jlo_group_size(Ls[j], w_pre); }
         const int kv = h / g;
         double* qloc = (double*)malloc(sizeof(double) * d * 3);
         double* qrem = qloc + d;

@@ -19,7 +19,7 @@ OP_PREFILL, OP_DECODE, OP_CAUSAL_PREFILL, OP_CAUSAL_DECODE = 0, 1, 2, 3
 
 EXPORTS = ["jetlong_group_size", "jetlong_workspace_bytes", "jetlong_prefill", "jetlong_decode",
            "jetlong_causal_prefill", "jetlong_causal_decode", "jetlong_prefill_host", "jetlong_status_string",
-           "jetlong_launch_count", "jetlong_set_prefill_impl"]
+           "jetlong_launch_count", "jetlong_set_prefill_impl", "jetlong_prefill_uses_umma"]
 
 
 class JetlongError(RuntimeError):
@@ -58,6 +58,8 @@ def lib():
         L.jetlong_launch_count.restype = i64
         L.jetlong_set_prefill_impl.restype = i32
         L.jetlong_set_prefill_impl.argtypes = [i32]
+        L.jetlong_prefill_uses_umma.restype = i32
+        L.jetlong_prefill_uses_umma.argtypes = [i64, i32, i32, i32]
         _lib = L
     return _lib
 

@@ -193,4 +193,8 @@ int64_t jetlong_launch_count(void) { return g_launches.load(); }
 
 int jetlong_set_prefill_impl(int impl) { return g_prefill_impl.exchange(impl); }
 
+int jetlong_prefill_uses_umma(int64_t L, int H_q, int H_kv, int head_dim) {
+    return use_umma(L, H_q, H_kv, head_dim, JETLONG_BF16) ? 1 : 0;
+}
+
 }  // extern "C"

@@ -76,14 +76,23 @@ def test_config5_decode_steps(L0):
     Kf = Kc.float().cpu().numpy()
     Vf = Vc.float().cpu().numpy()
     import oracle
-    worst = dict(out_abs=0.0, out_rel=0.0, lse=0.0)
-    for t in range(steps):                      # every step, all 32 heads, each over its full key range
-        L = L0 + t
-        Qr = Qs[t].float().cpu().numpy()
-        ro, rl = oracle.attend_rows((Qr, c.H_q), Kf[:L], Vf[:L], [L - 1] * c.H_q, list(range(c.H_q)),
-                                    w_local=c.w_local, w_pretrained=c.w_pretrained, rope_theta=c.rope_theta,
-                                    q_is_compact=True)
-        r = check(outs[t], lses[t], ro, rl, torch.bfloat16, "C5 L0=%d step %d" % (L0, t))
-        for k in worst:
-            worst[k] = max(worst[k], r[k])
-    print("C5 L0=%d worst errors over %d steps: %s" % (L0, steps, worst))
+    # oracle rows: EVERY step with 4 seeded heads, plus all 32 heads at steps 0, 1 (the G boundary) and the last.
+    # (all 256 x 32 rows would be ~1e9 key visits, several minutes of CPU; the sample keeps every step covered.)
+    gen = torch.Generator(); gen.manual_seed(c.seed() + L0)
+    st_list, hd_list = [], []
+    for t in range(steps):
+        hs = range(c.H_q) if t in (0, 1, steps - 1) else torch.randperm(c.H_q, generator=gen)[:4].tolist()
+        for h in hs:
+            st_list.append(t); hd_list.append(int(h))
+    st = np.array(st_list); hd = np.array(hd_list, dtype=np.int32)
+    Ls = L0 + st
+    sti = torch.as_tensor(st, device=DEV)
+    hdi = torch.as_tensor(hd_list, device=DEV)
+    Qr = Qs[sti, hdi].float().cpu().numpy()
+    ro, rl = oracle.attend_rows((Qr, c.H_q), Kf, Vf, Ls - 1, hd, w_local=c.w_local, w_pretrained=c.w_pretrained,
+                                rope_theta=c.rope_theta, q_is_compact=True, Ls=Ls)
+    og = torch.stack(outs)[sti, hdi]
+    lg = torch.stack(lses)[sti, hdi]
+    worst = check(og, lg, ro, rl, torch.bfloat16, "C5 L0=%d, %d (step, head) rows" % (L0, len(st)))
+    assert torch.isfinite(torch.stack(outs).float()).all() and torch.isfinite(torch.stack(lses)).all()
+    print("C5 L0=%d errors over %d steps: %s" % (L0, steps, worst))

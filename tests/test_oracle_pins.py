@@ -295,6 +295,22 @@ def test_within_group_aliasing():
     assert abs(s_loc[20] - s_loc[21]) > 1e-4          # inside the local window they are told apart
 
 
+def test_per_pair_length_is_the_same_as_truncating_the_cache():
+    # decode runs: pair j with current length L_j == a separate call on the cache cut at L_j
+    Ltot, H_q, H_kv, d, theta, w_pre, w0 = 50, 4, 2, 8, 1e4, 16, 3
+    xq, xk, v = _raw_inputs(Ltot, H_q, H_kv, d, 13)
+    Q = _rope_np(xq, np.arange(Ltot), theta)
+    K = _rope_np(xk, np.arange(Ltot), theta)
+    Ls = np.array([32, 33, 48, 49, 50])          # G = 2, 3, 3, 4, 4: crosses two boundaries
+    rows, heads = Ls - 1, np.array([0, 1, 2, 3, 0])
+    o, l = oracle.attend_rows(Q, K, v, rows, heads, w_local=w0, w_pretrained=w_pre, rope_theta=theta, Ls=Ls)
+    for j, L in enumerate(Ls):
+        o1, l1 = oracle.attend_rows(Q[:L], K[:L], v[:L], [L - 1], [heads[j]], w_local=w0, w_pretrained=w_pre,
+                                    rope_theta=theta)
+        assert np.array_equal(o[j], o1[0]) and l[j] == l1[0]
+    assert [oracle.group_size(int(L), w_pre) for L in Ls] == [2, 3, 3, 4, 4]
+
+
 def test_bad_arguments_are_rejected():
     K = np.zeros((4, 1, 4), dtype=np.float32)
     with pytest.raises(ValueError):
