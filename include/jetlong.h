@@ -105,6 +105,14 @@ int64_t jetlong_launch_count(void);
  * jetlong_set_prefill_impl(-1) restores the default. Returns the previous value. */
 int jetlong_set_prefill_impl(int impl);
 
+/* Operand precision of the REMOTE Q'K'^T on the tcgen05 path.
+ * COMPENSATED (default): rotated operands split hi + lo in fp16, S = Q'hi K'hi + Q'hi K'lo + Q'lo K'hi; meets the
+ * lse tolerance (1e-3) on outlier-channel inputs.  FAST: Q'hi K'hi only (one UMMA group instead of three);
+ * lse errors up to ~2.5e-3 on such inputs.  Local tiles, the control and decode are unaffected.
+ * Returns the previous mode; an unknown mode changes nothing. */
+enum { JETLONG_PRECISION_COMPENSATED = 0, JETLONG_PRECISION_FAST = 1 };
+int jetlong_set_prefill_precision(int mode);
+
 /* 1 if a bf16 prefill of these shapes runs on the tcgen05 UMMA kernel under the current setting, else 0. */
 int jetlong_prefill_uses_umma(int64_t L, int H_q, int H_kv, int head_dim);
 

@@ -16,10 +16,12 @@ _lib = None
 OK, INVALID_ARG, UNSUPPORTED, CUDA_ERROR = 0, 1, 2, 3
 BF16, FP32 = 0, 1
 OP_PREFILL, OP_DECODE, OP_CAUSAL_PREFILL, OP_CAUSAL_DECODE = 0, 1, 2, 3
+PRECISION_COMPENSATED, PRECISION_FAST = 0, 1
 
 EXPORTS = ["jetlong_group_size", "jetlong_workspace_bytes", "jetlong_prefill", "jetlong_decode",
            "jetlong_causal_prefill", "jetlong_causal_decode", "jetlong_prefill_host", "jetlong_status_string",
-           "jetlong_launch_count", "jetlong_set_prefill_impl", "jetlong_prefill_uses_umma"]
+           "jetlong_launch_count", "jetlong_set_prefill_impl", "jetlong_prefill_uses_umma",
+           "jetlong_set_prefill_precision"]
 
 
 class JetlongError(RuntimeError):
@@ -60,6 +62,8 @@ def lib():
         L.jetlong_set_prefill_impl.argtypes = [i32]
         L.jetlong_prefill_uses_umma.restype = i32
         L.jetlong_prefill_uses_umma.argtypes = [i64, i32, i32, i32]
+        L.jetlong_set_prefill_precision.restype = i32
+        L.jetlong_set_prefill_precision.argtypes = [i32]
         _lib = L
     return _lib
 
@@ -95,6 +99,10 @@ def jetlong_launch_count():
 
 def jetlong_set_prefill_impl(impl):
     return int(lib().jetlong_set_prefill_impl(int(impl)))
+
+
+def jetlong_set_prefill_precision(mode):
+    return int(lib().jetlong_set_prefill_precision(int(mode)))
 
 
 def alloc_workspace(op, L, H_q, H_kv, head_dim, dtype, device="cuda"):

@@ -10,6 +10,7 @@ namespace jetlong {
 static std::atomic<long long> g_launches{0};
 static thread_local char g_err[256] = "no CUDA error recorded";
 static std::atomic<int> g_prefill_impl{-1};
+static std::atomic<int> g_prefill_precision{JETLONG_PRECISION_COMPENSATED};
 
 void note_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
 
@@ -24,7 +25,7 @@ int check_launch(const char* what) {
 bool umma_prefill_supported(long long L, int H_q, int H_kv, int d, int dtype);
 size_t umma_prefill_workspace_bytes(long long L, int H_q, int H_kv, int d);
 int launch_prefill_umma(const void* Q, const void* K, const void* V, void* out, float* lse, long long L, int H_q,
-                        int H_kv, int d, long long w0, long long G, double theta, bool bifocal, void* ws,
+                        int H_kv, int d, long long w0, long long G, double theta, bool bifocal, bool precise, void* ws,
                         size_t ws_bytes, cudaStream_t st);
 
 static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; }
@@ -76,7 +77,8 @@ static int prefill_common(const void* Q, const void* K, const void* V, void* out
     if (rc != JETLONG_OK) return rc;
     cudaStream_t st = (cudaStream_t)stream;
     if (use_umma(L, H_q, H_kv, d, dtype))
-        return launch_prefill_umma(Q, K, V, out, lse, L, H_q, H_kv, d, w0, G, theta, bifocal, ws, ws_bytes, st);
+        return launch_prefill_umma(Q, K, V, out, lse, L, H_q, H_kv, d, w0, G, theta, bifocal,
+                                   g_prefill_precision.load() != JETLONG_PRECISION_FAST, ws, ws_bytes, st);
     const float2* tab = nullptr;
     if (bifocal) {
         rc = build_key_table((float2*)ws, L, G, d, theta, st);
@@ -192,6 +194,11 @@ const char* jetlong_status_string(int status) {
 int64_t jetlong_launch_count(void) { return g_launches.load(); }
 
 int jetlong_set_prefill_impl(int impl) { return g_prefill_impl.exchange(impl); }
+
+int jetlong_set_prefill_precision(int mode) {
+    if (mode != JETLONG_PRECISION_COMPENSATED && mode != JETLONG_PRECISION_FAST) return g_prefill_precision.load();
+    return g_prefill_precision.exchange(mode);
+}
 
 int jetlong_prefill_uses_umma(int64_t L, int H_q, int H_kv, int head_dim) {
     return use_umma(L, H_q, H_kv, head_dim, JETLONG_BF16) ? 1 : 0;

@@ -1,21 +1,27 @@
 // prefill_umma.cu -- tcgen05 UMMA bifocal / causal prefill for bf16, head_dim 128 (steps a3-a8, a10).
 //
-// One CTA = 128 query rows x 2 query heads of one KV group ("tile A", "tile B"): both see the same keys,
-// the same positions and therefore the same tile classification, so one TMA-loaded K tile, one V tile and
-// one in-smem RoPE correction (Eq.(6)) serve both.  Warp roles (512 threads):
-//   warp 0      TMA producer: Q (once), then one K and one V tile per visit, SWIZZLE_128B boxes
-//   warp 1      MMA issuer: S_t = Q_t K^T (tcgen05.mma SS), O_t += P_t V (tcgen05.mma TS, P from TMEM)
-//   warps 4-7   rotate group: remote visits rotate the K tile in shared memory between the TMA load and the
-//               MMA (bf16 -> fp32 rotate -> fp16, in place); once per CTA it turns Q into Q' = R(Delta q) Q
-//   warps 8-11  softmax group of tile A; warps 12-15 softmax group of tile B (one thread per query row)
-// TMEM (512 columns): S_A | S_B | O_A | O_B, 128 fp32 columns each; P_t (bf16) aliases S_t columns 0..63.
+// One CTA PAIR (cluster of 2, tcgen05 cta_group::2) = 128 query rows x 2 query heads of one KV group: both
+// heads see the same keys, the same positions and therefore the same tile classification.  Every UMMA is
+// M = 256 across the pair (CTA c owns head h0 + c), so each CTA stages and -- on remote visits -- rotates only
+// HALF of every K tile (its 64 keys) and loads half of every V tile (its 64 channels).
+// Warp roles (384 threads per CTA):
+//   warp 0      TMA producer: its half of K and V per visit, SWIZZLE_128B boxes, NS-stage ring
+//   warp 1      MMA issuer (leader CTA only, one thread): S_b = Q K^T (A = Q from TMEM), O += P V (A = P from TMEM)
+//   warps 4-7   rotate group: stages Q into TMEM; on remote visits rotates its K half in shared memory between
+//               the TMA load and the MMA (Eq.(6): bf16 -> fp32 rotate -> fp16 hi (+ fp16 lo)); once per CTA
+//               it replaces Q in TMEM by Q' = R(Delta q) Q (hi, lo)
+//   warps 8-11  softmax group: one thread per query row, online softmax over the visits, epilogue
+// TMEM (512 columns): S0 | S1 | O | Qa | Qb  (128, 128, 128, 64, 64).  P (bf16) aliases columns 0..63 of its S.
+// S is double-buffered over consecutive visits so QK^T of visit v+1 overlaps the softmax of visit v.
 //
-// Visit order per CTA: local visits first (diagonal tile, then the band down to q - w0), then the Q -> Q'
+// Visit order per pair: local visits first (diagonal tile, then the band down to q - w0), then the Q -> Q'
 // switch, then the remote visits.  The straddle tile is visited twice with complementary masks (step a6).
 // All visits feed ONE running (m, l, O) per row: the additive form of the Eq.(7) merge.
 //
-// Precision: local visits multiply the stored bf16 Q, K.  Remote operands are rounded once to fp16
-// (kind::f16 takes fp16 as well as bf16; values are far inside the fp16 range), see DESIGN.md.
+// Precision: local visits multiply the stored bf16 Q, K exactly.  Remote
+// operands are fp32-rotated and split hi + lo in fp16; S = Q'hi K'hi + Q'hi K'lo + Q'lo K'hi (three UMMA
+// groups, "compensated").  The fast mode keeps only Q'hi K'hi (one group) and misses the lse tolerance on
+// outlier-channel inputs; it is opt-in (jetlong_set_prefill_precision).
 #include <cuda.h>
 #include <math.h>
 
@@ -29,28 +35,38 @@ namespace {
 using namespace ptx;
 
 constexpr int D = 128, BM = 128, BN = 128;
-constexpr int KS = 3, VS = 2;                         // K / V ring depths
-constexpr int TILE_BYTES = BM * D * 2;                // 32 KB: two 16 KB SWIZZLE_128B boxes (cols 0-63 | 64-127)
-constexpr int BOX_BYTES = 128 * 128;
-constexpr int NTHREADS = 512;
+constexpr int NS = 4;                                 // K/V ring depth
+constexpr int KH_BYTES = 64 * D * 2;                  // this CTA's 64 keys: two 8 KB SWIZZLE_128B boxes (ch 0-63 | 64-127)
+constexpr int KBOX = 64 * 128;                        // one K box: 64 rows x 128 B
+constexpr int VH_BYTES = BN * 64 * 2;                 // this CTA's 64 channels of 128 keys: one 16 KB box
+constexpr int STAGE_BYTES = 2 * KH_BYTES + VH_BYTES;  // K (hi in place) | K lo | V
+constexpr int NTHREADS = 384;
 constexpr float kLog2e = 1.4426950408889634f;
+constexpr uint32_t TM_S = 0, TM_O = 256, TM_QA = 384, TM_QB = 448;
 
 struct Bars {
-    uint64_t q_full, q_local_done, q_rot_done, o_full;
-    uint64_t k_full[KS], k_ready[KS], k_empty[KS];
-    uint64_t v_full[VS], v_empty[VS];
-    uint64_t s_full[2], p_full[2];
+    uint64_t kv_full[NS];      // local: TMA bytes of this CTA's K/V halves landed
+    uint64_t kv_ready[NS];     // leader: both rotate groups are done with stage s (8 warp arrivals)
+    uint64_t kv_empty[NS];     // both: MMAs reading stage s have completed (multicast commit)
+    uint64_t s_full[2];        // both: S_b holds Q K^T of a visit
+    uint64_t p_full[2];        // leader: both softmax groups wrote P_b and are done reading S_b (8 warp arrivals)
+    uint64_t pv_done;          // both: O += P V of a visit has completed
+    uint64_t o_full;           // both: all MMAs done
+    uint64_t q_ready;          // leader: Q staged in TMEM by both rotate groups
+    uint64_t q_local_done;     // both: the last local Q K^T has completed, Qa may be overwritten
+    uint64_t q_rot_done;       // leader: Q' (hi, lo) staged in TMEM
     uint32_t tmem_base;
 };
 
-constexpr size_t SMEM_BYTES = 1024 /*align slack*/ + (size_t)(2 + KS + VS) * TILE_BYTES + 1024 /*Bars*/;
+constexpr size_t SMEM_BYTES = 1024 /*align slack*/ + (size_t)NS * STAGE_BYTES + 1024 /*Bars*/;
 
 struct Params {
+    const __nv_bfloat16* Q;
     __nv_bfloat16* out;
     float* lse;
     long long L, w0, G;
     int H_q, H_kv, g;
-    int bifocal;
+    int bifocal, precise;
     const float2* lo;
     const float2* hi;
 };
@@ -79,197 +95,262 @@ struct Plan {
     }
 };
 
-// ---- step a4 / a5: in-place correction rotation of a [128 rows][128 ch] SWIZZLE_128B tile, bf16 -> fp16 ----
-// Row r of the tile sits at absolute position pos0 + r.  Thread t of the 128-thread rotate group owns the
-// 16-byte chunk c = t & 7 (channels 8c..8c+7 of box 0 and their partners 64+8c.. of box 1) of rows 8(t>>3)+m.
-__device__ __forceinline__ void rotate_tile(unsigned char* tile, long long pos0, long long G,
-                                            const float2* __restrict__ lo, const float2* __restrict__ hi, int t) {
-    const int c = t & 7;
-#pragma unroll 2
-    for (int m = 0; m < 8; ++m) {
-        const int r = 8 * (t >> 3) + m;
-        const long long pos = pos0 + r;
-        const long long n = pos - pos / G;                              // -Delta(pos) >= 0, Eq.(5)
-        const float4* ph = reinterpret_cast<const float4*>(hi + (n >> 8) * 64 + 8 * c);
-        const float4* pl = reinterpret_cast<const float4*>(lo + (n & 255) * 64 + 8 * c);
-        float cs_c[8], cs_s[8];
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            const float4 h = __ldg(ph + j), l = __ldg(pl + j);
-            cs_c[2 * j] = h.x * l.x - h.y * l.y;      cs_s[2 * j] = h.y * l.x + h.x * l.y;
-            cs_c[2 * j + 1] = h.z * l.z - h.w * l.w;  cs_s[2 * j + 1] = h.w * l.z + h.z * l.w;
-        }
-        unsigned char* p1 = tile + r * 128 + ((c ^ (r & 7)) << 4);
-        unsigned char* p2 = p1 + BOX_BYTES;
-        const uint4 u1 = *reinterpret_cast<const uint4*>(p1);
-        const uint4 u2 = *reinterpret_cast<const uint4*>(p2);
-        const uint32_t a[4] = {u1.x, u1.y, u1.z, u1.w}, b[4] = {u2.x, u2.y, u2.z, u2.w};
-        uint32_t o1[4], o2[4];
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            const float x1l = __uint_as_float(a[j] << 16), x1h = __uint_as_float(a[j] & 0xffff0000u);
-            const float x2l = __uint_as_float(b[j] << 16), x2h = __uint_as_float(b[j] & 0xffff0000u);
-            const float y1l = x1l * cs_c[2 * j] - x2l * cs_s[2 * j];
-            const float y2l = x1l * cs_s[2 * j] + x2l * cs_c[2 * j];
-            const float y1h = x1h * cs_c[2 * j + 1] - x2h * cs_s[2 * j + 1];
-            const float y2h = x1h * cs_s[2 * j + 1] + x2h * cs_c[2 * j + 1];
-            __half2 h1 = __floats2half2_rn(y1l, y1h), h2 = __floats2half2_rn(y2l, y2h);
-            o1[j] = *reinterpret_cast<uint32_t*>(&h1);
-            o2[j] = *reinterpret_cast<uint32_t*>(&h2);
-        }
-        *reinterpret_cast<uint4*>(p1) = make_uint4(o1[0], o1[1], o1[2], o1[3]);
-        *reinterpret_cast<uint4*>(p2) = make_uint4(o2[0], o2[1], o2[2], o2[3]);
-    }
-}
-
 __device__ __forceinline__ float ex2(float x) {
     float y;
     asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
 }
 
-constexpr uint32_t IDESC_QK_BF16 = idesc_f16(1, 1, 0, 0, BM, BN);
-constexpr uint32_t IDESC_QK_F16 = idesc_f16(0, 0, 0, 0, BM, BN);
-constexpr uint32_t IDESC_PV = idesc_f16(1, 1, 0, 1, BM, D);      // A = P (TMEM, bf16), B = V (smem, MN-major)
+// (cos, sin)(Delta(pos) theta_i) for 8 consecutive frequencies i = i0 .. i0+7 from the two-level table
+// (HI[n >> 8] * LO[n & 255] as complex numbers, n = -Delta(pos) >= 0, Eq.(5))
+__device__ __forceinline__ void cs8(const float2* __restrict__ lo, const float2* __restrict__ hi, long long pos,
+                                    long long G, int i0, float* cs_c, float* cs_s) {
+    const long long n = pos - pos / G;
+    const float4* ph = reinterpret_cast<const float4*>(hi + (n >> 8) * 64 + i0);
+    const float4* pl = reinterpret_cast<const float4*>(lo + (n & 255) * 64 + i0);
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const float4 h = __ldg(ph + j), l = __ldg(pl + j);
+        cs_c[2 * j] = h.x * l.x - h.y * l.y;      cs_s[2 * j] = h.y * l.x + h.x * l.y;
+        cs_c[2 * j + 1] = h.z * l.z - h.w * l.w;  cs_s[2 * j + 1] = h.w * l.z + h.z * l.w;
+    }
+}
 
-__global__ void __launch_bounds__(NTHREADS, 1)
-prefill_umma_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
-                    const __grid_constant__ CUtensorMap tmV, const Params p) {
+// rotate 8 pairs: a[4] = bf16 words of channels i0..i0+7, b[4] = their partners i0+64..; fp32 rotation, then
+// fp16 hi words (h1, h2) and fp16 lo words (l1, l2) of the residual y - hi.
+__device__ __forceinline__ void rot8(const uint32_t* a, const uint32_t* b, const float* cs_c, const float* cs_s,
+                                     uint32_t* h1, uint32_t* h2, uint32_t* l1, uint32_t* l2) {
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const float x1l = __uint_as_float(a[j] << 16), x1h = __uint_as_float(a[j] & 0xffff0000u);
+        const float x2l = __uint_as_float(b[j] << 16), x2h = __uint_as_float(b[j] & 0xffff0000u);
+        const float y1l = x1l * cs_c[2 * j] - x2l * cs_s[2 * j];
+        const float y2l = x1l * cs_s[2 * j] + x2l * cs_c[2 * j];
+        const float y1h = x1h * cs_c[2 * j + 1] - x2h * cs_s[2 * j + 1];
+        const float y2h = x1h * cs_s[2 * j + 1] + x2h * cs_c[2 * j + 1];
+        const __half2 a1 = __floats2half2_rn(y1l, y1h), a2 = __floats2half2_rn(y2l, y2h);
+        const float2 f1 = __half22float2(a1), f2 = __half22float2(a2);
+        const __half2 r1 = __floats2half2_rn(y1l - f1.x, y1h - f1.y), r2 = __floats2half2_rn(y2l - f2.x, y2h - f2.y);
+        h1[j] = *reinterpret_cast<const uint32_t*>(&a1);
+        h2[j] = *reinterpret_cast<const uint32_t*>(&a2);
+        l1[j] = *reinterpret_cast<const uint32_t*>(&r1);
+        l2[j] = *reinterpret_cast<const uint32_t*>(&r2);
+    }
+}
+
+// ---- step a5: correction rotation of this CTA's 64 keys of a K tile, in shared memory -----------------------
+// kh: [2 boxes][64 rows][128 B] SWIZZLE_128B, bf16 in, fp16 hi out (in place); kl: same layout, fp16 lo out.
+// Row r sits at absolute position pos0 + r.  Thread t of the 128-thread rotate group owns the 16-byte chunk
+// c = t & 7 (channels 8c..8c+7 of box 0 and their partners 64+8c.. of box 1) of rows 4(t>>3)+m, m = 0..3.
+__device__ __forceinline__ void rotate_k_half(unsigned char* kh, unsigned char* kl, long long pos0, long long G,
+                                              const float2* __restrict__ lo, const float2* __restrict__ hi, int t,
+                                              bool precise) {
+    const int c = t & 7;
+#pragma unroll 2
+    for (int m = 0; m < 4; ++m) {
+        const int r = 4 * (t >> 3) + m;
+        float cs_c[8], cs_s[8];
+        cs8(lo, hi, pos0 + r, G, 8 * c, cs_c, cs_s);
+        const int off = r * 128 + ((c ^ (r & 7)) << 4);
+        const uint4 u1 = *reinterpret_cast<const uint4*>(kh + off);
+        const uint4 u2 = *reinterpret_cast<const uint4*>(kh + KBOX + off);
+        const uint32_t a[4] = {u1.x, u1.y, u1.z, u1.w}, b[4] = {u2.x, u2.y, u2.z, u2.w};
+        uint32_t h1[4], h2[4], l1[4], l2[4];
+        rot8(a, b, cs_c, cs_s, h1, h2, l1, l2);
+        *reinterpret_cast<uint4*>(kh + off) = make_uint4(h1[0], h1[1], h1[2], h1[3]);
+        *reinterpret_cast<uint4*>(kh + KBOX + off) = make_uint4(h2[0], h2[1], h2[2], h2[3]);
+        if (precise) {
+            *reinterpret_cast<uint4*>(kl + off) = make_uint4(l1[0], l1[1], l1[2], l1[3]);
+            *reinterpret_cast<uint4*>(kl + KBOX + off) = make_uint4(l2[0], l2[1], l2[2], l2[3]);
+        }
+    }
+}
+
+// ---- Q staging (step a4): thread = one query row; TMEM column c of Qa/Qb holds channels (2c, 2c+1) ------------
+__device__ __forceinline__ void stage_q_raw(const __nv_bfloat16* qrow, bool valid, uint32_t tQa) {
+#pragma unroll
+    for (int j = 0; j < 16; ++j) {
+        uint4 u = make_uint4(0, 0, 0, 0);
+        if (valid) u = __ldg(reinterpret_cast<const uint4*>(qrow) + j);
+        tmem_st4(tQa + 4 * j, u.x, u.y, u.z, u.w);
+    }
+}
+__device__ __forceinline__ void stage_q_rot(const __nv_bfloat16* qrow, bool valid, long long q, long long G,
+                                            const float2* __restrict__ lo, const float2* __restrict__ hi,
+                                            uint32_t tQa, uint32_t tQb) {
+#pragma unroll 2
+    for (int j = 0; j < 8; ++j) {                         // channels 8j..8j+7 and 64+8j..
+        uint4 u1 = make_uint4(0, 0, 0, 0), u2 = u1;
+        if (valid) {
+            u1 = __ldg(reinterpret_cast<const uint4*>(qrow) + j);
+            u2 = __ldg(reinterpret_cast<const uint4*>(qrow) + 8 + j);
+        }
+        float cs_c[8], cs_s[8];
+        cs8(lo, hi, q, G, 8 * j, cs_c, cs_s);
+        const uint32_t a[4] = {u1.x, u1.y, u1.z, u1.w}, b[4] = {u2.x, u2.y, u2.z, u2.w};
+        uint32_t h1[4], h2[4], l1[4], l2[4];
+        rot8(a, b, cs_c, cs_s, h1, h2, l1, l2);
+        tmem_st4(tQa + 4 * j, h1[0], h1[1], h1[2], h1[3]);
+        tmem_st4(tQa + 32 + 4 * j, h2[0], h2[1], h2[2], h2[3]);
+        tmem_st4(tQb + 4 * j, l1[0], l1[1], l1[2], l1[3]);
+        tmem_st4(tQb + 32 + 4 * j, l2[0], l2[1], l2[2], l2[3]);
+    }
+}
+
+constexpr uint32_t IDESC_QK_BF16 = idesc_f16(1, 1, 0, 0, 2 * BM, BN);
+constexpr uint32_t IDESC_QK_F16 = idesc_f16(0, 0, 0, 0, 2 * BM, BN);
+constexpr uint32_t IDESC_PV = idesc_f16(1, 1, 0, 1, 2 * BM, D);  // A = P (TMEM, bf16), B = V (smem, MN-major)
+
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1)
+prefill_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV, const Params p) {
     extern __shared__ unsigned char smem_raw[];
     unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-    unsigned char* sQ = smem;
-    unsigned char* sK = sQ + 2 * TILE_BYTES;
-    unsigned char* sV = sK + KS * TILE_BYTES;
-    Bars* bars = reinterpret_cast<Bars*>(sV + VS * TILE_BYTES);
+    Bars* bars = reinterpret_cast<Bars*>(smem + NS * STAGE_BYTES);
+    auto sK = [&](int s) { return smem + s * STAGE_BYTES; };
+    auto sKl = [&](int s) { return smem + s * STAGE_BYTES + KH_BYTES; };
+    auto sV = [&](int s) { return smem + s * STAGE_BYTES + 2 * KH_BYTES; };
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int cta = (int)cluster_ctarank();
+    const int pair = (int)(blockIdx.x >> 1);
     const int n_qb = (int)((p.L + BM - 1) / BM);
     const int pairs = p.H_q / 2;
-    const int qb = n_qb - 1 - (int)(blockIdx.x / pairs);          // heaviest row blocks first
-    const int h0 = 2 * (int)(blockIdx.x % pairs);
+    const int qb = n_qb - 1 - pair / pairs;                       // heaviest row blocks first
+    const int h0 = 2 * (pair % pairs);
+    const int head = h0 + cta;
     const int kvh = h0 / p.g;
     const long long q0 = (long long)qb * BM;
     const bool bifocal = p.bifocal != 0;
+    const bool precise = p.precise != 0;
     const Plan plan(qb, p.w0, bifocal);
 
     if (tid == 0) {
-        mbar_init(&bars->q_full, 1); mbar_init(&bars->q_local_done, 1); mbar_init(&bars->q_rot_done, 128);
-        mbar_init(&bars->o_full, 1);
-        for (int i = 0; i < KS; ++i) { mbar_init(&bars->k_full[i], 1); mbar_init(&bars->k_ready[i], 128); mbar_init(&bars->k_empty[i], 1); }
-        for (int i = 0; i < VS; ++i) { mbar_init(&bars->v_full[i], 1); mbar_init(&bars->v_empty[i], 1); }
-        for (int i = 0; i < 2; ++i) { mbar_init(&bars->s_full[i], 1); mbar_init(&bars->p_full[i], 128); }
+        for (int i = 0; i < NS; ++i) { mbar_init(&bars->kv_full[i], 1); mbar_init(&bars->kv_ready[i], 8); mbar_init(&bars->kv_empty[i], 1); }
+        for (int i = 0; i < 2; ++i) { mbar_init(&bars->s_full[i], 1); mbar_init(&bars->p_full[i], 8); }
+        mbar_init(&bars->pv_done, 1); mbar_init(&bars->o_full, 1); mbar_init(&bars->q_ready, 8);
+        mbar_init(&bars->q_local_done, 1); mbar_init(&bars->q_rot_done, 8);
         fence_barrier_init();
-        prefetch_tmap(&tmQ); prefetch_tmap(&tmK); prefetch_tmap(&tmV);
+        prefetch_tmap(&tmK); prefetch_tmap(&tmV);
     }
-    if (warp == 1) tmem_alloc<512>(&bars->tmem_base);
+    if (warp == 1) tmem_alloc2<512>(&bars->tmem_base);
     tc_fence_before();
-    __syncthreads();
+    cluster_sync_all();                                            // barriers of both CTAs initialised, TMEM allocated
     tc_fence_after();
     const uint32_t tmem = bars->tmem_base;
 
     if (warp == 0) {
-        // ===================== TMA producer =====================
+        // ===================== TMA producer (each CTA loads its halves) =====================
         if (lane == 0) {
-            mbar_arrive_expect_tx(&bars->q_full, 2 * TILE_BYTES);
-            for (int t = 0; t < 2; ++t)
-                for (int b = 0; b < 2; ++b)
-                    tma_load_3d(sQ + t * TILE_BYTES + b * BOX_BYTES, &tmQ, &bars->q_full, 64 * b, h0 + t, (int)q0);
             for (int v = 0; v < plan.nv; ++v) {
                 const Visit x = plan.at(v, bifocal);
-                const int s = v % KS, sv = v % VS;
-                if (v >= KS) mbar_wait(&bars->k_empty[s], ((v / KS) - 1) & 1);
-                mbar_arrive_expect_tx(&bars->k_full[s], TILE_BYTES);
-                for (int b = 0; b < 2; ++b)
-                    tma_load_3d(sK + s * TILE_BYTES + b * BOX_BYTES, &tmK, &bars->k_full[s], 64 * b, kvh, x.kt * BN);
-                if (v >= VS) mbar_wait(&bars->v_empty[sv], ((v / VS) - 1) & 1);
-                mbar_arrive_expect_tx(&bars->v_full[sv], TILE_BYTES);
-                for (int b = 0; b < 2; ++b)
-                    tma_load_3d(sV + sv * TILE_BYTES + b * BOX_BYTES, &tmV, &bars->v_full[sv], 64 * b, kvh, x.kt * BN);
+                const int s = v % NS;
+                if (v >= NS) mbar_wait(&bars->kv_empty[s], ((v / NS) - 1) & 1);
+                mbar_arrive_expect_tx(&bars->kv_full[s], KH_BYTES + VH_BYTES);
+                tma_load_3d(sK(s), &tmK, &bars->kv_full[s], 0, kvh, x.kt * BN + 64 * cta);
+                tma_load_3d(sK(s) + KBOX, &tmK, &bars->kv_full[s], 64, kvh, x.kt * BN + 64 * cta);
+                tma_load_3d(sV(s), &tmV, &bars->kv_full[s], 64 * cta, kvh, x.kt * BN);
             }
         }
     } else if (warp == 1) {
-        // ===================== MMA issuer (one thread) =====================
-        if (lane == 0) {
-            auto issue_qk = [&](int v, int t) {
+        // ===================== MMA issuer (one thread of the leader CTA) =====================
+        if (cta == 0 && lane == 0) {
+            auto issue_qk = [&](int v) {
                 const Visit x = plan.at(v, bifocal);
-                const uint32_t idesc = x.mode == 2 ? IDESC_QK_F16 : IDESC_QK_BF16;
-                const uint32_t a0 = smem_u32(sQ + t * TILE_BYTES), b0 = smem_u32(sK + (v % KS) * TILE_BYTES);
+                const uint32_t dS = tmem + TM_S + (v & 1) * 128;
+                const uint32_t kb = smem_u32(sK(v % NS)), klb = kb + KH_BYTES;
+                if (x.mode != 2) {
 #pragma unroll
-                for (int ks = 0; ks < D / 16; ++ks) {
-                    const uint32_t off = (ks >> 2) * BOX_BYTES + (ks & 3) * 32;
-                    umma_ss(tmem + t * 128, smem_desc_sw128(a0 + off, 16, 1024), smem_desc_sw128(b0 + off, 16, 1024),
-                            idesc, ks > 0);
-                }
-                umma_commit(&bars->s_full[t]);
-            };
-            auto issue_pv = [&](int v, int t) {
-                const uint32_t b0 = smem_u32(sV + (v % VS) * TILE_BYTES);
+                    for (int ks = 0; ks < D / 16; ++ks)
+                        umma2_ts(dS, tmem + TM_QA + ks * 8,
+                                 smem_desc_sw128(kb + (ks >> 2) * KBOX + (ks & 3) * 32, 16, 1024), IDESC_QK_BF16, ks > 0);
+                } else {
 #pragma unroll
-                for (int ks = 0; ks < BN / 16; ++ks)
-                    umma_ts(tmem + 256 + t * 128, tmem + t * 128 + ks * 8,
-                            smem_desc_sw128(b0 + ks * 2048, BOX_BYTES, 1024), IDESC_PV, (v > 0 || ks > 0) ? 1u : 0u);
-            };
-            mbar_wait(&bars->q_full, 0);
-            mbar_wait(&bars->k_ready[0], 0);
-            tc_fence_after();
-            issue_qk(0, 0);
-            issue_qk(0, 1);
-            umma_commit(&bars->k_empty[0]);
-            if (plan.n_remote > 0 && plan.n_local == 1) umma_commit(&bars->q_local_done);
-            for (int v = 0; v < plan.nv; ++v) {
-                const int sv = v % VS;
-                for (int t = 0; t < 2; ++t) {
-                    mbar_wait(&bars->p_full[t], v & 1);
-                    if (t == 0) mbar_wait(&bars->v_full[sv], (v / VS) & 1);
-                    tc_fence_after();
-                    issue_pv(v, t);
-                    if (t == 1) umma_commit(&bars->v_empty[sv]);
-                    if (v + 1 < plan.nv) {
-                        if (t == 0) {
-                            if (v + 1 == plan.n_local) mbar_wait(&bars->q_rot_done, 0);
-                            mbar_wait(&bars->k_ready[(v + 1) % KS], ((v + 1) / KS) & 1);
-                            tc_fence_after();
-                        }
-                        issue_qk(v + 1, t);
-                        if (t == 1) {
-                            umma_commit(&bars->k_empty[(v + 1) % KS]);
-                            if (plan.n_remote > 0 && v + 1 == plan.n_local - 1) umma_commit(&bars->q_local_done);
-                        }
+                    for (int ks = 0; ks < D / 16; ++ks)
+                        umma2_ts(dS, tmem + TM_QA + ks * 8,
+                                 smem_desc_sw128(kb + (ks >> 2) * KBOX + (ks & 3) * 32, 16, 1024), IDESC_QK_F16, ks > 0);
+                    if (precise) {
+#pragma unroll
+                        for (int ks = 0; ks < D / 16; ++ks)
+                            umma2_ts(dS, tmem + TM_QA + ks * 8,
+                                     smem_desc_sw128(klb + (ks >> 2) * KBOX + (ks & 3) * 32, 16, 1024), IDESC_QK_F16, 1);
+#pragma unroll
+                        for (int ks = 0; ks < D / 16; ++ks)
+                            umma2_ts(dS, tmem + TM_QB + ks * 8,
+                                     smem_desc_sw128(kb + (ks >> 2) * KBOX + (ks & 3) * 32, 16, 1024), IDESC_QK_F16, 1);
                     }
                 }
+                umma2_commit(&bars->s_full[v & 1]);
+                if (plan.n_remote > 0 && v == plan.n_local - 1) umma2_commit(&bars->q_local_done);
+            };
+            auto issue_pv = [&](int v) {
+                const uint32_t vb = smem_u32(sV(v % NS));
+#pragma unroll
+                for (int ks = 0; ks < BN / 16; ++ks)
+                    umma2_ts(tmem + TM_O, tmem + TM_S + (v & 1) * 128 + ks * 8,
+                             smem_desc_sw128(vb + ks * 2048, VH_BYTES, 1024), IDESC_PV, (v > 0 || ks > 0) ? 1u : 0u);
+                umma2_commit(&bars->kv_empty[v % NS]);
+                umma2_commit(&bars->pv_done);
+            };
+            mbar_wait_cluster(&bars->q_ready, 0);
+            mbar_wait_cluster(&bars->kv_ready[0], 0);
+            tc_fence_after();
+            issue_qk(0);
+            for (int v = 0; v < plan.nv; ++v) {
+                if (v + 1 < plan.nv) {
+                    if (plan.n_remote > 0 && v + 1 == plan.n_local) mbar_wait_cluster(&bars->q_rot_done, 0);
+                    mbar_wait_cluster(&bars->kv_ready[(v + 1) % NS], ((v + 1) / NS) & 1);
+                    tc_fence_after();
+                    issue_qk(v + 1);
+                }
+                mbar_wait_cluster(&bars->p_full[v & 1], (v >> 1) & 1);
+                tc_fence_after();
+                issue_pv(v);
             }
-            umma_commit(&bars->o_full);
+            umma2_commit(&bars->o_full);
         }
     } else if (warp >= 4 && warp < 8) {
         // ===================== rotate group (steps a4, a5) =====================
         const int t = tid - 128;
+        const uint32_t lane_base = (uint32_t)((warp & 3) << 5) << 16;
+        const long long q = q0 + t;
+        const bool valid = q < p.L;
+        const __nv_bfloat16* qrow = p.Q + ((size_t)(valid ? q : 0) * p.H_q + head) * D;
+        stage_q_raw(qrow, valid, tmem + lane_base + TM_QA);
+        tmem_st_wait();
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive_leader(&bars->q_ready);
         for (int v = 0; v < plan.nv; ++v) {
             const Visit x = plan.at(v, bifocal);
-            const int s = v % KS;
-            mbar_wait(&bars->k_full[s], (v / KS) & 1);
+            const int s = v % NS;
+            mbar_wait(&bars->kv_full[s], (v / NS) & 1);
             if (x.mode == 2) {
                 if (v == plan.n_local) {                              // first remote visit: Q -> Q' = R(Delta q) Q
                     mbar_wait(&bars->q_local_done, 0);
-                    rotate_tile(sQ, q0, p.G, p.lo, p.hi, t);
-                    rotate_tile(sQ + TILE_BYTES, q0, p.G, p.lo, p.hi, t);
-                    fence_proxy_async_smem();
-                    mbar_arrive(&bars->q_rot_done);
+                    tc_fence_after();
+                    stage_q_rot(qrow, valid, q, p.G, p.lo, p.hi, tmem + lane_base + TM_QA, tmem + lane_base + TM_QB);
+                    tmem_st_wait();
+                    tc_fence_before();
                 }
-                rotate_tile(sK + s * TILE_BYTES, (long long)x.kt * BN, p.G, p.lo, p.hi, t);
+                rotate_k_half(sK(s), sKl(s), (long long)x.kt * BN + 64 * cta, p.G, p.lo, p.hi, t, precise);
                 fence_proxy_async_smem();
             }
-            mbar_arrive(&bars->k_ready[s]);
+            __syncwarp();
+            if (lane == 0) {
+                if (x.mode == 2 && v == plan.n_local) mbar_arrive_leader(&bars->q_rot_done);
+                mbar_arrive_leader(&bars->kv_ready[s]);
+            }
         }
     } else if (warp >= 8) {
-        // ===================== softmax groups (steps a6-a8): one thread per query row =====================
-        const int t = (warp - 8) >> 2;
+        // ===================== softmax group (steps a6-a8): one thread per query row =====================
         const int r = ((warp & 3) << 5) | lane;
         const uint32_t lane_base = (uint32_t)((warp & 3) << 5) << 16;
-        const uint32_t tS = tmem + lane_base + t * 128, tO = tmem + lane_base + 256 + t * 128;
+        const uint32_t tO = tmem + lane_base + TM_O;
         const float sl2 = (1.0f / sqrtf((float)D)) * kLog2e;
         float m_ref = -INFINITY, l = 0.f;
         for (int v = 0; v < plan.nv; ++v) {
             const Visit x = plan.at(v, bifocal);
+            const uint32_t tS = tmem + lane_base + TM_S + (v & 1) * 128;
             const long long k0 = (long long)x.kt * BN;
             const long long qrel = q0 + r - k0;
             int lo = 0, hi = BN - 1;
@@ -285,7 +366,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_consta
                 hi = a < hi ? (int)a : hi;
                 masked = true;
             }
-            mbar_wait(&bars->s_full[t], v & 1);
+            mbar_wait(&bars->s_full[v & 1], (v >> 1) & 1);
             tc_fence_after();
             uint32_t rg[32];
             float mx = -INFINITY;
@@ -310,6 +391,8 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_consta
             } else {
                 const bool need = mnew > m_ref + 8.0f;                 // lazy rescale: only on a jump of 2^8
                 if (__any_sync(0xffffffffu, need)) {
+                    mbar_wait(&bars->pv_done, (v - 1) & 1);            // O += P V of visit v-1 must have landed
+                    tc_fence_after();
                     const float alpha = need ? ex2(m_ref - mnew) : 1.0f;
                     if (need) m_ref = mnew;
                     l *= alpha;
@@ -347,14 +430,15 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_consta
             l += sum;
             tmem_st_wait();
             tc_fence_before();
-            mbar_arrive(&bars->p_full[t]);
+            __syncwarp();
+            if (lane == 0) mbar_arrive_leader(&bars->p_full[v & 1]);
         }
         // ---- epilogue (step a8) ----
         mbar_wait(&bars->o_full, 0);
         tc_fence_after();
         const long long q = q0 + r;
         const float inv = 1.0f / l;
-        __nv_bfloat16* orow = p.out + ((size_t)q * p.H_q + (h0 + t)) * D;
+        __nv_bfloat16* orow = p.out + ((size_t)(q < p.L ? q : 0) * p.H_q + head) * D;
 #pragma unroll
         for (int ch = 0; ch < 4; ++ch) {
             uint32_t rg[32];
@@ -374,11 +458,11 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_consta
                 }
             }
         }
-        if (q < p.L) p.lse[(size_t)(h0 + t) * p.L + q] = (m_ref + log2f(l)) * 0.6931471805599453f;
+        if (q < p.L) p.lse[(size_t)head * p.L + q] = (m_ref + log2f(l)) * 0.6931471805599453f;
     }
     tc_fence_before();
-    __syncthreads();
-    if (warp == 1) tmem_dealloc<512>(tmem);
+    cluster_sync_all();                                            // the peer may still be reading our smem / TMEM
+    if (warp == 1) tmem_dealloc2<512>(tmem);
 }
 
 // ---- host side ------------------------------------------------------------------------------------------
@@ -398,13 +482,13 @@ EncodeTiledFn encode_fn() {
     return fn;
 }
 
-// [L, H, 128] bf16 tensor seen as (d, H, L); box = 64 channels x 1 head x 128 rows, SWIZZLE_128B, OOB rows -> 0
-bool make_map(CUtensorMap* m, const void* base, long long L, int H) {
+// [L, H, 128] bf16 tensor seen as (d, H, L); box = 64 channels x 1 head x `rows` rows, SWIZZLE_128B, OOB rows -> 0
+bool make_map(CUtensorMap* m, const void* base, long long L, int H, int rows) {
     EncodeTiledFn fn = encode_fn();
     if (!fn) return false;
     cuuint64_t dims[3] = {(cuuint64_t)D, (cuuint64_t)H, (cuuint64_t)L};
     cuuint64_t strides[2] = {(cuuint64_t)D * 2, (cuuint64_t)H * D * 2};
-    cuuint32_t box[3] = {64, 1, 128};
+    cuuint32_t box[3] = {64, 1, (cuuint32_t)rows};
     cuuint32_t es[3] = {1, 1, 1};
     return fn(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(base), dims, strides, box, es,
               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
@@ -422,18 +506,19 @@ bool umma_prefill_supported(long long L, int H_q, int H_kv, int d, int dtype) {
 size_t umma_prefill_workspace_bytes(long long L, int, int, int d) { return two_level_bytes(L + 256, d); }
 
 int launch_prefill_umma(const void* Q, const void* K, const void* V, void* out, float* lse, long long L, int H_q,
-                        int H_kv, int d, long long w0, long long G, double theta, bool bifocal, void* ws,
+                        int H_kv, int d, long long w0, long long G, double theta, bool bifocal, bool precise, void* ws,
                         size_t ws_bytes, cudaStream_t st) {
     (void)ws_bytes;
-    CUtensorMap tmQ, tmK, tmV;
-    if (!make_map(&tmQ, Q, L, H_q) || !make_map(&tmK, K, L, H_kv) || !make_map(&tmV, V, L, H_kv))
-        return JETLONG_UNSUPPORTED;
+    CUtensorMap tmK, tmV;
+    if (!make_map(&tmK, K, L, H_kv, 64) || !make_map(&tmV, V, L, H_kv, 128)) return JETLONG_UNSUPPORTED;
     Params p;
+    p.Q = (const __nv_bfloat16*)Q;
     p.out = (__nv_bfloat16*)out;
     p.lse = lse;
     p.L = L; p.w0 = w0; p.G = G;
     p.H_q = H_q; p.H_kv = H_kv; p.g = H_q / H_kv;
     p.bifocal = bifocal ? 1 : 0;
+    p.precise = precise ? 1 : 0;
     p.lo = nullptr; p.hi = nullptr;
     if (bifocal) {
         int rc = build_two_level(ws, L + 256, d, theta, st);
@@ -449,8 +534,8 @@ int launch_prefill_umma(const void* Q, const void* K, const void* V, void* out, 
         attr_set = true;
     }
     const int n_qb = (int)((L + BM - 1) / BM);
-    const unsigned grid = (unsigned)n_qb * (unsigned)(H_q / 2);
-    prefill_umma_kernel<<<grid, NTHREADS, SMEM_BYTES, st>>>(tmQ, tmK, tmV, p);
+    const unsigned grid = 2u * (unsigned)n_qb * (unsigned)(H_q / 2);
+    prefill_umma_kernel<<<grid, NTHREADS, SMEM_BYTES, st>>>(tmK, tmV, p);
     note_launch();
     return check_launch("prefill_umma_kernel");
 }
