@@ -4,13 +4,14 @@
 // heads see the same keys, the same positions and therefore the same tile classification.  Every UMMA is
 // M = 256 across the pair (CTA c owns head h0 + c), so each CTA stages and -- on remote visits -- rotates only
 // HALF of every K tile (its 64 keys) and loads half of every V tile (its 64 channels).
-// Warp roles (384 threads per CTA):
+// Warp roles (448 threads per CTA; ptxas caps >384 threads at 128 registers, the kernel uses 124, no spills):
 //   warp 0      TMA producer: its half of K and V per visit, SWIZZLE_128B boxes, NS-stage ring
 //   warp 1      MMA issuer (leader CTA only, one thread): S_b = Q K^T (A = Q from TMEM), O += P V (A = P from TMEM)
-//   warps 4-7   rotate group: stages Q into TMEM; on remote visits rotates its K half in shared memory between
+//   warps 2-5   rotate group: stages Q into TMEM; on remote visits rotates its K half in shared memory between
 //               the TMA load and the MMA (Eq.(6): bf16 -> fp32 rotate -> fp16 hi (+ fp16 lo)); once per CTA
 //               it replaces Q in TMEM by Q' = R(Delta q) Q (hi, lo)
-//   warps 8-11  softmax group: one thread per query row, online softmax over the visits, epilogue
+//   warps 6-13  softmax groups: two threads per query row (64 keys of the tile each, S kept in registers, row max
+//               combined through shared memory), online softmax over the visits, epilogue
 // TMEM (512 columns): S0 | S1 | O | Qa | Qb  (128, 128, 128, 64, 64).  P (bf16) aliases columns 0..63 of its S.
 // S is double-buffered over consecutive visits so QK^T of visit v+1 overlaps the softmax of visit v.
 //
@@ -40,7 +41,7 @@ constexpr int KH_BYTES = 64 * D * 2;                  // this CTA's 64 keys: two
 constexpr int KBOX = 64 * 128;                        // one K box: 64 rows x 128 B
 constexpr int VH_BYTES = BN * 64 * 2;                 // this CTA's 64 channels of 128 keys: one 16 KB box
 constexpr int STAGE_BYTES = 2 * KH_BYTES + VH_BYTES;  // K (hi in place) | K lo | V
-constexpr int NTHREADS = 384;
+constexpr int NTHREADS = 448;
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr uint32_t TM_S = 0, TM_O = 256, TM_QA = 384, TM_QB = 448;
 
@@ -56,9 +57,10 @@ struct Bars {
     uint64_t q_local_done;     // both: the last local Q K^T has completed, Qa may be overwritten
     uint64_t q_rot_done;       // leader: Q' (hi, lo) staged in TMEM
     uint32_t tmem_base;
+    float xchg[4 * BM];        // row-max / row-sum exchange between the two column halves of a row
 };
 
-constexpr size_t SMEM_BYTES = 1024 /*align slack*/ + (size_t)NS * STAGE_BYTES + 1024 /*Bars*/;
+constexpr size_t SMEM_BYTES = 1024 /*align slack*/ + (size_t)NS * STAGE_BYTES + 4096 /*Bars*/;
 
 struct Params {
     const __nv_bfloat16* Q;
@@ -99,6 +101,46 @@ __device__ __forceinline__ float ex2(float x) {
     float y;
     asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
+}
+
+__device__ __forceinline__ float max3(float a, float b, float c) {
+    float y;
+    asm("max.f32 %0, %1, %2, %3;" : "=f"(y) : "f"(a), "f"(b), "f"(c));
+    return y;
+}
+// packed fp32x2 arithmetic (FFMA2 / FADD2 / FMUL2 on sm_100)
+__device__ __forceinline__ uint64_t pack2(float lo, float hi) {
+    uint64_t y;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(y) : "f"(lo), "f"(hi));
+    return y;
+}
+__device__ __forceinline__ void unpack2(uint64_t v, float& lo, float& hi) {
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ uint64_t ffma2(uint64_t a, uint64_t b, uint64_t c) {
+    uint64_t y;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(y) : "l"(a), "l"(b), "l"(c));
+    return y;
+}
+__device__ __forceinline__ uint64_t fadd2(uint64_t a, uint64_t b) {
+    uint64_t y;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(y) : "l"(a), "l"(b));
+    return y;
+}
+__device__ __forceinline__ uint64_t fmul2(uint64_t a, uint64_t b) {
+    uint64_t y;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(y) : "l"(a), "l"(b));
+    return y;
+}
+__device__ __forceinline__ uint32_t bf16x2(float lo, float hi) {
+    uint32_t y;
+    asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(y) : "f"(hi), "f"(lo));
+    return y;
+}
+template <int N> __device__ __forceinline__ void reg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
+template <int N> __device__ __forceinline__ void reg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
+__device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
 
 // (cos, sin)(Delta(pos) theta_i) for 8 consecutive frequencies i = i0 .. i0+7 from the two-level table
@@ -226,7 +268,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_consta
 
     if (tid == 0) {
         for (int i = 0; i < NS; ++i) { mbar_init(&bars->kv_full[i], 1); mbar_init(&bars->kv_ready[i], 8); mbar_init(&bars->kv_empty[i], 1); }
-        for (int i = 0; i < 2; ++i) { mbar_init(&bars->s_full[i], 1); mbar_init(&bars->p_full[i], 8); }
+        for (int i = 0; i < 2; ++i) { mbar_init(&bars->s_full[i], 1); mbar_init(&bars->p_full[i], 16); }
         mbar_init(&bars->pv_done, 1); mbar_init(&bars->o_full, 1); mbar_init(&bars->q_ready, 8);
         mbar_init(&bars->q_local_done, 1); mbar_init(&bars->q_rot_done, 8);
         fence_barrier_init();
@@ -237,6 +279,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_consta
     cluster_sync_all();                                            // barriers of both CTAs initialised, TMEM allocated
     tc_fence_after();
     const uint32_t tmem = bars->tmem_base;
+    float* xchg = bars->xchg;
 
     if (warp == 0) {
         // ===================== TMA producer (each CTA loads its halves) =====================
@@ -291,28 +334,28 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_consta
                 umma2_commit(&bars->kv_empty[v % NS]);
                 umma2_commit(&bars->pv_done);
             };
-            mbar_wait_cluster(&bars->q_ready, 0);
-            mbar_wait_cluster(&bars->kv_ready[0], 0);
+            mbar_wait(&bars->q_ready, 0);
+            mbar_wait(&bars->kv_ready[0], 0);
             tc_fence_after();
             issue_qk(0);
             for (int v = 0; v < plan.nv; ++v) {
                 if (v + 1 < plan.nv) {
-                    if (plan.n_remote > 0 && v + 1 == plan.n_local) mbar_wait_cluster(&bars->q_rot_done, 0);
-                    mbar_wait_cluster(&bars->kv_ready[(v + 1) % NS], ((v + 1) / NS) & 1);
+                    if (plan.n_remote > 0 && v + 1 == plan.n_local) mbar_wait(&bars->q_rot_done, 0);
+                    mbar_wait(&bars->kv_ready[(v + 1) % NS], ((v + 1) / NS) & 1);
                     tc_fence_after();
                     issue_qk(v + 1);
                 }
-                mbar_wait_cluster(&bars->p_full[v & 1], (v >> 1) & 1);
+                mbar_wait(&bars->p_full[v & 1], (v >> 1) & 1);
                 tc_fence_after();
                 issue_pv(v);
             }
             umma2_commit(&bars->o_full);
         }
-    } else if (warp >= 4 && warp < 8) {
+    } else if (warp >= 2 && warp < 6) {
         // ===================== rotate group (steps a4, a5) =====================
-        const int t = tid - 128;
-        const uint32_t lane_base = (uint32_t)((warp & 3) << 5) << 16;
-        const long long q = q0 + t;
+        const int t = tid - 64;                                       // work index for the K rotation
+        const uint32_t lane_base = (uint32_t)((warp & 3) << 5) << 16; // TMEM lanes a warp may touch: 32 (warp % 4) ..
+        const long long q = q0 + (((warp & 3) << 5) | lane);
         const bool valid = q < p.L;
         const __nv_bfloat16* qrow = p.Q + ((size_t)(valid ? q : 0) * p.H_q + head) * D;
         stage_q_raw(qrow, valid, tmem + lane_base + TM_QA);
@@ -341,13 +384,19 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_consta
                 mbar_arrive_leader(&bars->kv_ready[s]);
             }
         }
-    } else if (warp >= 8) {
-        // ===================== softmax group (steps a6-a8): one thread per query row =====================
-        const int r = ((warp & 3) << 5) | lane;
-        const uint32_t lane_base = (uint32_t)((warp & 3) << 5) << 16;
-        const uint32_t tO = tmem + lane_base + TM_O;
+    } else if (warp >= 6) {
+        // ===================== softmax groups (steps a6-a8) =====================
+        // Two threads per query row: warps w and w+4 hold the same 32 rows, column half `half` (64 keys) each.
+        // The S values are loaded ONCE into registers; the row max is combined through shared memory.
+        const int half = (warp - 6) >> 2;
+        const int quad = warp & 3;
+        const int r = (quad << 5) | lane;
+        const uint32_t lane_base = (uint32_t)(quad << 5) << 16;
+        const uint32_t tO = tmem + lane_base + TM_O + 64 * half;
         const float sl2 = (1.0f / sqrtf((float)D)) * kLog2e;
-        float m_ref = -INFINITY, l = 0.f;
+        const uint64_t sl2x2 = pack2(sl2, sl2);
+        float m_ref = -INFINITY;
+        uint64_t l2a = 0, l2b = 0;                                     // packed fp32x2 partial row sums
         for (int v = 0; v < plan.nv; ++v) {
             const Visit x = plan.at(v, bifocal);
             const uint32_t tS = tmem + lane_base + TM_S + (v & 1) * 128;
@@ -366,25 +415,36 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_consta
                 hi = a < hi ? (int)a : hi;
                 masked = true;
             }
+            lo -= 64 * half; hi -= 64 * half;                          // in this thread's 64 columns
             mbar_wait(&bars->s_full[v & 1], (v >> 1) & 1);
             tc_fence_after();
-            uint32_t rg[32];
-            float mx = -INFINITY;
+            uint32_t sa[32], sb[32];
+            tmem_ld32(tS + 64 * half, sa);
+            tmem_ld32(tS + 64 * half + 32, sb);
+            tmem_ld_wait();
+            if (masked) {
 #pragma unroll
-            for (int ch = 0; ch < 4; ++ch) {
-                tmem_ld32(tS + ch * 32, rg);
-                tmem_ld_wait();
-                if (masked) {
-#pragma unroll
-                    for (int j = 0; j < 32; ++j) {
-                        const int c = ch * 32 + j;
-                        mx = fmaxf(mx, (c >= lo && c <= hi) ? __uint_as_float(rg[j]) : -INFINITY);
-                    }
-                } else {
-#pragma unroll
-                    for (int j = 0; j < 32; ++j) mx = fmaxf(mx, __uint_as_float(rg[j]));
+                for (int j = 0; j < 32; ++j) {
+                    if (j < lo || j > hi) sa[j] = 0xff800000u;         // -inf: exp2 -> 0, never wins the max
+                    if (j + 32 < lo || j + 32 > hi) sb[j] = 0xff800000u;
                 }
             }
+            float mx0 = -INFINITY, mx1 = -INFINITY, mx2 = -INFINITY, mx3 = -INFINITY;
+#pragma unroll
+            for (int j = 0; j < 32; j += 8) {
+                mx0 = max3(mx0, __uint_as_float(sa[j]), __uint_as_float(sa[j + 1]));
+                mx1 = max3(mx1, __uint_as_float(sa[j + 2]), __uint_as_float(sa[j + 3]));
+                mx2 = max3(mx2, __uint_as_float(sa[j + 4]), __uint_as_float(sa[j + 5]));
+                mx3 = max3(mx3, __uint_as_float(sa[j + 6]), __uint_as_float(sa[j + 7]));
+                mx0 = max3(mx0, __uint_as_float(sb[j]), __uint_as_float(sb[j + 1]));
+                mx1 = max3(mx1, __uint_as_float(sb[j + 2]), __uint_as_float(sb[j + 3]));
+                mx2 = max3(mx2, __uint_as_float(sb[j + 4]), __uint_as_float(sb[j + 5]));
+                mx3 = max3(mx3, __uint_as_float(sb[j + 6]), __uint_as_float(sb[j + 7]));
+            }
+            float mx = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3));
+            xchg[((v & 1) * 2 + half) * BM + r] = mx;
+            named_bar_sync(1 + quad, 64);                              // the two warps of this row quadrant
+            mx = fmaxf(mx, xchg[((v & 1) * 2 + (half ^ 1)) * BM + r]);
             const float mnew = mx * sl2;
             if (v == 0) {
                 m_ref = mnew;
@@ -395,52 +455,60 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_consta
                     tc_fence_after();
                     const float alpha = need ? ex2(m_ref - mnew) : 1.0f;
                     if (need) m_ref = mnew;
-                    l *= alpha;
-#pragma unroll
+                    const uint64_t al2 = pack2(alpha, alpha);
+                    l2a = fmul2(l2a, al2); l2b = fmul2(l2b, al2);
+                    uint32_t rg[16];
+#pragma unroll 1
                     for (int ch = 0; ch < 4; ++ch) {
-                        tmem_ld32(tO + ch * 32, rg);
+                        tmem_ld16(tO + ch * 16, rg);
                         tmem_ld_wait();
 #pragma unroll
-                        for (int j = 0; j < 32; ++j) rg[j] = __float_as_uint(__uint_as_float(rg[j]) * alpha);
-                        tmem_st32(tO + ch * 32, rg);
+                        for (int j = 0; j < 16; ++j) rg[j] = __float_as_uint(__uint_as_float(rg[j]) * alpha);
+                        tmem_st16(tO + ch * 16, rg);
                     }
                 }
             }
-            float sum = 0.f;
+            // a row whose every key so far is masked has m_ref = -inf: keep exp2 arguments finite (-> p = 0)
+            const float mneg = (m_ref == -INFINITY) ? 0.f : -m_ref;
+            const uint64_t mneg2 = pack2(mneg, mneg);
+            uint32_t pk[16];
 #pragma unroll
-            for (int ch = 0; ch < 4; ++ch) {
-                tmem_ld32(tS + ch * 32, rg);
-                tmem_ld_wait();
-                uint32_t pk[16];
-#pragma unroll
-                for (int j = 0; j < 32; j += 2) {
-                    const int c = ch * 32 + j;
-                    float a = ex2(fmaf(__uint_as_float(rg[j]), sl2, -m_ref));
-                    float b = ex2(fmaf(__uint_as_float(rg[j + 1]), sl2, -m_ref));
-                    if (masked) {
-                        if (c < lo || c > hi) a = 0.f;
-                        if (c + 1 < lo || c + 1 > hi) b = 0.f;
-                    }
-                    sum += a + b;
-                    __nv_bfloat162 h = __floats2bfloat162_rn(a, b);
-                    pk[j >> 1] = *reinterpret_cast<uint32_t*>(&h);
-                }
-                tmem_st16(tS + ch * 16, pk);
+            for (int j = 0; j < 32; j += 2) {
+                float x0, x1;
+                unpack2(ffma2(pack2(__uint_as_float(sa[j]), __uint_as_float(sa[j + 1])), sl2x2, mneg2), x0, x1);
+                const float p0 = ex2(x0), p1 = ex2(x1);
+                if (j & 2) l2b = fadd2(l2b, pack2(p0, p1)); else l2a = fadd2(l2a, pack2(p0, p1));
+                pk[j >> 1] = bf16x2(p0, p1);
             }
-            l += sum;
+            tmem_st16(tS + 32 * half, pk);
+#pragma unroll
+            for (int j = 0; j < 32; j += 2) {
+                float x0, x1;
+                unpack2(ffma2(pack2(__uint_as_float(sb[j]), __uint_as_float(sb[j + 1])), sl2x2, mneg2), x0, x1);
+                const float p0 = ex2(x0), p1 = ex2(x1);
+                if (j & 2) l2b = fadd2(l2b, pack2(p0, p1)); else l2a = fadd2(l2a, pack2(p0, p1));
+                pk[j >> 1] = bf16x2(p0, p1);
+            }
+            tmem_st16(tS + 32 * half + 16, pk);
             tmem_st_wait();
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive_leader(&bars->p_full[v & 1]);
         }
         // ---- epilogue (step a8) ----
+        float la, lb, lc, ld;
+        unpack2(l2a, la, lb); unpack2(l2b, lc, ld);
+        float l = (la + lb) + (lc + ld);
+        xchg[(2 + half) * BM + r] = l;                                 // slot parity 1 of the last visit's pair is free:
+        named_bar_sync(1 + quad, 64);                                  //   (nv-1)&1 may be 1, so use a dedicated sync
+        l += xchg[(2 + (half ^ 1)) * BM + r];
         mbar_wait(&bars->o_full, 0);
         tc_fence_after();
         const long long q = q0 + r;
         const float inv = 1.0f / l;
-        __nv_bfloat16* orow = p.out + ((size_t)(q < p.L ? q : 0) * p.H_q + head) * D;
+        __nv_bfloat16* orow = p.out + ((size_t)(q < p.L ? q : 0) * p.H_q + head) * D + 64 * half;
 #pragma unroll
-        for (int ch = 0; ch < 4; ++ch) {
+        for (int ch = 0; ch < 2; ++ch) {
             uint32_t rg[32];
             tmem_ld32(tO + ch * 32, rg);
             tmem_ld_wait();
@@ -449,16 +517,13 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_consta
                 for (int j = 0; j < 32; j += 8) {
                     uint32_t w[4];
 #pragma unroll
-                    for (int e = 0; e < 4; ++e) {
-                        __nv_bfloat162 h = __floats2bfloat162_rn(__uint_as_float(rg[j + 2 * e]) * inv,
-                                                                 __uint_as_float(rg[j + 2 * e + 1]) * inv);
-                        w[e] = *reinterpret_cast<uint32_t*>(&h);
-                    }
+                    for (int e = 0; e < 4; ++e)
+                        w[e] = bf16x2(__uint_as_float(rg[j + 2 * e]) * inv, __uint_as_float(rg[j + 2 * e + 1]) * inv);
                     *reinterpret_cast<uint4*>(orow + ch * 32 + j) = make_uint4(w[0], w[1], w[2], w[3]);
                 }
             }
         }
-        if (q < p.L) p.lse[(size_t)head * p.L + q] = (m_ref + log2f(l)) * 0.6931471805599453f;
+        if (half == 0 && q < p.L) p.lse[(size_t)head * p.L + q] = (m_ref + log2f(l)) * 0.6931471805599453f;
     }
     tc_fence_before();
     cluster_sync_all();                                            // the peer may still be reading our smem / TMEM
