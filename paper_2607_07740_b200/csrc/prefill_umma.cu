@@ -182,23 +182,96 @@ __device__ __forceinline__ void rot8(const uint32_t* a, const uint32_t* b, const
 
 // ---- step a5: correction rotation of this CTA's 64 keys of a K tile, in shared memory -----------------------
 // kh: [2 boxes][64 rows][128 B] SWIZZLE_128B, bf16 in, fp16 hi out (in place); kl: same layout, fp16 lo out.
-// Row r sits at absolute position pos0 + r.  Thread t of the 128-thread rotate group owns the 16-byte chunk
-// c = t & 7 (channels 8c..8c+7 of box 0 and their partners 64+8c.. of box 1) of rows 4(t>>3)+m, m = 0..3.
-__device__ __forceinline__ void rotate_k_half(unsigned char* kh, unsigned char* kl, long long pos0, long long G,
-                                              const float2* __restrict__ lo, const float2* __restrict__ hi, int t,
+// Thread t of the 128-thread rotate group owns the 16-byte chunk c = t & 7 (channels 8c..8c+7 of box 0 and
+// their partners 64+8c.. of box 1, i.e. frequencies 8c..8c+7) of the 4 consecutive rows 4(t>>3)+m.
+// (cos, sin) of the first row come from the two-level table, fetched ONE VISIT AHEAD (KRot::prefetch) so no
+// global-load latency sits between the TMA arrival and the MMA; rows 1..3 follow by the exact recurrence
+// cs(n+1) = cs(n) * cs(1) (n = -Delta grows by 1 per key, by 0 when the key position is a multiple of G).
+// All arithmetic is packed fp32x2 (FFMA2/FMUL2): a bf16 word holds two adjacent channels = two frequencies.
+struct KRot {
+    uint64_t sc[4], ss[4];          // unit step cs(-theta_i), pairs of frequencies (8c+2j, 8c+2j+1)
+    float4 nh[4], nl[4];            // prefetched HI / LO table entries of the next visit's first row
+    const float2* lo; const float2* hi;
+    int c, r0;
+    unsigned G;
+    __device__ __forceinline__ void init(const float2* lo_, const float2* hi_, int t, long long G_) {
+        lo = lo_; hi = hi_; c = t & 7; r0 = 4 * (t >> 3); G = (unsigned)G_;
+        const float4* p1 = reinterpret_cast<const float4*>(lo + 64 + 8 * c);       // LO[1][8c..]
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const float4 l = __ldg(p1 + j);
+            sc[j] = pack2(l.x, l.z); ss[j] = pack2(l.y, l.w);
+        }
+    }
+    // pos0 = absolute position of this CTA's first key row of the tile
+    __device__ __forceinline__ void prefetch(unsigned pos0) {
+        const unsigned pos = pos0 + r0;
+        const unsigned n = pos - pos / G;
+        const float4* ph = reinterpret_cast<const float4*>(hi + (size_t)(n >> 8) * 64 + 8 * c);
+        const float4* pl = reinterpret_cast<const float4*>(lo + (size_t)(n & 255) * 64 + 8 * c);
+#pragma unroll
+        for (int j = 0; j < 4; ++j) { nh[j] = __ldg(ph + j); nl[j] = __ldg(pl + j); }
+    }
+};
+
+__device__ __forceinline__ uint64_t neg2(uint64_t v) { return v ^ 0x8000000080000000ull; }
+__device__ __forceinline__ uint64_t bf16x2_to_f32x2(uint32_t w) {
+    return (uint64_t)(w << 16) | ((uint64_t)(w & 0xffff0000u) << 32);
+}
+__device__ __forceinline__ uint32_t f16x2_rn(float lo, float hi) {
+    uint32_t y;
+    asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(y) : "f"(hi), "f"(lo));
+    return y;
+}
+// y (packed f32x2) -> fp16x2 hi word and fp16x2 word of the residual y - hi
+__device__ __forceinline__ void split_hi_lo(uint64_t y, uint32_t& h, uint32_t& l, bool precise) {
+    float a, b;
+    unpack2(y, a, b);
+    h = f16x2_rn(a, b);
+    if (precise) {
+        const float2 f = __half22float2(*reinterpret_cast<const __half2*>(&h));
+        l = f16x2_rn(a - f.x, b - f.y);
+    }
+}
+
+__device__ __forceinline__ void rotate_k_half(unsigned char* kh, unsigned char* kl, unsigned pos0, KRot& R,
                                               bool precise) {
-    const int c = t & 7;
-#pragma unroll 2
+    // first-row (cos, sin) from the prefetched table entries: HI * LO as complex numbers
+    uint64_t cc[4], cs[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const float4 h = R.nh[j], l = R.nl[j];
+        cc[j] = pack2(h.x * l.x - h.y * l.y, h.z * l.z - h.w * l.w);
+        cs[j] = pack2(h.y * l.x + h.x * l.y, h.w * l.z + h.z * l.w);
+    }
+    unsigned rem = (pos0 + R.r0) % R.G;
+#pragma unroll
     for (int m = 0; m < 4; ++m) {
-        const int r = 4 * (t >> 3) + m;
-        float cs_c[8], cs_s[8];
-        cs8(lo, hi, pos0 + r, G, 8 * c, cs_c, cs_s);
-        const int off = r * 128 + ((c ^ (r & 7)) << 4);
+        const int r = R.r0 + m;
+        if (m > 0) {
+            rem = (rem + 1 == R.G) ? 0u : rem + 1;
+            if (rem != 0) {                                           // n grows by one: advance by the unit step
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const uint64_t c2 = ffma2(neg2(cs[j]), R.ss[j], fmul2(cc[j], R.sc[j]));
+                    cs[j] = ffma2(cc[j], R.ss[j], fmul2(cs[j], R.sc[j]));
+                    cc[j] = c2;
+                }
+            }
+        }
+        const int off = r * 128 + ((R.c ^ (r & 7)) << 4);
         const uint4 u1 = *reinterpret_cast<const uint4*>(kh + off);
         const uint4 u2 = *reinterpret_cast<const uint4*>(kh + KBOX + off);
         const uint32_t a[4] = {u1.x, u1.y, u1.z, u1.w}, b[4] = {u2.x, u2.y, u2.z, u2.w};
         uint32_t h1[4], h2[4], l1[4], l2[4];
-        rot8(a, b, cs_c, cs_s, h1, h2, l1, l2);
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const uint64_t x1 = bf16x2_to_f32x2(a[j]), x2 = bf16x2_to_f32x2(b[j]);
+            const uint64_t y1 = ffma2(neg2(x2), cs[j], fmul2(x1, cc[j]));      // x1 c - x2 s
+            const uint64_t y2 = ffma2(x1, cs[j], fmul2(x2, cc[j]));            // x1 s + x2 c
+            split_hi_lo(y1, h1[j], l1[j], precise);
+            split_hi_lo(y2, h2[j], l2[j], precise);
+        }
         *reinterpret_cast<uint4*>(kh + off) = make_uint4(h1[0], h1[1], h1[2], h1[3]);
         *reinterpret_cast<uint4*>(kh + KBOX + off) = make_uint4(h2[0], h2[1], h2[2], h2[3]);
         if (precise) {
@@ -295,44 +368,54 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_consta
             }
         }
     } else if (warp == 1) {
-        // ===================== MMA issuer (one thread of the leader CTA) =====================
-        if (cta == 0 && lane == 0) {
+        // ===================== MMA issuer (warp 1 of the leader CTA; one elected lane issues) =====================
+        // The whole warp runs the loop convergently so that descriptors and TMEM addresses stay in uniform
+        // registers; a divergent single-lane issuer costs ~100 cycles of R2UR/ELECT waterfall per MMA (measured).
+        if (cta == 0) {
+            const uint32_t tm = __shfl_sync(0xffffffffu, tmem, 0);
+            const uint32_t smem0 = __shfl_sync(0xffffffffu, smem_u32(smem), 0);
             auto issue_qk = [&](int v) {
                 const Visit x = plan.at(v, bifocal);
-                const uint32_t dS = tmem + TM_S + (v & 1) * 128;
-                const uint32_t kb = smem_u32(sK(v % NS)), klb = kb + KH_BYTES;
-                if (x.mode != 2) {
-#pragma unroll
-                    for (int ks = 0; ks < D / 16; ++ks)
-                        umma2_ts(dS, tmem + TM_QA + ks * 8,
-                                 smem_desc_sw128(kb + (ks >> 2) * KBOX + (ks & 3) * 32, 16, 1024), IDESC_QK_BF16, ks > 0);
-                } else {
-#pragma unroll
-                    for (int ks = 0; ks < D / 16; ++ks)
-                        umma2_ts(dS, tmem + TM_QA + ks * 8,
-                                 smem_desc_sw128(kb + (ks >> 2) * KBOX + (ks & 3) * 32, 16, 1024), IDESC_QK_F16, ks > 0);
-                    if (precise) {
+                const uint32_t dS = tm + TM_S + (v & 1) * 128;
+                const uint32_t kb = smem0 + (v % NS) * STAGE_BYTES, klb = kb + KH_BYTES;
+                if (elect_one()) {
+                    if (x.mode != 2) {
 #pragma unroll
                         for (int ks = 0; ks < D / 16; ++ks)
-                            umma2_ts(dS, tmem + TM_QA + ks * 8,
-                                     smem_desc_sw128(klb + (ks >> 2) * KBOX + (ks & 3) * 32, 16, 1024), IDESC_QK_F16, 1);
+                            umma2_ts(dS, tm + TM_QA + ks * 8,
+                                     smem_desc_sw128(kb + (ks >> 2) * KBOX + (ks & 3) * 32, 16, 1024), IDESC_QK_BF16, ks > 0);
+                    } else {
 #pragma unroll
                         for (int ks = 0; ks < D / 16; ++ks)
-                            umma2_ts(dS, tmem + TM_QB + ks * 8,
-                                     smem_desc_sw128(kb + (ks >> 2) * KBOX + (ks & 3) * 32, 16, 1024), IDESC_QK_F16, 1);
+                            umma2_ts(dS, tm + TM_QA + ks * 8,
+                                     smem_desc_sw128(kb + (ks >> 2) * KBOX + (ks & 3) * 32, 16, 1024), IDESC_QK_F16, ks > 0);
+                        if (precise) {
+#pragma unroll
+                            for (int ks = 0; ks < D / 16; ++ks)
+                                umma2_ts(dS, tm + TM_QA + ks * 8,
+                                         smem_desc_sw128(klb + (ks >> 2) * KBOX + (ks & 3) * 32, 16, 1024), IDESC_QK_F16, 1);
+#pragma unroll
+                            for (int ks = 0; ks < D / 16; ++ks)
+                                umma2_ts(dS, tm + TM_QB + ks * 8,
+                                         smem_desc_sw128(kb + (ks >> 2) * KBOX + (ks & 3) * 32, 16, 1024), IDESC_QK_F16, 1);
+                        }
                     }
+                    umma2_commit(&bars->s_full[v & 1]);
+                    if (plan.n_remote > 0 && v == plan.n_local - 1) umma2_commit(&bars->q_local_done);
                 }
-                umma2_commit(&bars->s_full[v & 1]);
-                if (plan.n_remote > 0 && v == plan.n_local - 1) umma2_commit(&bars->q_local_done);
+                __syncwarp();
             };
             auto issue_pv = [&](int v) {
-                const uint32_t vb = smem_u32(sV(v % NS));
+                const uint32_t vb = smem0 + (v % NS) * STAGE_BYTES + 2 * KH_BYTES;
+                if (elect_one()) {
 #pragma unroll
-                for (int ks = 0; ks < BN / 16; ++ks)
-                    umma2_ts(tmem + TM_O, tmem + TM_S + (v & 1) * 128 + ks * 8,
-                             smem_desc_sw128(vb + ks * 2048, VH_BYTES, 1024), IDESC_PV, (v > 0 || ks > 0) ? 1u : 0u);
-                umma2_commit(&bars->kv_empty[v % NS]);
-                umma2_commit(&bars->pv_done);
+                    for (int ks = 0; ks < BN / 16; ++ks)
+                        umma2_ts(tm + TM_O, tm + TM_S + (v & 1) * 128 + ks * 8,
+                                 smem_desc_sw128(vb + ks * 2048, VH_BYTES, 1024), IDESC_PV, (v > 0 || ks > 0) ? 1u : 0u);
+                    umma2_commit(&bars->kv_empty[v % NS]);
+                    umma2_commit(&bars->pv_done);
+                }
+                __syncwarp();
             };
             mbar_wait(&bars->q_ready, 0);
             mbar_wait(&bars->kv_ready[0], 0);
@@ -349,7 +432,8 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_consta
                 tc_fence_after();
                 issue_pv(v);
             }
-            umma2_commit(&bars->o_full);
+            if (elect_one()) umma2_commit(&bars->o_full);
+            __syncwarp();
         }
     } else if (warp >= 2 && warp < 6) {
         // ===================== rotate group (steps a4, a5) =====================
@@ -363,6 +447,11 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_consta
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive_leader(&bars->q_ready);
+        KRot rot;
+        if (plan.n_remote > 0) {
+            rot.init(p.lo, p.hi, t, p.G);
+            rot.prefetch((unsigned)(plan.kt_hi * BN + 64 * cta));     // first remote visit
+        }
         for (int v = 0; v < plan.nv; ++v) {
             const Visit x = plan.at(v, bifocal);
             const int s = v % NS;
@@ -375,8 +464,9 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_consta
                     tmem_st_wait();
                     tc_fence_before();
                 }
-                rotate_k_half(sK(s), sKl(s), (long long)x.kt * BN + 64 * cta, p.G, p.lo, p.hi, t, precise);
+                rotate_k_half(sK(s), sKl(s), (unsigned)(x.kt * BN + 64 * cta), rot, precise);
                 fence_proxy_async_smem();
+                if (x.kt > 0) rot.prefetch((unsigned)((x.kt - 1) * BN + 64 * cta));   // next remote visit's first row
             }
             __syncwarp();
             if (lane == 0) {
@@ -606,3 +696,4 @@ int launch_prefill_umma(const void* Q, const void* K, const void* V, void* out, 
 }
 
 }  // namespace jetlong
+
