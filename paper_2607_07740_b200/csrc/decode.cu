@@ -373,11 +373,21 @@ Plan make_plan(long long L, int H_q, int H_kv) {
 
 }  // namespace
 
+// decode_umma.cu
+bool umma_decode_supported(int H_q, int H_kv, int d, int dtype);
+void umma_decode_plan(long long L, int H_kv, int* nsplit, long long* kps);
+int launch_decode_umma(const void* q, const void* K, const void* V, float* part, long long L, int H_q, int H_kv,
+                       long long w0, long long G, bool bifocal, const float2* lo, const float2* hi, int* nsplit_out,
+                       cudaStream_t st);
+
 size_t decode_workspace_bytes(long long L, int H_q, int H_kv, int d) {
-    // worst-case split count (1024) is small; size for the plan's own count at this L, but never less
-    // than what a shorter L of the same call sequence would need: nsplit is non-decreasing in L.
+    // room for the partials of either implementation (SIMT or tcgen05) at this L
     Plan pl = make_plan(L, H_q, H_kv);
-    return two_level_bytes(L, d) + align256((size_t)pl.nsplit * H_q * (d + 2) * sizeof(float));
+    int ns = pl.nsplit, nu = 0;
+    long long kps = 0;
+    umma_decode_plan(L, H_kv, &nu, &kps);
+    if (nu > ns) ns = nu;
+    return two_level_bytes(L, d) + align256((size_t)ns * H_q * (d + 2) * sizeof(float));
 }
 
 template <typename T, int D>
@@ -398,6 +408,14 @@ static int launch_decode_td(const void* q, const void* K, const void* V, void* o
     p.H_q = H_q; p.H_kv = H_kv; p.HPB = pl.HPB;
     p.lo = reinterpret_cast<const float2*>(base + 256);
     p.hi = p.lo + 256 * (D / 2);
+    if (umma_decode_supported(H_q, H_kv, D, sizeof(T) == 2 ? JETLONG_BF16 : JETLONG_FP32)) {
+        int ns = 0;
+        int rc = launch_decode_umma(q, K, V, p.part, L, H_q, H_kv, w0, G, bifocal, p.lo, p.hi, &ns, st);
+        if (rc != JETLONG_OK) return rc;
+        decode_merge_kernel<T, D><<<H_q, D, 0, st>>>(p.part, ns, H_q, (T*)out, lse);
+        note_launch();
+        return check_launch("decode_merge_kernel");
+    }
     const size_t cs_bytes = 2 * (size_t)CK * (D / 2) * sizeof(float2);
     constexpr int EPL = Lane<T>::EPL;
     const size_t st_bytes = (size_t)NW * (32 / (D / EPL)) * 4 * (D + 2) * sizeof(float);

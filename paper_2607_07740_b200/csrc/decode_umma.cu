@@ -1,0 +1,419 @@
+// decode_umma.cu -- tcgen05 split-KV batch-1 decode for bf16, head_dim 128, up to 16 query heads per KV head
+// (steps a9, a7, a8).  HBM-bound scan: the KV cache is streamed once, by TMA, at full bandwidth; nothing but the
+// correction rotation of remote keys touches the ALUs per cache element.
+//
+// A CTA owns one KV head and a contiguous key range.  Per 128-key tile (KEYS on the UMMA M axis):
+//   S^T[key, head] = K[key, :] . Q[head, :]        UMMA M=128 (keys), N=16 (heads, zero padded), K=128 (channels)
+//   P[head, key]   = exp2(S^T * scale*log2e - m)   one thread per key, 16 values each
+//   O^T[ch, head] += V^T[ch, key] . P[head, key]   UMMA M=128 (channels), N=16, K=128 (keys); A = V tile, MN-major
+// Remote tiles (k < L-1-w0): the rotate group turns the TMA-loaded K tile into K' = R(Delta k) K in shared memory
+// (fp32 rotate, fp16 hi in place + fp16 lo in a side buffer), Q' = R(Delta q) Q is prepared once per CTA, and
+// S^T = K'hi Q'hi + K'lo Q'hi + K'hi Q'lo (compensated; the MMAs are ~free here).  The cache is only read.
+// Warp roles (320 threads): warp 0 TMA producer, warp 1 MMA issuer, warps 2-5 rotate group, warps 6-9 softmax.
+// Partial (m, l, O) states go to the workspace and are merged by decode_merge_kernel (additive LSE merge).
+#include <cuda.h>
+#include <math.h>
+
+#include "common.cuh"
+#include "umma.cuh"
+#include "rot.cuh"
+
+namespace jetlong {
+
+namespace {
+
+using namespace ptx;
+using namespace dev;
+
+constexpr int D = 128, BN = 128;
+constexpr int NH = 16;                               // UMMA N: query heads of one KV group, zero padded
+constexpr int KS = 3, VS = 2;                        // K / V ring depths
+constexpr int BOXB = BN * 128;                       // one SWIZZLE_128B box: 128 rows x 128 B = 16 KB
+constexpr int TILE = 2 * BOXB;                       // 32 KB (channels 0-63 | 64-127)
+constexpr int QBUF = 2 * NH * 128;                   // [2 boxes][16 rows][128 B] = 4 KB
+constexpr int NTHREADS = 320;
+constexpr float kLog2e = 1.4426950408889634f;
+constexpr uint32_t TM_S = 0, TM_O = 32;              // S0 | S1 | O, 16 fp32 columns each
+
+struct Bars {
+    uint64_t k_full[KS], k_ready[KS], k_empty[KS];
+    uint64_t v_full[VS], v_empty[VS];
+    uint64_t s_full[2], p_full[2];
+    uint64_t pv_done, o_full, q_ready;
+    uint32_t tmem_base;
+    float red[4 * NH];                               // cross-warp max / sum exchange of the softmax group
+};
+
+// smem: K ring | V ring | K lo | Q raw | Q' hi | Q' lo | P0 | P1 | Bars
+constexpr size_t OFF_V = (size_t)KS * TILE, OFF_KLO = OFF_V + (size_t)VS * TILE, OFF_Q = OFF_KLO + TILE,
+                 OFF_P = OFF_Q + 3 * QBUF, OFF_BARS = OFF_P + 2 * QBUF;
+constexpr size_t SMEM_BYTES = 1024 + OFF_BARS + 1024;
+
+struct Params {
+    const __nv_bfloat16* q;
+    float* part;                                     // [nsplit][H_q][D+2]
+    long long L, w0, G, kps;                         // kps = keys per split, a multiple of BN
+    int H_q, H_kv, g, bifocal;
+    const float2* lo;
+    const float2* hi;
+};
+
+// byte offset of element (row n, k) in a [2 boxes][16 rows][128 B] SWIZZLE_128B K-major operand (16-bit elements)
+__device__ __forceinline__ int bop_off(int n, int k) {
+    return (k >> 6) * (NH * 128) + n * 128 + ((((k & 63) >> 3) ^ (n & 7)) << 4) + (k & 7) * 2;
+}
+
+constexpr uint32_t IDESC_S_BF16 = idesc_f16(1, 1, 0, 0, BN, NH);
+constexpr uint32_t IDESC_S_F16 = idesc_f16(0, 0, 0, 0, BN, NH);
+constexpr uint32_t IDESC_PV = idesc_f16(1, 1, 1, 0, D, NH);      // A = V^T (smem, MN-major), B = P (smem, K-major)
+
+struct DPlan {
+    long long ks, ke, re, ls;
+    int kt_r0, nr, kt_l0, nl, nv;
+    __device__ DPlan(const Params& p, int split) {
+        ks = (long long)split * p.kps;
+        ke = ks + p.kps < p.L ? ks + p.kps : p.L;
+        const long long qpos = p.L - 1;
+        const long long kb = (p.bifocal && qpos - p.w0 > 0) ? qpos - p.w0 : 0;     // keys >= kb are local (R1)
+        re = ke < kb ? ke : kb;
+        ls = ks > kb ? ks : kb;
+        kt_r0 = (int)(ks / BN);
+        nr = re > ks ? (int)((re - 1) / BN) - kt_r0 + 1 : 0;
+        kt_l0 = (int)(ls / BN);
+        nl = ke > ls ? (int)((ke - 1) / BN) - kt_l0 + 1 : 0;
+        nv = nr + nl;
+    }
+    __device__ int kt(int v) const { return v < nr ? kt_r0 + v : kt_l0 + (v - nr); }
+    __device__ bool remote(int v) const { return v < nr; }
+};
+
+__global__ void __launch_bounds__(NTHREADS, 1)
+decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV, const Params p) {
+    extern __shared__ unsigned char smem_raw[];
+    unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    unsigned char* sKlo = smem + OFF_KLO;
+    unsigned char* sQ = smem + OFF_Q;                              // raw | hi | lo
+    unsigned char* sP = smem + OFF_P;                              // P0 | P1
+    Bars* bars = reinterpret_cast<Bars*>(smem + OFF_BARS);
+    auto sK = [&](int s) { return smem + (size_t)s * TILE; };
+    auto sV = [&](int s) { return smem + OFF_V + (size_t)s * TILE; };
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int split = blockIdx.x, kvh = blockIdx.y;
+    const DPlan plan(p, split);
+    const float sl2 = (1.0f / sqrtf((float)D)) * kLog2e;
+
+    if (tid == 0) {
+        for (int i = 0; i < KS; ++i) { mbar_init(&bars->k_full[i], 1); mbar_init(&bars->k_ready[i], 4); mbar_init(&bars->k_empty[i], 1); }
+        for (int i = 0; i < VS; ++i) { mbar_init(&bars->v_full[i], 1); mbar_init(&bars->v_empty[i], 1); }
+        for (int i = 0; i < 2; ++i) { mbar_init(&bars->s_full[i], 1); mbar_init(&bars->p_full[i], 4); }
+        mbar_init(&bars->pv_done, 1); mbar_init(&bars->o_full, 1); mbar_init(&bars->q_ready, 4);
+        fence_barrier_init();
+        prefetch_tmap(&tmK); prefetch_tmap(&tmV);
+    }
+    if (warp == 1) tmem_alloc<64>(&bars->tmem_base);
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = bars->tmem_base;
+
+    if (warp == 0) {
+        // ===================== TMA producer =====================
+        if (lane == 0) {
+            for (int v = 0; v < plan.nv; ++v) {
+                const int row0 = plan.kt(v) * BN;
+                const int s = v % KS, sv = v % VS;
+                if (v >= KS) mbar_wait(&bars->k_empty[s], ((v / KS) - 1) & 1);
+                mbar_arrive_expect_tx(&bars->k_full[s], TILE);
+                tma_load_3d(sK(s), &tmK, &bars->k_full[s], 0, kvh, row0);
+                tma_load_3d(sK(s) + BOXB, &tmK, &bars->k_full[s], 64, kvh, row0);
+                if (v >= VS) mbar_wait(&bars->v_empty[sv], ((v / VS) - 1) & 1);
+                mbar_arrive_expect_tx(&bars->v_full[sv], TILE);
+                tma_load_3d(sV(sv), &tmV, &bars->v_full[sv], 0, kvh, row0);
+                tma_load_3d(sV(sv) + BOXB, &tmV, &bars->v_full[sv], 64, kvh, row0);
+            }
+        }
+    } else if (warp == 1) {
+        // ===================== MMA issuer (convergent warp, one elected lane issues) =====================
+        const uint32_t tm = __shfl_sync(0xffffffffu, tmem, 0);
+        const uint32_t smem0 = __shfl_sync(0xffffffffu, smem_u32(smem), 0);
+        auto issue_s = [&](int v) {
+            const uint32_t dS = tm + TM_S + (v & 1) * NH;
+            const uint32_t ka = smem0 + (v % KS) * TILE, kla = smem0 + (uint32_t)OFF_KLO;
+            const uint32_t qa = smem0 + (uint32_t)OFF_Q;
+            const bool rem = plan.remote(v);
+            if (elect_one()) {
+                if (!rem) {
+#pragma unroll
+                    for (int ks = 0; ks < D / 16; ++ks)
+                        umma_ss(dS, smem_desc_sw128(ka + (ks >> 2) * BOXB + (ks & 3) * 32, 16, 1024),
+                                smem_desc_sw128(qa + (ks >> 2) * (NH * 128) + (ks & 3) * 32, 16, 1024), IDESC_S_BF16, ks > 0);
+                } else {
+#pragma unroll
+                    for (int ks = 0; ks < D / 16; ++ks)        // K'hi Q'hi
+                        umma_ss(dS, smem_desc_sw128(ka + (ks >> 2) * BOXB + (ks & 3) * 32, 16, 1024),
+                                smem_desc_sw128(qa + QBUF + (ks >> 2) * (NH * 128) + (ks & 3) * 32, 16, 1024), IDESC_S_F16, ks > 0);
+#pragma unroll
+                    for (int ks = 0; ks < D / 16; ++ks)        // K'lo Q'hi
+                        umma_ss(dS, smem_desc_sw128(kla + (ks >> 2) * BOXB + (ks & 3) * 32, 16, 1024),
+                                smem_desc_sw128(qa + QBUF + (ks >> 2) * (NH * 128) + (ks & 3) * 32, 16, 1024), IDESC_S_F16, 1);
+#pragma unroll
+                    for (int ks = 0; ks < D / 16; ++ks)        // K'hi Q'lo
+                        umma_ss(dS, smem_desc_sw128(ka + (ks >> 2) * BOXB + (ks & 3) * 32, 16, 1024),
+                                smem_desc_sw128(qa + 2 * QBUF + (ks >> 2) * (NH * 128) + (ks & 3) * 32, 16, 1024), IDESC_S_F16, 1);
+                }
+                umma_commit(&bars->s_full[v & 1]);
+                umma_commit(&bars->k_empty[v % KS]);
+            }
+            __syncwarp();
+        };
+        auto issue_pv = [&](int v) {
+            const uint32_t va = smem0 + (uint32_t)OFF_V + (v % VS) * TILE;
+            const uint32_t pa = smem0 + (uint32_t)OFF_P + (v & 1) * QBUF;
+            if (elect_one()) {
+#pragma unroll
+                for (int ks = 0; ks < BN / 16; ++ks)
+                    umma_ss(tm + TM_O, smem_desc_sw128(va + ks * 2048, BOXB, 1024),
+                            smem_desc_sw128(pa + (ks >> 2) * (NH * 128) + (ks & 3) * 32, 16, 1024), IDESC_PV,
+                            (v > 0 || ks > 0) ? 1u : 0u);
+                umma_commit(&bars->v_empty[v % VS]);
+                umma_commit(&bars->pv_done);
+            }
+            __syncwarp();
+        };
+        mbar_wait(&bars->q_ready, 0);
+        for (int v = 0; v <= plan.nv; ++v) {
+            if (v < plan.nv) {
+                mbar_wait(&bars->k_ready[v % KS], (v / KS) & 1);
+                tc_fence_after();
+                issue_s(v);
+            }
+            if (v > 0) {
+                const int u = v - 1;
+                mbar_wait(&bars->p_full[u & 1], (u >> 1) & 1);
+                mbar_wait(&bars->v_full[u % VS], (u / VS) & 1);
+                tc_fence_after();
+                issue_pv(u);
+            }
+        }
+        if (elect_one()) umma_commit(&bars->o_full);
+        __syncwarp();
+    } else if (warp >= 2 && warp < 6) {
+        // ===================== rotate group (steps a4, a5) =====================
+        const int t = tid - 64;
+        const long long qpos = p.L - 1;
+        // Q operands [16 heads][128 ch]: raw bf16 for local tiles; Q' = R(Delta q) Q as fp16 hi / lo for remote tiles
+        for (int i = t; i < 3 * QBUF / 4; i += 128) reinterpret_cast<uint32_t*>(sQ)[i] = 0u;
+        for (int i = t; i < 2 * QBUF / 4; i += 128) reinterpret_cast<uint32_t*>(sP)[i] = 0u;
+        named_bar_sync(1, 128);
+        const long long nq = qpos - qpos / p.G;                      // -Delta(q) >= 0, Eq.(5)
+        for (int idx = t; idx < p.g * 64; idx += 128) {
+            const int h = idx >> 6, i = idx & 63;
+            const __nv_bfloat16* qh = p.q + (size_t)(kvh * p.g + h) * D;
+            const __nv_bfloat16 b1 = qh[i], b2 = qh[i + 64];
+            *reinterpret_cast<__nv_bfloat16*>(sQ + bop_off(h, i)) = b1;
+            *reinterpret_cast<__nv_bfloat16*>(sQ + bop_off(h, i + 64)) = b2;
+            if (plan.nr > 0) {
+                const float2 ch = __ldg(&p.hi[(nq >> 8) * 64 + i]), cl = __ldg(&p.lo[(nq & 255) * 64 + i]);
+                const float c = ch.x * cl.x - ch.y * cl.y, s = ch.y * cl.x + ch.x * cl.y;
+                const float x1 = __bfloat162float(b1), x2 = __bfloat162float(b2);
+                const float y1 = x1 * c - x2 * s, y2 = x1 * s + x2 * c;
+                const __half h1 = __float2half_rn(y1), h2 = __float2half_rn(y2);
+                *reinterpret_cast<__half*>(sQ + QBUF + bop_off(h, i)) = h1;
+                *reinterpret_cast<__half*>(sQ + QBUF + bop_off(h, i + 64)) = h2;
+                *reinterpret_cast<__half*>(sQ + 2 * QBUF + bop_off(h, i)) = __float2half_rn(y1 - __half2float(h1));
+                *reinterpret_cast<__half*>(sQ + 2 * QBUF + bop_off(h, i + 64)) = __float2half_rn(y2 - __half2float(h2));
+            }
+        }
+        fence_proxy_async_smem();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&bars->q_ready);
+        KRot<8> rot;
+        if (plan.nr > 0) {
+            rot.init(p.lo, p.hi, t, p.G);
+            rot.prefetch((unsigned)(plan.kt(0) * BN));
+        }
+        for (int v = 0; v < plan.nv; ++v) {
+            const int s = v % KS;
+            mbar_wait(&bars->k_full[s], (v / KS) & 1);
+            if (plan.remote(v)) {
+                if (v > 0) mbar_wait(&bars->k_empty[(v - 1) % KS], ((v - 1) / KS) & 1);   // K lo of visit v-1 consumed
+                rotate_k_rows<8, BOXB>(sK(s), sKlo, (unsigned)(plan.kt(v) * BN), rot, true);
+                fence_proxy_async_smem();
+                if (plan.remote(v + 1)) rot.prefetch((unsigned)(plan.kt(v + 1) * BN));
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&bars->k_ready[s]);
+        }
+    } else {
+        // ===================== softmax group (steps a6-a8): one thread per key of the tile =====================
+        const int wq = warp & 3;                                     // TMEM lane quadrant of this warp
+        const int j = (wq << 5) | lane;                              // key row in the tile == TMEM lane
+        const uint32_t lane_base = (uint32_t)(wq << 5) << 16;
+        const int g = p.g;
+        float m_ref[NH], l[NH];
+#pragma unroll
+        for (int h = 0; h < NH; ++h) { m_ref[h] = -INFINITY; l[h] = 0.f; }
+        for (int v = 0; v < plan.nv; ++v) {
+            const long long key = (long long)plan.kt(v) * BN + j;
+            const bool valid = plan.remote(v) ? (key >= plan.ks && key < plan.re) : (key >= plan.ls && key < plan.ke);
+            mbar_wait(&bars->s_full[v & 1], (v >> 1) & 1);
+            tc_fence_after();
+            uint32_t sr[16];
+            tmem_ld16(tmem + lane_base + TM_S + (v & 1) * NH, sr);
+            tmem_ld_wait();
+            float x[NH], tmax[NH];
+#pragma unroll
+            for (int h = 0; h < NH; ++h) {
+                x[h] = (valid && h < g) ? __uint_as_float(sr[h]) * sl2 : -INFINITY;
+                float w = x[h];
+                if (h < g) {
+#pragma unroll
+                    for (int off = 16; off >= 1; off >>= 1) w = fmaxf(w, __shfl_xor_sync(0xffffffffu, w, off));
+                }
+                tmax[h] = w;
+            }
+            float* red = bars->red;                                  // single buffer, two barriers per visit
+            if (lane < NH) {
+                float w = -INFINITY;
+#pragma unroll
+                for (int h = 0; h < NH; ++h) if (lane == h) w = tmax[h];
+                red[wq * NH + lane] = w;
+            }
+            named_bar_sync(2, 128);
+            bool need = false;
+#pragma unroll
+            for (int h = 0; h < NH; ++h) {
+                if (h < g) {
+                    tmax[h] = fmaxf(fmaxf(red[h], red[NH + h]), fmaxf(red[2 * NH + h], red[3 * NH + h]));
+                    need |= tmax[h] > m_ref[h] + 8.0f;               // lazy rescale: only on a jump of 2^8 (or from -inf)
+                }
+            }
+            named_bar_sync(2, 128);                                  // everyone has read red before the next visit writes it
+            if (need) {                                              // uniform over the 128 threads
+                float alpha[NH];
+#pragma unroll
+                for (int h = 0; h < NH; ++h) {
+                    alpha[h] = 1.0f;
+                    if (h < g && tmax[h] > m_ref[h]) {
+                        alpha[h] = (m_ref[h] == -INFINITY) ? 0.0f : exp2f(m_ref[h] - tmax[h]);
+                        m_ref[h] = tmax[h];
+                        l[h] *= alpha[h];
+                    }
+                }
+                if (v > 0) {                                         // O^T row of channel j: scale column h by alpha[h]
+                    mbar_wait(&bars->pv_done, (v - 1) & 1);
+                    tc_fence_after();
+                    uint32_t og[16];
+                    tmem_ld16(tmem + lane_base + TM_O, og);
+                    tmem_ld_wait();
+#pragma unroll
+                    for (int h = 0; h < NH; ++h) og[h] = __float_as_uint(__uint_as_float(og[h]) * alpha[h]);
+                    tmem_st16(tmem + lane_base + TM_O, og);
+                    tmem_st_wait();
+                    tc_fence_before();
+                }
+            }
+            unsigned char* pb = sP + (v & 1) * QBUF;
+#pragma unroll
+            for (int h = 0; h < NH; ++h) {
+                if (h < g) {
+                    const float pr = (x[h] == -INFINITY) ? 0.0f : exp2f(x[h] - m_ref[h]);
+                    l[h] += pr;
+                    *reinterpret_cast<__nv_bfloat16*>(pb + bop_off(h, j)) = __float2bfloat16_rn(pr);
+                }
+            }
+            fence_proxy_async_smem();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&bars->p_full[v & 1]);
+        }
+        // ---- partial state of this split (steps a7, a8): l summed over the 128 key lanes, O^T from TMEM ----------
+#pragma unroll
+        for (int h = 0; h < NH; ++h) {
+            if (h < g) {
+#pragma unroll
+                for (int off = 16; off >= 1; off >>= 1) l[h] += __shfl_xor_sync(0xffffffffu, l[h], off);
+            }
+        }
+        if (lane < NH) {
+            float w = 0.f;
+#pragma unroll
+            for (int h = 0; h < NH; ++h) if (lane == h) w = l[h];
+            bars->red[wq * NH + lane] = w;
+        }
+        named_bar_sync(2, 128);
+        mbar_wait(&bars->o_full, 0);
+        tc_fence_after();
+        uint32_t og[16];
+        if (plan.nv > 0) {
+            tmem_ld16(tmem + lane_base + TM_O, og);
+            tmem_ld_wait();
+        } else {
+#pragma unroll
+            for (int h = 0; h < NH; ++h) og[h] = 0u;
+        }
+        constexpr int SS = D + 2;
+#pragma unroll
+        for (int h = 0; h < NH; ++h) {
+            if (h < g) {
+                float* dst = p.part + ((size_t)split * p.H_q + (size_t)kvh * g + h) * SS;
+                dst[j] = __uint_as_float(og[h]);
+                if (j == 0) {
+                    dst[D] = m_ref[h];
+                    dst[D + 1] = bars->red[h] + bars->red[NH + h] + bars->red[2 * NH + h] + bars->red[3 * NH + h];
+                }
+            }
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 1) tmem_dealloc<64>(tmem);
+}
+
+}  // namespace
+
+bool umma_decode_supported(int H_q, int H_kv, int d, int dtype) {
+    if (dtype != JETLONG_BF16 || d != 128 || H_kv < 1 || H_q % H_kv) return false;
+    return H_q / H_kv <= NH;
+}
+
+// split plan: one CTA per SM (the kernel needs ~215 KB of shared memory), key ranges are multiples of the 128-key tile
+void umma_decode_plan(long long L, int H_kv, int* nsplit, long long* kps) {
+    const long long ntiles = (L + BN - 1) / BN;
+    long long ns = 148 / H_kv;
+    if (ns < 1) ns = 1;
+    if (ns > ntiles) ns = ntiles;
+    if (ns > 1024) ns = 1024;
+    const long long tps = (ntiles + ns - 1) / ns;
+    *kps = tps * BN;
+    *nsplit = (int)((ntiles + tps - 1) / tps);
+}
+
+int launch_decode_umma(const void* q, const void* K, const void* V, float* part, long long L, int H_q, int H_kv,
+                       long long w0, long long G, bool bifocal, const float2* lo, const float2* hi, int* nsplit_out,
+                       cudaStream_t st) {
+    CUtensorMap tmK, tmV;
+    if (!make_kv_tensor_map(&tmK, K, L, H_kv, BN) || !make_kv_tensor_map(&tmV, V, L, H_kv, BN)) return JETLONG_UNSUPPORTED;
+    Params p;
+    p.q = (const __nv_bfloat16*)q;
+    p.part = part;
+    p.L = L; p.w0 = w0; p.G = G;
+    int ns;
+    umma_decode_plan(L, H_kv, &ns, &p.kps);
+    p.H_q = H_q; p.H_kv = H_kv; p.g = H_q / H_kv;
+    p.bifocal = bifocal ? 1 : 0;
+    p.lo = lo; p.hi = hi;
+    static bool attr_set = false;
+    if (!attr_set) {
+        if (cudaFuncSetAttribute(decode_umma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES) !=
+            cudaSuccess)
+            return check_launch("decode_umma attr");
+        attr_set = true;
+    }
+    decode_umma_kernel<<<dim3(ns, H_kv), NTHREADS, SMEM_BYTES, st>>>(tmK, tmV, p);
+    note_launch();
+    *nsplit_out = ns;
+    return check_launch("decode_umma_kernel");
+}
+
+}  // namespace jetlong

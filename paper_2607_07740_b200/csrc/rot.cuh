@@ -1,0 +1,198 @@
+// rot.cuh -- device helpers shared by the tcgen05 prefill and decode kernels: packed fp32x2 arithmetic, the
+// two-level (cos, sin) table lookup and the in-shared-memory correction rotation of K tiles (Eq.(5)-(6) P:101-106).
+#pragma once
+#include <cuda_bf16.h>
+#include <cuda_fp16.h>
+#include <stdint.h>
+
+namespace jetlong {
+namespace dev {
+
+__device__ __forceinline__ float ex2(float x) {
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+__device__ __forceinline__ float max3(float a, float b, float c) {
+    float y;
+    asm("max.f32 %0, %1, %2, %3;" : "=f"(y) : "f"(a), "f"(b), "f"(c));
+    return y;
+}
+// packed fp32x2 arithmetic (FFMA2 / FADD2 / FMUL2 on sm_100)
+__device__ __forceinline__ uint64_t pack2(float lo, float hi) {
+    uint64_t y;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(y) : "f"(lo), "f"(hi));
+    return y;
+}
+__device__ __forceinline__ void unpack2(uint64_t v, float& lo, float& hi) {
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ uint64_t ffma2(uint64_t a, uint64_t b, uint64_t c) {
+    uint64_t y;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(y) : "l"(a), "l"(b), "l"(c));
+    return y;
+}
+__device__ __forceinline__ uint64_t fadd2(uint64_t a, uint64_t b) {
+    uint64_t y;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(y) : "l"(a), "l"(b));
+    return y;
+}
+__device__ __forceinline__ uint64_t fmul2(uint64_t a, uint64_t b) {
+    uint64_t y;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(y) : "l"(a), "l"(b));
+    return y;
+}
+__device__ __forceinline__ uint32_t bf16x2(float lo, float hi) {
+    uint32_t y;
+    asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(y) : "f"(hi), "f"(lo));
+    return y;
+}
+template <int N> __device__ __forceinline__ void reg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
+template <int N> __device__ __forceinline__ void reg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
+__device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+
+// (cos, sin)(Delta(pos) theta_i) for 8 consecutive frequencies i = i0 .. i0+7 from the two-level table
+// (HI[n >> 8] * LO[n & 255] as complex numbers, n = -Delta(pos) >= 0, Eq.(5))
+__device__ __forceinline__ void cs8(const float2* __restrict__ lo, const float2* __restrict__ hi, long long pos,
+                                    long long G, int i0, float* cs_c, float* cs_s) {
+    const long long n = pos - pos / G;
+    const float4* ph = reinterpret_cast<const float4*>(hi + (n >> 8) * 64 + i0);
+    const float4* pl = reinterpret_cast<const float4*>(lo + (n & 255) * 64 + i0);
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const float4 h = __ldg(ph + j), l = __ldg(pl + j);
+        cs_c[2 * j] = h.x * l.x - h.y * l.y;      cs_s[2 * j] = h.y * l.x + h.x * l.y;
+        cs_c[2 * j + 1] = h.z * l.z - h.w * l.w;  cs_s[2 * j + 1] = h.w * l.z + h.z * l.w;
+    }
+}
+
+// rotate 8 pairs: a[4] = bf16 words of channels i0..i0+7, b[4] = their partners i0+64..; fp32 rotation, then
+// fp16 hi words (h1, h2) and fp16 lo words (l1, l2) of the residual y - hi.
+__device__ __forceinline__ void rot8(const uint32_t* a, const uint32_t* b, const float* cs_c, const float* cs_s,
+                                     uint32_t* h1, uint32_t* h2, uint32_t* l1, uint32_t* l2) {
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const float x1l = __uint_as_float(a[j] << 16), x1h = __uint_as_float(a[j] & 0xffff0000u);
+        const float x2l = __uint_as_float(b[j] << 16), x2h = __uint_as_float(b[j] & 0xffff0000u);
+        const float y1l = x1l * cs_c[2 * j] - x2l * cs_s[2 * j];
+        const float y2l = x1l * cs_s[2 * j] + x2l * cs_c[2 * j];
+        const float y1h = x1h * cs_c[2 * j + 1] - x2h * cs_s[2 * j + 1];
+        const float y2h = x1h * cs_s[2 * j + 1] + x2h * cs_c[2 * j + 1];
+        const __half2 a1 = __floats2half2_rn(y1l, y1h), a2 = __floats2half2_rn(y2l, y2h);
+        const float2 f1 = __half22float2(a1), f2 = __half22float2(a2);
+        const __half2 r1 = __floats2half2_rn(y1l - f1.x, y1h - f1.y), r2 = __floats2half2_rn(y2l - f2.x, y2h - f2.y);
+        h1[j] = *reinterpret_cast<const uint32_t*>(&a1);
+        h2[j] = *reinterpret_cast<const uint32_t*>(&a2);
+        l1[j] = *reinterpret_cast<const uint32_t*>(&r1);
+        l2[j] = *reinterpret_cast<const uint32_t*>(&r2);
+    }
+}
+
+// ---- step a5: correction rotation of 16 ROWS key rows of a K tile, in shared memory ---------------------------
+// kh: [2 boxes of KBOX bytes][rows][128 B] SWIZZLE_128B, bf16 in, fp16 hi out (in place); kl: same layout, fp16
+// lo out.  Thread t of the 128-thread rotate group owns the 16-byte chunk c = t & 7 (channels 8c..8c+7 of box 0
+// and their partners 64+8c.. of box 1, i.e. frequencies 8c..8c+7) of the ROWS consecutive rows ROWS(t>>3)+m.
+// (cos, sin) of the first row come from the two-level table, fetched ONE VISIT AHEAD (KRot::prefetch) so no
+// global-load latency sits between the TMA arrival and the MMA; rows 1..3 follow by the exact recurrence
+// cs(n+1) = cs(n) * cs(1) (n = -Delta grows by 1 per key, by 0 when the key position is a multiple of G);
+// the recurrence runs at most 7 steps from a table value, so it adds no measurable error.
+// All arithmetic is packed fp32x2 (FFMA2/FMUL2): a bf16 word holds two adjacent channels = two frequencies.
+template <int ROWS> struct KRot {
+    uint64_t sc[4], ss[4];          // unit step cs(-theta_i), pairs of frequencies (8c+2j, 8c+2j+1)
+    float4 nh[4], nl[4];            // prefetched HI / LO table entries of the next visit's first row
+    const float2* lo; const float2* hi;
+    int c, r0;
+    unsigned G;
+    __device__ __forceinline__ void init(const float2* lo_, const float2* hi_, int t, long long G_) {
+        lo = lo_; hi = hi_; c = t & 7; r0 = ROWS * (t >> 3); G = (unsigned)G_;
+        const float4* p1 = reinterpret_cast<const float4*>(lo + 64 + 8 * c);       // LO[1][8c..]
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const float4 l = __ldg(p1 + j);
+            sc[j] = pack2(l.x, l.z); ss[j] = pack2(l.y, l.w);
+        }
+    }
+    // pos0 = absolute position of this CTA's first key row of the tile
+    __device__ __forceinline__ void prefetch(unsigned pos0) {
+        const unsigned pos = pos0 + r0;
+        const unsigned n = pos - pos / G;
+        const float4* ph = reinterpret_cast<const float4*>(hi + (size_t)(n >> 8) * 64 + 8 * c);
+        const float4* pl = reinterpret_cast<const float4*>(lo + (size_t)(n & 255) * 64 + 8 * c);
+#pragma unroll
+        for (int j = 0; j < 4; ++j) { nh[j] = __ldg(ph + j); nl[j] = __ldg(pl + j); }
+    }
+};
+
+__device__ __forceinline__ uint64_t neg2(uint64_t v) { return v ^ 0x8000000080000000ull; }
+__device__ __forceinline__ uint64_t bf16x2_to_f32x2(uint32_t w) {
+    return (uint64_t)(w << 16) | ((uint64_t)(w & 0xffff0000u) << 32);
+}
+__device__ __forceinline__ uint32_t f16x2_rn(float lo, float hi) {
+    uint32_t y;
+    asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(y) : "f"(hi), "f"(lo));
+    return y;
+}
+// y (packed f32x2) -> fp16x2 hi word and fp16x2 word of the residual y - hi
+__device__ __forceinline__ void split_hi_lo(uint64_t y, uint32_t& h, uint32_t& l, bool precise) {
+    float a, b;
+    unpack2(y, a, b);
+    h = f16x2_rn(a, b);
+    if (precise) {
+        const float2 f = __half22float2(*reinterpret_cast<const __half2*>(&h));
+        l = f16x2_rn(a - f.x, b - f.y);
+    }
+}
+
+template <int ROWS, int KBOX>
+__device__ __forceinline__ void rotate_k_rows(unsigned char* kh, unsigned char* kl, unsigned pos0, KRot<ROWS>& R,
+                                              bool precise) {
+    // first-row (cos, sin) from the prefetched table entries: HI * LO as complex numbers
+    uint64_t cc[4], cs[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const float4 h = R.nh[j], l = R.nl[j];
+        cc[j] = pack2(h.x * l.x - h.y * l.y, h.z * l.z - h.w * l.w);
+        cs[j] = pack2(h.y * l.x + h.x * l.y, h.w * l.z + h.z * l.w);
+    }
+    unsigned rem = (pos0 + R.r0) % R.G;
+#pragma unroll
+    for (int m = 0; m < ROWS; ++m) {
+        const int r = R.r0 + m;
+        if (m > 0) {
+            rem = (rem + 1 == R.G) ? 0u : rem + 1;
+            if (rem != 0) {                                           // n grows by one: advance by the unit step
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const uint64_t c2 = ffma2(neg2(cs[j]), R.ss[j], fmul2(cc[j], R.sc[j]));
+                    cs[j] = ffma2(cc[j], R.ss[j], fmul2(cs[j], R.sc[j]));
+                    cc[j] = c2;
+                }
+            }
+        }
+        const int off = r * 128 + ((R.c ^ (r & 7)) << 4);
+        const uint4 u1 = *reinterpret_cast<const uint4*>(kh + off);
+        const uint4 u2 = *reinterpret_cast<const uint4*>(kh + KBOX + off);
+        const uint32_t a[4] = {u1.x, u1.y, u1.z, u1.w}, b[4] = {u2.x, u2.y, u2.z, u2.w};
+        uint32_t h1[4], h2[4], l1[4], l2[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const uint64_t x1 = bf16x2_to_f32x2(a[j]), x2 = bf16x2_to_f32x2(b[j]);
+            const uint64_t y1 = ffma2(neg2(x2), cs[j], fmul2(x1, cc[j]));      // x1 c - x2 s
+            const uint64_t y2 = ffma2(x1, cs[j], fmul2(x2, cc[j]));            // x1 s + x2 c
+            split_hi_lo(y1, h1[j], l1[j], precise);
+            split_hi_lo(y2, h2[j], l2[j], precise);
+        }
+        *reinterpret_cast<uint4*>(kh + off) = make_uint4(h1[0], h1[1], h1[2], h1[3]);
+        *reinterpret_cast<uint4*>(kh + KBOX + off) = make_uint4(h2[0], h2[1], h2[2], h2[3]);
+        if (precise) {
+            *reinterpret_cast<uint4*>(kl + off) = make_uint4(l1[0], l1[1], l1[2], l1[3]);
+            *reinterpret_cast<uint4*>(kl + KBOX + off) = make_uint4(l2[0], l2[1], l2[2], l2[3]);
+        }
+    }
+}
+
+}  // namespace dev
+}  // namespace jetlong

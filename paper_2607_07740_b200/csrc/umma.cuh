@@ -4,6 +4,11 @@
 #include <stdint.h>
 
 namespace jetlong {
+
+// host: tensor map of a [L, H, 128] bf16 tensor seen as (d, H, L); box = 64 channels x 1 head x `rows` rows,
+// SWIZZLE_128B, out-of-bounds rows read as zero (defined in prefill_umma.cu)
+bool make_kv_tensor_map(CUtensorMap* m, const void* base, long long L, int H, int rows);
+
 namespace ptx {
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
