@@ -9,7 +9,7 @@
 // Remote tiles (k < L-1-w0): the rotate group turns the TMA-loaded K tile into K' = R(Delta k) K in shared memory
 // (fp32 rotate, fp16 hi in place + fp16 lo in a side buffer), Q' = R(Delta q) Q is prepared once per CTA, and
 // S^T = K'hi Q'hi + K'lo Q'hi + K'hi Q'lo (compensated; the MMAs are ~free here).  The cache is only read.
-// Warp roles (320 threads): warp 0 TMA producer, warp 1 MMA issuer, warps 2-5 rotate group, warps 6-9 softmax.
+// Warp roles (448 threads): warp 0 TMA producer, warp 1 MMA issuer, warps 2-9 rotate group, warps 10-13 softmax.
 // Partial (m, l, O) states go to the workspace and are merged by decode_merge_kernel (additive LSE merge).
 #include <cuda.h>
 #include <math.h>
@@ -27,11 +27,14 @@ using namespace dev;
 
 constexpr int D = 128, BN = 128;
 constexpr int NH = 16;                               // UMMA N: query heads of one KV group, zero padded
-constexpr int KS = 3, VS = 2;                        // K / V ring depths
+constexpr int KS = 2, VS = 2;                        // K / V ring depths; a K stage is K (hi in place) | K lo
 constexpr int BOXB = BN * 128;                       // one SWIZZLE_128B box: 128 rows x 128 B = 16 KB
 constexpr int TILE = 2 * BOXB;                       // 32 KB (channels 0-63 | 64-127)
 constexpr int QBUF = 2 * NH * 128;                   // [2 boxes][16 rows][128 B] = 4 KB
-constexpr int NTHREADS = 320;
+constexpr int RW = 8;                                // rotate warps
+constexpr int RT = RW * 32;                          // rotate threads
+constexpr int RROWS = 1024 / RT;                     // key rows per rotate thread (8 chunks x 128 rows / RT)
+constexpr int NTHREADS = 64 + RT + 128;
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr uint32_t TM_S = 0, TM_O = 32;              // S0 | S1 | O, 16 fp32 columns each
 
@@ -44,9 +47,9 @@ struct Bars {
     float red[4 * NH];                               // cross-warp max / sum exchange of the softmax group
 };
 
-// smem: K ring | V ring | K lo | Q raw | Q' hi | Q' lo | P0 | P1 | Bars
-constexpr size_t OFF_V = (size_t)KS * TILE, OFF_KLO = OFF_V + (size_t)VS * TILE, OFF_Q = OFF_KLO + TILE,
-                 OFF_P = OFF_Q + 3 * QBUF, OFF_BARS = OFF_P + 2 * QBUF;
+// smem: K ring (K | K lo per stage) | V ring | Q raw | Q' hi | Q' lo | P0 | P1 | Bars
+constexpr size_t OFF_V = (size_t)KS * 2 * TILE, OFF_Q = OFF_V + (size_t)VS * TILE, OFF_P = OFF_Q + 3 * QBUF,
+                 OFF_BARS = OFF_P + 2 * QBUF;
 constexpr size_t SMEM_BYTES = 1024 + OFF_BARS + 1024;
 
 struct Params {
@@ -61,6 +64,27 @@ struct Params {
 // byte offset of element (row n, k) in a [2 boxes][16 rows][128 B] SWIZZLE_128B K-major operand (16-bit elements)
 __device__ __forceinline__ int bop_off(int n, int k) {
     return (k >> 6) * (NH * 128) + n * 128 + ((((k & 63) >> 3) ^ (n & 7)) << 4) + (k & 7) * 2;
+}
+
+__device__ __forceinline__ float ex2(float x) {
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+// OR of `pred` over the `nthreads` threads that meet at named barrier `id`
+__device__ __forceinline__ bool bar_red_or(int id, int nthreads, bool pred) {
+    uint32_t r;
+    asm volatile(
+        "{\n\t.reg .pred p, q;\n\tsetp.ne.u32 p, %3, 0;\n\t"
+        "barrier.red.or.pred q, %1, %2, p;\n\t"
+        "selp.u32 %0, 1, 0, q;\n\t}"
+        : "=r"(r) : "r"(id), "r"(nthreads), "r"((uint32_t)pred) : "memory");
+    return r != 0;
+}
+__device__ __forceinline__ void sts16(uint32_t a, uint16_t v) { asm volatile("st.shared.u16 [%0], %1;" ::"r"(a), "h"(v) : "memory"); }
+__device__ __forceinline__ uint16_t bf16_bits(float f) {
+    const __nv_bfloat16 b = __float2bfloat16_rn(f);
+    return *reinterpret_cast<const uint16_t*>(&b);
 }
 
 constexpr uint32_t IDESC_S_BF16 = idesc_f16(1, 1, 0, 0, BN, NH);
@@ -87,15 +111,15 @@ struct DPlan {
     __device__ bool remote(int v) const { return v < nr; }
 };
 
+template <int NG>                                    // NG = query heads per KV head, rounded up to a power of two
 __global__ void __launch_bounds__(NTHREADS, 1)
 decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV, const Params p) {
     extern __shared__ unsigned char smem_raw[];
     unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-    unsigned char* sKlo = smem + OFF_KLO;
     unsigned char* sQ = smem + OFF_Q;                              // raw | hi | lo
     unsigned char* sP = smem + OFF_P;                              // P0 | P1
     Bars* bars = reinterpret_cast<Bars*>(smem + OFF_BARS);
-    auto sK = [&](int s) { return smem + (size_t)s * TILE; };
+    auto sK = [&](int s) { return smem + (size_t)s * 2 * TILE; };                // K lo of the stage sits at + TILE
     auto sV = [&](int s) { return smem + OFF_V + (size_t)s * TILE; };
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -104,10 +128,10 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
     const float sl2 = (1.0f / sqrtf((float)D)) * kLog2e;
 
     if (tid == 0) {
-        for (int i = 0; i < KS; ++i) { mbar_init(&bars->k_full[i], 1); mbar_init(&bars->k_ready[i], 4); mbar_init(&bars->k_empty[i], 1); }
+        for (int i = 0; i < KS; ++i) { mbar_init(&bars->k_full[i], 1); mbar_init(&bars->k_ready[i], RW); mbar_init(&bars->k_empty[i], 1); }
         for (int i = 0; i < VS; ++i) { mbar_init(&bars->v_full[i], 1); mbar_init(&bars->v_empty[i], 1); }
         for (int i = 0; i < 2; ++i) { mbar_init(&bars->s_full[i], 1); mbar_init(&bars->p_full[i], 4); }
-        mbar_init(&bars->pv_done, 1); mbar_init(&bars->o_full, 1); mbar_init(&bars->q_ready, 4);
+        mbar_init(&bars->pv_done, 1); mbar_init(&bars->o_full, 1); mbar_init(&bars->q_ready, RW);
         fence_barrier_init();
         prefetch_tmap(&tmK); prefetch_tmap(&tmV);
     }
@@ -139,7 +163,7 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
         const uint32_t smem0 = __shfl_sync(0xffffffffu, smem_u32(smem), 0);
         auto issue_s = [&](int v) {
             const uint32_t dS = tm + TM_S + (v & 1) * NH;
-            const uint32_t ka = smem0 + (v % KS) * TILE, kla = smem0 + (uint32_t)OFF_KLO;
+            const uint32_t ka = smem0 + (v % KS) * 2 * TILE, kla = ka + TILE;
             const uint32_t qa = smem0 + (uint32_t)OFF_Q;
             const bool rem = plan.remote(v);
             if (elect_one()) {
@@ -198,16 +222,16 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
         }
         if (elect_one()) umma_commit(&bars->o_full);
         __syncwarp();
-    } else if (warp >= 2 && warp < 6) {
+    } else if (warp >= 2 && warp < 2 + RW) {
         // ===================== rotate group (steps a4, a5) =====================
         const int t = tid - 64;
         const long long qpos = p.L - 1;
         // Q operands [16 heads][128 ch]: raw bf16 for local tiles; Q' = R(Delta q) Q as fp16 hi / lo for remote tiles
-        for (int i = t; i < 3 * QBUF / 4; i += 128) reinterpret_cast<uint32_t*>(sQ)[i] = 0u;
-        for (int i = t; i < 2 * QBUF / 4; i += 128) reinterpret_cast<uint32_t*>(sP)[i] = 0u;
-        named_bar_sync(1, 128);
+        for (int i = t; i < 3 * QBUF / 4; i += RT) reinterpret_cast<uint32_t*>(sQ)[i] = 0u;
+        for (int i = t; i < 2 * QBUF / 4; i += RT) reinterpret_cast<uint32_t*>(sP)[i] = 0u;
+        named_bar_sync(1, RT);
         const long long nq = qpos - qpos / p.G;                      // -Delta(q) >= 0, Eq.(5)
-        for (int idx = t; idx < p.g * 64; idx += 128) {
+        for (int idx = t; idx < p.g * 64; idx += RT) {
             const int h = idx >> 6, i = idx & 63;
             const __nv_bfloat16* qh = p.q + (size_t)(kvh * p.g + h) * D;
             const __nv_bfloat16 b1 = qh[i], b2 = qh[i + 64];
@@ -228,7 +252,7 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
         fence_proxy_async_smem();
         __syncwarp();
         if (lane == 0) mbar_arrive(&bars->q_ready);
-        KRot<8> rot;
+        KRot<RROWS> rot;
         if (plan.nr > 0) {
             rot.init(p.lo, p.hi, t, p.G);
             rot.prefetch((unsigned)(plan.kt(0) * BN));
@@ -237,8 +261,7 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
             const int s = v % KS;
             mbar_wait(&bars->k_full[s], (v / KS) & 1);
             if (plan.remote(v)) {
-                if (v > 0) mbar_wait(&bars->k_empty[(v - 1) % KS], ((v - 1) / KS) & 1);   // K lo of visit v-1 consumed
-                rotate_k_rows<8, BOXB>(sK(s), sKlo, (unsigned)(plan.kt(v) * BN), rot, true);
+                rotate_k_rows<RROWS, BOXB>(smem_u32(sK(s)), smem_u32(sK(s)) + TILE, (unsigned)(plan.kt(v) * BN), rot, true);
                 fence_proxy_async_smem();
                 if (plan.remote(v + 1)) rot.prefetch((unsigned)(plan.kt(v + 1) * BN));
             }
@@ -251,9 +274,11 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
         const int j = (wq << 5) | lane;                              // key row in the tile == TMEM lane
         const uint32_t lane_base = (uint32_t)(wq << 5) << 16;
         const int g = p.g;
-        float m_ref[NH], l[NH];
+        const uint32_t pj = smem_u32(sP) + (j >> 6) * (NH * 128) + (j & 7) * 2;   // P[h][j] = pj + h*128 + ((cj ^ (h&7)) << 4)
+        const int cj = (j & 63) >> 3;
+        float m_ref[NG], l[NG];
 #pragma unroll
-        for (int h = 0; h < NH; ++h) { m_ref[h] = -INFINITY; l[h] = 0.f; }
+        for (int h = 0; h < NG; ++h) { m_ref[h] = -INFINITY; l[h] = 0.f; }
         for (int v = 0; v < plan.nv; ++v) {
             const long long key = (long long)plan.kt(v) * BN + j;
             const bool valid = plan.remote(v) ? (key >= plan.ks && key < plan.re) : (key >= plan.ls && key < plan.ke);
@@ -262,45 +287,42 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
             uint32_t sr[16];
             tmem_ld16(tmem + lane_base + TM_S + (v & 1) * NH, sr);
             tmem_ld_wait();
-            float x[NH], tmax[NH];
+            float x[NG];
+            bool jump = false;
 #pragma unroll
-            for (int h = 0; h < NH; ++h) {
+            for (int h = 0; h < NG; ++h) {
                 x[h] = (valid && h < g) ? __uint_as_float(sr[h]) * sl2 : -INFINITY;
-                float w = x[h];
-                if (h < g) {
+                jump |= x[h] > m_ref[h] + 8.0f;                      // lazy rescale: only on a jump of 2^8 (or from -inf)
+            }
+            if (bar_red_or(2, 128, jump)) {                          // rare; uniform over the 128 threads
+                float tmax[NG];
+#pragma unroll
+                for (int h = 0; h < NG; ++h) {
+                    float w = x[h];
 #pragma unroll
                     for (int off = 16; off >= 1; off >>= 1) w = fmaxf(w, __shfl_xor_sync(0xffffffffu, w, off));
+                    tmax[h] = w;
                 }
-                tmax[h] = w;
-            }
-            float* red = bars->red;                                  // single buffer, two barriers per visit
-            if (lane < NH) {
-                float w = -INFINITY;
+                if (lane < NG) {
+                    float w = -INFINITY;
 #pragma unroll
-                for (int h = 0; h < NH; ++h) if (lane == h) w = tmax[h];
-                red[wq * NH + lane] = w;
-            }
-            named_bar_sync(2, 128);
-            bool need = false;
-#pragma unroll
-            for (int h = 0; h < NH; ++h) {
-                if (h < g) {
-                    tmax[h] = fmaxf(fmaxf(red[h], red[NH + h]), fmaxf(red[2 * NH + h], red[3 * NH + h]));
-                    need |= tmax[h] > m_ref[h] + 8.0f;               // lazy rescale: only on a jump of 2^8 (or from -inf)
+                    for (int h = 0; h < NG; ++h) if (lane == h) w = tmax[h];
+                    bars->red[wq * NH + lane] = w;
                 }
-            }
-            named_bar_sync(2, 128);                                  // everyone has read red before the next visit writes it
-            if (need) {                                              // uniform over the 128 threads
-                float alpha[NH];
+                named_bar_sync(2, 128);
+                float alpha[NG];
 #pragma unroll
-                for (int h = 0; h < NH; ++h) {
+                for (int h = 0; h < NG; ++h) {
+                    const float* red = bars->red;
+                    const float tm_h = fmaxf(fmaxf(red[h], red[NH + h]), fmaxf(red[2 * NH + h], red[3 * NH + h]));
                     alpha[h] = 1.0f;
-                    if (h < g && tmax[h] > m_ref[h]) {
-                        alpha[h] = (m_ref[h] == -INFINITY) ? 0.0f : exp2f(m_ref[h] - tmax[h]);
-                        m_ref[h] = tmax[h];
+                    if (tm_h > m_ref[h]) {
+                        alpha[h] = (m_ref[h] == -INFINITY) ? 0.0f : ex2(m_ref[h] - tm_h);
+                        m_ref[h] = tm_h;
                         l[h] *= alpha[h];
                     }
                 }
+                named_bar_sync(2, 128);                              // red[] may be rewritten by the next slow path
                 if (v > 0) {                                         // O^T row of channel j: scale column h by alpha[h]
                     mbar_wait(&bars->pv_done, (v - 1) & 1);
                     tc_fence_after();
@@ -308,20 +330,18 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
                     tmem_ld16(tmem + lane_base + TM_O, og);
                     tmem_ld_wait();
 #pragma unroll
-                    for (int h = 0; h < NH; ++h) og[h] = __float_as_uint(__uint_as_float(og[h]) * alpha[h]);
+                    for (int h = 0; h < NG; ++h) og[h] = __float_as_uint(__uint_as_float(og[h]) * alpha[h]);
                     tmem_st16(tmem + lane_base + TM_O, og);
                     tmem_st_wait();
                     tc_fence_before();
                 }
             }
-            unsigned char* pb = sP + (v & 1) * QBUF;
+            const uint32_t pb = pj + (v & 1) * QBUF;
 #pragma unroll
-            for (int h = 0; h < NH; ++h) {
-                if (h < g) {
-                    const float pr = (x[h] == -INFINITY) ? 0.0f : exp2f(x[h] - m_ref[h]);
-                    l[h] += pr;
-                    *reinterpret_cast<__nv_bfloat16*>(pb + bop_off(h, j)) = __float2bfloat16_rn(pr);
-                }
+            for (int h = 0; h < NG; ++h) {
+                const float pr = (x[h] == -INFINITY) ? 0.0f : ex2(x[h] - m_ref[h]);
+                l[h] += pr;
+                if (h < g) sts16(pb + h * 128 + ((cj ^ (h & 7)) << 4), bf16_bits(pr));
             }
             fence_proxy_async_smem();
             __syncwarp();
@@ -329,16 +349,14 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
         }
         // ---- partial state of this split (steps a7, a8): l summed over the 128 key lanes, O^T from TMEM ----------
 #pragma unroll
-        for (int h = 0; h < NH; ++h) {
-            if (h < g) {
+        for (int h = 0; h < NG; ++h) {
 #pragma unroll
-                for (int off = 16; off >= 1; off >>= 1) l[h] += __shfl_xor_sync(0xffffffffu, l[h], off);
-            }
+            for (int off = 16; off >= 1; off >>= 1) l[h] += __shfl_xor_sync(0xffffffffu, l[h], off);
         }
-        if (lane < NH) {
+        if (lane < NG) {
             float w = 0.f;
 #pragma unroll
-            for (int h = 0; h < NH; ++h) if (lane == h) w = l[h];
+            for (int h = 0; h < NG; ++h) if (lane == h) w = l[h];
             bars->red[wq * NH + lane] = w;
         }
         named_bar_sync(2, 128);
@@ -350,11 +368,11 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
             tmem_ld_wait();
         } else {
 #pragma unroll
-            for (int h = 0; h < NH; ++h) og[h] = 0u;
+            for (int h = 0; h < 16; ++h) og[h] = 0u;
         }
         constexpr int SS = D + 2;
 #pragma unroll
-        for (int h = 0; h < NH; ++h) {
+        for (int h = 0; h < NG; ++h) {
             if (h < g) {
                 float* dst = p.part + ((size_t)split * p.H_q + (size_t)kvh * g + h) * SS;
                 dst[j] = __uint_as_float(og[h]);
@@ -403,14 +421,11 @@ int launch_decode_umma(const void* q, const void* K, const void* V, float* part,
     p.H_q = H_q; p.H_kv = H_kv; p.g = H_q / H_kv;
     p.bifocal = bifocal ? 1 : 0;
     p.lo = lo; p.hi = hi;
-    static bool attr_set = false;
-    if (!attr_set) {
-        if (cudaFuncSetAttribute(decode_umma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES) !=
-            cudaSuccess)
-            return check_launch("decode_umma attr");
-        attr_set = true;
-    }
-    decode_umma_kernel<<<dim3(ns, H_kv), NTHREADS, SMEM_BYTES, st>>>(tmK, tmV, p);
+    auto kern = p.g <= 1 ? decode_umma_kernel<1> : p.g <= 2 ? decode_umma_kernel<2> : p.g <= 4 ? decode_umma_kernel<4>
+              : p.g <= 8 ? decode_umma_kernel<8> : decode_umma_kernel<16>;
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES) != cudaSuccess)
+        return check_launch("decode_umma attr");
+    kern<<<dim3(ns, H_kv), NTHREADS, SMEM_BYTES, st>>>(tmK, tmV, p);
     note_launch();
     *nsplit_out = ns;
     return check_launch("decode_umma_kernel");

@@ -282,7 +282,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_consta
                     tmem_st_wait();
                     tc_fence_before();
                 }
-                rotate_k_rows<4, KBOX>(sK(s), sKl(s), (unsigned)(x.kt * BN + 64 * cta), rot, precise);
+                rotate_k_rows<4, KBOX>(smem_u32(sK(s)), smem_u32(sKl(s)), (unsigned)(x.kt * BN + 64 * cta), rot, precise);
                 fence_proxy_async_smem();
                 if (x.kt > 0) rot.prefetch((unsigned)((x.kt - 1) * BN + 64 * cta));   // next remote visit's first row
             }

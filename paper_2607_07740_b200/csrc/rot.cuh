@@ -146,9 +146,19 @@ __device__ __forceinline__ void split_hi_lo(uint64_t y, uint32_t& h, uint32_t& l
     }
 }
 
+// explicit shared-space 128-bit accesses (pointers that pass through lambdas degrade to generic LD/ST otherwise)
+__device__ __forceinline__ uint4 lds128(uint32_t a) {
+    uint4 v;
+    asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a) : "memory");
+    return v;
+}
+__device__ __forceinline__ void sts128(uint32_t a, uint32_t x, uint32_t y, uint32_t z, uint32_t w) {
+    asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" ::"r"(a), "r"(x), "r"(y), "r"(z), "r"(w) : "memory");
+}
+
 template <int ROWS, int KBOX>
-__device__ __forceinline__ void rotate_k_rows(unsigned char* kh, unsigned char* kl, unsigned pos0, KRot<ROWS>& R,
-                                              bool precise) {
+__device__ __forceinline__ void rotate_k_rows(uint32_t kh, uint32_t kl, unsigned pos0, KRot<ROWS>& R,
+                                              bool precise) {   // kh, kl: shared-space addresses
     // first-row (cos, sin) from the prefetched table entries: HI * LO as complex numbers
     uint64_t cc[4], cs[4];
 #pragma unroll
@@ -173,8 +183,8 @@ __device__ __forceinline__ void rotate_k_rows(unsigned char* kh, unsigned char* 
             }
         }
         const int off = r * 128 + ((R.c ^ (r & 7)) << 4);
-        const uint4 u1 = *reinterpret_cast<const uint4*>(kh + off);
-        const uint4 u2 = *reinterpret_cast<const uint4*>(kh + KBOX + off);
+        const uint4 u1 = lds128(kh + off);
+        const uint4 u2 = lds128(kh + KBOX + off);
         const uint32_t a[4] = {u1.x, u1.y, u1.z, u1.w}, b[4] = {u2.x, u2.y, u2.z, u2.w};
         uint32_t h1[4], h2[4], l1[4], l2[4];
 #pragma unroll
@@ -185,11 +195,11 @@ __device__ __forceinline__ void rotate_k_rows(unsigned char* kh, unsigned char* 
             split_hi_lo(y1, h1[j], l1[j], precise);
             split_hi_lo(y2, h2[j], l2[j], precise);
         }
-        *reinterpret_cast<uint4*>(kh + off) = make_uint4(h1[0], h1[1], h1[2], h1[3]);
-        *reinterpret_cast<uint4*>(kh + KBOX + off) = make_uint4(h2[0], h2[1], h2[2], h2[3]);
+        sts128(kh + off, h1[0], h1[1], h1[2], h1[3]);
+        sts128(kh + KBOX + off, h2[0], h2[1], h2[2], h2[3]);
         if (precise) {
-            *reinterpret_cast<uint4*>(kl + off) = make_uint4(l1[0], l1[1], l1[2], l1[3]);
-            *reinterpret_cast<uint4*>(kl + KBOX + off) = make_uint4(l2[0], l2[1], l2[2], l2[3]);
+            sts128(kl + off, l1[0], l1[1], l1[2], l1[3]);
+            sts128(kl + KBOX + off, l2[0], l2[1], l2[2], l2[3]);
         }
     }
 }
