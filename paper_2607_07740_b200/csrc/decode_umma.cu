@@ -30,13 +30,14 @@ constexpr int NH = 16;                               // UMMA N: query heads of o
 constexpr int KS = 2, VS = 2;                        // K / V ring depths; a K stage is K (hi in place) | K lo
 constexpr int BOXB = BN * 128;                       // one SWIZZLE_128B box: 128 rows x 128 B = 16 KB
 constexpr int TILE = 2 * BOXB;                       // 32 KB (channels 0-63 | 64-127)
-constexpr int QBUF = 2 * NH * 128;                   // [2 boxes][16 rows][128 B] = 4 KB
+constexpr int QBUF = 2 * NH * 128;                   // [2 boxes][16 rows][128 B] = 4 KB (raw Q, P)
+constexpr int QCBUF = 2 * 2 * NH * 128;              // [2 boxes][32 rows][128 B] = 8 KB: rows 0-15 Q'hi, rows 16-31 Q'lo
 constexpr int RW = 8;                                // rotate warps
 constexpr int RT = RW * 32;                          // rotate threads
 constexpr int RROWS = 1024 / RT;                     // key rows per rotate thread (8 chunks x 128 rows / RT)
 constexpr int NTHREADS = 64 + RT + 128;
 constexpr float kLog2e = 1.4426950408889634f;
-constexpr uint32_t TM_S = 0, TM_O = 32;              // S0 | S1 | O, 16 fp32 columns each
+constexpr uint32_t TM_S = 0, TM_O = 64;              // S0 | S1 (32 fp32 columns each: K'hi Q'hi | K'hi Q'lo) | O (16)
 
 struct Bars {
     uint64_t k_full[KS], k_ready[KS], k_empty[KS];
@@ -47,8 +48,8 @@ struct Bars {
     float red[4 * NH];                               // cross-warp max / sum exchange of the softmax group
 };
 
-// smem: K ring (K | K lo per stage) | V ring | Q raw | Q' hi | Q' lo | P0 | P1 | Bars
-constexpr size_t OFF_V = (size_t)KS * 2 * TILE, OFF_Q = OFF_V + (size_t)VS * TILE, OFF_P = OFF_Q + 3 * QBUF,
+// smem: K ring (K | K lo per stage) | V ring | Q raw | Q' (hi rows | lo rows) | P0 | P1 | Bars
+constexpr size_t OFF_V = (size_t)KS * 2 * TILE, OFF_Q = OFF_V + (size_t)VS * TILE, OFF_P = OFF_Q + QBUF + QCBUF,
                  OFF_BARS = OFF_P + 2 * QBUF;
 constexpr size_t SMEM_BYTES = 1024 + OFF_BARS + 1024;
 
@@ -62,8 +63,8 @@ struct Params {
 };
 
 // byte offset of element (row n, k) in a [2 boxes][16 rows][128 B] SWIZZLE_128B K-major operand (16-bit elements)
-__device__ __forceinline__ int bop_off(int n, int k) {
-    return (k >> 6) * (NH * 128) + n * 128 + ((((k & 63) >> 3) ^ (n & 7)) << 4) + (k & 7) * 2;
+template <int ROWS = NH> __device__ __forceinline__ int bop_off(int n, int k) {
+    return (k >> 6) * (ROWS * 128) + n * 128 + ((((k & 63) >> 3) ^ (n & 7)) << 4) + (k & 7) * 2;
 }
 
 __device__ __forceinline__ float ex2(float x) {
@@ -89,6 +90,7 @@ __device__ __forceinline__ uint16_t bf16_bits(float f) {
 
 constexpr uint32_t IDESC_S_BF16 = idesc_f16(1, 1, 0, 0, BN, NH);
 constexpr uint32_t IDESC_S_F16 = idesc_f16(0, 0, 0, 0, BN, NH);
+constexpr uint32_t IDESC_S_F16_N32 = idesc_f16(0, 0, 0, 0, BN, 2 * NH);
 constexpr uint32_t IDESC_PV = idesc_f16(1, 1, 1, 0, D, NH);      // A = V^T (smem, MN-major), B = P (smem, K-major)
 
 struct DPlan {
@@ -135,7 +137,7 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
         fence_barrier_init();
         prefetch_tmap(&tmK); prefetch_tmap(&tmV);
     }
-    if (warp == 1) tmem_alloc<64>(&bars->tmem_base);
+    if (warp == 1) tmem_alloc<128>(&bars->tmem_base);
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
@@ -162,7 +164,7 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
         const uint32_t tm = __shfl_sync(0xffffffffu, tmem, 0);
         const uint32_t smem0 = __shfl_sync(0xffffffffu, smem_u32(smem), 0);
         auto issue_s = [&](int v) {
-            const uint32_t dS = tm + TM_S + (v & 1) * NH;
+            const uint32_t dS = tm + TM_S + (v & 1) * 2 * NH;
             const uint32_t ka = smem0 + (v % KS) * 2 * TILE, kla = ka + TILE;
             const uint32_t qa = smem0 + (uint32_t)OFF_Q;
             const bool rem = plan.remote(v);
@@ -173,18 +175,15 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
                         umma_ss(dS, smem_desc_sw128(ka + (ks >> 2) * BOXB + (ks & 3) * 32, 16, 1024),
                                 smem_desc_sw128(qa + (ks >> 2) * (NH * 128) + (ks & 3) * 32, 16, 1024), IDESC_S_BF16, ks > 0);
                 } else {
+                    const uint32_t qc = qa + QBUF;                  // rows 0-15 Q'hi, rows 16-31 Q'lo
 #pragma unroll
-                    for (int ks = 0; ks < D / 16; ++ks)        // K'hi Q'hi
+                    for (int ks = 0; ks < D / 16; ++ks)        // K'hi [Q'hi ; Q'lo]: one pass over the K tile, N = 32
                         umma_ss(dS, smem_desc_sw128(ka + (ks >> 2) * BOXB + (ks & 3) * 32, 16, 1024),
-                                smem_desc_sw128(qa + QBUF + (ks >> 2) * (NH * 128) + (ks & 3) * 32, 16, 1024), IDESC_S_F16, ks > 0);
+                                smem_desc_sw128(qc + (ks >> 2) * (2 * NH * 128) + (ks & 3) * 32, 16, 1024), IDESC_S_F16_N32, ks > 0);
 #pragma unroll
-                    for (int ks = 0; ks < D / 16; ++ks)        // K'lo Q'hi
+                    for (int ks = 0; ks < D / 16; ++ks)        // K'lo Q'hi into columns 0-15
                         umma_ss(dS, smem_desc_sw128(kla + (ks >> 2) * BOXB + (ks & 3) * 32, 16, 1024),
-                                smem_desc_sw128(qa + QBUF + (ks >> 2) * (NH * 128) + (ks & 3) * 32, 16, 1024), IDESC_S_F16, 1);
-#pragma unroll
-                    for (int ks = 0; ks < D / 16; ++ks)        // K'hi Q'lo
-                        umma_ss(dS, smem_desc_sw128(ka + (ks >> 2) * BOXB + (ks & 3) * 32, 16, 1024),
-                                smem_desc_sw128(qa + 2 * QBUF + (ks >> 2) * (NH * 128) + (ks & 3) * 32, 16, 1024), IDESC_S_F16, 1);
+                                smem_desc_sw128(qc + (ks >> 2) * (2 * NH * 128) + (ks & 3) * 32, 16, 1024), IDESC_S_F16, 1);
                 }
                 umma_commit(&bars->s_full[v & 1]);
                 umma_commit(&bars->k_empty[v % KS]);
@@ -227,7 +226,7 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
         const int t = tid - 64;
         const long long qpos = p.L - 1;
         // Q operands [16 heads][128 ch]: raw bf16 for local tiles; Q' = R(Delta q) Q as fp16 hi / lo for remote tiles
-        for (int i = t; i < 3 * QBUF / 4; i += RT) reinterpret_cast<uint32_t*>(sQ)[i] = 0u;
+        for (int i = t; i < (QBUF + QCBUF) / 4; i += RT) reinterpret_cast<uint32_t*>(sQ)[i] = 0u;
         for (int i = t; i < 2 * QBUF / 4; i += RT) reinterpret_cast<uint32_t*>(sP)[i] = 0u;
         named_bar_sync(1, RT);
         const long long nq = qpos - qpos / p.G;                      // -Delta(q) >= 0, Eq.(5)
@@ -243,10 +242,10 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
                 const float x1 = __bfloat162float(b1), x2 = __bfloat162float(b2);
                 const float y1 = x1 * c - x2 * s, y2 = x1 * s + x2 * c;
                 const __half h1 = __float2half_rn(y1), h2 = __float2half_rn(y2);
-                *reinterpret_cast<__half*>(sQ + QBUF + bop_off(h, i)) = h1;
-                *reinterpret_cast<__half*>(sQ + QBUF + bop_off(h, i + 64)) = h2;
-                *reinterpret_cast<__half*>(sQ + 2 * QBUF + bop_off(h, i)) = __float2half_rn(y1 - __half2float(h1));
-                *reinterpret_cast<__half*>(sQ + 2 * QBUF + bop_off(h, i + 64)) = __float2half_rn(y2 - __half2float(h2));
+                *reinterpret_cast<__half*>(sQ + QBUF + bop_off<2 * NH>(h, i)) = h1;
+                *reinterpret_cast<__half*>(sQ + QBUF + bop_off<2 * NH>(h, i + 64)) = h2;
+                *reinterpret_cast<__half*>(sQ + QBUF + bop_off<2 * NH>(NH + h, i)) = __float2half_rn(y1 - __half2float(h1));
+                *reinterpret_cast<__half*>(sQ + QBUF + bop_off<2 * NH>(NH + h, i + 64)) = __float2half_rn(y2 - __half2float(h2));
             }
         }
         fence_proxy_async_smem();
@@ -284,14 +283,16 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
             const bool valid = plan.remote(v) ? (key >= plan.ks && key < plan.re) : (key >= plan.ls && key < plan.ke);
             mbar_wait(&bars->s_full[v & 1], (v >> 1) & 1);
             tc_fence_after();
-            uint32_t sr[16];
-            tmem_ld16(tmem + lane_base + TM_S + (v & 1) * NH, sr);
+            uint32_t sr[32];
+            tmem_ld32(tmem + lane_base + TM_S + (v & 1) * 2 * NH, sr);
             tmem_ld_wait();
+            const bool rem = plan.remote(v);                          // remote: columns 16.. hold the K'hi Q'lo term
             float x[NG];
             bool jump = false;
 #pragma unroll
             for (int h = 0; h < NG; ++h) {
-                x[h] = (valid && h < g) ? __uint_as_float(sr[h]) * sl2 : -INFINITY;
+                const float sc = __uint_as_float(sr[h]) + (rem ? __uint_as_float(sr[NH + h]) : 0.0f);
+                x[h] = (valid && h < g) ? sc * sl2 : -INFINITY;
                 jump |= x[h] > m_ref[h] + 8.0f;                      // lazy rescale: only on a jump of 2^8 (or from -inf)
             }
             if (bar_red_or(2, 128, jump)) {                          // rare; uniform over the 128 threads
@@ -385,7 +386,7 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
     }
     tc_fence_before();
     __syncthreads();
-    if (warp == 1) tmem_dealloc<64>(tmem);
+    if (warp == 1) tmem_dealloc<128>(tmem);
 }
 
 }  // namespace
