@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the libjetlong hot path on synthetic Qwen3-shaped data.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--variant ...] [--no-extras]
 
 A "step" is one bifocal prefill call (scope rows a1-a8) on BASELINE.json configs[1]
 (Qwen3-1.7B-shaped, L=65536, H_q=16, H_kv=8, d=128, w_local=4096, w_pretrained=32768, G=2).
@@ -33,10 +33,11 @@ def flops_causal(L, H_q, d):
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons sampled during the timed region (B200_PROFILING.md)."""
-    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
-         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
-         "clocks_event_reasons.sw_power_cap")
+    """nvidia-smi clocks / throttle reasons; started before the warm-up, samples are kept only if their timestamp
+    falls inside the timed region (B200_PROFILING.md)."""
+    Q = ("timestamp,index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
     def __init__(self, index):
         self.index = index
@@ -46,7 +47,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
-                                          "--format=csv,noheader,nounits", "-lms", "100"], stdout=subprocess.PIPE,
+                                          "--format=csv,noheader,nounits", "-lms", "20"], stdout=subprocess.PIPE,
                                          stderr=subprocess.DEVNULL, text=True)
             self.th = threading.Thread(target=self._read, daemon=True)
             self.th.start()
@@ -55,9 +56,9 @@ class ClockSampler:
 
     def _read(self):
         for line in self.proc.stdout:
-            self.lines.append(line.strip())
+            self.lines.append((time.time(), line.strip()))
 
-    def stop(self):
+    def stop(self, t_begin=None, t_end=None):
         if not self.proc:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
         self.proc.terminate()
@@ -65,21 +66,24 @@ class ClockSampler:
             self.proc.wait(timeout=2)
         except Exception:
             self.proc.kill()
-        sm, mx, pw, reasons = [], [], [], set()
-        for ln in self.lines:
+        sm, mx, pw, reasons, n_all = [], [], [], set(), 0
+        for (tl, ln) in self.lines:
             f = [x.strip() for x in ln.split(",")]
-            if len(f) < 9:
+            if len(f) < 10:
+                continue
+            n_all += 1
+            if t_begin is not None and not (t_begin <= tl <= t_end + 0.05):
                 continue
             try:
-                sm.append(float(f[1])); mx.append(float(f[2])); pw.append(float(f[3]))
+                sm.append(float(f[2])); mx.append(float(f[3])); pw.append(float(f[4]))
             except ValueError:
                 continue
-            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[5:9]):
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[6:10]):
                 if v.lower().startswith("active"):
                     reasons.add(name)
         if not sm:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
-        return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "power_w_max": max(pw),
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples in the timed region (%d outside)" % n_all]}
+        return {"sm_mhz": statistics.median(sm), "sm_min_mhz": min(sm), "sm_max_mhz": max(mx), "power_w_max": max(pw),
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
@@ -124,7 +128,7 @@ def run_reference(args, cfg):
     from paper_2607_07740_b200 import workloads as W
     dev = "cuda" if torch.cuda.is_available() else "cpu"
     Q, K, V = W.make_config_inputs(cfg, dev)
-    n_pairs = 24
+    n_pairs = 512
     vals = []
     for i in range(args.warmup + args.steps):
         r = oracle_sample(cfg, n_pairs, Q, K, V)
@@ -156,9 +160,12 @@ def workload_config(cfg):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--variant", default="bifocal", choices=["bifocal", "fast", "control", "decode", "decode-control"],
+                    help="what the timed loop runs (default: the bifocal prefill in its default, compensated "
+                         "precision); the other values exist for profiling one kernel at a time")
     ap.add_argument("--no-extras", action="store_true", help="skip control / decode / e2e / oracle legs (profiling)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" and not args.no_extras else args.warmup
@@ -187,6 +194,14 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
+    pk = peaks()
+    if args.variant in ("decode", "decode-control"):              # profiling aid: only the decode kernel(s)
+        r = bench_decode(J, B, W, dev, pk, L0=131072, steps=max(args.steps, 8),
+                         only="bifocal" if args.variant == "decode" else "control")
+        if rank == 0:
+            print(json.dumps({"metric": METRIC, "variant": args.variant, "decode": r}))
+        return
+
     Q, K, V = W.make_config_inputs(cfg, dev)
     out = torch.empty_like(Q)
     lse = torch.empty((cfg.H_q, cfg.L), dtype=torch.float32, device=dev)
@@ -194,27 +209,42 @@ def main():
     kw = dict(w_local=cfg.w_local, w_pretrained=cfg.w_pretrained, rope_theta=cfg.rope_theta)
     fl = flops_causal(cfg.L, cfg.H_q, cfg.d)
 
-    def step():
-        J.jetlong_prefill(Q, K, V, out=out, lse=lse, workspace=ws, **kw)
+    def make_step(variant):
+        if variant == "control":
+            return lambda: J.jetlong_causal_prefill(Q, K, V, out=out, lse=lse, workspace=ws)
+        mode = B.PRECISION_FAST if variant == "fast" else B.PRECISION_COMPENSATED
 
-    for _ in range(args.warmup):
-        step()
-    barrier()
+        def f():
+            J.jetlong_set_prefill_precision(mode)
+            J.jetlong_prefill(Q, K, V, out=out, lse=lse, workspace=ws, **kw)
+        return f
+
+    def timed(fn, steps, warmup, sampler=None):
+        """K steps bracketed by barrier + synchronize; CUDA events on the launching (current torch) stream."""
+        for _ in range(warmup):
+            fn()
+        barrier()
+        evs = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
+        barrier()
+        t_begin = time.time()
+        evs[0].record()
+        for i in range(steps):
+            fn()
+            evs[i + 1].record()
+        barrier()
+        t_end = time.time()
+        per = [evs[i].elapsed_time(evs[i + 1]) for i in range(steps)]
+        return evs[0].elapsed_time(evs[-1]), per, (t_begin, t_end)
+
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
+        time.sleep(0.3)                                          # let nvidia-smi start sampling before the region
+    step = make_step(args.variant)
     n0 = J.jetlong_launch_count()
-    evs = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
-    barrier()
-    evs[0].record()
-    for i in range(args.steps):
-        step()
-        evs[i + 1].record()
-    barrier()
-    launches = J.jetlong_launch_count() - n0
-    clocks = sampler.stop() if rank == 0 else None
-    total_ms = evs[0].elapsed_time(evs[-1])
-    per = [evs[i].elapsed_time(evs[i + 1]) for i in range(args.steps)]
+    total_ms, per, (t_begin, t_end) = timed(step, args.steps, args.warmup)
+    launches = (J.jetlong_launch_count() - n0) * args.steps // (args.steps + args.warmup)
+    clocks = sampler.stop(t_begin, t_end) if rank == 0 else None
     t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
     if dist is not None:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
@@ -222,45 +252,50 @@ def main():
     ms_per_step = total_ms / args.steps
     value = world * fl / (ms_per_step * 1e-3) / 1e12
 
+    cfgd = workload_config(cfg)
+    cfgd["variant"] = {"bifocal": "bifocal prefill, default precision (compensated remote QK^T, meets the lse tolerance)",
+                       "fast": "bifocal prefill, JETLONG_PRECISION_FAST (misses the lse tolerance on outlier inputs)",
+                       "control": "matched causal control kernel"}[args.variant]
     line = {"metric": METRIC, "value": value, "unit": "TFLOP/s", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "bf16", "data": "synthetic", "config": workload_config(cfg),
+            "vs_baseline": None, "dtype": "bf16", "data": "synthetic", "config": cfgd,
             "tokens_per_s": world * cfg.L / (ms_per_step * 1e-3), "gpu_launches": int(launches), "clocks": clocks,
             "ms_per_step_min": min(per), "ms_per_step_median": statistics.median(per)}
 
-    pk = peaks()
     if rank == 0 and not args.no_extras:
-        # ---- roofline of the dominant kernel (the prefill kernel is >99% of a step) ---------------------
+        # ---- roofline of the dominant kernel (the prefill kernel is >99.9% of a step, profiles/) ----------
         impl = "tcgen05 UMMA" if _umma_active(B, cfg) else "SIMT fp32 FMA"
-        kern_ms = statistics.median(per)
+        kern_ms = sum(per) / len(per)                             # the step is one prefill kernel + 2 table kernels (~10 us)
         ach = fl / (kern_ms * 1e-3) / 1e12
         traffic = None
         tp = os.path.join(ROOT, "profiles", "traffic.json")
         if os.path.exists(tp):
             traffic = json.load(open(tp)).get("prefill_dram_bytes_per_launch")
         if impl == "tcgen05 UMMA":
-            peak, bound, which = pk["tflops_sustained"], "tensor", "sustained cuBLAS bf16, " + pk["source"]
+            peak, bound = pk["tflops_sustained"], "tensor"
+            which = "sustained cuBLAS bf16 (the kernel is timed back to back for %d steps), %s" % (args.steps, pk["source"])
         else:
-            # fp32 FMA path: 148 SMs x 128 lanes x 2 flop x max SM clock (alu roofline)
             peak, bound, which = 148 * 128 * 2 * 1.965e9 / 1e12, "alu", "148 SM x 128 FMA lanes x 2 x 1965 MHz (derived)"
         line["roofline"] = {"bound": bound, "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
-                            "traffic": traffic, "kernel": "prefill (" + impl + ")", "peak_source": which,
-                            "frac_of_bf16_burst_peak": ach / pk["tflops_burst"],
-                            "frac_of_nominal_2250": ach / 2250.0}
-        # ---- matched control (a10) on the same buffers ---------------------------------------------------
-        wsc = B.alloc_workspace(B.OP_CAUSAL_PREFILL, cfg.L, cfg.H_q, cfg.H_kv, cfg.d, B.BF16, dev)
-        for _ in range(2):
-            J.jetlong_causal_prefill(Q, K, V, out=out, lse=lse, workspace=wsc)
-        torch.cuda.synchronize()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        nrep = max(3, min(args.steps, 10))
-        e0.record()
-        for _ in range(nrep):
-            J.jetlong_causal_prefill(Q, K, V, out=out, lse=lse, workspace=wsc)
-        e1.record()
-        torch.cuda.synchronize()
-        cms = e0.elapsed_time(e1) / nrep
-        line["control"] = {"ms": cms, "tflops": fl / (cms * 1e-3) / 1e12, "bifocal_over_control": cms / ms_per_step}
+                            "traffic": traffic, "kernel": "prefill_umma_kernel (" + impl + ")", "peak_source": which,
+                            "algorithmic_flops_per_launch": fl,
+                            "frac_of_bf16_burst_peak": ach / pk["tflops_burst"], "bf16_burst_peak": pk["tflops_burst"],
+                            "frac_of_nominal_2250": ach / 2250.0,
+                            "note": "FLOPs = 2*d*H_q*L*(L+1); the two extra remote QK^T groups of the default "
+                                    "precision and the straddle revisit are executed but not credited"}
+        # ---- the other prefill variants on the same buffers, interleaved after the main loop ---------------
+        others = {}
+        for name in ("control", "fast", "bifocal"):
+            if name == args.variant:
+                continue
+            tot, pp, _ = timed(make_step(name), max(3, min(args.steps, 10)), 2)
+            ms = tot / len(pp)
+            others[name] = {"ms": ms, "tflops": fl / (ms * 1e-3) / 1e12,
+                            "frac_of_bf16_burst_peak": fl / (ms * 1e-3) / 1e12 / pk["tflops_burst"]}
+        line["prefill_variants"] = others
+        if "control" in others and args.variant != "control":
+            line["control"] = dict(others["control"], bifocal_over_control=others["control"]["ms"] / ms_per_step)
+        J.jetlong_set_prefill_precision(B.PRECISION_COMPENSATED)
         # ---- end to end through the host-buffer C-ABI call -----------------------------------------------
         Qh, Kh, Vh = Q.cpu().pin_memory(), K.cpu().pin_memory(), V.cpu().pin_memory()
         oh = torch.empty_like(Qh).pin_memory()
@@ -276,10 +311,11 @@ def main():
                        "d2h_bytes_per_step": oh.numel() * 2 + lh.numel() * 4,
                        "api": "jetlong_prefill_host (pinned host buffers; cudaMalloc + H2D + kernels + D2H + sync)"}
         del Qh, Kh, Vh, oh, lh
-        # ---- decode (a9): config 5 at L0 = 131072 ---------------------------------------------------------
-        line["decode"] = bench_decode(J, B, W, dev, pk)
+        # ---- decode (a9): config 5 at both cache lengths -------------------------------------------------
+        line["decode"] = bench_decode(J, B, W, dev, pk, L0=131072, steps=256)
+        line["decode_64k"] = bench_decode(J, B, W, dev, pk, L0=65536, steps=256)
         # ---- the CPU oracle on a bounded sample ---------------------------------------------------------
-        cb = oracle_sample(cfg, 24, Q, K, V)
+        cb = oracle_sample(cfg, 3072, Q, K, V)
         cb.pop("seconds")
         line["cpu_baseline"] = cb
     if rank == 0:
@@ -296,14 +332,20 @@ def _umma_active(B, cfg):
         return False
 
 
-def bench_decode(J, B, W, dev, pk, L0=131072, steps=64):
+def bench_decode(J, B, W, dev, pk, L0=131072, steps=256, only=None):
+    """Config 5: `steps` consecutive decode steps, step t at L = L0 + t (G is recomputed from L each step, R14).
+    KV-read GB/s = 2*L*H_kv*d*2 B / step time; the cache (268 / 537 MB) exceeds the 126 MB L2."""
     c = W.C5
     Qs, Kc, Vc = W.make_decode_inputs(c, L0, steps, dev)
     ws = B.alloc_workspace(B.OP_DECODE, L0 + steps, c.H_q, c.H_kv, c.d, B.BF16, dev)
     o = torch.empty((c.H_q, c.d), dtype=torch.bfloat16, device=dev)
     l = torch.empty((c.H_q,), dtype=torch.float32, device=dev)
     res = {}
+    kv_bytes = 2.0 * (L0 + (steps - 1) / 2) * c.H_kv * c.d * 2
     for name in ("bifocal", "control"):
+        if only and name != only:
+            continue
+
         def run(t):
             if name == "bifocal":
                 J.jetlong_decode(Qs[t], Kc, Vc, L0 + t, w_local=c.w_local, w_pretrained=c.w_pretrained,
@@ -314,19 +356,37 @@ def bench_decode(J, B, W, dev, pk, L0=131072, steps=64):
             run(t)
         torch.cuda.synchronize()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        n0 = J.jetlong_launch_count()
         e0.record()
         for t in range(steps):
             run(t)
         e1.record()
         torch.cuda.synchronize()
         us = e0.elapsed_time(e1) / steps * 1e3
-        kv_bytes = 2.0 * (L0 + steps / 2) * c.H_kv * c.d * 2
         res[name] = {"us_per_step": us, "kv_read_gbs": kv_bytes / (us * 1e-6) / 1e9,
-                     "frac_hbm_peak": kv_bytes / (us * 1e-6) / 1e9 / pk["hbm_gbs"]}
+                     "frac_hbm_peak": kv_bytes / (us * 1e-6) / 1e9 / pk["hbm_gbs"],
+                     "launches_per_step": (J.jetlong_launch_count() - n0) / steps}
+        # the same steps replayed from one CUDA graph (the paper measures decode under CUDA graphs)
+        try:
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g):
+                for t in range(steps):
+                    run(t)
+            g.replay()
+            torch.cuda.synchronize()
+            e0.record()
+            g.replay()
+            e1.record()
+            torch.cuda.synchronize()
+            gus = e0.elapsed_time(e1) / steps * 1e3
+            res[name]["cuda_graph"] = {"us_per_step": gus, "kv_read_gbs": kv_bytes / (gus * 1e-6) / 1e9,
+                                       "frac_hbm_peak": kv_bytes / (gus * 1e-6) / 1e9 / pk["hbm_gbs"]}
+        except Exception as e:                                     # capture is an extra, never the headline
+            res[name]["cuda_graph"] = {"unavailable": str(e)[:120]}
     res["workload"] = "BASELINE.json configs[4]: Qwen3-8B-shaped batch-1 decode, L0=%d, %d steps, KV cache %.0f MB > L2" % (
         L0, steps, 2.0 * L0 * c.H_kv * c.d * 2 / 1e6)
-    res["hbm_peak_gbs"] = pk["hbm_gbs"]
-    res["peak_source"] = pk["source"]
+    res["roofline"] = {"bound": "hbm", "unit": "GB/s", "peak": pk["hbm_gbs"], "peak_source": pk["source"],
+                       "algorithmic_bytes_per_step": kv_bytes, "kernel": "decode_umma_kernel"}
     return res
 
 
