@@ -105,12 +105,16 @@ int64_t jetlong_launch_count(void);
  * jetlong_set_prefill_impl(-1) restores the default. Returns the previous value. */
 int jetlong_set_prefill_impl(int impl);
 
-/* Operand precision of the REMOTE Q'K'^T on the tcgen05 path.
- * COMPENSATED (default): rotated operands split hi + lo in fp16, S = Q'hi K'hi + Q'hi K'lo + Q'lo K'hi; meets the
- * lse tolerance (1e-3) on outlier-channel inputs.  FAST: Q'hi K'hi only (one UMMA group instead of three);
- * lse errors up to ~2.5e-3 on such inputs.  Local tiles, the control and decode are unaffected.
+/* Operand precision of the REMOTE Q'K'^T on the tcgen05 prefill path.  Rotated operands must be
+ * re-rounded for the tensor core; with one fp16 rounding (11 bits) the lse error reaches ~3e-3 on outlier-channel
+ * inputs (tolerance 1e-3).  With y = hi + lo (hi = fp16(y), lo = y - hi):
+ *   COMPENSATED (default): S = Q'hi K'hi (fp16 UMMA) + Q' K'lo + Q'lo K' with the two cross terms in e5m2
+ *                          (kind::f8f6f4, half the tensor cycles of fp16); lse error ~2e-4.
+ *   COMPENSATED_F16:       the two cross terms in fp16 as well (three fp16 UMMA groups); lse error ~1e-5.
+ *   FAST:                  Q'hi K'hi only; lse error up to ~3e-3 on such inputs (out still within tolerance).
+ * Local tiles, the control and decode are unaffected (decode always uses the fp16 cross terms).
  * Returns the previous mode; an unknown mode changes nothing. */
-enum { JETLONG_PRECISION_COMPENSATED = 0, JETLONG_PRECISION_FAST = 1 };
+enum { JETLONG_PRECISION_COMPENSATED = 0, JETLONG_PRECISION_FAST = 1, JETLONG_PRECISION_COMPENSATED_F16 = 2 };
 int jetlong_set_prefill_precision(int mode);
 
 /* 1 if a bf16 prefill of these shapes runs on the tcgen05 UMMA kernel under the current setting, else 0. */

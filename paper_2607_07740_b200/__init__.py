@@ -2,4 +2,4 @@
 from .binding import (BF16, FP32, JetlongError, jetlong_causal_decode, jetlong_causal_prefill,  # noqa: F401
                       jetlong_decode, jetlong_group_size, jetlong_launch_count, jetlong_prefill,
                       jetlong_prefill_host, jetlong_set_prefill_impl, jetlong_set_prefill_precision,
-                      jetlong_workspace_bytes, PRECISION_COMPENSATED, PRECISION_FAST)
+                      jetlong_workspace_bytes, PRECISION_COMPENSATED, PRECISION_COMPENSATED_F16, PRECISION_FAST)

@@ -25,7 +25,7 @@ int check_launch(const char* what) {
 bool umma_prefill_supported(long long L, int H_q, int H_kv, int d, int dtype);
 size_t umma_prefill_workspace_bytes(long long L, int H_q, int H_kv, int d);
 int launch_prefill_umma(const void* Q, const void* K, const void* V, void* out, float* lse, long long L, int H_q,
-                        int H_kv, int d, long long w0, long long G, double theta, bool bifocal, bool precise, void* ws,
+                        int H_kv, int d, long long w0, long long G, double theta, bool bifocal, int precise, void* ws,
                         size_t ws_bytes, cudaStream_t st);
 
 static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; }
@@ -76,9 +76,10 @@ static int prefill_common(const void* Q, const void* K, const void* V, void* out
     rc = device_ok();
     if (rc != JETLONG_OK) return rc;
     cudaStream_t st = (cudaStream_t)stream;
+    const int prec = g_prefill_precision.load();
     if (use_umma(L, H_q, H_kv, d, dtype))
         return launch_prefill_umma(Q, K, V, out, lse, L, H_q, H_kv, d, w0, G, theta, bifocal,
-                                   g_prefill_precision.load() != JETLONG_PRECISION_FAST, ws, ws_bytes, st);
+                                   prec == JETLONG_PRECISION_FAST ? 0 : (prec == JETLONG_PRECISION_COMPENSATED_F16 ? 1 : 2), ws, ws_bytes, st);
     const float2* tab = nullptr;
     if (bifocal) {
         rc = build_key_table((float2*)ws, L, G, d, theta, st);
@@ -196,7 +197,8 @@ int64_t jetlong_launch_count(void) { return g_launches.load(); }
 int jetlong_set_prefill_impl(int impl) { return g_prefill_impl.exchange(impl); }
 
 int jetlong_set_prefill_precision(int mode) {
-    if (mode != JETLONG_PRECISION_COMPENSATED && mode != JETLONG_PRECISION_FAST) return g_prefill_precision.load();
+    if (mode != JETLONG_PRECISION_COMPENSATED && mode != JETLONG_PRECISION_FAST && mode != JETLONG_PRECISION_COMPENSATED_F16)
+        return g_prefill_precision.load();
     return g_prefill_precision.exchange(mode);
 }
 

@@ -46,6 +46,7 @@ constexpr int STAGE_BYTES = 2 * KH_BYTES + VH_BYTES;  // K (hi in place) | K lo 
 constexpr int NTHREADS = 448;
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr uint32_t TM_S = 0, TM_O = 256, TM_QA = 384, TM_QB = 448;
+constexpr uint32_t TM_QY = 448, TM_QR = 480;         // precision mode 2: Q' and Q' lo as e5m2 (32 columns each) in place of Qb
 
 struct Bars {
     uint64_t kv_full[NS];      // local: TMA bytes of this CTA's K/V halves landed
@@ -110,7 +111,7 @@ __device__ __forceinline__ void stage_q_raw(const __nv_bfloat16* qrow, bool vali
 }
 __device__ __forceinline__ void stage_q_rot(const __nv_bfloat16* qrow, bool valid, long long q, long long G,
                                             const float2* __restrict__ lo, const float2* __restrict__ hi,
-                                            uint32_t tQa, uint32_t tQb) {
+                                            uint32_t tQa, uint32_t tQb, int precise) {
 #pragma unroll 2
     for (int j = 0; j < 8; ++j) {                         // channels 8j..8j+7 and 64+8j..
         uint4 u1 = make_uint4(0, 0, 0, 0), u2 = u1;
@@ -125,13 +126,21 @@ __device__ __forceinline__ void stage_q_rot(const __nv_bfloat16* qrow, bool vali
         rot8(a, b, cs_c, cs_s, h1, h2, l1, l2);
         tmem_st4(tQa + 4 * j, h1[0], h1[1], h1[2], h1[3]);
         tmem_st4(tQa + 32 + 4 * j, h2[0], h2[1], h2[2], h2[3]);
-        tmem_st4(tQb + 4 * j, l1[0], l1[1], l1[2], l1[3]);
-        tmem_st4(tQb + 32 + 4 * j, l2[0], l2[1], l2[2], l2[3]);
+        if (precise == 2) {                                   // e5m2 copies: column c of QY / QR holds channels 4c..4c+3
+            tmem_st2(tQb + 2 * j, e5m2x4(h1[0], h1[1]), e5m2x4(h1[2], h1[3]));
+            tmem_st2(tQb + 16 + 2 * j, e5m2x4(h2[0], h2[1]), e5m2x4(h2[2], h2[3]));
+            tmem_st2(tQb + 32 + 2 * j, e5m2x4(l1[0], l1[1]), e5m2x4(l1[2], l1[3]));
+            tmem_st2(tQb + 48 + 2 * j, e5m2x4(l2[0], l2[1]), e5m2x4(l2[2], l2[3]));
+        } else {
+            tmem_st4(tQb + 4 * j, l1[0], l1[1], l1[2], l1[3]);
+            tmem_st4(tQb + 32 + 4 * j, l2[0], l2[1], l2[2], l2[3]);
+        }
     }
 }
 
 constexpr uint32_t IDESC_QK_BF16 = idesc_f16(1, 1, 0, 0, 2 * BM, BN);
 constexpr uint32_t IDESC_QK_F16 = idesc_f16(0, 0, 0, 0, 2 * BM, BN);
+constexpr uint32_t IDESC_QK_E5M2 = idesc_f16(1, 1, 0, 0, 2 * BM, BN);   // kind::f8f6f4: format code 1 = e5m2
 constexpr uint32_t IDESC_PV = idesc_f16(1, 1, 0, 1, 2 * BM, D);  // A = P (TMEM, bf16), B = V (smem, MN-major)
 
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1)
@@ -154,7 +163,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_consta
     const int kvh = h0 / p.g;
     const long long q0 = (long long)qb * BM;
     const bool bifocal = p.bifocal != 0;
-    const bool precise = p.precise != 0;
+    const int precise = p.precise;                                // 0 fast, 1 fp16 cross terms, 2 e5m2 cross terms
     const Plan plan(qb, p.w0, bifocal);
 
     if (tid == 0) {
@@ -207,7 +216,16 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_consta
                         for (int ks = 0; ks < D / 16; ++ks)
                             umma2_ts(dS, tm + TM_QA + ks * 8,
                                      smem_desc_sw128(kb + (ks >> 2) * KBOX + (ks & 3) * 32, 16, 1024), IDESC_QK_F16, ks > 0);
-                        if (precise) {
+                        if (precise == 2) {
+#pragma unroll
+                            for (int ks = 0; ks < D / 32; ++ks)      // Q' (e5m2) . K' lo (e5m2)
+                                umma2_ts_f8(dS, tm + TM_QY + ks * 8, smem_desc_sw128(klb + KBOX + ks * 32, 16, 1024),
+                                            IDESC_QK_E5M2, 1);
+#pragma unroll
+                            for (int ks = 0; ks < D / 32; ++ks)      // Q' lo (e5m2) . K' (e5m2)
+                                umma2_ts_f8(dS, tm + TM_QR + ks * 8, smem_desc_sw128(klb + ks * 32, 16, 1024),
+                                            IDESC_QK_E5M2, 1);
+                        } else if (precise == 1) {
 #pragma unroll
                             for (int ks = 0; ks < D / 16; ++ks)
                                 umma2_ts(dS, tm + TM_QA + ks * 8,
@@ -278,7 +296,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_consta
                 if (v == plan.n_local) {                              // first remote visit: Q -> Q' = R(Delta q) Q
                     mbar_wait(&bars->q_local_done, 0);
                     tc_fence_after();
-                    stage_q_rot(qrow, valid, q, p.G, p.lo, p.hi, tmem + lane_base + TM_QA, tmem + lane_base + TM_QB);
+                    stage_q_rot(qrow, valid, q, p.G, p.lo, p.hi, tmem + lane_base + TM_QA, tmem + lane_base + TM_QB, precise);
                     tmem_st_wait();
                     tc_fence_before();
                 }
@@ -480,7 +498,7 @@ bool umma_prefill_supported(long long L, int H_q, int H_kv, int d, int dtype) {
 size_t umma_prefill_workspace_bytes(long long L, int, int, int d) { return two_level_bytes(L + 256, d); }
 
 int launch_prefill_umma(const void* Q, const void* K, const void* V, void* out, float* lse, long long L, int H_q,
-                        int H_kv, int d, long long w0, long long G, double theta, bool bifocal, bool precise, void* ws,
+                        int H_kv, int d, long long w0, long long G, double theta, bool bifocal, int precise, void* ws,
                         size_t ws_bytes, cudaStream_t st) {
     (void)ws_bytes;
     CUtensorMap tmK, tmV;
@@ -492,7 +510,7 @@ int launch_prefill_umma(const void* Q, const void* K, const void* V, void* out, 
     p.L = L; p.w0 = w0; p.G = G;
     p.H_q = H_q; p.H_kv = H_kv; p.g = H_q / H_kv;
     p.bifocal = bifocal ? 1 : 0;
-    p.precise = precise ? 1 : 0;
+    p.precise = precise;
     p.lo = nullptr; p.hi = nullptr;
     if (bifocal) {
         int rc = build_two_level(ws, L + 256, d, theta, st);

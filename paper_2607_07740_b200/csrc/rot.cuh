@@ -146,6 +146,14 @@ __device__ __forceinline__ void split_hi_lo(uint64_t y, uint32_t& h, uint32_t& l
     }
 }
 
+// four e5m2 bytes from two fp16x2 words: e5m2 is the top byte of fp16 (same exponent bias); +0x80 rounds to nearest
+__device__ __forceinline__ uint32_t e5m2x4(uint32_t w0, uint32_t w1) {
+    return __byte_perm(w0 + 0x00800080u, w1 + 0x00800080u, 0x7531);
+}
+__device__ __forceinline__ void sts64(uint32_t a, uint32_t x, uint32_t y) {
+    asm volatile("st.shared.v2.u32 [%0], {%1,%2};" ::"r"(a), "r"(x), "r"(y) : "memory");
+}
+
 // explicit shared-space 128-bit accesses (pointers that pass through lambdas degrade to generic LD/ST otherwise)
 __device__ __forceinline__ uint4 lds128(uint32_t a) {
     uint4 v;
@@ -158,7 +166,9 @@ __device__ __forceinline__ void sts128(uint32_t a, uint32_t x, uint32_t y, uint3
 
 template <int ROWS, int KBOX>
 __device__ __forceinline__ void rotate_k_rows(uint32_t kh, uint32_t kl, unsigned pos0, KRot<ROWS>& R,
-                                              bool precise) {   // kh, kl: shared-space addresses
+                                              int precise) {   // kh, kl: shared-space addresses
+    // precise: 0 = hi only; 1 = fp16 lo at kl (same layout as kh); 2 = e5m2 copies for the cross terms at kl:
+    //          [box of KBOX bytes: K' as e5m2, rows x 128 channels][box: K' lo as e5m2], SWIZZLE_128B
     // first-row (cos, sin) from the prefetched table entries: HI * LO as complex numbers
     uint64_t cc[4], cs[4];
 #pragma unroll
@@ -192,14 +202,22 @@ __device__ __forceinline__ void rotate_k_rows(uint32_t kh, uint32_t kl, unsigned
             const uint64_t x1 = bf16x2_to_f32x2(a[j]), x2 = bf16x2_to_f32x2(b[j]);
             const uint64_t y1 = ffma2(neg2(x2), cs[j], fmul2(x1, cc[j]));      // x1 c - x2 s
             const uint64_t y2 = ffma2(x1, cs[j], fmul2(x2, cc[j]));            // x1 s + x2 c
-            split_hi_lo(y1, h1[j], l1[j], precise);
-            split_hi_lo(y2, h2[j], l2[j], precise);
+            split_hi_lo(y1, h1[j], l1[j], precise != 0);
+            split_hi_lo(y2, h2[j], l2[j], precise != 0);
         }
         sts128(kh + off, h1[0], h1[1], h1[2], h1[3]);
         sts128(kh + KBOX + off, h2[0], h2[1], h2[2], h2[3]);
-        if (precise) {
+        if (precise == 1) {
             sts128(kl + off, l1[0], l1[1], l1[2], l1[3]);
             sts128(kl + KBOX + off, l2[0], l2[1], l2[2], l2[3]);
+        } else if (precise == 2) {
+            // byte b of an e5m2 row is channel b: channels 8c.. sit in 16-byte chunk c/2, channels 64+8c.. in chunk 4+c/2
+            const uint32_t o1 = r * 128 + ((((R.c >> 1)) ^ (r & 7)) << 4) + (R.c & 1) * 8;
+            const uint32_t o2 = r * 128 + (((4 + (R.c >> 1)) ^ (r & 7)) << 4) + (R.c & 1) * 8;
+            sts64(kl + o1, e5m2x4(h1[0], h1[1]), e5m2x4(h1[2], h1[3]));
+            sts64(kl + o2, e5m2x4(h2[0], h2[1]), e5m2x4(h2[2], h2[3]));
+            sts64(kl + KBOX + o1, e5m2x4(l1[0], l1[1]), e5m2x4(l1[2], l1[3]));
+            sts64(kl + KBOX + o2, e5m2x4(l2[0], l2[1]), e5m2x4(l2[2], l2[3]));
         }
     }
 }
