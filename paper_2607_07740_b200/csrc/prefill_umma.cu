@@ -45,6 +45,9 @@ constexpr int VH_BYTES = BN * 64 * 2;                 // this CTA's 64 channels 
 constexpr int STAGE_BYTES = 2 * KH_BYTES + VH_BYTES;  // K (hi in place) | K lo | V
 constexpr int NTHREADS = 448;
 constexpr float kLog2e = 1.4426950408889634f;
+constexpr int POLY_OF_4 = 0;                          // of every 4 exponential pairs, this many use the FMA-pipe polynomial.
+// Measured on C2 (same box, back to back): 0 -> 25.5 ms, 1 -> 25.4 ms, 2 -> 27.2 ms (default precision); the kernel runs
+// under the power cap (~1.45 GHz), where extra FMA instructions cost more clock than the freed MUFU cycles return.
 constexpr uint32_t TM_S = 0, TM_O = 256, TM_QA = 384, TM_QB = 448;
 constexpr uint32_t TM_QY = 448, TM_QR = 480;         // precision mode 2: Q' and Q' lo as e5m2 (32 columns each) in place of Qb
 
@@ -135,6 +138,27 @@ __device__ __forceinline__ void stage_q_rot(const __nv_bfloat16* qrow, bool vali
             tmem_st4(tQb + 4 * j, l1[0], l1[1], l1[2], l1[3]);
             tmem_st4(tQb + 32 + 4 * j, l2[0], l2[1], l2[2], l2[3]);
         }
+    }
+}
+
+// p = exp2(s * sl2 - m) for 32 scores of a row, packed row sums, bf16 P words.  POLY: of every 4 pairs, POLY_OF_4
+// use the FMA-pipe polynomial instead of MUFU.EX2 (never on masked tiles, whose -inf entries need MUFU semantics).
+template <bool POLY>
+__device__ __forceinline__ void exp_block(const uint32_t (&sx)[32], uint64_t sl2x2, uint64_t mneg2, uint64_t& l2a,
+                                          uint64_t& l2b, uint32_t (&pk)[16]) {
+#pragma unroll
+    for (int j = 0; j < 32; j += 2) {
+        const uint64_t xx = ffma2(pack2(__uint_as_float(sx[j]), __uint_as_float(sx[j + 1])), sl2x2, mneg2);
+        float p0, p1;
+        if (POLY && (j & 6) < 2 * POLY_OF_4) {
+            exp2_poly2(xx, p0, p1);
+        } else {
+            float x0, x1;
+            unpack2(xx, x0, x1);
+            p0 = ex2(x0); p1 = ex2(x1);
+        }
+        if (j & 2) l2b = fadd2(l2b, pack2(p0, p1)); else l2a = fadd2(l2a, pack2(p0, p1));
+        pk[j >> 1] = bf16x2(p0, p1);
     }
 }
 
@@ -398,23 +422,9 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_consta
             const float mneg = (m_ref == -INFINITY) ? 0.f : -m_ref;
             const uint64_t mneg2 = pack2(mneg, mneg);
             uint32_t pk[16];
-#pragma unroll
-            for (int j = 0; j < 32; j += 2) {
-                float x0, x1;
-                unpack2(ffma2(pack2(__uint_as_float(sa[j]), __uint_as_float(sa[j + 1])), sl2x2, mneg2), x0, x1);
-                const float p0 = ex2(x0), p1 = ex2(x1);
-                if (j & 2) l2b = fadd2(l2b, pack2(p0, p1)); else l2a = fadd2(l2a, pack2(p0, p1));
-                pk[j >> 1] = bf16x2(p0, p1);
-            }
+            if (masked) exp_block<false>(sa, sl2x2, mneg2, l2a, l2b, pk); else exp_block<true>(sa, sl2x2, mneg2, l2a, l2b, pk);
             tmem_st16(tS + 32 * half, pk);
-#pragma unroll
-            for (int j = 0; j < 32; j += 2) {
-                float x0, x1;
-                unpack2(ffma2(pack2(__uint_as_float(sb[j]), __uint_as_float(sb[j + 1])), sl2x2, mneg2), x0, x1);
-                const float p0 = ex2(x0), p1 = ex2(x1);
-                if (j & 2) l2b = fadd2(l2b, pack2(p0, p1)); else l2a = fadd2(l2a, pack2(p0, p1));
-                pk[j >> 1] = bf16x2(p0, p1);
-            }
+            if (masked) exp_block<false>(sb, sl2x2, mneg2, l2a, l2b, pk); else exp_block<true>(sb, sl2x2, mneg2, l2a, l2b, pk);
             tmem_st16(tS + 32 * half + 16, pk);
             tmem_st_wait();
             tc_fence_before();

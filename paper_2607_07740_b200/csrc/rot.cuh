@@ -43,6 +43,31 @@ __device__ __forceinline__ uint64_t fmul2(uint64_t a, uint64_t b) {
     asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(y) : "l"(a), "l"(b));
     return y;
 }
+__device__ __forceinline__ uint64_t fsub2(uint64_t a, uint64_t b) {
+    uint64_t y;
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(y) : "l"(a), "l"(b));
+    return y;
+}
+// 2^x for two values on the FMA/ALU pipes (no MUFU): x = n + f, n = round(x), f in [-0.5, 0.5];
+// 2^f by a degree-3 minimax polynomial (max relative error 7.5e-5), 2^n by adding n to the exponent field.
+// Valid for -126 <= x < 128 after the clamp; used for half of the softmax exponentials so the 16/clk/SM MUFU
+// pipe stops being the limiter.
+__device__ __forceinline__ void exp2_poly2(uint64_t x2, float& r0, float& r1) {
+    float x0, x1;
+    unpack2(x2, x0, x1);
+    const uint64_t xc = pack2(fmaxf(x0, -126.0f), fmaxf(x1, -126.0f));
+    const uint64_t MAG = pack2(12582912.0f, 12582912.0f);              // 1.5 * 2^23: the add rounds x to an integer
+    const uint64_t t = fadd2(xc, MAG);
+    const uint64_t f = fsub2(xc, fsub2(t, MAG));
+    uint64_t pl = ffma2(pack2(5.517165290e-02f, 5.517165290e-02f), f, pack2(2.426111210e-01f, 2.426111210e-01f));
+    pl = ffma2(pl, f, pack2(6.932609884e-01f, 6.932609884e-01f));
+    pl = ffma2(pl, f, pack2(9.999280737e-01f, 9.999280737e-01f));
+    float p0, p1, t0, t1;
+    unpack2(pl, p0, p1);
+    unpack2(t, t0, t1);
+    r0 = __uint_as_float(__float_as_uint(p0) + (__float_as_uint(t0) << 23));
+    r1 = __uint_as_float(__float_as_uint(p1) + (__float_as_uint(t1) << 23));
+}
 __device__ __forceinline__ uint32_t bf16x2(float lo, float hi) {
     uint32_t y;
     asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(y) : "f"(hi), "f"(lo));
