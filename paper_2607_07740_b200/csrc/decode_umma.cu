@@ -9,7 +9,9 @@
 // Remote tiles (k < L-1-w0): the rotate group turns the TMA-loaded K tile into K' = R(Delta k) K in shared memory
 // (fp32 rotate, fp16 hi in place + fp16 lo in a side buffer), Q' = R(Delta q) Q is prepared once per CTA, and
 // S^T = K'hi Q'hi + K'lo Q'hi + K'hi Q'lo (compensated; the MMAs are ~free here).  The cache is only read.
-// Warp roles (448 threads): warp 0 TMA producer, warp 1 MMA issuer, warps 2-9 rotate group, warps 10-13 softmax.
+// S^T = K'hi [Q'hi; Q'lo] (fp16, one pass over the K tile, N = 32) + K'lo Q'hi (e5m2, kind::f8f6f4).
+// Warp roles (480 threads): warp 0 K producer (TMA), warp 1 MMA issuer, warp 2 V producer (TMA), warps 3-10 rotate
+// group, warps 11-14 softmax.
 // Partial (m, l, O) states go to the workspace and are merged by decode_merge_kernel (additive LSE merge).
 #include <cuda.h>
 #include <math.h>
@@ -27,15 +29,17 @@ using namespace dev;
 
 constexpr int D = 128, BN = 128;
 constexpr int NH = 16;                               // UMMA N: query heads of one KV group, zero padded
-constexpr int KS = 2, VS = 2;                        // K / V ring depths; a K stage is K (hi in place) | K lo
+constexpr int KS = 3, VS = 2;                        // K / V ring depths; a K stage is K (hi in place) | K lo (e5m2)
 constexpr int BOXB = BN * 128;                       // one SWIZZLE_128B box: 128 rows x 128 B = 16 KB
 constexpr int TILE = 2 * BOXB;                       // 32 KB (channels 0-63 | 64-127)
+constexpr int KSTAGE = TILE + BOXB;                  // K tile + its e5m2 lo copy [128 rows][128 B]: 48 KB
 constexpr int QBUF = 2 * NH * 128;                   // [2 boxes][16 rows][128 B] = 4 KB (raw Q, P)
 constexpr int QCBUF = 2 * 2 * NH * 128;              // [2 boxes][32 rows][128 B] = 8 KB: rows 0-15 Q'hi, rows 16-31 Q'lo
+constexpr int QYBUF = NH * 128;                      // [16 rows][128 B] = 2 KB: Q'hi as e5m2
 constexpr int RW = 8;                                // rotate warps
 constexpr int RT = RW * 32;                          // rotate threads
 constexpr int RROWS = 1024 / RT;                     // key rows per rotate thread (8 chunks x 128 rows / RT)
-constexpr int NTHREADS = 64 + RT + 128;
+constexpr int NTHREADS = 96 + RT + 128;             // warps: 0 K producer, 1 MMA, 2 V producer, 3.. rotate, last 4 softmax
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr uint32_t TM_S = 0, TM_O = 64;              // S0 | S1 (32 fp32 columns each: K'hi Q'hi | K'hi Q'lo) | O (16)
 
@@ -48,10 +52,11 @@ struct Bars {
     float red[4 * NH];                               // cross-warp max / sum exchange of the softmax group
 };
 
-// smem: K ring (K | K lo per stage) | V ring | Q raw | Q' (hi rows | lo rows) | P0 | P1 | Bars
-constexpr size_t OFF_V = (size_t)KS * 2 * TILE, OFF_Q = OFF_V + (size_t)VS * TILE, OFF_P = OFF_Q + QBUF + QCBUF,
-                 OFF_BARS = OFF_P + 2 * QBUF;
-constexpr size_t SMEM_BYTES = 1024 + OFF_BARS + 1024;
+// smem: K ring (K | K lo e5m2 per stage) | V ring | Q raw | Q' (hi rows | lo rows) | Q'hi e5m2 | P | Bars
+constexpr size_t OFF_V = (size_t)KS * KSTAGE, OFF_Q = OFF_V + (size_t)VS * TILE, OFF_P = OFF_Q + QBUF + QCBUF + QYBUF,
+                 OFF_BARS = OFF_P + QBUF;
+constexpr size_t SMEM_BYTES = OFF_BARS + 1024;       // = 227 KB exactly; the dynamic smem base must be 1024-aligned
+static_assert(SMEM_BYTES <= 232448, "shared memory budget");
 
 struct Params {
     const __nv_bfloat16* q;
@@ -91,6 +96,7 @@ __device__ __forceinline__ uint16_t bf16_bits(float f) {
 constexpr uint32_t IDESC_S_BF16 = idesc_f16(1, 1, 0, 0, BN, NH);
 constexpr uint32_t IDESC_S_F16 = idesc_f16(0, 0, 0, 0, BN, NH);
 constexpr uint32_t IDESC_S_F16_N32 = idesc_f16(0, 0, 0, 0, BN, 2 * NH);
+constexpr uint32_t IDESC_S_E5M2 = idesc_f16(1, 1, 0, 0, BN, NH);  // kind::f8f6f4: format code 1 = e5m2
 constexpr uint32_t IDESC_PV = idesc_f16(1, 1, 1, 0, D, NH);      // A = V^T (smem, MN-major), B = P (smem, K-major)
 
 struct DPlan {
@@ -116,12 +122,12 @@ struct DPlan {
 template <int NG>                                    // NG = query heads per KV head, rounded up to a power of two
 __global__ void __launch_bounds__(NTHREADS, 1)
 decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV, const Params p) {
-    extern __shared__ unsigned char smem_raw[];
-    unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    extern __shared__ __align__(1024) unsigned char smem[];
+    if ((smem_u32(smem) & 1023u) != 0) __trap();               // SWIZZLE_128B operands need the 1024-byte alignment
     unsigned char* sQ = smem + OFF_Q;                              // raw | hi | lo
-    unsigned char* sP = smem + OFF_P;                              // P0 | P1
+    unsigned char* sP = smem + OFF_P;
     Bars* bars = reinterpret_cast<Bars*>(smem + OFF_BARS);
-    auto sK = [&](int s) { return smem + (size_t)s * 2 * TILE; };                // K lo of the stage sits at + TILE
+    auto sK = [&](int s) { return smem + (size_t)s * KSTAGE; };                  // K lo (e5m2) of the stage sits at + TILE
     auto sV = [&](int s) { return smem + OFF_V + (size_t)s * TILE; };
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -148,11 +154,20 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
         if (lane == 0) {
             for (int v = 0; v < plan.nv; ++v) {
                 const int row0 = plan.kt(v) * BN;
-                const int s = v % KS, sv = v % VS;
+                const int s = v % KS;
                 if (v >= KS) mbar_wait(&bars->k_empty[s], ((v / KS) - 1) & 1);
                 mbar_arrive_expect_tx(&bars->k_full[s], TILE);
                 tma_load_3d(sK(s), &tmK, &bars->k_full[s], 0, kvh, row0);
                 tma_load_3d(sK(s) + BOXB, &tmK, &bars->k_full[s], 64, kvh, row0);
+            }
+        }
+    } else if (warp == 2) {
+        // ===================== TMA producer for V (its own thread: a V stage lives until O += V^T P of its visit,
+        // much longer than a K stage, and must not hold back the K loads) =====================
+        if (lane == 0) {
+            for (int v = 0; v < plan.nv; ++v) {
+                const int row0 = plan.kt(v) * BN;
+                const int sv = v % VS;
                 if (v >= VS) mbar_wait(&bars->v_empty[sv], ((v / VS) - 1) & 1);
                 mbar_arrive_expect_tx(&bars->v_full[sv], TILE);
                 tma_load_3d(sV(sv), &tmV, &bars->v_full[sv], 0, kvh, row0);
@@ -165,7 +180,7 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
         const uint32_t smem0 = __shfl_sync(0xffffffffu, smem_u32(smem), 0);
         auto issue_s = [&](int v) {
             const uint32_t dS = tm + TM_S + (v & 1) * 2 * NH;
-            const uint32_t ka = smem0 + (v % KS) * 2 * TILE, kla = ka + TILE;
+            const uint32_t ka = smem0 + (v % KS) * KSTAGE, kla = ka + TILE;
             const uint32_t qa = smem0 + (uint32_t)OFF_Q;
             const bool rem = plan.remote(v);
             if (elect_one()) {
@@ -181,9 +196,9 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
                         umma_ss(dS, smem_desc_sw128(ka + (ks >> 2) * BOXB + (ks & 3) * 32, 16, 1024),
                                 smem_desc_sw128(qc + (ks >> 2) * (2 * NH * 128) + (ks & 3) * 32, 16, 1024), IDESC_S_F16_N32, ks > 0);
 #pragma unroll
-                    for (int ks = 0; ks < D / 16; ++ks)        // K'lo Q'hi into columns 0-15
-                        umma_ss(dS, smem_desc_sw128(kla + (ks >> 2) * BOXB + (ks & 3) * 32, 16, 1024),
-                                smem_desc_sw128(qc + (ks >> 2) * (2 * NH * 128) + (ks & 3) * 32, 16, 1024), IDESC_S_F16, 1);
+                    for (int ks = 0; ks < D / 32; ++ks)        // K'lo (e5m2) Q'hi (e5m2) into columns 0-15
+                        umma_ss_f8(dS, smem_desc_sw128(kla + ks * 32, 16, 1024),
+                                   smem_desc_sw128(qc + QCBUF + ks * 32, 16, 1024), IDESC_S_E5M2, 1);
                 }
                 umma_commit(&bars->s_full[v & 1]);
                 umma_commit(&bars->k_empty[v % KS]);
@@ -192,7 +207,7 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
         };
         auto issue_pv = [&](int v) {
             const uint32_t va = smem0 + (uint32_t)OFF_V + (v % VS) * TILE;
-            const uint32_t pa = smem0 + (uint32_t)OFF_P + (v & 1) * QBUF;
+            const uint32_t pa = smem0 + (uint32_t)OFF_P;
             if (elect_one()) {
 #pragma unroll
                 for (int ks = 0; ks < BN / 16; ++ks)
@@ -221,13 +236,13 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
         }
         if (elect_one()) umma_commit(&bars->o_full);
         __syncwarp();
-    } else if (warp >= 2 && warp < 2 + RW) {
+    } else if (warp >= 3 && warp < 3 + RW) {
         // ===================== rotate group (steps a4, a5) =====================
-        const int t = tid - 64;
+        const int t = tid - 96;
         const long long qpos = p.L - 1;
         // Q operands [16 heads][128 ch]: raw bf16 for local tiles; Q' = R(Delta q) Q as fp16 hi / lo for remote tiles
-        for (int i = t; i < (QBUF + QCBUF) / 4; i += RT) reinterpret_cast<uint32_t*>(sQ)[i] = 0u;
-        for (int i = t; i < 2 * QBUF / 4; i += RT) reinterpret_cast<uint32_t*>(sP)[i] = 0u;
+        for (int i = t; i < (QBUF + QCBUF + QYBUF) / 4; i += RT) reinterpret_cast<uint32_t*>(sQ)[i] = 0u;
+        for (int i = t; i < QBUF / 4; i += RT) reinterpret_cast<uint32_t*>(sP)[i] = 0u;
         named_bar_sync(1, RT);
         const long long nq = qpos - qpos / p.G;                      // -Delta(q) >= 0, Eq.(5)
         for (int idx = t; idx < p.g * 64; idx += RT) {
@@ -246,6 +261,10 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
                 *reinterpret_cast<__half*>(sQ + QBUF + bop_off<2 * NH>(h, i + 64)) = h2;
                 *reinterpret_cast<__half*>(sQ + QBUF + bop_off<2 * NH>(NH + h, i)) = __float2half_rn(y1 - __half2float(h1));
                 *reinterpret_cast<__half*>(sQ + QBUF + bop_off<2 * NH>(NH + h, i + 64)) = __float2half_rn(y2 - __half2float(h2));
+                // Q'hi as e5m2 (top byte of the fp16, rounded): byte ch of row h, 16-byte chunks swizzled by (h & 7)
+                unsigned char* qy = sQ + QBUF + QCBUF + h * 128;
+                qy[(((i >> 4) ^ (h & 7)) << 4) + (i & 15)] = (unsigned char)((__half_as_ushort(h1) + 0x80) >> 8);
+                qy[((((i + 64) >> 4) ^ (h & 7)) << 4) + (i & 15)] = (unsigned char)((__half_as_ushort(h2) + 0x80) >> 8);
             }
         }
         fence_proxy_async_smem();
@@ -260,7 +279,7 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
             const int s = v % KS;
             mbar_wait(&bars->k_full[s], (v / KS) & 1);
             if (plan.remote(v)) {
-                rotate_k_rows<RROWS, BOXB>(smem_u32(sK(s)), smem_u32(sK(s)) + TILE, (unsigned)(plan.kt(v) * BN), rot, true);
+                rotate_k_rows<RROWS, BOXB>(smem_u32(sK(s)), smem_u32(sK(s)) + TILE, (unsigned)(plan.kt(v) * BN), rot, 3);
                 fence_proxy_async_smem();
                 if (plan.remote(v + 1)) rot.prefetch((unsigned)(plan.kt(v + 1) * BN));
             }
@@ -273,7 +292,7 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
         const int j = (wq << 5) | lane;                              // key row in the tile == TMEM lane
         const uint32_t lane_base = (uint32_t)(wq << 5) << 16;
         const int g = p.g;
-        const uint32_t pj = smem_u32(sP) + (j >> 6) * (NH * 128) + (j & 7) * 2;   // P[h][j] = pj + h*128 + ((cj ^ (h&7)) << 4)
+        const uint32_t pb = smem_u32(sP) + (j >> 6) * (NH * 128) + (j & 7) * 2;   // P[h][j] = pb + h*128 + ((cj ^ (h&7)) << 4)
         const int cj = (j & 63) >> 3;
         float m_ref[NG], l[NG];
 #pragma unroll
@@ -337,7 +356,7 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
                     tc_fence_before();
                 }
             }
-            const uint32_t pb = pj + (v & 1) * QBUF;
+            if (v > 0) mbar_wait(&bars->pv_done, (v - 1) & 1);        // single P buffer: O += V^T P of visit v-1 has read it
 #pragma unroll
             for (int h = 0; h < NG; ++h) {
                 const float pr = (x[h] == -INFINITY) ? 0.0f : ex2(x[h] - m_ref[h]);

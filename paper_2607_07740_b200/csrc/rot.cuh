@@ -193,7 +193,8 @@ template <int ROWS, int KBOX>
 __device__ __forceinline__ void rotate_k_rows(uint32_t kh, uint32_t kl, unsigned pos0, KRot<ROWS>& R,
                                               int precise) {   // kh, kl: shared-space addresses
     // precise: 0 = hi only; 1 = fp16 lo at kl (same layout as kh); 2 = e5m2 copies for the cross terms at kl:
-    //          [box of KBOX bytes: K' as e5m2, rows x 128 channels][box: K' lo as e5m2], SWIZZLE_128B
+    //          [box of KBOX bytes: K' as e5m2, rows x 128 channels][box: K' lo as e5m2], SWIZZLE_128B;
+    //          3 = only K' lo as e5m2 at kl (one box)
     // first-row (cos, sin) from the prefetched table entries: HI * LO as complex numbers
     uint64_t cc[4], cs[4];
 #pragma unroll
@@ -243,6 +244,11 @@ __device__ __forceinline__ void rotate_k_rows(uint32_t kh, uint32_t kl, unsigned
             sts64(kl + o2, e5m2x4(h2[0], h2[1]), e5m2x4(h2[2], h2[3]));
             sts64(kl + KBOX + o1, e5m2x4(l1[0], l1[1]), e5m2x4(l1[2], l1[3]));
             sts64(kl + KBOX + o2, e5m2x4(l2[0], l2[1]), e5m2x4(l2[2], l2[3]));
+        } else if (precise == 3) {
+            const uint32_t o1 = r * 128 + ((((R.c >> 1)) ^ (r & 7)) << 4) + (R.c & 1) * 8;
+            const uint32_t o2 = r * 128 + (((4 + (R.c >> 1)) ^ (r & 7)) << 4) + (R.c & 1) * 8;
+            sts64(kl + o1, e5m2x4(l1[0], l1[1]), e5m2x4(l1[2], l1[3]));
+            sts64(kl + o2, e5m2x4(l2[0], l2[1]), e5m2x4(l2[2], l2[3]));
         }
     }
 }
