@@ -46,47 +46,40 @@ size_t two_level_bytes(long long L, int d) {
     return 256 + align256((size_t)(256 + n_hi) * (d / 2) * sizeof(float2));
 }
 
-__global__ void two_level_kernel(unsigned char* __restrict__ region, long long n_hi, int half, double theta,
-                                 double log2_theta, int d) {
+// One CTA.  Every call launches it; when the header already describes (theta, n_hi, d) it returns at once (decode
+// steps 1..n), otherwise it rebuilds the table and then seals the header.
+__global__ void __launch_bounds__(1024) two_level_kernel(unsigned char* __restrict__ region, long long n_hi, int half,
+                                                         double theta, double log2_theta, int d) {
     TableHeader* hdr = reinterpret_cast<TableHeader*>(region);
-    // header already valid for these parameters: nothing to do (decode steps 1..n hit this path)
-    if (hdr->magic == kMagic && hdr->theta == theta && hdr->n_hi == n_hi && hdr->d == d) return;
+    if (hdr->magic == kMagic && hdr->theta == theta && hdr->n_hi == n_hi && hdr->d == d) return;   // uniform
     float2* lo = reinterpret_cast<float2*>(region + 256);
     float2* hi = lo + 256 * half;
-    long long total = (256 + n_hi) * half;
-    for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < total;
-         idx += (long long)gridDim.x * blockDim.x) {
-        long long row = idx / half;
-        int i = (int)(idx - row * half);
-        double th = exp2(-2.0 * (double)i / (double)d * log2_theta);
-        double n = row < 256 ? (double)row : 256.0 * (double)(row - 256);
+    const long long total = (256 + n_hi) * half;
+    for (long long idx = threadIdx.x; idx < total; idx += blockDim.x) {
+        const long long row = idx / half;
+        const int i = (int)(idx - row * half);
+        const double th = exp2(-2.0 * (double)i / (double)d * log2_theta);
+        const double n = row < 256 ? (double)row : 256.0 * (double)(row - 256);
         double s, c;
         sincos(-n * th, &s, &c);
         (row < 256 ? lo : hi)[(row < 256 ? row : row - 256) * half + i] = make_float2((float)c, (float)s);
     }
-}
-
-__global__ void two_level_seal_kernel(unsigned char* region, long long n_hi, double theta, int d) {
-    TableHeader* hdr = reinterpret_cast<TableHeader*>(region);
-    if (hdr->magic == kMagic && hdr->theta == theta && hdr->n_hi == n_hi && hdr->d == d) return;
-    hdr->theta = theta;
-    hdr->n_hi = n_hi;
-    hdr->d = d;
-    hdr->pad = 0;
     __threadfence();
-    hdr->magic = kMagic;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        hdr->theta = theta;
+        hdr->n_hi = n_hi;
+        hdr->d = d;
+        hdr->pad = 0;
+        __threadfence();
+        hdr->magic = kMagic;
+    }
 }
 
 int build_two_level(void* region, long long L, int d, double theta, cudaStream_t st) {
-    long long n_hi = (L + 255) / 256 + 1;
-    int half = d / 2;
-    long long total = (256 + n_hi) * half;
-    int threads = 256;
-    int blocks = (int)((total + threads - 1) / threads);
-    if (blocks > 1024) blocks = 1024;
-    two_level_kernel<<<blocks, threads, 0, st>>>((unsigned char*)region, n_hi, half, theta, log2(theta), d);
-    two_level_seal_kernel<<<1, 1, 0, st>>>((unsigned char*)region, n_hi, theta, d);
-    note_launch(2);
+    const long long n_hi = (L + 255) / 256 + 1;
+    two_level_kernel<<<1, 1024, 0, st>>>((unsigned char*)region, n_hi, d / 2, theta, log2(theta), d);
+    note_launch(1);
     return check_launch("two_level_kernel");
 }
 
