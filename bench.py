@@ -157,6 +157,20 @@ def workload_config(cfg):
             "l2": "inputs+outputs (0.8 GB) exceed the 126 MB L2; no flush needed between iterations"}
 
 
+def max_over_ranks(ms, dist, device):
+    """Device time of the slowest rank (the contract's max-over-ranks); identity on one rank."""
+    if dist is None:
+        return float(ms)
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def replicas_value(world, flops_per_replica, ms_per_step):
+    """Whole-job TFLOP/s of `world` independent replicas ("replicas only": no exchange step exists on the path)."""
+    return world * flops_per_replica / (ms_per_step * 1e-3) / 1e12
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -245,12 +259,9 @@ def main():
     total_ms, per, (t_begin, t_end) = timed(step, args.steps, args.warmup)
     launches = (J.jetlong_launch_count() - n0) * args.steps // (args.steps + args.warmup)
     clocks = sampler.stop(t_begin, t_end) if rank == 0 else None
-    t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-    if dist is not None:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms = float(t.item())
+    total_ms = max_over_ranks(total_ms, dist, dev)
     ms_per_step = total_ms / args.steps
-    value = world * fl / (ms_per_step * 1e-3) / 1e12
+    value = replicas_value(world, fl, ms_per_step)
 
     cfgd = workload_config(cfg)
     cfgd["variant"] = {"bifocal": "bifocal prefill, default precision (compensated remote QK^T, meets the lse tolerance)",

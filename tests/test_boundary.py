@@ -79,3 +79,11 @@ def test_product_does_not_import_the_oracle():
             if f.endswith((".py", ".cu", ".cuh", ".h")):
                 txt = open(os.path.join(dirpath, f)).read()
                 assert "import oracle" not in txt and "from oracle" not in txt and "jetlong_oracle" not in txt, f
+
+
+def test_prefill_precision_switch_is_host_state():
+    assert B.jetlong_set_prefill_precision(B.PRECISION_FAST) == B.PRECISION_COMPENSATED       # returns the previous mode
+    assert B.jetlong_set_prefill_precision(B.PRECISION_COMPENSATED_F16) == B.PRECISION_FAST
+    assert B.jetlong_set_prefill_precision(77) == B.PRECISION_COMPENSATED_F16                  # unknown: unchanged
+    assert B.jetlong_set_prefill_precision(B.PRECISION_COMPENSATED) == B.PRECISION_COMPENSATED_F16
+    assert B.jetlong_set_prefill_precision(B.PRECISION_COMPENSATED) == B.PRECISION_COMPENSATED
