@@ -43,7 +43,8 @@ typedef enum {
 enum { JETLONG_BF16 = 0, JETLONG_FP32 = 1 };
 
 /* op codes for jetlong_workspace_bytes */
-enum { JETLONG_OP_PREFILL = 0, JETLONG_OP_DECODE = 1, JETLONG_OP_CAUSAL_PREFILL = 2, JETLONG_OP_CAUSAL_DECODE = 3 };
+enum { JETLONG_OP_PREFILL = 0, JETLONG_OP_DECODE = 1, JETLONG_OP_CAUSAL_PREFILL = 2, JETLONG_OP_CAUSAL_DECODE = 3,
+       JETLONG_OP_PREFILL_PREROTATED = 4 };
 
 /* Eq.(2): G = max(1, ceil(L / w_pretrained)), integer arithmetic on the host.
  * Returns -1 if L < 1 or w_pretrained < 1. */
@@ -65,6 +66,21 @@ int jetlong_prefill(const void* Q, const void* K, const void* V, void* out, floa
                     int64_t L, int H_q, int H_kv, int head_dim,
                     int64_t w_local, int64_t w_pretrained, double rope_theta,
                     int dtype, void* workspace, size_t workspace_bytes, void* stream);
+
+/*
+ * Workspace variant of the bifocal prefill (an ablation that prices the on-the-fly key correction; the paper
+ * keeps "no second key view").  Same arguments and result as jetlong_prefill, but the correction
+ * rotation K' = R(Delta k) K (Eq.(5)-(6) P:101-106) is applied ONCE into a scratch inside the workspace
+ * (K' as fp16 plus the two e5m2 cross-term operands: 4 bytes per key channel, e.g. 268 MB at L = 65536,
+ * H_kv = 8) and the remote tiles are then TMA-loaded from it; the stored K is still never written.
+ * bf16, head_dim 128, even H_q / H_kv only (JETLONG_UNSUPPORTED otherwise); the workspace must be at
+ * least jetlong_workspace_bytes(JETLONG_OP_PREFILL_PREROTATED, ...).  The fp16 cross-term precision
+ * mode is served with the e5m2 cross terms.
+ */
+int jetlong_prefill_prerotated(const void* Q, const void* K, const void* V, void* out, float* lse,
+                               int64_t L, int H_q, int H_kv, int head_dim,
+                               int64_t w_local, int64_t w_pretrained, double rope_theta,
+                               int dtype, void* workspace, size_t workspace_bytes, void* stream);
 
 /*
  * Bifocal batch-1 decode: one query row per head at position L-1 against cache rows

@@ -15,7 +15,7 @@ _lib = None
 
 OK, INVALID_ARG, UNSUPPORTED, CUDA_ERROR = 0, 1, 2, 3
 BF16, FP32 = 0, 1
-OP_PREFILL, OP_DECODE, OP_CAUSAL_PREFILL, OP_CAUSAL_DECODE = 0, 1, 2, 3
+OP_PREFILL, OP_DECODE, OP_CAUSAL_PREFILL, OP_CAUSAL_DECODE, OP_PREFILL_PREROTATED = 0, 1, 2, 3, 4
 PRECISION_COMPENSATED, PRECISION_FAST, PRECISION_COMPENSATED_F16 = 0, 1, 2
 
 EXPORTS = ["jetlong_group_size", "jetlong_workspace_bytes", "jetlong_prefill", "jetlong_decode",
@@ -46,6 +46,8 @@ def lib():
         tail = [i64, i32, i32, i32, i64, i64, dbl, i32, vp, sz, vp]
         L.jetlong_prefill.restype = i32
         L.jetlong_prefill.argtypes = [vp] * 5 + tail
+        L.jetlong_prefill_prerotated.restype = i32
+        L.jetlong_prefill_prerotated.argtypes = [vp] * 5 + tail
         L.jetlong_decode.restype = i32
         L.jetlong_decode.argtypes = [vp] * 5 + tail
         ctail = [i64, i32, i32, i32, i32, vp, sz, vp]
@@ -131,6 +133,18 @@ def jetlong_prefill(Q, K, V, *, w_local, w_pretrained, rope_theta, out=None, lse
     _check(lib().jetlong_prefill(Q.data_ptr(), K.data_ptr(), V.data_ptr(), out.data_ptr(), lse.data_ptr(), L, H_q,
                                  H_kv, d, int(w_local), int(w_pretrained), float(rope_theta), dt,
                                  workspace.data_ptr(), workspace.numel(), _stream()))
+    return out, lse
+
+
+def jetlong_prefill_prerotated(Q, K, V, *, w_local, w_pretrained, rope_theta, out=None, lse=None, workspace=None):
+    """Workspace variant of the bifocal prefill: K is correction-rotated once into a scratch in the workspace."""
+    L, H_q, H_kv, d, out, lse = _prefill_args(Q, K, V, out, lse)
+    dt = _dt(Q)
+    if workspace is None:
+        workspace = alloc_workspace(OP_PREFILL_PREROTATED, L, H_q, H_kv, d, dt, Q.device)
+    _check(lib().jetlong_prefill_prerotated(Q.data_ptr(), K.data_ptr(), V.data_ptr(), out.data_ptr(), lse.data_ptr(),
+                                            L, H_q, H_kv, d, int(w_local), int(w_pretrained), float(rope_theta), dt,
+                                            workspace.data_ptr(), workspace.numel(), _stream()))
     return out, lse
 
 

@@ -24,9 +24,10 @@ int check_launch(const char* what) {
 // prefill_umma.cu
 bool umma_prefill_supported(long long L, int H_q, int H_kv, int d, int dtype);
 size_t umma_prefill_workspace_bytes(long long L, int H_q, int H_kv, int d);
+size_t umma_prefill_prerot_workspace_bytes(long long L, int H_kv, int d);
 int launch_prefill_umma(const void* Q, const void* K, const void* V, void* out, float* lse, long long L, int H_q,
                         int H_kv, int d, long long w0, long long G, double theta, bool bifocal, int precise, void* ws,
-                        size_t ws_bytes, cudaStream_t st);
+                        size_t ws_bytes, cudaStream_t st, bool prerot);
 
 static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; }
 
@@ -66,20 +67,22 @@ static size_t prefill_ws(long long L, int H_q, int H_kv, int d, int dtype, bool 
 
 static int prefill_common(const void* Q, const void* K, const void* V, void* out, float* lse, long long L, int H_q,
                           int H_kv, int d, long long w0, long long w_pre, double theta, int dtype, void* ws,
-                          size_t ws_bytes, void* stream, bool bifocal) {
+                          size_t ws_bytes, void* stream, bool bifocal, bool prerot = false) {
     int rc = validate(Q, K, V, out, lse, L, H_q, H_kv, d, w0, w_pre, theta, dtype);
     if (rc != JETLONG_OK) return rc;
+    if (prerot && !umma_prefill_supported(L, H_q, H_kv, d, dtype)) return JETLONG_UNSUPPORTED;
     long long G = bifocal ? jetlong_group_size(L, w_pre) : 1;
     if (G == 1 || w0 >= L - 1) bifocal = false;          // step a2: G = 1 (or an all-covering window) is the control
-    const size_t need = prefill_ws(L, H_q, H_kv, d, dtype, bifocal);
+    const size_t need = (prerot && bifocal) ? umma_prefill_prerot_workspace_bytes(L, H_kv, d) : prefill_ws(L, H_q, H_kv, d, dtype, bifocal);
     if (need > 0 && (!ws || ws_bytes < need || !aligned16(ws))) return JETLONG_INVALID_ARG;
     rc = device_ok();
     if (rc != JETLONG_OK) return rc;
     cudaStream_t st = (cudaStream_t)stream;
     const int prec = g_prefill_precision.load();
-    if (use_umma(L, H_q, H_kv, d, dtype))
+    if (prerot || use_umma(L, H_q, H_kv, d, dtype))
         return launch_prefill_umma(Q, K, V, out, lse, L, H_q, H_kv, d, w0, G, theta, bifocal,
-                                   prec == JETLONG_PRECISION_FAST ? 0 : (prec == JETLONG_PRECISION_COMPENSATED_F16 ? 1 : 2), ws, ws_bytes, st);
+                                   prec == JETLONG_PRECISION_FAST ? 0 : (prec == JETLONG_PRECISION_COMPENSATED_F16 ? 1 : 2), ws, ws_bytes, st,
+                                   prerot && bifocal);
     const float2* tab = nullptr;
     if (bifocal) {
         rc = build_key_table((float2*)ws, L, G, d, theta, st);
@@ -123,6 +126,8 @@ size_t jetlong_workspace_bytes(int op, int64_t L, int H_q, int H_kv, int head_di
         case JETLONG_OP_CAUSAL_PREFILL: return prefill_ws(L, H_q, H_kv, head_dim, dtype, false);
         case JETLONG_OP_DECODE:
         case JETLONG_OP_CAUSAL_DECODE: return decode_workspace_bytes(L, H_q, H_kv, head_dim);
+        case JETLONG_OP_PREFILL_PREROTATED:
+            return umma_prefill_supported(L, H_q, H_kv, head_dim, dtype) ? umma_prefill_prerot_workspace_bytes(L, H_kv, head_dim) : 0;
         default: return 0;
     }
 }
@@ -132,6 +137,13 @@ int jetlong_prefill(const void* Q, const void* K, const void* V, void* out, floa
                     size_t workspace_bytes, void* stream) {
     return prefill_common(Q, K, V, out, lse, L, H_q, H_kv, head_dim, w_local, w_pretrained, rope_theta, dtype,
                           workspace, workspace_bytes, stream, true);
+}
+
+int jetlong_prefill_prerotated(const void* Q, const void* K, const void* V, void* out, float* lse, int64_t L, int H_q,
+                               int H_kv, int head_dim, int64_t w_local, int64_t w_pretrained, double rope_theta, int dtype,
+                               void* workspace, size_t workspace_bytes, void* stream) {
+    return prefill_common(Q, K, V, out, lse, L, H_q, H_kv, head_dim, w_local, w_pretrained, rope_theta, dtype,
+                          workspace, workspace_bytes, stream, true, true);
 }
 
 int jetlong_causal_prefill(const void* Q, const void* K, const void* V, void* out, float* lse, int64_t L, int H_q,

@@ -75,6 +75,7 @@ struct Params {
     long long L, w0, G;
     int H_q, H_kv, g;
     int bifocal, precise;
+    int prerot;                                       // remote K tiles come pre-rotated from the workspace (8(f)-1)
     const float2* lo;
     const float2* hi;
 };
@@ -168,7 +169,9 @@ constexpr uint32_t IDESC_QK_E5M2 = idesc_f16(1, 1, 0, 0, 2 * BM, BN);   // kind:
 constexpr uint32_t IDESC_PV = idesc_f16(1, 1, 0, 1, 2 * BM, D);  // A = P (TMEM, bf16), B = V (smem, MN-major)
 
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1)
-prefill_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV, const Params p) {
+prefill_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV,
+                    const __grid_constant__ CUtensorMap tmKh, const __grid_constant__ CUtensorMap tmKe,
+                    const __grid_constant__ CUtensorMap tmKl, const Params p) {
     extern __shared__ unsigned char smem_raw[];
     unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
     Bars* bars = reinterpret_cast<Bars*>(smem + NS * STAGE_BYTES);
@@ -197,6 +200,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_consta
         mbar_init(&bars->q_local_done, 1); mbar_init(&bars->q_rot_done, 8);
         fence_barrier_init();
         prefetch_tmap(&tmK); prefetch_tmap(&tmV);
+        if (p.prerot) { prefetch_tmap(&tmKh); prefetch_tmap(&tmKe); prefetch_tmap(&tmKl); }
     }
     if (warp == 1) tmem_alloc2<512>(&bars->tmem_base);
     tc_fence_before();
@@ -212,9 +216,20 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_consta
                 const Visit x = plan.at(v, bifocal);
                 const int s = v % NS;
                 if (v >= NS) mbar_wait(&bars->kv_empty[s], ((v / NS) - 1) & 1);
-                mbar_arrive_expect_tx(&bars->kv_full[s], KH_BYTES + VH_BYTES);
-                tma_load_3d(sK(s), &tmK, &bars->kv_full[s], 0, kvh, x.kt * BN + 64 * cta);
-                tma_load_3d(sK(s) + KBOX, &tmK, &bars->kv_full[s], 64, kvh, x.kt * BN + 64 * cta);
+                if (p.prerot && x.mode == 2) {
+                    // pre-rotated variant: K' hi (fp16) and the e5m2 copies of K' and K' lo come from the workspace
+                    mbar_arrive_expect_tx(&bars->kv_full[s], KH_BYTES + VH_BYTES + (precise == 2 ? 2 * KBOX : 0));
+                    tma_load_3d(sK(s), &tmKh, &bars->kv_full[s], 0, kvh, x.kt * BN + 64 * cta);
+                    tma_load_3d(sK(s) + KBOX, &tmKh, &bars->kv_full[s], 64, kvh, x.kt * BN + 64 * cta);
+                    if (precise == 2) {
+                        tma_load_3d(sKl(s), &tmKe, &bars->kv_full[s], 0, kvh, x.kt * BN + 64 * cta);
+                        tma_load_3d(sKl(s) + KBOX, &tmKl, &bars->kv_full[s], 0, kvh, x.kt * BN + 64 * cta);
+                    }
+                } else {
+                    mbar_arrive_expect_tx(&bars->kv_full[s], KH_BYTES + VH_BYTES);
+                    tma_load_3d(sK(s), &tmK, &bars->kv_full[s], 0, kvh, x.kt * BN + 64 * cta);
+                    tma_load_3d(sK(s) + KBOX, &tmK, &bars->kv_full[s], 64, kvh, x.kt * BN + 64 * cta);
+                }
                 tma_load_3d(sV(s), &tmV, &bars->kv_full[s], 64 * cta, kvh, x.kt * BN);
             }
         }
@@ -308,7 +323,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_consta
         __syncwarp();
         if (lane == 0) mbar_arrive_leader(&bars->q_ready);
         KRot<4> rot;
-        if (plan.n_remote > 0) {
+        if (plan.n_remote > 0 && !p.prerot) {
             rot.init(p.lo, p.hi, t, p.G);
             rot.prefetch((unsigned)(plan.kt_hi * BN + 64 * cta));     // first remote visit
         }
@@ -324,9 +339,11 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_consta
                     tmem_st_wait();
                     tc_fence_before();
                 }
-                rotate_k_rows<4, KBOX>(smem_u32(sK(s)), smem_u32(sKl(s)), (unsigned)(x.kt * BN + 64 * cta), rot, precise);
-                fence_proxy_async_smem();
-                if (x.kt > 0) rot.prefetch((unsigned)((x.kt - 1) * BN + 64 * cta));   // next remote visit's first row
+                if (!p.prerot) {
+                    rotate_k_rows<4, KBOX>(smem_u32(sK(s)), smem_u32(sKl(s)), (unsigned)(x.kt * BN + 64 * cta), rot, precise);
+                    fence_proxy_async_smem();
+                    if (x.kt > 0) rot.prefetch((unsigned)((x.kt - 1) * BN + 64 * cta));   // next remote visit's first row
+                }
             }
             __syncwarp();
             if (lane == 0) {
@@ -466,6 +483,33 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_consta
     if (warp == 1) tmem_dealloc2<512>(tmem);
 }
 
+// ---- 8(f)-1: rotate K once into a scratch (the workspace variant) -------------------------------------------
+// K'hi [L, H_kv, 128] fp16, K'e5 [L, H_kv, 128] e5m2 (K' rounded), K'lo [L, H_kv, 128] e5m2 (K' - K'hi): exactly the
+// three operands the rotate group otherwise produces per visit.  Thread = (key k, KV head, 16-byte chunk c).
+__global__ void __launch_bounds__(256) prerotate_k_kernel(const __nv_bfloat16* __restrict__ K, __half* __restrict__ Kh,
+                                                          unsigned char* __restrict__ Ke, unsigned char* __restrict__ Kl,
+                                                          long long L, int H_kv, long long G,
+                                                          const float2* __restrict__ lo, const float2* __restrict__ hi) {
+    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= L * H_kv * 8) return;
+    const int c = (int)(idx & 7);
+    const long long row = idx >> 3;                                   // k * H_kv + kvh
+    const long long k = row / H_kv;
+    const uint4 u1 = __ldg(reinterpret_cast<const uint4*>(K + row * D) + c);
+    const uint4 u2 = __ldg(reinterpret_cast<const uint4*>(K + row * D) + 8 + c);
+    float cs_c[8], cs_s[8];
+    cs8(lo, hi, k, G, 8 * c, cs_c, cs_s);
+    const uint32_t a[4] = {u1.x, u1.y, u1.z, u1.w}, b[4] = {u2.x, u2.y, u2.z, u2.w};
+    uint32_t h1[4], h2[4], l1[4], l2[4];
+    rot8(a, b, cs_c, cs_s, h1, h2, l1, l2);
+    reinterpret_cast<uint4*>(Kh + row * D)[c] = make_uint4(h1[0], h1[1], h1[2], h1[3]);
+    reinterpret_cast<uint4*>(Kh + row * D)[8 + c] = make_uint4(h2[0], h2[1], h2[2], h2[3]);
+    reinterpret_cast<uint2*>(Ke + row * D)[c] = make_uint2(e5m2x4(h1[0], h1[1]), e5m2x4(h1[2], h1[3]));
+    reinterpret_cast<uint2*>(Ke + row * D)[8 + c] = make_uint2(e5m2x4(h2[0], h2[1]), e5m2x4(h2[2], h2[3]));
+    reinterpret_cast<uint2*>(Kl + row * D)[c] = make_uint2(e5m2x4(l1[0], l1[1]), e5m2x4(l1[2], l1[3]));
+    reinterpret_cast<uint2*>(Kl + row * D)[8 + c] = make_uint2(e5m2x4(l2[0], l2[1]), e5m2x4(l2[2], l2[3]));
+}
+
 }  // namespace
 
 // ---- host side ------------------------------------------------------------------------------------------
@@ -486,18 +530,21 @@ static EncodeTiledFn encode_fn() {
 }
 
 // [L, H, 128] bf16 tensor seen as (d, H, L); box = 64 channels x 1 head x `rows` rows, SWIZZLE_128B, OOB rows -> 0
-bool make_kv_tensor_map(CUtensorMap* m, const void* base, long long L, int H, int rows) {
+// bytes = 1: the same tensor with one-byte elements (the e5m2 copies), box = 128 channels x 1 head x `rows` rows
+static bool make_tensor_map(CUtensorMap* m, const void* base, long long L, int H, int rows, int bytes) {
     EncodeTiledFn fn = encode_fn();
     if (!fn) return false;
     cuuint64_t dims[3] = {(cuuint64_t)D, (cuuint64_t)H, (cuuint64_t)L};
-    cuuint64_t strides[2] = {(cuuint64_t)D * 2, (cuuint64_t)H * D * 2};
-    cuuint32_t box[3] = {64, 1, (cuuint32_t)rows};
+    cuuint64_t strides[2] = {(cuuint64_t)D * bytes, (cuuint64_t)H * D * bytes};
+    cuuint32_t box[3] = {(cuuint32_t)(128 / bytes), 1, (cuuint32_t)rows};
     cuuint32_t es[3] = {1, 1, 1};
-    return fn(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(base), dims, strides, box, es,
+    return fn(m, bytes == 2 ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16 : CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<void*>(base), dims, strides, box, es,
               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
-
+bool make_kv_tensor_map(CUtensorMap* m, const void* base, long long L, int H, int rows) {
+    return make_tensor_map(m, base, L, H, rows, 2);
+}
 
 bool umma_prefill_supported(long long L, int H_q, int H_kv, int d, int dtype) {
     if (dtype != JETLONG_BF16 || d != 128 || H_kv < 1 || H_q % H_kv) return false;
@@ -507,9 +554,15 @@ bool umma_prefill_supported(long long L, int H_q, int H_kv, int d, int dtype) {
 
 size_t umma_prefill_workspace_bytes(long long L, int, int, int d) { return two_level_bytes(L + 256, d); }
 
+// pre-rotated variant: tables, then K'hi (fp16), K' (e5m2), K'lo (e5m2), each [L, H_kv, 128]
+size_t umma_prefill_prerot_workspace_bytes(long long L, int H_kv, int d) {
+    const size_t n = (size_t)L * H_kv * d;
+    return two_level_bytes(L + 256, d) + align256(2 * n) + 2 * align256(n);
+}
+
 int launch_prefill_umma(const void* Q, const void* K, const void* V, void* out, float* lse, long long L, int H_q,
                         int H_kv, int d, long long w0, long long G, double theta, bool bifocal, int precise, void* ws,
-                        size_t ws_bytes, cudaStream_t st) {
+                        size_t ws_bytes, cudaStream_t st, bool prerot) {
     (void)ws_bytes;
     CUtensorMap tmK, tmV;
     if (!make_kv_tensor_map(&tmK, K, L, H_kv, 64) || !make_kv_tensor_map(&tmV, V, L, H_kv, 128)) return JETLONG_UNSUPPORTED;
@@ -521,12 +574,32 @@ int launch_prefill_umma(const void* Q, const void* K, const void* V, void* out, 
     p.H_q = H_q; p.H_kv = H_kv; p.g = H_q / H_kv;
     p.bifocal = bifocal ? 1 : 0;
     p.precise = precise;
+    p.prerot = 0;
+    CUtensorMap tmKh = tmK, tmKe = tmK, tmKl = tmK;
     p.lo = nullptr; p.hi = nullptr;
     if (bifocal) {
         int rc = build_two_level(ws, L + 256, d, theta, st);
         if (rc != JETLONG_OK) return rc;
         p.lo = reinterpret_cast<const float2*>((unsigned char*)ws + 256);
         p.hi = p.lo + 256 * (d / 2);
+        if (prerot) {
+            if (precise == 1) precise = p.precise = 2;               // the scratch holds the e5m2 cross-term operands only
+            const size_t n = (size_t)L * H_kv * d;
+            unsigned char* base = (unsigned char*)ws + two_level_bytes(L + 256, d);
+            __half* Kh = reinterpret_cast<__half*>(base);
+            unsigned char* Ke = base + align256(2 * n);
+            unsigned char* Kl = Ke + align256(n);
+            const long long items = L * H_kv * 8;
+            prerotate_k_kernel<<<(unsigned)((items + 255) / 256), 256, 0, st>>>((const __nv_bfloat16*)K, Kh, Ke, Kl, L, H_kv, G,
+                                                                               p.lo, p.hi);
+            note_launch();
+            rc = check_launch("prerotate_k_kernel");
+            if (rc != JETLONG_OK) return rc;
+            if (!make_tensor_map(&tmKh, Kh, L, H_kv, 64, 2) || !make_tensor_map(&tmKe, Ke, L, H_kv, 64, 1) ||
+                !make_tensor_map(&tmKl, Kl, L, H_kv, 64, 1))
+                return JETLONG_UNSUPPORTED;
+            p.prerot = 1;
+        }
     }
     static bool attr_set = false;
     if (!attr_set) {
@@ -537,7 +610,7 @@ int launch_prefill_umma(const void* Q, const void* K, const void* V, void* out, 
     }
     const int n_qb = (int)((L + BM - 1) / BM);
     const unsigned grid = 2u * (unsigned)n_qb * (unsigned)(H_q / 2);
-    prefill_umma_kernel<<<grid, NTHREADS, SMEM_BYTES, st>>>(tmK, tmV, p);
+    prefill_umma_kernel<<<grid, NTHREADS, SMEM_BYTES, st>>>(tmK, tmV, tmKh, tmKe, tmKl, p);
     note_launch();
     return check_launch("prefill_umma_kernel");
 }

@@ -142,3 +142,38 @@ def test_precision_modes_of_the_remote_scores():
     assert errs["default"][1] <= 1e-3 and errs["f16"][1] <= 1e-4, errs
     assert all(e[0] <= 2e-2 for e in errs.values()), errs
     assert errs["fast"][1] <= 1e-2, errs                           # bounded, but it is NOT within the 1e-3 tolerance
+
+
+# ---- workspace variant (K correction-rotated once into a scratch) ---------------------------
+@pytest.mark.parametrize("L,H_q,H_kv,w_pre,w0", [
+    (777, 4, 2, 200, 100),        # G=4, ragged tail, straddle not tile aligned
+    (640, 8, 2, 320, 128),        # G=2, g=4, tile-aligned window
+    (1300, 2, 1, 300, 0),         # G=5, w0=0
+])
+def test_prerotated_small_shapes_full(L, H_q, H_kv, w_pre, w0):
+    Q, K, V = W.make_qkv(L, H_q, H_kv, 128, 1e6, "bf16", 4321 + L, True, DEV)
+    k0 = K.clone()
+    out, lse = J.jetlong_prefill_prerotated(Q, K, V, w_local=w0, w_pretrained=w_pre, rope_theta=1e6)
+    torch.cuda.synchronize()
+    assert torch.equal(K, k0)                                          # the stored K is still never written
+    rows, heads = all_pairs(L, H_q)
+    ro, rl = oracle_rows(Q, K, V, rows, heads, w_local=w0, w_pretrained=w_pre, rope_theta=1e6)
+    check(*gather(out, lse, rows, heads), ro, rl, Q.dtype, "prerotated L=%d" % L)
+
+
+def test_prerotated_config2_sampled_rows():
+    c = W.C2
+    Q, K, V = W.make_config_inputs(c, DEV)
+    out, lse = J.jetlong_prefill_prerotated(Q, K, V, w_local=c.w_local, w_pretrained=c.w_pretrained, rope_theta=c.rope_theta)
+    torch.cuda.synchronize()
+    rows, heads = W.sample_pairs(c.L, c.H_q, 256, c.seed(), c.w_local, J.jetlong_group_size(c.L, c.w_pretrained))
+    ro, rl = oracle_rows(Q, K, V, rows, heads, w_local=c.w_local, w_pretrained=c.w_pretrained, rope_theta=c.rope_theta)
+    check(*gather(out, lse, rows, heads), ro, rl, Q.dtype, "prerotated C2")
+
+
+def test_prerotated_unsupported_shapes_are_refused():
+    from paper_2607_07740_b200 import binding as B
+    Q, K, V = W.make_qkv(300, 2, 1, 64, 1e4, "fp32", 3, False, DEV)
+    with pytest.raises(B.JetlongError):
+        J.jetlong_prefill_prerotated(Q, K, V, w_local=7, w_pretrained=100, rope_theta=1e4,
+                                     workspace=torch.zeros(1 << 20, dtype=torch.uint8, device=DEV))
