@@ -78,6 +78,7 @@ struct Params {
     int prerot;                                       // remote K tiles come pre-rotated from the workspace (8(f)-1)
     const float2* lo;
     const float2* hi;
+    const uint32_t* selinfo;                          // [H_kv][16]: 8 PRMT selectors (two pairs per 8-pair chunk), full-mode flag
 };
 
 struct Visit { int kt; int mode; };                   // mode 0 = causal/control, 1 = local, 2 = remote
@@ -115,29 +116,46 @@ __device__ __forceinline__ void stage_q_raw(const __nv_bfloat16* qrow, bool vali
 }
 __device__ __forceinline__ void stage_q_rot(const __nv_bfloat16* qrow, bool valid, long long q, long long G,
                                             const float2* __restrict__ lo, const float2* __restrict__ hi,
-                                            uint32_t tQa, uint32_t tQb, int precise) {
-#pragma unroll 2
-    for (int j = 0; j < 8; ++j) {                         // channels 8j..8j+7 and 64+8j..
-        uint4 u1 = make_uint4(0, 0, 0, 0), u2 = u1;
-        if (valid) {
-            u1 = __ldg(reinterpret_cast<const uint4*>(qrow) + j);
-            u2 = __ldg(reinterpret_cast<const uint4*>(qrow) + 8 + j);
+                                            uint32_t tQa, uint32_t tQb, int precise, const uint32_t* __restrict__ sel) {
+#pragma unroll 1
+    for (int jp = 0; jp < 4; ++jp) {
+        uint32_t w[4] = {0u, 0u, 0u, 0u};                    // precise 3: compact hi1 | hi2 | lo1 | lo2 words of chunks 2jp, 2jp+1
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+            const int j = 2 * jp + u;                         // channels 8j..8j+7 and 64+8j..
+            uint4 u1 = make_uint4(0, 0, 0, 0), u2 = u1;
+            if (valid) {
+                u1 = __ldg(reinterpret_cast<const uint4*>(qrow) + j);
+                u2 = __ldg(reinterpret_cast<const uint4*>(qrow) + 8 + j);
+            }
+            float cs_c[8], cs_s[8];
+            cs8(lo, hi, q, G, 8 * j, cs_c, cs_s);
+            const uint32_t a[4] = {u1.x, u1.y, u1.z, u1.w}, b[4] = {u2.x, u2.y, u2.z, u2.w};
+            uint32_t h1[4], h2[4], l1[4], l2[4];
+            rot8(a, b, cs_c, cs_s, h1, h2, l1, l2);
+            tmem_st4(tQa + 4 * j, h1[0], h1[1], h1[2], h1[3]);
+            tmem_st4(tQa + 32 + 4 * j, h2[0], h2[1], h2[2], h2[3]);
+            if (precise == 2) {                                   // e5m2 copies: column c of QY / QR holds channels 4c..4c+3
+                tmem_st2(tQb + 2 * j, e5m2x4(h1[0], h1[1]), e5m2x4(h1[2], h1[3]));
+                tmem_st2(tQb + 16 + 2 * j, e5m2x4(h2[0], h2[1]), e5m2x4(h2[2], h2[3]));
+                tmem_st2(tQb + 32 + 2 * j, e5m2x4(l1[0], l1[1]), e5m2x4(l1[2], l1[3]));
+                tmem_st2(tQb + 48 + 2 * j, e5m2x4(l2[0], l2[1]), e5m2x4(l2[2], l2[3]));
+            } else if (precise == 3) {                            // the two selected pairs of this chunk, as e5m2
+                const uint32_t sj = __ldg(sel + j);
+                w[0] |= (__byte_perm(e5m2x4(h1[0], h1[1]), e5m2x4(h1[2], h1[3]), sj) & 0xffffu) << (16 * u);
+                w[1] |= (__byte_perm(e5m2x4(h2[0], h2[1]), e5m2x4(h2[2], h2[3]), sj) & 0xffffu) << (16 * u);
+                w[2] |= (__byte_perm(e5m2x4(l1[0], l1[1]), e5m2x4(l1[2], l1[3]), sj) & 0xffffu) << (16 * u);
+                w[3] |= (__byte_perm(e5m2x4(l2[0], l2[1]), e5m2x4(l2[2], l2[3]), sj) & 0xffffu) << (16 * u);
+            } else {
+                tmem_st4(tQb + 4 * j, l1[0], l1[1], l1[2], l1[3]);
+                tmem_st4(tQb + 32 + 4 * j, l2[0], l2[1], l2[2], l2[3]);
+            }
         }
-        float cs_c[8], cs_s[8];
-        cs8(lo, hi, q, G, 8 * j, cs_c, cs_s);
-        const uint32_t a[4] = {u1.x, u1.y, u1.z, u1.w}, b[4] = {u2.x, u2.y, u2.z, u2.w};
-        uint32_t h1[4], h2[4], l1[4], l2[4];
-        rot8(a, b, cs_c, cs_s, h1, h2, l1, l2);
-        tmem_st4(tQa + 4 * j, h1[0], h1[1], h1[2], h1[3]);
-        tmem_st4(tQa + 32 + 4 * j, h2[0], h2[1], h2[2], h2[3]);
-        if (precise == 2) {                                   // e5m2 copies: column c of QY / QR holds channels 4c..4c+3
-            tmem_st2(tQb + 2 * j, e5m2x4(h1[0], h1[1]), e5m2x4(h1[2], h1[3]));
-            tmem_st2(tQb + 16 + 2 * j, e5m2x4(h2[0], h2[1]), e5m2x4(h2[2], h2[3]));
-            tmem_st2(tQb + 32 + 2 * j, e5m2x4(l1[0], l1[1]), e5m2x4(l1[2], l1[3]));
-            tmem_st2(tQb + 48 + 2 * j, e5m2x4(l2[0], l2[1]), e5m2x4(l2[2], l2[3]));
-        } else {
-            tmem_st4(tQb + 4 * j, l1[0], l1[1], l1[2], l1[3]);
-            tmem_st4(tQb + 32 + 4 * j, l2[0], l2[1], l2[2], l2[3]);
+        if (precise == 3) {          // QY' = [hi1 | hi2] in columns 0-7 of Qb, QR' = [lo1 | lo2] in columns 8-15
+            tmem_st1(tQb + jp, w[0]);
+            tmem_st1(tQb + 4 + jp, w[1]);
+            tmem_st1(tQb + 8 + jp, w[2]);
+            tmem_st1(tQb + 12 + jp, w[3]);
         }
     }
 }
@@ -190,7 +208,10 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_consta
     const int kvh = h0 / p.g;
     const long long q0 = (long long)qb * BM;
     const bool bifocal = p.bifocal != 0;
-    const int precise = p.precise;                                // 0 fast, 1 fp16 cross terms, 2 e5m2 cross terms
+    // 0 fast, 1 fp16 cross terms, 2 e5m2 cross terms, 3 (pre-rotated variant only) e5m2 cross terms over the two
+    // highest-energy pairs of every 8-pair chunk; a KV head whose other channels are too loud falls back to 2
+    int precise = p.precise;
+    if (precise == 3 && __ldg(p.selinfo + kvh * 16 + 8) != 0u) precise = 2;
     const Plan plan(qb, p.w0, bifocal);
 
     if (tid == 0) {
@@ -218,13 +239,11 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_consta
                 if (v >= NS) mbar_wait(&bars->kv_empty[s], ((v / NS) - 1) & 1);
                 if (p.prerot && x.mode == 2) {
                     // pre-rotated variant: K' hi (fp16) and the e5m2 copies of K' and K' lo come from the workspace
-                    mbar_arrive_expect_tx(&bars->kv_full[s], KH_BYTES + VH_BYTES + (precise == 2 ? 2 * KBOX : 0));
+                    mbar_arrive_expect_tx(&bars->kv_full[s], KH_BYTES + VH_BYTES + (precise == 2 ? 2 * KBOX : precise == 3 ? KBOX : 0));
                     tma_load_3d(sK(s), &tmKh, &bars->kv_full[s], 0, kvh, x.kt * BN + 64 * cta);
                     tma_load_3d(sK(s) + KBOX, &tmKh, &bars->kv_full[s], 64, kvh, x.kt * BN + 64 * cta);
-                    if (precise == 2) {
-                        tma_load_3d(sKl(s), &tmKe, &bars->kv_full[s], 0, kvh, x.kt * BN + 64 * cta);
-                        tma_load_3d(sKl(s) + KBOX, &tmKl, &bars->kv_full[s], 0, kvh, x.kt * BN + 64 * cta);
-                    }
+                    if (precise >= 2) tma_load_3d(sKl(s), &tmKe, &bars->kv_full[s], 0, kvh, x.kt * BN + 64 * cta);
+                    if (precise == 2) tma_load_3d(sKl(s) + KBOX, &tmKl, &bars->kv_full[s], 0, kvh, x.kt * BN + 64 * cta);
                 } else {
                     mbar_arrive_expect_tx(&bars->kv_full[s], KH_BYTES + VH_BYTES);
                     tma_load_3d(sK(s), &tmK, &bars->kv_full[s], 0, kvh, x.kt * BN + 64 * cta);
@@ -264,6 +283,10 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_consta
                             for (int ks = 0; ks < D / 32; ++ks)      // Q' lo (e5m2) . K' (e5m2)
                                 umma2_ts_f8(dS, tm + TM_QR + ks * 8, smem_desc_sw128(klb + ks * 32, 16, 1024),
                                             IDESC_QK_E5M2, 1);
+                        } else if (precise == 3) {
+                            // compact operands: K row = [lo1 | lo2 | hi1 | hi2] (16 B each), Q' = [hi1 | hi2], [lo1 | lo2]
+                            umma2_ts_f8(dS, tm + TM_QY, smem_desc_sw128(klb, 16, 1024), IDESC_QK_E5M2, 1);
+                            umma2_ts_f8(dS, tm + TM_QY + 8, smem_desc_sw128(klb + 32, 16, 1024), IDESC_QK_E5M2, 1);
                         } else if (precise == 1) {
 #pragma unroll
                             for (int ks = 0; ks < D / 16; ++ks)
@@ -335,7 +358,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_consta
                 if (v == plan.n_local) {                              // first remote visit: Q -> Q' = R(Delta q) Q
                     mbar_wait(&bars->q_local_done, 0);
                     tc_fence_after();
-                    stage_q_rot(qrow, valid, q, p.G, p.lo, p.hi, tmem + lane_base + TM_QA, tmem + lane_base + TM_QB, precise);
+                    stage_q_rot(qrow, valid, q, p.G, p.lo, p.hi, tmem + lane_base + TM_QA, tmem + lane_base + TM_QB, precise, p.selinfo + kvh * 16);
                     tmem_st_wait();
                     tc_fence_before();
                 }
@@ -486,10 +509,60 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_consta
 // ---- 8(f)-1: rotate K once into a scratch (the workspace variant) -------------------------------------------
 // K'hi [L, H_kv, 128] fp16, K'e5 [L, H_kv, 128] e5m2 (K' rounded), K'lo [L, H_kv, 128] e5m2 (K' - K'hi): exactly the
 // three operands the rotate group otherwise produces per visit.  Thread = (key k, KV head, 16-byte chunk c).
+// Mean pair energies for the selective compensation: e[(h / gdiv) * 64 + i] += x_i^2 + x_{i+64}^2 over the sampled rows
+// of head h.  grid (blocks, H), 256 threads: pair i = t & 63, row lane t >> 6.
+__global__ void __launch_bounds__(256) pair_energy_kernel(const __nv_bfloat16* __restrict__ X, float* __restrict__ e,
+                                                          long long L, int H, int gdiv, int stride) {
+    __shared__ float red[256];
+    const int i = threadIdx.x & 63, sub = threadIdx.x >> 6, h = blockIdx.y;
+    float acc = 0.f;
+    for (long long k = ((long long)blockIdx.x * 4 + sub) * stride; k < L; k += (long long)gridDim.x * 4 * stride) {
+        const __nv_bfloat16* r = X + ((size_t)k * H + h) * D;
+        const float x1 = __bfloat162float(r[i]), x2 = __bfloat162float(r[i + 64]);
+        acc += x1 * x1 + x2 * x2;
+    }
+    red[threadIdx.x] = acc;
+    __syncthreads();
+    if (sub == 0) atomicAdd(&e[(h / gdiv) * 64 + i], red[i] + red[64 + i] + red[128 + i] + red[192 + i]);
+}
+
+// Per KV head: weight w_i = mean pair energy of K times that of Q; in every chunk of 8 pairs the two heaviest are
+// compensated (PRMT selector j0 | j1 << 4).  The pairs left out add rounding noise of about
+// sigma = scale * 2^-10 / (1.44 sqrt(12)) * sqrt(sum of their w_i) to a remote score; above
+// SEL_SIGMA_MAX the head falls back to the full e5m2 cross terms (flag at [8]).
+constexpr float SEL_SIGMA_MAX = 3.0e-4f;
+__global__ void __launch_bounds__(64) select_pairs_kernel(const float* __restrict__ eK, const float* __restrict__ eQ,
+                                                          uint32_t* __restrict__ selinfo, float inv_nk, float inv_nq) {
+    __shared__ float w[64];
+    __shared__ float resid[8];
+    const int kvh = blockIdx.x, t = threadIdx.x;
+    w[t] = (eK[kvh * 64 + t] * inv_nk) * (eQ[kvh * 64 + t] * inv_nq);
+    __syncthreads();
+    if (t < 8) {
+        int j0 = 0;
+        for (int j = 1; j < 8; ++j) if (w[8 * t + j] > w[8 * t + j0]) j0 = j;
+        int j1 = j0 == 0 ? 1 : 0;
+        for (int j = 0; j < 8; ++j) if (j != j0 && w[8 * t + j] > w[8 * t + j1]) j1 = j;
+        float r = 0.f;
+        for (int j = 0; j < 8; ++j) if (j != j0 && j != j1) r += w[8 * t + j];
+        resid[t] = r;
+        const int a = j0 < j1 ? j0 : j1, b = j0 < j1 ? j1 : j0;
+        selinfo[kvh * 16 + t] = (uint32_t)(a | (b << 4));
+    }
+    __syncthreads();
+    if (t == 0) {
+        float r = 0.f;
+        for (int c = 0; c < 8; ++c) r += resid[c];
+        const float sigma = rsqrtf((float)D) * 1.96e-4f * sqrtf(r);
+        selinfo[kvh * 16 + 8] = (sigma > SEL_SIGMA_MAX || !(sigma == sigma)) ? 1u : 0u;
+    }
+}
+
 __global__ void __launch_bounds__(256) prerotate_k_kernel(const __nv_bfloat16* __restrict__ K, __half* __restrict__ Kh,
                                                           unsigned char* __restrict__ Ke, unsigned char* __restrict__ Kl,
                                                           long long L, int H_kv, long long G,
-                                                          const float2* __restrict__ lo, const float2* __restrict__ hi) {
+                                                          const float2* __restrict__ lo, const float2* __restrict__ hi,
+                                                          const uint32_t* __restrict__ selinfo) {
     const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= L * H_kv * 8) return;
     const int c = (int)(idx & 7);
@@ -504,10 +577,23 @@ __global__ void __launch_bounds__(256) prerotate_k_kernel(const __nv_bfloat16* _
     rot8(a, b, cs_c, cs_s, h1, h2, l1, l2);
     reinterpret_cast<uint4*>(Kh + row * D)[c] = make_uint4(h1[0], h1[1], h1[2], h1[3]);
     reinterpret_cast<uint4*>(Kh + row * D)[8 + c] = make_uint4(h2[0], h2[1], h2[2], h2[3]);
-    reinterpret_cast<uint2*>(Ke + row * D)[c] = make_uint2(e5m2x4(h1[0], h1[1]), e5m2x4(h1[2], h1[3]));
-    reinterpret_cast<uint2*>(Ke + row * D)[8 + c] = make_uint2(e5m2x4(h2[0], h2[1]), e5m2x4(h2[2], h2[3]));
-    reinterpret_cast<uint2*>(Kl + row * D)[c] = make_uint2(e5m2x4(l1[0], l1[1]), e5m2x4(l1[2], l1[3]));
-    reinterpret_cast<uint2*>(Kl + row * D)[8 + c] = make_uint2(e5m2x4(l2[0], l2[1]), e5m2x4(l2[2], l2[3]));
+    const uint2 eh1 = make_uint2(e5m2x4(h1[0], h1[1]), e5m2x4(h1[2], h1[3])), eh2 = make_uint2(e5m2x4(h2[0], h2[1]), e5m2x4(h2[2], h2[3]));
+    const uint2 el1 = make_uint2(e5m2x4(l1[0], l1[1]), e5m2x4(l1[2], l1[3])), el2 = make_uint2(e5m2x4(l2[0], l2[1]), e5m2x4(l2[2], l2[3]));
+    const int kvh = (int)(row - k * H_kv);
+    if (selinfo != nullptr && selinfo[kvh * 16 + 8] == 0u) {
+        // selective mode: one 128-byte row per key = [lo1 | lo2 | hi1 | hi2] (16 B each: two pairs per chunk) | unused
+        const uint32_t sj = selinfo[kvh * 16 + c];
+        unsigned short* dst = reinterpret_cast<unsigned short*>(Ke + row * D);
+        dst[c] = (unsigned short)__byte_perm(el1.x, el1.y, sj);
+        dst[8 + c] = (unsigned short)__byte_perm(el2.x, el2.y, sj);
+        dst[16 + c] = (unsigned short)__byte_perm(eh1.x, eh1.y, sj);
+        dst[24 + c] = (unsigned short)__byte_perm(eh2.x, eh2.y, sj);
+    } else {
+        reinterpret_cast<uint2*>(Ke + row * D)[c] = eh1;
+        reinterpret_cast<uint2*>(Ke + row * D)[8 + c] = eh2;
+        reinterpret_cast<uint2*>(Kl + row * D)[c] = el1;
+        reinterpret_cast<uint2*>(Kl + row * D)[8 + c] = el2;
+    }
 }
 
 }  // namespace
@@ -557,7 +643,8 @@ size_t umma_prefill_workspace_bytes(long long L, int, int, int d) { return two_l
 // pre-rotated variant: tables, then K'hi (fp16), K' (e5m2), K'lo (e5m2), each [L, H_kv, 128]
 size_t umma_prefill_prerot_workspace_bytes(long long L, int H_kv, int d) {
     const size_t n = (size_t)L * H_kv * d;
-    return two_level_bytes(L + 256, d) + align256(2 * n) + 2 * align256(n);
+    return two_level_bytes(L + 256, d) + align256(2 * n) + 2 * align256(n) + align256((size_t)H_kv * 64 * 4 * 2) +
+           align256((size_t)H_kv * 16 * 4);       // + pair energies of K and Q, selection table
 }
 
 int launch_prefill_umma(const void* Q, const void* K, const void* V, void* out, float* lse, long long L, int H_q,
@@ -575,6 +662,7 @@ int launch_prefill_umma(const void* Q, const void* K, const void* V, void* out, 
     p.bifocal = bifocal ? 1 : 0;
     p.precise = precise;
     p.prerot = 0;
+    p.selinfo = nullptr;
     CUtensorMap tmKh = tmK, tmKe = tmK, tmKl = tmK;
     p.lo = nullptr; p.hi = nullptr;
     if (bifocal) {
@@ -583,15 +671,34 @@ int launch_prefill_umma(const void* Q, const void* K, const void* V, void* out, 
         p.lo = reinterpret_cast<const float2*>((unsigned char*)ws + 256);
         p.hi = p.lo + 256 * (d / 2);
         if (prerot) {
-            if (precise == 1) precise = p.precise = 2;               // the scratch holds the e5m2 cross-term operands only
+            // the scratch holds e5m2 cross-term operands only: the fp16 mode is served by the full e5m2 terms (2),
+            // the default by the selective e5m2 terms (3) with a per-head fallback to 2
+            precise = p.precise = (precise == 0 ? 0 : precise == 1 ? 2 : 3);
             const size_t n = (size_t)L * H_kv * d;
             unsigned char* base = (unsigned char*)ws + two_level_bytes(L + 256, d);
             __half* Kh = reinterpret_cast<__half*>(base);
             unsigned char* Ke = base + align256(2 * n);
             unsigned char* Kl = Ke + align256(n);
+            uint32_t* selinfo = nullptr;
+            if (precise == 3) {
+                float* eK = reinterpret_cast<float*>(Kl + align256(n));
+                float* eQ = eK + (size_t)H_kv * 64;
+                selinfo = reinterpret_cast<uint32_t*>(reinterpret_cast<unsigned char*>(eK) + align256((size_t)H_kv * 64 * 4 * 2));
+                if (cudaMemsetAsync(eK, 0, (size_t)H_kv * 64 * 4 * 2, st) != cudaSuccess) return check_launch("memset");
+                const int sk = 1, sq = 8;                              // every key row, every 8th query row
+                const unsigned bk = (unsigned)((L / sk + 255) / 256), bq = (unsigned)((L / sq + 255) / 256);
+                pair_energy_kernel<<<dim3(bk ? bk : 1, H_kv), 256, 0, st>>>((const __nv_bfloat16*)K, eK, L, H_kv, 1, sk);
+                pair_energy_kernel<<<dim3(bq ? bq : 1, H_q), 256, 0, st>>>((const __nv_bfloat16*)Q, eQ, L, H_q, H_q / H_kv, sq);
+                const double nk = (double)((L + sk - 1) / sk), nq = (double)((L + sq - 1) / sq) * (H_q / H_kv);
+                select_pairs_kernel<<<H_kv, 64, 0, st>>>(eK, eQ, selinfo, (float)(1.0 / nk), (float)(1.0 / nq));
+                note_launch(3);
+                rc = check_launch("select_pairs_kernel");
+                if (rc != JETLONG_OK) return rc;
+                p.selinfo = selinfo;
+            }
             const long long items = L * H_kv * 8;
             prerotate_k_kernel<<<(unsigned)((items + 255) / 256), 256, 0, st>>>((const __nv_bfloat16*)K, Kh, Ke, Kl, L, H_kv, G,
-                                                                               p.lo, p.hi);
+                                                                               p.lo, p.hi, selinfo);
             note_launch();
             rc = check_launch("prerotate_k_kernel");
             if (rc != JETLONG_OK) return rc;

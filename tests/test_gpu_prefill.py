@@ -177,3 +177,27 @@ def test_prerotated_unsupported_shapes_are_refused():
     with pytest.raises(B.JetlongError):
         J.jetlong_prefill_prerotated(Q, K, V, w_local=7, w_pretrained=100, rope_theta=1e4,
                                      workspace=torch.zeros(1 << 20, dtype=torch.uint8, device=DEV))
+
+
+def test_prerotated_selective_compensation_and_its_fallback():
+    """The default precision of the workspace variant compensates two pairs per 8-pair chunk (chosen from the pair
+    energies of K and Q); a head whose remaining channels are too loud falls back to the full e5m2 cross terms.
+    Both must meet the lse tolerance; COMPENSATED_F16 selects the full cross terms for every head."""
+    from paper_2607_07740_b200 import binding as B
+    L, H_q, H_kv, d, theta, w_pre, w0 = 4096, 4, 2, 128, 1e6, 1024, 128
+    rows, heads = all_pairs(L, H_q)
+    pick = np.random.RandomState(1).choice(len(rows), 2048, replace=False)
+    rows, heads = rows[pick], heads[pick]
+    for name, scale_all in (("4 outlier channels", 1.0), ("every K channel x1.5 (fallback)", 1.5)):
+        Q, K, V = W.make_qkv(L, H_q, H_kv, d, theta, "bf16", 12, True, DEV)
+        if scale_all != 1.0:
+            K = (K.float() * scale_all).to(torch.bfloat16)
+        ro, rl = oracle_rows(Q, K, V, rows, heads, w_local=w0, w_pretrained=w_pre, rope_theta=theta)
+        try:
+            for mode in (B.PRECISION_COMPENSATED, B.PRECISION_COMPENSATED_F16):
+                J.jetlong_set_prefill_precision(mode)
+                out, lse = J.jetlong_prefill_prerotated(Q, K, V, w_local=w0, w_pretrained=w_pre, rope_theta=theta)
+                torch.cuda.synchronize()
+                check(*gather(out, lse, rows, heads), ro, rl, Q.dtype, "prerotated, %s, mode %d" % (name, mode))
+        finally:
+            J.jetlong_set_prefill_precision(B.PRECISION_COMPENSATED)
