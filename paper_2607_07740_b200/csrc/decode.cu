@@ -328,6 +328,7 @@ __global__ void __launch_bounds__(D) decode_merge_kernel(const float* __restrict
     __shared__ float w_s[1024];
     __shared__ float red[2];
     const int h = blockIdx.x, tid = threadIdx.x, lane = tid & 31;
+    asm volatile("griddepcontrol.wait;" ::: "memory");           // launched programmatically behind the scan kernel
     if (tid < 32) {
         float M = -INFINITY;
         for (int s = lane; s < nsplit; s += 32) M = fmaxf(M, part[((size_t)s * H_q + h) * SS + D]);
@@ -412,7 +413,16 @@ static int launch_decode_td(const void* q, const void* K, const void* V, void* o
         int ns = 0;
         int rc = launch_decode_umma(q, K, V, p.part, L, H_q, H_kv, w0, G, bifocal, p.lo, p.hi, &ns, st);
         if (rc != JETLONG_OK) return rc;
-        decode_merge_kernel<T, D><<<H_q, D, 0, st>>>(p.part, ns, H_q, (T*)out, lse);
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(H_q);
+        cfg.blockDim = dim3(D);
+        cfg.stream = st;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = at;
+        cfg.numAttrs = 1;
+        cudaLaunchKernelEx(&cfg, decode_merge_kernel<T, D>, (const float*)p.part, ns, H_q, (T*)out, lse);
         note_launch();
         return check_launch("decode_merge_kernel");
     }

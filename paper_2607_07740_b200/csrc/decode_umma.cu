@@ -93,6 +93,11 @@ __device__ __forceinline__ uint16_t bf16_bits(float f) {
     return *reinterpret_cast<const uint16_t*>(&b);
 }
 
+// programmatic dependent launch: the kernel starts while its stream predecessor (the table check, or the previous
+// step's merge) is still draining; griddep_wait() returns once that grid has completed and its writes are visible
+__device__ __forceinline__ void griddep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void griddep_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 constexpr uint32_t IDESC_S_BF16 = idesc_f16(1, 1, 0, 0, BN, NH);
 constexpr uint32_t IDESC_S_F16 = idesc_f16(0, 0, 0, 0, BN, NH);
 constexpr uint32_t IDESC_S_F16_N32 = idesc_f16(0, 0, 0, 0, BN, 2 * NH);
@@ -135,6 +140,21 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
     const DPlan plan(p, split);
     const float sl2 = (1.0f / sqrtf((float)D)) * kLog2e;
 
+    // the query loads go out before the TMA streams start: behind ~14 MB of in-flight cache tiles they take microseconds
+    const int rt = tid - 96;                                           // rotate-group thread index
+    __nv_bfloat16 qv1[NH * 64 / RT], qv2[NH * 64 / RT];
+    if (warp >= 3 && warp < 3 + RW) {
+#pragma unroll
+        for (int it = 0; it < NH * 64 / RT; ++it) {
+            const int idx = rt + it * RT;
+            if (idx < p.g * 64) {
+                const __nv_bfloat16* qh = p.q + (size_t)(kvh * p.g + (idx >> 6)) * D;
+                qv1[it] = qh[idx & 63];
+                qv2[it] = qh[(idx & 63) + 64];
+            }
+        }
+    }
+    griddep_launch_dependents();                                       // the merge kernel may queue up behind us
     if (tid == 0) {
         for (int i = 0; i < KS; ++i) { mbar_init(&bars->k_full[i], 1); mbar_init(&bars->k_ready[i], RW); mbar_init(&bars->k_empty[i], 1); }
         for (int i = 0; i < VS; ++i) { mbar_init(&bars->v_full[i], 1); mbar_init(&bars->v_empty[i], 1); }
@@ -245,10 +265,13 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
         for (int i = t; i < QBUF / 4; i += RT) reinterpret_cast<uint32_t*>(sP)[i] = 0u;
         named_bar_sync(1, RT);
         const long long nq = qpos - qpos / p.G;                      // -Delta(q) >= 0, Eq.(5)
-        for (int idx = t; idx < p.g * 64; idx += RT) {
+        if (plan.nr > 0) griddep_wait();                             // the rotation tables come from the preceding kernel
+#pragma unroll
+        for (int it = 0; it < NH * 64 / RT; ++it) {
+            const int idx = t + it * RT;
+            if (idx >= p.g * 64) break;
             const int h = idx >> 6, i = idx & 63;
-            const __nv_bfloat16* qh = p.q + (size_t)(kvh * p.g + h) * D;
-            const __nv_bfloat16 b1 = qh[i], b2 = qh[i + 64];
+            const __nv_bfloat16 b1 = qv1[it], b2 = qv2[it];
             *reinterpret_cast<__nv_bfloat16*>(sQ + bop_off(h, i)) = b1;
             *reinterpret_cast<__nv_bfloat16*>(sQ + bop_off(h, i + 64)) = b2;
             if (plan.nr > 0) {
@@ -391,6 +414,7 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
             for (int h = 0; h < 16; ++h) og[h] = 0u;
         }
         constexpr int SS = D + 2;
+        griddep_wait();                                              // the previous step's merge may still be reading the partials
 #pragma unroll
         for (int h = 0; h < NG; ++h) {
             if (h < g) {
@@ -445,7 +469,17 @@ int launch_decode_umma(const void* q, const void* K, const void* V, float* part,
               : p.g <= 8 ? decode_umma_kernel<8> : decode_umma_kernel<16>;
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES) != cudaSuccess)
         return check_launch("decode_umma attr");
-    kern<<<dim3(ns, H_kv), NTHREADS, SMEM_BYTES, st>>>(tmK, tmV, p);
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(ns, H_kv);
+    cfg.blockDim = dim3(NTHREADS);
+    cfg.dynamicSmemBytes = SMEM_BYTES;
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    cudaLaunchKernelEx(&cfg, kern, tmK, tmV, p);
     note_launch();
     *nsplit_out = ns;
     return check_launch("decode_umma_kernel");

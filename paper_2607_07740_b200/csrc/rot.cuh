@@ -152,8 +152,10 @@ template <int ROWS> struct KRot {
 };
 
 __device__ __forceinline__ uint64_t neg2(uint64_t v) { return v ^ 0x8000000080000000ull; }
+// both halves on the ALU pipe (PRMT, LOP3): ptxas turns `w << 16` into IMAD.SHL, which competes with the rotation's
+// FFMA2/FMUL2 for the FMA pipe -- the pipe that bounds the rotate group (measured)
 __device__ __forceinline__ uint64_t bf16x2_to_f32x2(uint32_t w) {
-    return (uint64_t)(w << 16) | ((uint64_t)(w & 0xffff0000u) << 32);
+    return (uint64_t)__byte_perm(w, 0u, 0x1044) | ((uint64_t)(w & 0xffff0000u) << 32);
 }
 __device__ __forceinline__ uint32_t f16x2_rn(float lo, float hi) {
     uint32_t y;
@@ -167,7 +169,9 @@ __device__ __forceinline__ void split_hi_lo(uint64_t y, uint32_t& h, uint32_t& l
     h = f16x2_rn(a, b);
     if (precise) {
         const float2 f = __half22float2(*reinterpret_cast<const __half2*>(&h));
-        l = f16x2_rn(a - f.x, b - f.y);
+        float ra, rb;
+        unpack2(fsub2(y, pack2(f.x, f.y)), ra, rb);                   // one packed subtract for the two residuals
+        l = f16x2_rn(ra, rb);
     }
 }
 

@@ -50,6 +50,7 @@ size_t two_level_bytes(long long L, int d) {
 // steps 1..n), otherwise it rebuilds the table and then seals the header.
 __global__ void __launch_bounds__(1024) two_level_kernel(unsigned char* __restrict__ region, long long n_hi, int half,
                                                          double theta, double log2_theta, int d) {
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");   // a programmatically launched consumer (decode) may start
     TableHeader* hdr = reinterpret_cast<TableHeader*>(region);
     if (hdr->magic == kMagic && hdr->theta == theta && hdr->n_hi == n_hi && hdr->d == d) return;   // uniform
     float2* lo = reinterpret_cast<float2*>(region + 256);
