@@ -177,7 +177,7 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--variant", default="bifocal", choices=["bifocal", "fast", "control", "decode", "decode-control"],
+    ap.add_argument("--variant", default="bifocal", choices=["bifocal", "fast", "control", "prerotated", "unfused", "decode", "decode-control"],
                     help="what the timed loop runs (default: the bifocal prefill in its default, compensated "
                          "precision); the other values exist for profiling one kernel at a time")
     ap.add_argument("--no-extras", action="store_true", help="skip control / decode / e2e / oracle legs (profiling)")
@@ -220,6 +220,7 @@ def main():
     out = torch.empty_like(Q)
     lse = torch.empty((cfg.H_q, cfg.L), dtype=torch.float32, device=dev)
     ws = B.alloc_workspace(B.OP_PREFILL, cfg.L, cfg.H_q, cfg.H_kv, cfg.d, B.BF16, dev)
+    wsp = B.alloc_workspace(B.OP_PREFILL_PREROTATED, cfg.L, cfg.H_q, cfg.H_kv, cfg.d, B.BF16, dev)
     kw = dict(w_local=cfg.w_local, w_pretrained=cfg.w_pretrained, rope_theta=cfg.rope_theta)
     fl = flops_causal(cfg.L, cfg.H_q, cfg.d)
 
@@ -227,6 +228,14 @@ def main():
         if variant == "control":
             return lambda: J.jetlong_causal_prefill(Q, K, V, out=out, lse=lse, workspace=ws)
         mode = B.PRECISION_FAST if variant == "fast" else B.PRECISION_COMPENSATED
+        if variant == "unfused":                                  # the paper's three calls + Eq.(7)
+            wsu = B.alloc_workspace(B.OP_PREFILL_UNFUSED, cfg.L, cfg.H_q, cfg.H_kv, cfg.d, B.BF16, dev)
+            return lambda: J.jetlong_prefill_unfused(Q, K, V, out=out, lse=lse, workspace=wsu, **kw)
+        if variant == "prerotated":                               # K rotated once into a scratch
+            def g():
+                J.jetlong_set_prefill_precision(mode)
+                J.jetlong_prefill_prerotated(Q, K, V, out=out, lse=lse, workspace=wsp, **kw)
+            return g
 
         def f():
             J.jetlong_set_prefill_precision(mode)
@@ -266,6 +275,9 @@ def main():
     cfgd = workload_config(cfg)
     cfgd["variant"] = {"bifocal": "bifocal prefill, default precision (compensated remote QK^T, meets the lse tolerance)",
                        "fast": "bifocal prefill, JETLONG_PRECISION_FAST (misses the lse tolerance on outlier inputs)",
+                       "unfused": "the paper's unfused three-call procedure (A + B - C, Eq.(7)) on the same kernel: a baseline",
+                       "prerotated": "bifocal prefill, workspace variant (jetlong_prefill_prerotated: K' written once to a "
+                                     "scratch, selective e5m2 compensation; meets the lse tolerance)",
                        "control": "matched causal control kernel"}[args.variant]
     line = {"metric": METRIC, "value": value, "unit": "TFLOP/s", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
@@ -296,7 +308,7 @@ def main():
                                     "precision and the straddle revisit are executed but not credited"}
         # ---- the other prefill variants on the same buffers, interleaved after the main loop ---------------
         others = {}
-        for name in ("control", "fast", "bifocal"):
+        for name in ("control", "fast", "prerotated", "unfused", "bifocal"):
             if name == args.variant:
                 continue
             tot, pp, _ = timed(make_step(name), max(3, min(args.steps, 10)), 2)
@@ -306,6 +318,18 @@ def main():
         line["prefill_variants"] = others
         if "control" in others and args.variant != "control":
             line["control"] = dict(others["control"], bifocal_over_control=others["control"]["ms"] / ms_per_step)
+            if "prerotated" in others:
+                others["prerotated"]["over_control"] = others["control"]["ms"] / others["prerotated"]["ms"]
+                others["prerotated"]["note"] = ("SURVEY.md 8(f)-1 ablation: the same kernel with the in-loop key rotation "
+                                                "replaced by one pass that writes K' (fp16 + e5m2 cross-term operands) "
+                                                "to a workspace scratch; the stored K is still never written")
+            if "unfused" in others:
+                others["unfused"]["fused_speedup"] = others["unfused"]["ms"] / ms_per_step
+                others["unfused"]["note"] = ("SURVEY.md 8(f)-2: window(Q,K) + causal(Q',K') + window(Q',K') + merge with the minus "
+                                             "sign; the paper reports fused 1.43-1.56x faster than unfused on H100 (P:226); lse "
+                                             "only ~3e-3 here (one fp16 rounding, no compensation)")
+        # ---- the same three kernels at 128K (BASELINE.json configs[2], Qwen3-4B-shaped) --------------------
+        line["prefill_128k"] = bench_prefill_128k(J, B, W, dev, pk, timed)
         J.jetlong_set_prefill_precision(B.PRECISION_COMPENSATED)
         # ---- end to end through the host-buffer C-ABI call -----------------------------------------------
         Qh, Kh, Vh = Q.cpu().pin_memory(), K.cpu().pin_memory(), V.cpu().pin_memory()
@@ -333,6 +357,29 @@ def main():
         print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()
+
+
+def bench_prefill_128k(J, B, W, dev, pk, timed):
+    """configs[2]: L=131072, H_q=32, H_kv=8 (G=4): control, bifocal (on the fly) and the workspace variant, 3 calls each."""
+    c = W.C3
+    Q, K, V = W.make_config_inputs(c, dev)
+    out = torch.empty_like(Q)
+    lse = torch.empty((c.H_q, c.L), dtype=torch.float32, device=dev)
+    wsp = B.alloc_workspace(B.OP_PREFILL_PREROTATED, c.L, c.H_q, c.H_kv, c.d, B.BF16, dev)
+    kw = dict(w_local=c.w_local, w_pretrained=c.w_pretrained, rope_theta=c.rope_theta)
+    fl = flops_causal(c.L, c.H_q, c.d)
+    J.jetlong_set_prefill_precision(B.PRECISION_COMPENSATED)
+    res = {"workload": "BASELINE.json configs[2]: Qwen3-4B-shaped single-layer prefill, L=131072, H_q=32, H_kv=8, G=4, w_local=4096"}
+    for name, fn in (("control", lambda: J.jetlong_causal_prefill(Q, K, V, out=out, lse=lse, workspace=wsp)),
+                     ("bifocal", lambda: J.jetlong_prefill(Q, K, V, out=out, lse=lse, workspace=wsp, **kw)),
+                     ("prerotated", lambda: J.jetlong_prefill_prerotated(Q, K, V, out=out, lse=lse, workspace=wsp, **kw))):
+        tot, pp, _ = timed(fn, 3, 1)
+        ms = tot / len(pp)
+        res[name] = {"ms": ms, "tflops": fl / (ms * 1e-3) / 1e12,
+                     "frac_of_bf16_burst_peak": fl / (ms * 1e-3) / 1e12 / pk["tflops_burst"]}
+    for name in ("bifocal", "prerotated"):
+        res[name]["over_control"] = res["control"]["ms"] / res[name]["ms"]
+    return res
 
 
 def _umma_active(B, cfg):

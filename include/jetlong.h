@@ -44,7 +44,7 @@ enum { JETLONG_BF16 = 0, JETLONG_FP32 = 1 };
 
 /* op codes for jetlong_workspace_bytes */
 enum { JETLONG_OP_PREFILL = 0, JETLONG_OP_DECODE = 1, JETLONG_OP_CAUSAL_PREFILL = 2, JETLONG_OP_CAUSAL_DECODE = 3,
-       JETLONG_OP_PREFILL_PREROTATED = 4 };
+       JETLONG_OP_PREFILL_PREROTATED = 4, JETLONG_OP_PREFILL_UNFUSED = 5 };
 
 /* Eq.(2): G = max(1, ceil(L / w_pretrained)), integer arithmetic on the host.
  * Returns -1 if L < 1 or w_pretrained < 1. */
@@ -81,6 +81,23 @@ int jetlong_prefill_prerotated(const void* Q, const void* K, const void* V, void
                                int64_t L, int H_q, int H_kv, int head_dim,
                                int64_t w_local, int64_t w_pretrained, double rope_theta,
                                int dtype, void* workspace, size_t workspace_bytes, void* stream);
+
+/*
+ * The paper's UNFUSED procedure on the GPU (Section 3.3, "Jet-Long (unfused)" of Table 7), a baseline
+ * for the fused kernel, never the product path: three launches of the same tcgen05 attention kernel --
+ *   A: sliding-window attention (0 <= q-k <= w_local) on the stored Q, K;
+ *   B: full causal attention on Q' = R(Delta q) Q, K' = R(Delta k) K (both written once to the workspace as fp16);
+ *   C: sliding-window attention on Q', K' --
+ * each returning (O_X, l_X), then Eq.(7) WITH the minus sign: O = (W_A O_A + W_B O_B - W_C O_C) / (W_A + W_B - W_C).
+ * The band is computed three times and the remote operands carry one fp16 rounding without compensation, so on
+ * outlier-channel inputs lse is only good to ~3e-3 (the fused default: ~3e-4); out stays within the bf16 tolerance.
+ * bf16, head_dim 128, even H_q / H_kv; workspace >= jetlong_workspace_bytes(JETLONG_OP_PREFILL_UNFUSED, ...)
+ * (tables + Q', K', O_B, O_C, l_B, l_C: about 4.5x the size of Q).
+ */
+int jetlong_prefill_unfused(const void* Q, const void* K, const void* V, void* out, float* lse,
+                            int64_t L, int H_q, int H_kv, int head_dim,
+                            int64_t w_local, int64_t w_pretrained, double rope_theta,
+                            int dtype, void* workspace, size_t workspace_bytes, void* stream);
 
 /*
  * Bifocal batch-1 decode: one query row per head at position L-1 against cache rows

@@ -15,13 +15,14 @@ _lib = None
 
 OK, INVALID_ARG, UNSUPPORTED, CUDA_ERROR = 0, 1, 2, 3
 BF16, FP32 = 0, 1
-OP_PREFILL, OP_DECODE, OP_CAUSAL_PREFILL, OP_CAUSAL_DECODE, OP_PREFILL_PREROTATED = 0, 1, 2, 3, 4
+OP_PREFILL, OP_DECODE, OP_CAUSAL_PREFILL, OP_CAUSAL_DECODE, OP_PREFILL_PREROTATED, OP_PREFILL_UNFUSED = \
+    0, 1, 2, 3, 4, 5
 PRECISION_COMPENSATED, PRECISION_FAST, PRECISION_COMPENSATED_F16 = 0, 1, 2
 
 EXPORTS = ["jetlong_group_size", "jetlong_workspace_bytes", "jetlong_prefill", "jetlong_decode",
            "jetlong_causal_prefill", "jetlong_causal_decode", "jetlong_prefill_host", "jetlong_status_string",
            "jetlong_launch_count", "jetlong_set_prefill_impl", "jetlong_prefill_uses_umma",
-           "jetlong_set_prefill_precision"]
+           "jetlong_set_prefill_precision", "jetlong_prefill_prerotated", "jetlong_prefill_unfused"]
 
 
 class JetlongError(RuntimeError):
@@ -48,6 +49,8 @@ def lib():
         L.jetlong_prefill.argtypes = [vp] * 5 + tail
         L.jetlong_prefill_prerotated.restype = i32
         L.jetlong_prefill_prerotated.argtypes = [vp] * 5 + tail
+        L.jetlong_prefill_unfused.restype = i32
+        L.jetlong_prefill_unfused.argtypes = [vp] * 5 + tail
         L.jetlong_decode.restype = i32
         L.jetlong_decode.argtypes = [vp] * 5 + tail
         ctail = [i64, i32, i32, i32, i32, vp, sz, vp]
@@ -145,6 +148,18 @@ def jetlong_prefill_prerotated(Q, K, V, *, w_local, w_pretrained, rope_theta, ou
     _check(lib().jetlong_prefill_prerotated(Q.data_ptr(), K.data_ptr(), V.data_ptr(), out.data_ptr(), lse.data_ptr(),
                                             L, H_q, H_kv, d, int(w_local), int(w_pretrained), float(rope_theta), dt,
                                             workspace.data_ptr(), workspace.numel(), _stream()))
+    return out, lse
+
+
+def jetlong_prefill_unfused(Q, K, V, *, w_local, w_pretrained, rope_theta, out=None, lse=None, workspace=None):
+    """The paper's unfused three-call procedure (A + B - C, Eq.(7)) on the GPU: a baseline, not the product path."""
+    L, H_q, H_kv, d, out, lse = _prefill_args(Q, K, V, out, lse)
+    dt = _dt(Q)
+    if workspace is None:
+        workspace = alloc_workspace(OP_PREFILL_UNFUSED, L, H_q, H_kv, d, dt, Q.device)
+    _check(lib().jetlong_prefill_unfused(Q.data_ptr(), K.data_ptr(), V.data_ptr(), out.data_ptr(), lse.data_ptr(),
+                                         L, H_q, H_kv, d, int(w_local), int(w_pretrained), float(rope_theta), dt,
+                                         workspace.data_ptr(), workspace.numel(), _stream()))
     return out, lse
 
 

@@ -25,6 +25,9 @@ int check_launch(const char* what) {
 bool umma_prefill_supported(long long L, int H_q, int H_kv, int d, int dtype);
 size_t umma_prefill_workspace_bytes(long long L, int H_q, int H_kv, int d);
 size_t umma_prefill_prerot_workspace_bytes(long long L, int H_kv, int d);
+size_t umma_prefill_unfused_workspace_bytes(long long L, int H_q, int H_kv, int d);
+int launch_prefill_unfused(const void* Q, const void* K, const void* V, void* out, float* lse, long long L, int H_q,
+                           int H_kv, int d, long long w0, long long G, double theta, void* ws, cudaStream_t st);
 int launch_prefill_umma(const void* Q, const void* K, const void* V, void* out, float* lse, long long L, int H_q,
                         int H_kv, int d, long long w0, long long G, double theta, bool bifocal, int precise, void* ws,
                         size_t ws_bytes, cudaStream_t st, bool prerot);
@@ -126,6 +129,8 @@ size_t jetlong_workspace_bytes(int op, int64_t L, int H_q, int H_kv, int head_di
         case JETLONG_OP_CAUSAL_PREFILL: return prefill_ws(L, H_q, H_kv, head_dim, dtype, false);
         case JETLONG_OP_DECODE:
         case JETLONG_OP_CAUSAL_DECODE: return decode_workspace_bytes(L, H_q, H_kv, head_dim);
+        case JETLONG_OP_PREFILL_UNFUSED:
+            return umma_prefill_supported(L, H_q, H_kv, head_dim, dtype) ? umma_prefill_unfused_workspace_bytes(L, H_q, H_kv, head_dim) : 0;
         case JETLONG_OP_PREFILL_PREROTATED:
             return umma_prefill_supported(L, H_q, H_kv, head_dim, dtype) ? umma_prefill_prerot_workspace_bytes(L, H_kv, head_dim) : 0;
         default: return 0;
@@ -144,6 +149,24 @@ int jetlong_prefill_prerotated(const void* Q, const void* K, const void* V, void
                                void* workspace, size_t workspace_bytes, void* stream) {
     return prefill_common(Q, K, V, out, lse, L, H_q, H_kv, head_dim, w_local, w_pretrained, rope_theta, dtype,
                           workspace, workspace_bytes, stream, true, true);
+}
+
+int jetlong_prefill_unfused(const void* Q, const void* K, const void* V, void* out, float* lse, int64_t L, int H_q,
+                            int H_kv, int head_dim, int64_t w_local, int64_t w_pretrained, double rope_theta, int dtype,
+                            void* workspace, size_t workspace_bytes, void* stream) {
+    int rc = validate(Q, K, V, out, lse, L, H_q, H_kv, head_dim, w_local, w_pretrained, rope_theta, dtype);
+    if (rc != JETLONG_OK) return rc;
+    if (!umma_prefill_supported(L, H_q, H_kv, head_dim, dtype)) return JETLONG_UNSUPPORTED;
+    const long long G = jetlong_group_size(L, w_pretrained);
+    if (G == 1 || w_local >= L - 1)                          // nothing is remote: the control, as in jetlong_prefill
+        return prefill_common(Q, K, V, out, lse, L, H_q, H_kv, head_dim, w_local, w_pretrained, rope_theta, dtype,
+                              workspace, workspace_bytes, stream, true);
+    const size_t need = umma_prefill_unfused_workspace_bytes(L, H_q, H_kv, head_dim);
+    if (!workspace || workspace_bytes < need || !aligned16(workspace)) return JETLONG_INVALID_ARG;
+    rc = device_ok();
+    if (rc != JETLONG_OK) return rc;
+    return launch_prefill_unfused(Q, K, V, out, lse, L, H_q, H_kv, head_dim, w_local, G, rope_theta, workspace,
+                                  (cudaStream_t)stream);
 }
 
 int jetlong_causal_prefill(const void* Q, const void* K, const void* V, void* out, float* lse, int64_t L, int H_q,

@@ -76,6 +76,8 @@ struct Params {
     int H_q, H_kv, g;
     int bifocal, precise;
     int prerot;                                       // remote K tiles come pre-rotated from the workspace (8(f)-1)
+    int window_only;                                  // only the local band 0 <= q-k <= w0 (calls A and C of the unfused path)
+    int qk_f16;                                       // Q and K hold fp16 (pre-rotated operands of calls B and C), not bf16
     const float2* lo;
     const float2* hi;
     const uint32_t* selinfo;                          // [H_kv][16]: 8 PRMT selectors (two pairs per 8-pair chunk), full-mode flag
@@ -85,7 +87,7 @@ struct Visit { int kt; int mode; };                   // mode 0 = causal/control
 
 struct Plan {
     int qb, n_local, n_remote, kt_hi, nv;
-    __device__ Plan(int qb_, long long w0, bool bifocal) : qb(qb_) {
+    __device__ Plan(int qb_, long long w0, bool bifocal, bool window_only = false) : qb(qb_) {
         const long long q0 = (long long)qb * BM;
         if (!bifocal) { n_local = qb + 1; n_remote = 0; kt_hi = -1; nv = n_local; return; }
         long long t = q0 - w0 - (BN - 1);                              // local iff k0 >= t
@@ -95,6 +97,7 @@ struct Plan {
         kt_hi = u < 0 ? -1 : (int)(u / BN);
         if (kt_hi > qb) kt_hi = qb;
         n_remote = kt_hi + 1;
+        if (window_only) { n_remote = 0; kt_hi = -1; }
         nv = n_local + n_remote;
     }
     __device__ Visit at(int v, bool bifocal) const {
@@ -212,7 +215,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_consta
     // highest-energy pairs of every 8-pair chunk; a KV head whose other channels are too loud falls back to 2
     int precise = p.precise;
     if (precise == 3 && __ldg(p.selinfo + kvh * 16 + 8) != 0u) precise = 2;
-    const Plan plan(qb, p.w0, bifocal);
+    const Plan plan(qb, p.w0, bifocal, p.window_only != 0);
 
     if (tid == 0) {
         for (int i = 0; i < NS; ++i) { mbar_init(&bars->kv_full[i], 1); mbar_init(&bars->kv_ready[i], 8); mbar_init(&bars->kv_empty[i], 1); }
@@ -265,10 +268,11 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_consta
                 const uint32_t kb = smem0 + (v % NS) * STAGE_BYTES, klb = kb + KH_BYTES;
                 if (elect_one()) {
                     if (x.mode != 2) {
+                        const uint32_t idesc = p.qk_f16 ? IDESC_QK_F16 : IDESC_QK_BF16;
 #pragma unroll
                         for (int ks = 0; ks < D / 16; ++ks)
                             umma2_ts(dS, tm + TM_QA + ks * 8,
-                                     smem_desc_sw128(kb + (ks >> 2) * KBOX + (ks & 3) * 32, 16, 1024), IDESC_QK_BF16, ks > 0);
+                                     smem_desc_sw128(kb + (ks >> 2) * KBOX + (ks & 3) * 32, 16, 1024), idesc, ks > 0);
                     } else {
 #pragma unroll
                         for (int ks = 0; ks < D / 16; ++ks)
@@ -596,6 +600,62 @@ __global__ void __launch_bounds__(256) prerotate_k_kernel(const __nv_bfloat16* _
     }
 }
 
+// ---- 8(f)-2: the unfused three-call baseline ("Jet-Long (unfused)") ------------------------------
+// X' = R(Delta pos) X as fp16, one rounding: the remote-position operands of calls B and C.  Thread = (row, head, chunk).
+__global__ void __launch_bounds__(256) prerotate_hi_kernel(const __nv_bfloat16* __restrict__ X, __half* __restrict__ Xr,
+                                                           long long L, int H, long long G,
+                                                           const float2* __restrict__ lo, const float2* __restrict__ hi) {
+    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= L * H * 8) return;
+    const int c = (int)(idx & 7);
+    const long long row = idx >> 3;
+    const long long pos = row / H;
+    const uint4 u1 = __ldg(reinterpret_cast<const uint4*>(X + row * D) + c);
+    const uint4 u2 = __ldg(reinterpret_cast<const uint4*>(X + row * D) + 8 + c);
+    float cs_c[8], cs_s[8];
+    cs8(lo, hi, pos, G, 8 * c, cs_c, cs_s);
+    const uint32_t a[4] = {u1.x, u1.y, u1.z, u1.w}, b[4] = {u2.x, u2.y, u2.z, u2.w};
+    uint32_t h1[4], h2[4], l1[4], l2[4];
+    rot8(a, b, cs_c, cs_s, h1, h2, l1, l2);
+    reinterpret_cast<uint4*>(Xr + row * D)[c] = make_uint4(h1[0], h1[1], h1[2], h1[3]);
+    reinterpret_cast<uint4*>(Xr + row * D)[8 + c] = make_uint4(h2[0], h2[1], h2[2], h2[3]);
+}
+
+// Eq.(7) P:114 with the minus sign: O = (W_A O_A + W_B O_B - W_C O_C) / (W_A + W_B - W_C), W_X = exp(l_X - M).
+// A is read from and the result written to (out, lse).  Thread = (row q, head h, 8 channels).
+__global__ void __launch_bounds__(256) merge_abc_kernel(__nv_bfloat16* __restrict__ out, float* __restrict__ lse,
+                                                        const __nv_bfloat16* __restrict__ oB, const float* __restrict__ lB,
+                                                        const __nv_bfloat16* __restrict__ oC, const float* __restrict__ lC,
+                                                        long long L, int H_q) {
+    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= L * H_q * 16) return;
+    const int c = (int)(idx & 15);
+    const long long row = idx >> 4;                                   // q * H_q + h
+    const long long q = row / H_q;
+    const int h = (int)(row - q * H_q);
+    const size_t li = (size_t)h * L + q;
+    const float a = lse[li], b = lB[li], cc = lC[li];
+    const float M = fmaxf(a, b);
+    const float wA = __expf(a - M), wB = __expf(b - M), wC = __expf(cc - M);
+    const float den = wA + wB - wC;
+    const float inv = 1.0f / den;
+    uint4 ua = reinterpret_cast<const uint4*>(out + row * D)[c];
+    const uint4 ub = reinterpret_cast<const uint4*>(oB + row * D)[c], uc = reinterpret_cast<const uint4*>(oC + row * D)[c];
+    uint32_t* pa = reinterpret_cast<uint32_t*>(&ua);
+    const uint32_t* pb = reinterpret_cast<const uint32_t*>(&ub);
+    const uint32_t* pc = reinterpret_cast<const uint32_t*>(&uc);
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const float a0 = __uint_as_float(pa[j] << 16), a1 = __uint_as_float(pa[j] & 0xffff0000u);
+        const float b0 = __uint_as_float(pb[j] << 16), b1 = __uint_as_float(pb[j] & 0xffff0000u);
+        const float c0 = __uint_as_float(pc[j] << 16), c1 = __uint_as_float(pc[j] & 0xffff0000u);
+        pa[j] = bf16x2((wA * a0 + wB * b0 - wC * c0) * inv, (wA * a1 + wB * b1 - wC * c1) * inv);
+    }
+    reinterpret_cast<uint4*>(out + row * D)[c] = ua;
+    __syncwarp();                                                     // the 16 threads of a (q, h) all read lse first
+    if (c == 0) lse[li] = M + __logf(den);
+}
+
 }  // namespace
 
 // ---- host side ------------------------------------------------------------------------------------------
@@ -632,6 +692,12 @@ bool make_kv_tensor_map(CUtensorMap* m, const void* base, long long L, int H, in
     return make_tensor_map(m, base, L, H, rows, 2);
 }
 
+size_t umma_prefill_unfused_workspace_bytes(long long L, int H_q, int H_kv, int d) {
+    const size_t nq = (size_t)L * H_q * d, nk = (size_t)L * H_kv * d;
+    // tables | Q' fp16 | K' fp16 | out_B | out_C | lse_B | lse_C
+    return two_level_bytes(L + 256, d) + 3 * align256(2 * nq) + align256(2 * nk) + 2 * align256((size_t)L * H_q * 4);
+}
+
 bool umma_prefill_supported(long long L, int H_q, int H_kv, int d, int dtype) {
     if (dtype != JETLONG_BF16 || d != 128 || H_kv < 1 || H_q % H_kv) return false;
     const int g = H_q / H_kv;
@@ -662,6 +728,8 @@ int launch_prefill_umma(const void* Q, const void* K, const void* V, void* out, 
     p.bifocal = bifocal ? 1 : 0;
     p.precise = precise;
     p.prerot = 0;
+    p.window_only = 0;
+    p.qk_f16 = 0;
     p.selinfo = nullptr;
     CUtensorMap tmKh = tmK, tmKe = tmK, tmKl = tmK;
     p.lo = nullptr; p.hi = nullptr;
@@ -724,3 +792,62 @@ int launch_prefill_umma(const void* Q, const void* K, const void* V, void* out, 
 
 }  // namespace jetlong
 
+
+namespace jetlong {
+
+// One launch of the tcgen05 kernel on given operands: window_only = the local band only, qk_f16 = fp16 Q/K operands.
+static int launch_plain(const void* Q, const void* K, const void* V, void* out, float* lse, long long L, int H_q, int H_kv,
+                        long long w0, bool window_only, bool qk_f16, cudaStream_t st) {
+    CUtensorMap tmK, tmV;
+    if (!make_kv_tensor_map(&tmK, K, L, H_kv, 64) || !make_kv_tensor_map(&tmV, V, L, H_kv, 128)) return JETLONG_UNSUPPORTED;
+    Params p;
+    p.Q = (const __nv_bfloat16*)Q;
+    p.out = (__nv_bfloat16*)out;
+    p.lse = lse;
+    p.L = L; p.w0 = w0; p.G = 1;
+    p.H_q = H_q; p.H_kv = H_kv; p.g = H_q / H_kv;
+    p.bifocal = window_only ? 1 : 0;
+    p.precise = 0;
+    p.prerot = 0;
+    p.window_only = window_only ? 1 : 0;
+    p.qk_f16 = qk_f16 ? 1 : 0;
+    p.lo = nullptr; p.hi = nullptr; p.selinfo = nullptr;
+    if (cudaFuncSetAttribute(prefill_umma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES) != cudaSuccess)
+        return check_launch("prefill_umma attr");
+    const int n_qb = (int)((L + BM - 1) / BM);
+    prefill_umma_kernel<<<2u * (unsigned)n_qb * (unsigned)(H_q / 2), NTHREADS, SMEM_BYTES, st>>>(tmK, tmV, tmK, tmK, tmK, p);
+    note_launch();
+    return check_launch("prefill_umma_kernel");
+}
+
+// A = window attention on the stored Q, K; B = full causal attention at the remote positions; C = window attention at
+// the remote positions; then Eq.(7) with the minus sign.  Remote operands are rounded once to fp16.
+int launch_prefill_unfused(const void* Q, const void* K, const void* V, void* out, float* lse, long long L, int H_q,
+                           int H_kv, int d, long long w0, long long G, double theta, void* ws, cudaStream_t st) {
+    int rc = build_two_level(ws, L + 256, d, theta, st);
+    if (rc != JETLONG_OK) return rc;
+    const float2* lo = reinterpret_cast<const float2*>((unsigned char*)ws + 256);
+    const float2* hi = lo + 256 * (d / 2);
+    const size_t nq = (size_t)L * H_q * d, nk = (size_t)L * H_kv * d;
+    unsigned char* base = (unsigned char*)ws + two_level_bytes(L + 256, d);
+    __half* Qr = reinterpret_cast<__half*>(base);
+    __half* Kr = reinterpret_cast<__half*>(base + align256(2 * nq));
+    unsigned char* oB = base + align256(2 * nq) + align256(2 * nk);
+    unsigned char* oC = oB + align256(2 * nq);
+    float* lB = reinterpret_cast<float*>(oC + align256(2 * nq));
+    float* lC = reinterpret_cast<float*>(reinterpret_cast<unsigned char*>(lB) + align256((size_t)L * H_q * 4));
+    prerotate_hi_kernel<<<(unsigned)((L * H_q * 8 + 255) / 256), 256, 0, st>>>((const __nv_bfloat16*)Q, Qr, L, H_q, G, lo, hi);
+    prerotate_hi_kernel<<<(unsigned)((L * H_kv * 8 + 255) / 256), 256, 0, st>>>((const __nv_bfloat16*)K, Kr, L, H_kv, G, lo, hi);
+    note_launch(2);
+    rc = check_launch("prerotate_hi_kernel");
+    if (rc != JETLONG_OK) return rc;
+    if ((rc = launch_plain(Q, K, V, out, lse, L, H_q, H_kv, w0, true, false, st)) != JETLONG_OK) return rc;     // A
+    if ((rc = launch_plain(Qr, Kr, V, oB, lB, L, H_q, H_kv, w0, false, true, st)) != JETLONG_OK) return rc;     // B
+    if ((rc = launch_plain(Qr, Kr, V, oC, lC, L, H_q, H_kv, w0, true, true, st)) != JETLONG_OK) return rc;      // C
+    merge_abc_kernel<<<(unsigned)((L * H_q * 16 + 255) / 256), 256, 0, st>>>((__nv_bfloat16*)out, lse, (const __nv_bfloat16*)oB, lB,
+                                                                          (const __nv_bfloat16*)oC, lC, L, H_q);
+    note_launch();
+    return check_launch("merge_abc_kernel");
+}
+
+}  // namespace jetlong
