@@ -32,6 +32,8 @@ int launch_prefill_umma(const void* Q, const void* K, const void* V, void* out, 
                         int H_kv, int d, long long w0, long long G, double theta, bool bifocal, int precise, void* ws,
                         size_t ws_bytes, cudaStream_t st, bool prerot);
 
+extern int g_share_clusters;   // prefill_umma.cu
+
 static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; }
 
 static int validate(const void* a, const void* b, const void* c, const void* o, const void* l, long long L, int H_q,
@@ -229,7 +231,10 @@ const char* jetlong_status_string(int status) {
 
 int64_t jetlong_launch_count(void) { return g_launches.load(); }
 
-int jetlong_set_prefill_impl(int impl) { return g_prefill_impl.exchange(impl); }
+int jetlong_set_prefill_impl(int impl) {
+    g_share_clusters = impl == 2 ? 1 : 0;
+    return g_prefill_impl.exchange(impl);
+}
 
 int jetlong_set_prefill_precision(int mode) {
     if (mode != JETLONG_PRECISION_COMPENSATED && mode != JETLONG_PRECISION_FAST && mode != JETLONG_PRECISION_COMPENSATED_F16)

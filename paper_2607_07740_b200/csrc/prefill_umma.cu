@@ -62,6 +62,10 @@ struct Bars {
     uint64_t q_ready;          // leader: Q staged in TMEM by both rotate groups
     uint64_t q_local_done;     // both: the last local Q K^T has completed, Qa may be overwritten
     uint64_t q_rot_done;       // leader: Q' (hi, lo) staged in TMEM
+    // cluster of four (SHARE): the other CTA pair rotates half of our rows and writes them into our stages
+    uint64_t peer_full[NS];    // local: the rows rotated by the other pair have landed in our stage (bulk copy, complete_tx)
+    uint64_t peer_empty[NS];   // both: the OTHER pair's MMAs reading ITS stage s have completed (its commit, multicast to us)
+    uint64_t peer_go;          // both: the other pair's last local visit has completed (all its stages are free)
     uint32_t tmem_base;
     float xchg[4 * BM];        // row-max / row-sum exchange between the two column halves of a row
 };
@@ -100,6 +104,8 @@ struct Plan {
         if (window_only) { n_remote = 0; kt_hi = -1; }
         nv = n_local + n_remote;
     }
+    // SHARE: the pair on the earlier query block walks the remote list of the later one (its extra tile is fully masked)
+    __device__ void adopt_remote(int kt_hi_) { kt_hi = kt_hi_; n_remote = kt_hi + 1; nv = n_local + n_remote; }
     __device__ Visit at(int v, bool bifocal) const {
         Visit x;
         if (v < n_local) { x.kt = qb - v; x.mode = bifocal ? 1 : 0; }
@@ -189,10 +195,13 @@ constexpr uint32_t IDESC_QK_F16 = idesc_f16(0, 0, 0, 0, 2 * BM, BN);
 constexpr uint32_t IDESC_QK_E5M2 = idesc_f16(1, 1, 0, 0, 2 * BM, BN);   // kind::f8f6f4: format code 1 = e5m2
 constexpr uint32_t IDESC_PV = idesc_f16(1, 1, 0, 1, 2 * BM, D);  // A = P (TMEM, bf16), B = V (smem, MN-major)
 
-__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1)
-prefill_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV,
-                    const __grid_constant__ CUtensorMap tmKh, const __grid_constant__ CUtensorMap tmKe,
-                    const __grid_constant__ CUtensorMap tmKl, const Params p) {
+// SHARE = false: a cluster is one CTA pair.  SHARE = true (bifocal, on the fly): a cluster is TWO pairs on adjacent query
+// blocks of the same two heads; in a remote visit every CTA loads and rotates only 32 key rows and writes them to its
+// own stage and to the stage of the CTA with the same parity in the other pair, so a rotated row serves 512 query rows.
+template <bool SHARE>
+__device__ __forceinline__ void prefill_body(const CUtensorMap& tmK, const CUtensorMap& tmV, const CUtensorMap& tmKh,
+                                             const CUtensorMap& tmKe, const CUtensorMap& tmKl, const CUtensorMap& tmK32,
+                                             const Params& p) {
     extern __shared__ unsigned char smem_raw[];
     unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
     Bars* bars = reinterpret_cast<Bars*>(smem + NS * STAGE_BYTES);
@@ -201,12 +210,15 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_consta
     auto sV = [&](int s) { return smem + s * STAGE_BYTES + 2 * KH_BYTES; };
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int cta = (int)cluster_ctarank();
-    const int pair = (int)(blockIdx.x >> 1);
+    const int rank = (int)cluster_ctarank();
+    const int cta = rank & 1;                                      // position in the CTA pair (0 = leader)
+    const int pr = SHARE ? (rank >> 1) : 0;                        // which pair of the cluster
     const int n_qb = (int)((p.L + BM - 1) / BM);
     const int pairs = p.H_q / 2;
-    const int qb = n_qb - 1 - pair / pairs;                       // heaviest row blocks first
-    const int h0 = 2 * (pair % pairs);
+    const int unit = SHARE ? (int)(blockIdx.x >> 2) : (int)(blockIdx.x >> 1);
+    const int qbA = SHARE ? n_qb - 1 - 2 * (unit / pairs) : n_qb - 1 - unit / pairs;   // heaviest row blocks first
+    const int qb = qbA - pr;                                       // SHARE: pair 1 takes the block below (-1 = none)
+    const int h0 = 2 * (unit % pairs);
     const int head = h0 + cta;
     const int kvh = h0 / p.g;
     const long long q0 = (long long)qb * BM;
@@ -215,15 +227,25 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_consta
     // highest-energy pairs of every 8-pair chunk; a KV head whose other channels are too loud falls back to 2
     int precise = p.precise;
     if (precise == 3 && __ldg(p.selinfo + kvh * 16 + 8) != 0u) precise = 2;
-    const Plan plan(qb, p.w0, bifocal, p.window_only != 0);
+    Plan plan(qb, p.w0, bifocal, p.window_only != 0);
+    int n_local_peer = 0;                                          // SHARE: local visits of the other pair
+    if (SHARE) {
+        const Plan pa(qbA, p.w0, bifocal), pb(qbA - 1, p.w0, bifocal);
+        if (pr == 1) plan.adopt_remote(pa.kt_hi);
+        n_local_peer = pr == 0 ? pb.n_local : pa.n_local;
+    }
+    const uint32_t own_mask = 3u << (2 * pr), peer_mask = 3u << (2 * (pr ^ 1));
 
     if (tid == 0) {
         for (int i = 0; i < NS; ++i) { mbar_init(&bars->kv_full[i], 1); mbar_init(&bars->kv_ready[i], 8); mbar_init(&bars->kv_empty[i], 1); }
         for (int i = 0; i < 2; ++i) { mbar_init(&bars->s_full[i], 1); mbar_init(&bars->p_full[i], 16); }
         mbar_init(&bars->pv_done, 1); mbar_init(&bars->o_full, 1); mbar_init(&bars->q_ready, 8);
         mbar_init(&bars->q_local_done, 1); mbar_init(&bars->q_rot_done, 8);
+        for (int i = 0; i < NS; ++i) { mbar_init(&bars->peer_full[i], 1); mbar_init(&bars->peer_empty[i], 1); }
+        mbar_init(&bars->peer_go, 1);
         fence_barrier_init();
         prefetch_tmap(&tmK); prefetch_tmap(&tmV);
+        if (SHARE) prefetch_tmap(&tmK32);
         if (p.prerot) { prefetch_tmap(&tmKh); prefetch_tmap(&tmKe); prefetch_tmap(&tmKl); }
     }
     if (warp == 1) tmem_alloc2<512>(&bars->tmem_base);
@@ -232,6 +254,11 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_consta
     tc_fence_after();
     const uint32_t tmem = bars->tmem_base;
     float* xchg = bars->xchg;
+    // arrive on the pair leader's copy of a barrier (the leader is rank & ~1 of the cluster)
+    auto arrive_leader = [&](uint64_t* bar) {
+        if (SHARE) mbar_arrive_cluster_addr(mapa_u32(smem_u32(bar), (uint32_t)(rank & ~1)));
+        else mbar_arrive_leader(bar);
+    };
 
     if (warp == 0) {
         // ===================== TMA producer (each CTA loads its halves) =====================
@@ -247,6 +274,11 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_consta
                     tma_load_3d(sK(s) + KBOX, &tmKh, &bars->kv_full[s], 64, kvh, x.kt * BN + 64 * cta);
                     if (precise >= 2) tma_load_3d(sKl(s), &tmKe, &bars->kv_full[s], 0, kvh, x.kt * BN + 64 * cta);
                     if (precise == 2) tma_load_3d(sKl(s) + KBOX, &tmKl, &bars->kv_full[s], 0, kvh, x.kt * BN + 64 * cta);
+                } else if (SHARE && x.mode == 2) {
+                    // shared remote visit: only the 32 rows this CTA rotates; the other 32 arrive rotated from the other pair
+                    mbar_arrive_expect_tx(&bars->kv_full[s], KH_BYTES / 2 + VH_BYTES);
+                    tma_load_3d(sK(s) + pr * 4096, &tmK32, &bars->kv_full[s], 0, kvh, x.kt * BN + 64 * cta + 32 * pr);
+                    tma_load_3d(sK(s) + KBOX + pr * 4096, &tmK32, &bars->kv_full[s], 64, kvh, x.kt * BN + 64 * cta + 32 * pr);
                 } else {
                     mbar_arrive_expect_tx(&bars->kv_full[s], KH_BYTES + VH_BYTES);
                     tma_load_3d(sK(s), &tmK, &bars->kv_full[s], 0, kvh, x.kt * BN + 64 * cta);
@@ -302,8 +334,8 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_consta
                                          smem_desc_sw128(kb + (ks >> 2) * KBOX + (ks & 3) * 32, 16, 1024), IDESC_QK_F16, 1);
                         }
                     }
-                    umma2_commit(&bars->s_full[v & 1]);
-                    if (plan.n_remote > 0 && v == plan.n_local - 1) umma2_commit(&bars->q_local_done);
+                    umma2_commit_mask(&bars->s_full[v & 1], own_mask);
+                    if (plan.n_remote > 0 && v == plan.n_local - 1) umma2_commit_mask(&bars->q_local_done, own_mask);
                 }
                 __syncwarp();
             };
@@ -314,27 +346,49 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_consta
                     for (int ks = 0; ks < BN / 16; ++ks)
                         umma2_ts(tm + TM_O, tm + TM_S + (v & 1) * 128 + ks * 8,
                                  smem_desc_sw128(vb + ks * 2048, VH_BYTES, 1024), IDESC_PV, (v > 0 || ks > 0) ? 1u : 0u);
-                    umma2_commit(&bars->kv_empty[v % NS]);
-                    umma2_commit(&bars->pv_done);
+                    umma2_commit_mask(&bars->kv_empty[v % NS], own_mask);
+                    if (SHARE) {                                      // the other pair may now overwrite ITS rows of our next use of the stage
+                        umma2_commit_mask(&bars->peer_empty[v % NS], peer_mask);
+                        if (v == plan.n_local - 1) umma2_commit_mask(&bars->peer_go, peer_mask);
+                    }
+                    umma2_commit_mask(&bars->pv_done, own_mask);
                 }
                 __syncwarp();
             };
+            // operands of visit v are in place: local visits (and every visit without SHARE) count the two rotate groups of
+            // the pair on kv_ready (in a shared visit each group arrives once the other pair's rows have landed too)
+            auto wait_ready = [&](int v) { mbar_wait(&bars->kv_ready[v % NS], (v / NS) & 1); };
+            if (SHARE && plan.n_local == 0 && elect_one()) umma2_commit_mask(&bars->peer_go, peer_mask);   // no local visit: all stages free
+            __syncwarp();
             mbar_wait(&bars->q_ready, 0);
-            mbar_wait(&bars->kv_ready[0], 0);
-            tc_fence_after();
-            issue_qk(0);
+            if (plan.nv > 0) {
+                if (plan.n_local == 0) mbar_wait(&bars->q_rot_done, 0);
+                wait_ready(0);
+                tc_fence_after();
+                issue_qk(0);
+            }
             for (int v = 0; v < plan.nv; ++v) {
+                // SHARE: the first shared visit can only become ready after OUR peer_go, which the P V of the last local
+                // visit commits -- so that one P V is issued before, not after, waiting for the next visit's operands
+                const bool pv_first = SHARE && v + 1 == plan.n_local;
+                if (pv_first) {
+                    mbar_wait(&bars->p_full[v & 1], (v >> 1) & 1);
+                    tc_fence_after();
+                    issue_pv(v);
+                }
                 if (v + 1 < plan.nv) {
                     if (plan.n_remote > 0 && v + 1 == plan.n_local) mbar_wait(&bars->q_rot_done, 0);
-                    mbar_wait(&bars->kv_ready[(v + 1) % NS], ((v + 1) / NS) & 1);
+                    wait_ready(v + 1);
                     tc_fence_after();
                     issue_qk(v + 1);
                 }
-                mbar_wait(&bars->p_full[v & 1], (v >> 1) & 1);
-                tc_fence_after();
-                issue_pv(v);
+                if (!pv_first) {
+                    mbar_wait(&bars->p_full[v & 1], (v >> 1) & 1);
+                    tc_fence_after();
+                    issue_pv(v);
+                }
             }
-            if (elect_one()) umma2_commit(&bars->o_full);
+            if (elect_one()) umma2_commit_mask(&bars->o_full, own_mask);
             __syncwarp();
         }
     } else if (warp >= 2 && warp < 6) {
@@ -342,42 +396,83 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_consta
         const int t = tid - 64;                                       // work index for the K rotation
         const uint32_t lane_base = (uint32_t)((warp & 3) << 5) << 16; // TMEM lanes a warp may touch: 32 (warp % 4) ..
         const long long q = q0 + (((warp & 3) << 5) | lane);
-        const bool valid = q < p.L;
+        const bool valid = q >= 0 && q < p.L;
         const __nv_bfloat16* qrow = p.Q + ((size_t)(valid ? q : 0) * p.H_q + head) * D;
         stage_q_raw(qrow, valid, tmem + lane_base + TM_QA);
         tmem_st_wait();
         tc_fence_before();
         __syncwarp();
-        if (lane == 0) mbar_arrive_leader(&bars->q_ready);
-        KRot<4> rot;
+        if (lane == 0) arrive_leader(&bars->q_ready);
+        constexpr int RR = SHARE ? 2 : 4;                             // key rows per rotate thread
+        KRot<RR> rot;
         if (plan.n_remote > 0 && !p.prerot) {
-            rot.init(p.lo, p.hi, t, p.G);
+            rot.init(p.lo, p.hi, t, p.G, SHARE ? 32 * pr : 0);
             rot.prefetch((unsigned)(plan.kt_hi * BN + 64 * cta));     // first remote visit
         }
+        // SHARE: the CTA of the same parity in the other pair receives a copy of the rows rotated here (bulk copy
+        // through the async proxy, counted on ITS peer_full barrier), and sends us the other 32 rows of each stage
+        const uint32_t peer_smem = SHARE ? mapa_u32(smem_u32(smem), (uint32_t)(rank ^ 2)) : 0u;
+        const uint32_t peer_full0 = SHARE ? mapa_u32(smem_u32(&bars->peer_full[0]), (uint32_t)(rank ^ 2)) : 0u;
+        // SHARE: the hand-over of a shared visit (wait for the other pair's rows, then arrive on kv_ready) is deferred to
+        // the start of the next iteration, so the rotation of visit u+1 never waits for the bulk copy of visit u
+        int pend_v = -1;
+        auto flush_pending = [&]() {
+            if (pend_v < 0) return;
+            const int u = pend_v - plan.n_local;
+            mbar_wait(&bars->peer_full[u % NS], (u / NS) & 1);       // the other 32 rows of that stage have landed
+            __syncwarp();
+            if (lane == 0) {
+                if (pend_v == plan.n_local) arrive_leader(&bars->q_rot_done);
+                arrive_leader(&bars->kv_ready[pend_v % NS]);
+            }
+            pend_v = -1;
+        };
         for (int v = 0; v < plan.nv; ++v) {
             const Visit x = plan.at(v, bifocal);
             const int s = v % NS;
+            if (SHARE) flush_pending();
             mbar_wait(&bars->kv_full[s], (v / NS) & 1);
             if (x.mode == 2) {
                 if (v == plan.n_local) {                              // first remote visit: Q -> Q' = R(Delta q) Q
-                    mbar_wait(&bars->q_local_done, 0);
+                    if (plan.n_local > 0) mbar_wait(&bars->q_local_done, 0);
                     tc_fence_after();
-                    stage_q_rot(qrow, valid, q, p.G, p.lo, p.hi, tmem + lane_base + TM_QA, tmem + lane_base + TM_QB, precise, p.selinfo + kvh * 16);
+                    stage_q_rot(qrow, valid, valid ? q : 0, p.G, p.lo, p.hi, tmem + lane_base + TM_QA, tmem + lane_base + TM_QB, precise, p.selinfo + kvh * 16);
                     tmem_st_wait();
                     tc_fence_before();
                 }
+                if (SHARE) {
+                    const int u = v - plan.n_local;                   // index of the shared remote visit
+                    const int vp = n_local_peer + u, sp = vp % NS;    // the other pair's visit number and stage
+                    const uint32_t nbox = precise == 0 ? 2u : 4u;     // 4 KB pieces: K'hi boxes (+ the two cross-term boxes)
+                    if (t == 0) mbar_arrive_expect_tx(&bars->peer_full[u % NS], nbox * 4096u);
+                    rotate_k_rows<RR, KBOX>(smem_u32(sK(s)), smem_u32(sKl(s)), (unsigned)(x.kt * BN + 64 * cta), rot, precise);
+                    fence_proxy_async_smem();
+                    named_bar_sync(8, 128);                           // every rotate thread has written and fenced its rows
+                    if (t == 0) {
+                        if (u == 0) mbar_wait(&bars->peer_go, 0);     // its local visits are over: all its stages are free
+                        if (u >= NS) mbar_wait(&bars->peer_empty[sp], ((vp / NS) - 1) & 1);
+                        const uint32_t src = smem_u32(smem) + (uint32_t)s * STAGE_BYTES + (uint32_t)pr * 4096u;
+                        const uint32_t dst = peer_smem + (uint32_t)sp * STAGE_BYTES + (uint32_t)pr * 4096u;
+                        const uint32_t mb = peer_full0 + 8u * (uint32_t)(u % NS);
+                        for (uint32_t b = 0; b < nbox; ++b) bulk_copy_to_peer(dst + b * KBOX, src + b * KBOX, 4096u, mb);
+                    }
+                    if (x.kt > 0) rot.prefetch((unsigned)((x.kt - 1) * BN + 64 * cta));
+                    pend_v = v;
+                    continue;
+                }
                 if (!p.prerot) {
-                    rotate_k_rows<4, KBOX>(smem_u32(sK(s)), smem_u32(sKl(s)), (unsigned)(x.kt * BN + 64 * cta), rot, precise);
+                    rotate_k_rows<RR, KBOX>(smem_u32(sK(s)), smem_u32(sKl(s)), (unsigned)(x.kt * BN + 64 * cta), rot, precise);
                     fence_proxy_async_smem();
                     if (x.kt > 0) rot.prefetch((unsigned)((x.kt - 1) * BN + 64 * cta));   // next remote visit's first row
                 }
             }
             __syncwarp();
             if (lane == 0) {
-                if (x.mode == 2 && v == plan.n_local) mbar_arrive_leader(&bars->q_rot_done);
-                mbar_arrive_leader(&bars->kv_ready[s]);
+                if (x.mode == 2 && v == plan.n_local) arrive_leader(&bars->q_rot_done);
+                arrive_leader(&bars->kv_ready[s]);
             }
         }
+        if (SHARE) flush_pending();
     } else if (warp >= 6) {
         // ===================== softmax groups (steps a6-a8) =====================
         // Two threads per query row: warps w and w+4 hold the same 32 rows, column half `half` (64 keys) each.
@@ -473,7 +568,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_consta
             tmem_st_wait();
             tc_fence_before();
             __syncwarp();
-            if (lane == 0) mbar_arrive_leader(&bars->p_full[v & 1]);
+            if (lane == 0) arrive_leader(&bars->p_full[v & 1]);
         }
         // ---- epilogue (step a8) ----
         float la, lb, lc, ld;
@@ -486,13 +581,14 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_consta
         tc_fence_after();
         const long long q = q0 + r;
         const float inv = 1.0f / l;
-        __nv_bfloat16* orow = p.out + ((size_t)(q < p.L ? q : 0) * p.H_q + head) * D + 64 * half;
+        const bool qok = q >= 0 && q < p.L;
+        __nv_bfloat16* orow = p.out + ((size_t)(qok ? q : 0) * p.H_q + head) * D + 64 * half;
 #pragma unroll
         for (int ch = 0; ch < 2; ++ch) {
             uint32_t rg[32];
             tmem_ld32(tO + ch * 32, rg);
             tmem_ld_wait();
-            if (q < p.L) {
+            if (qok) {
 #pragma unroll
                 for (int j = 0; j < 32; j += 8) {
                     uint32_t w[4];
@@ -503,11 +599,25 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_consta
                 }
             }
         }
-        if (half == 0 && q < p.L) p.lse[(size_t)head * p.L + q] = (m_ref + log2f(l)) * 0.6931471805599453f;
+        if (half == 0 && qok) p.lse[(size_t)head * p.L + q] = (m_ref + log2f(l)) * 0.6931471805599453f;
     }
     tc_fence_before();
     cluster_sync_all();                                            // the peer may still be reading our smem / TMEM
     if (warp == 1) tmem_dealloc2<512>(tmem);
+}
+
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1)
+prefill_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV,
+                    const __grid_constant__ CUtensorMap tmKh, const __grid_constant__ CUtensorMap tmKe,
+                    const __grid_constant__ CUtensorMap tmKl, const Params p) {
+    prefill_body<false>(tmK, tmV, tmKh, tmKe, tmKl, tmK, p);
+}
+
+// on-the-fly bifocal prefill: clusters of four CTAs (two pairs on adjacent query blocks) share every rotated K tile
+__global__ void __cluster_dims__(4, 1, 1) __launch_bounds__(NTHREADS, 1)
+prefill_umma_share_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV,
+                          const __grid_constant__ CUtensorMap tmK32, const Params p) {
+    prefill_body<true>(tmK, tmV, tmK, tmK, tmK, tmK32, p);
 }
 
 // ---- 8(f)-1: rotate K once into a scratch (the workspace variant) -------------------------------------------
@@ -698,6 +808,10 @@ size_t umma_prefill_unfused_workspace_bytes(long long L, int H_q, int H_kv, int 
     return two_level_bytes(L + 256, d) + 3 * align256(2 * nq) + align256(2 * nk) + 2 * align256((size_t)L * H_q * 4);
 }
 
+// 1: the on-the-fly bifocal prefill runs in clusters of four CTAs that share rotated K tiles (experimental, opt-in through
+// jetlong_set_prefill_impl(2): parity-green but not faster yet); 0: CTA pairs only (default)
+int g_share_clusters = 0;
+
 bool umma_prefill_supported(long long L, int H_q, int H_kv, int d, int dtype) {
     if (dtype != JETLONG_BF16 || d != 128 || H_kv < 1 || H_q % H_kv) return false;
     const int g = H_q / H_kv;
@@ -784,6 +898,22 @@ int launch_prefill_umma(const void* Q, const void* K, const void* V, void* out, 
         attr_set = true;
     }
     const int n_qb = (int)((L + BM - 1) / BM);
+    if (bifocal && !p.prerot && g_share_clusters) {
+        // on the fly: clusters of four CTAs, two query blocks per cluster share each rotated K tile
+        CUtensorMap tmK32;
+        if (!make_kv_tensor_map(&tmK32, K, L, H_kv, 32)) return JETLONG_UNSUPPORTED;
+        static bool attr4_set = false;
+        if (!attr4_set) {
+            if (cudaFuncSetAttribute(prefill_umma_share_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES) !=
+                cudaSuccess)
+                return check_launch("prefill_umma_share attr");
+            attr4_set = true;
+        }
+        const unsigned grid4 = 4u * (unsigned)((n_qb + 1) / 2) * (unsigned)(H_q / 2);
+        prefill_umma_share_kernel<<<grid4, NTHREADS, SMEM_BYTES, st>>>(tmK, tmV, tmK32, p);
+        note_launch();
+        return check_launch("prefill_umma_share_kernel");
+    }
     const unsigned grid = 2u * (unsigned)n_qb * (unsigned)(H_q / 2);
     prefill_umma_kernel<<<grid, NTHREADS, SMEM_BYTES, st>>>(tmK, tmV, tmKh, tmKe, tmKl, p);
     note_launch();

@@ -243,3 +243,26 @@ def test_unfused_G1_is_the_control():
     out, lse = J.jetlong_prefill_unfused(Q, K, V, w_local=10, w_pretrained=512, rope_theta=1e6)
     outc, lsec = J.jetlong_causal_prefill(Q, K, V)
     assert torch.equal(out, outc) and torch.equal(lse, lsec)
+
+
+# ---- experimental: on-the-fly prefill in clusters of four CTAs sharing rotated K tiles (jetlong_set_prefill_impl(2)) ----
+@pytest.mark.parametrize("L,H_q,H_kv,w_pre,w0", [
+    (777, 4, 2, 200, 100),        # odd number of query blocks: one cluster has a block-less second pair
+    (640, 8, 2, 320, 128),        # G=2, g=4
+    (1300, 2, 1, 300, 0),         # G=5, w0=0
+    (4096, 4, 2, 1024, 128),      # 32 query blocks, long shared phases
+])
+def test_cluster_of_four_sharing_matches_oracle(L, H_q, H_kv, w_pre, w0):
+    Q, K, V = W.make_qkv(L, H_q, H_kv, 128, 1e6, "bf16", 9753 + L, True, DEV)
+    try:
+        J.jetlong_set_prefill_impl(2)
+        out, lse = J.jetlong_prefill(Q, K, V, w_local=w0, w_pretrained=w_pre, rope_theta=1e6)
+        torch.cuda.synchronize()
+    finally:
+        J.jetlong_set_prefill_impl(-1)
+    rows, heads = all_pairs(L, H_q)
+    if L > 2000:
+        pick = np.random.RandomState(2).choice(len(rows), 2048, replace=False)
+        rows, heads = rows[pick], heads[pick]
+    ro, rl = oracle_rows(Q, K, V, rows, heads, w_local=w0, w_pretrained=w_pre, rope_theta=1e6)
+    check(*gather(out, lse, rows, heads), ro, rl, Q.dtype, "cluster-of-four L=%d" % L)
