@@ -448,13 +448,18 @@ __device__ __forceinline__ void prefill_body(const CUtensorMap& tmK, const CUten
                     rotate_k_rows<RR, KBOX>(smem_u32(sK(s)), smem_u32(sKl(s)), (unsigned)(x.kt * BN + 64 * cta), rot, precise);
                     fence_proxy_async_smem();
                     named_bar_sync(8, 128);                           // every rotate thread has written and fenced its rows
-                    if (t == 0) {
+                    if (t < 32) {
+                        // the whole first warp waits (a lone lane would share its issue slots with 31 lanes spinning on
+                        // peer_full below: measured 1 k cycles for this block), one lane issues the copies
                         if (u == 0) mbar_wait(&bars->peer_go, 0);     // its local visits are over: all its stages are free
                         if (u >= NS) mbar_wait(&bars->peer_empty[sp], ((vp / NS) - 1) & 1);
-                        const uint32_t src = smem_u32(smem) + (uint32_t)s * STAGE_BYTES + (uint32_t)pr * 4096u;
-                        const uint32_t dst = peer_smem + (uint32_t)sp * STAGE_BYTES + (uint32_t)pr * 4096u;
-                        const uint32_t mb = peer_full0 + 8u * (uint32_t)(u % NS);
-                        for (uint32_t b = 0; b < nbox; ++b) bulk_copy_to_peer(dst + b * KBOX, src + b * KBOX, 4096u, mb);
+                        if (lane == 0) {
+                            const uint32_t src = smem_u32(smem) + (uint32_t)s * STAGE_BYTES + (uint32_t)pr * 4096u;
+                            const uint32_t dst = peer_smem + (uint32_t)sp * STAGE_BYTES + (uint32_t)pr * 4096u;
+                            const uint32_t mb = peer_full0 + 8u * (uint32_t)(u % NS);
+                            for (uint32_t b = 0; b < nbox; ++b) bulk_copy_to_peer(dst + b * KBOX, src + b * KBOX, 4096u, mb);
+                        }
+                        __syncwarp();
                     }
                     if (x.kt > 0) rot.prefetch((unsigned)((x.kt - 1) * BN + 64 * cta));
                     pend_v = v;
