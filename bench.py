@@ -181,6 +181,9 @@ def main():
                     help="what the timed loop runs (default: the bifocal prefill in its default, compensated "
                          "precision); the other values exist for profiling one kernel at a time")
     ap.add_argument("--no-extras", action="store_true", help="skip control / decode / e2e / oracle legs (profiling)")
+    ap.add_argument("--config4", action="store_true",
+                    help="instead of the default run: BASELINE.json configs[3], the Qwen3-8B-shaped 36-layer stack at 128K for "
+                         "w_local in {2048, 4096, 8192}, bifocal / workspace variant / control on identical inputs (~2 min)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" and not args.no_extras else args.warmup
 
@@ -214,6 +217,12 @@ def main():
                          only="bifocal" if args.variant == "decode" else "control")
         if rank == 0:
             print(json.dumps({"metric": METRIC, "variant": args.variant, "decode": r}))
+        return
+
+    if args.config4:
+        r = bench_config4(J, B, W, dev, pk)
+        if rank == 0:
+            print(json.dumps({"metric": METRIC, "variant": "config4", "config4": r}))
         return
 
     Q, K, V = W.make_config_inputs(cfg, dev)
@@ -379,6 +388,41 @@ def bench_prefill_128k(J, B, W, dev, pk, timed):
                      "frac_of_bf16_burst_peak": fl / (ms * 1e-3) / 1e12 / pk["tflops_burst"]}
     for name in ("bifocal", "prerotated"):
         res[name]["over_control"] = res["control"]["ms"] / res[name]["ms"]
+    return res
+
+
+def bench_config4(J, B, W, dev, pk):
+    """configs[3]: 36 independent layers back to back (per-layer seeded inputs, buffers reused), L=131072, H_q=32, H_kv=8,
+    w_local in {2048, 4096, 8192}; per w_local the summed device time of the 36 calls of each kernel."""
+    c = W.C4
+    out = lse = wsp = None
+    fl = flops_causal(c.L, c.H_q, c.d) * W.C4_LAYERS
+    J.jetlong_set_prefill_precision(B.PRECISION_COMPENSATED)
+    tot = {w0: {"bifocal": 0.0, "prerotated": 0.0} for w0 in W.C4_W_LOCAL}
+    tot_control = 0.0
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+
+    def t(fn):
+        e0.record(); fn(); e1.record(); torch.cuda.synchronize()
+        return e0.elapsed_time(e1)
+    for layer in range(W.C4_LAYERS):
+        Q, K, V = W.make_config_inputs(c, dev, layer=layer)
+        if out is None:
+            out = torch.empty_like(Q)
+            lse = torch.empty((c.H_q, c.L), dtype=torch.float32, device=dev)
+            wsp = B.alloc_workspace(B.OP_PREFILL_PREROTATED, c.L, c.H_q, c.H_kv, c.d, B.BF16, dev)
+            J.jetlong_causal_prefill(Q, K, V, out=out, lse=lse, workspace=wsp)            # warm-up
+        tot_control += t(lambda: J.jetlong_causal_prefill(Q, K, V, out=out, lse=lse, workspace=wsp))
+        for w0 in W.C4_W_LOCAL:
+            kw = dict(w_local=w0, w_pretrained=c.w_pretrained, rope_theta=c.rope_theta)
+            tot[w0]["bifocal"] += t(lambda: J.jetlong_prefill(Q, K, V, out=out, lse=lse, workspace=wsp, **kw))
+            tot[w0]["prerotated"] += t(lambda: J.jetlong_prefill_prerotated(Q, K, V, out=out, lse=lse, workspace=wsp, **kw))
+        del Q, K, V
+    res = {"workload": "BASELINE.json configs[3]: Qwen3-8B-shaped stack, 36 layers x (L=131072, H_q=32, H_kv=8, G=4), "
+                       "FLOPs = 36 x 1.407e14", "control": {"ms": tot_control, "tflops": fl / tot_control / 1e9}}
+    for w0 in W.C4_W_LOCAL:
+        res["w_local=%d" % w0] = {k: {"ms": v, "tflops": fl / v / 1e9, "over_control": tot_control / v,
+                                       "frac_of_bf16_burst_peak": fl / v / 1e9 / pk["tflops_burst"]} for k, v in tot[w0].items()}
     return res
 
 

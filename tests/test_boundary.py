@@ -87,3 +87,36 @@ def test_prefill_precision_switch_is_host_state():
     assert B.jetlong_set_prefill_precision(77) == B.PRECISION_COMPENSATED_F16                  # unknown: unchanged
     assert B.jetlong_set_prefill_precision(B.PRECISION_COMPENSATED) == B.PRECISION_COMPENSATED_F16
     assert B.jetlong_set_prefill_precision(B.PRECISION_COMPENSATED) == B.PRECISION_COMPENSATED
+
+
+def test_workspace_sizes_of_the_prefill_variants():
+    """the workspace variant holds tables + K'hi (2 B) + two e5m2 buffers (1 B each) per key channel
+    + the selection scratch; the unfused baseline holds tables + Q', O_B, O_C (2 B per query channel) + K' + two lse."""
+    L, H_q, H_kv, d = 65536, 16, 8, 128
+    pre = B.jetlong_workspace_bytes(B.OP_PREFILL_PREROTATED, L, H_q, H_kv, d, B.BF16)
+    unf = B.jetlong_workspace_bytes(B.OP_PREFILL_UNFUSED, L, H_q, H_kv, d, B.BF16)
+    nk, nq = L * H_kv * d, L * H_q * d
+    slack = 1 << 20                                       # two-level rotation table (0.2 MB here) + alignment + selection scratch
+    assert 4 * nk <= pre <= 4 * nk + slack
+    assert 6 * nq + 2 * nk + 8 * L * H_q <= unf <= 6 * nq + 2 * nk + 8 * L * H_q + slack
+    # shapes the tcgen05 kernel does not serve have no such variants
+    assert B.jetlong_workspace_bytes(B.OP_PREFILL_PREROTATED, 1024, 4, 2, 64, B.FP32) == 0
+    assert B.jetlong_workspace_bytes(B.OP_PREFILL_UNFUSED, 1024, 3, 1, 128, B.BF16) == 0        # odd H_q / H_kv
+
+
+def test_prefill_variants_validate_before_any_launch():
+    L = B.lib()
+    buf = (ctypes.c_char * 4096)()
+    a = (ctypes.addressof(buf) + 15) & ~15
+    for fn in (L.jetlong_prefill_prerotated, L.jetlong_prefill_unfused):
+        assert fn(0, a, a, a, a, 256, 2, 1, 128, 1, 64, 1e4, B.BF16, a, 4096, None) == B.INVALID_ARG      # null Q
+        assert fn(a, a, a, a, a, 256, 2, 1, 128, -1, 64, 1e4, B.BF16, a, 4096, None) == B.INVALID_ARG     # w_local < 0
+        assert fn(a, a, a, a, a, 256, 2, 1, 64, 1, 64, 1e4, B.FP32, a, 4096, None) == B.UNSUPPORTED       # fp32 / d = 64
+        assert fn(a, a, a, a, a, 256, 2, 1, 128, 1, 64, 1e4, B.BF16, a, 16, None) == B.INVALID_ARG        # workspace too small
+
+
+def test_prefill_impl_switch_is_host_state():
+    prev = B.jetlong_set_prefill_impl(2)                  # experimental clusters of four
+    assert B.jetlong_set_prefill_impl(0) == 2
+    assert B.jetlong_set_prefill_impl(-1) == 0
+    assert B.jetlong_set_prefill_impl(prev) == -1
