@@ -64,6 +64,8 @@ struct Bars {
     uint64_t q_rot_done;       // leader: Q' (hi, lo) staged in TMEM
     // cluster of four (SHARE): the other CTA pair rotates half of our rows and writes them into our stages
     uint64_t peer_full[NS];    // local: the rows rotated by the other pair have landed in our stage (bulk copy, complete_tx)
+    uint64_t rows_done[NS];    // local: our four rotate warps have rotated and fenced their 32 rows of a shared visit
+    uint64_t kv_ready_sh[NS];  // leader: a shared visit is complete in a CTA of the pair (its own rows + the other pair's), 2 arrivals
     uint64_t peer_empty[NS];   // both: the OTHER pair's MMAs reading ITS stage s have completed (its commit, multicast to us)
     uint64_t peer_go;          // both: the other pair's last local visit has completed (all its stages are free)
     uint32_t tmem_base;
@@ -241,7 +243,8 @@ __device__ __forceinline__ void prefill_body(const CUtensorMap& tmK, const CUten
         for (int i = 0; i < 2; ++i) { mbar_init(&bars->s_full[i], 1); mbar_init(&bars->p_full[i], 16); }
         mbar_init(&bars->pv_done, 1); mbar_init(&bars->o_full, 1); mbar_init(&bars->q_ready, 8);
         mbar_init(&bars->q_local_done, 1); mbar_init(&bars->q_rot_done, 8);
-        for (int i = 0; i < NS; ++i) { mbar_init(&bars->peer_full[i], 1); mbar_init(&bars->peer_empty[i], 1); }
+        for (int i = 0; i < NS; ++i) { mbar_init(&bars->peer_full[i], 1); mbar_init(&bars->peer_empty[i], 1);
+                                       mbar_init(&bars->rows_done[i], 4); mbar_init(&bars->kv_ready_sh[i], 2); }
         mbar_init(&bars->peer_go, 1);
         fence_barrier_init();
         prefetch_tmap(&tmK); prefetch_tmap(&tmV);
@@ -262,7 +265,55 @@ __device__ __forceinline__ void prefill_body(const CUtensorMap& tmK, const CUten
 
     if (warp == 0) {
         // ===================== TMA producer (each CTA loads its halves) =====================
-        if (lane == 0) {
+        if (SHARE && lane == 0) {
+            // One thread, three duties, none of which may block the others (an event loop over non-blocking barrier tests):
+            //   load(v):  TMA of visit v once its stage is free; for a shared visit also arm peer_full with the incoming bytes
+            //   copy(u):  once our rotate warps have fenced their 32 rows of shared visit u and the other pair's stage is
+            //             free, send the rows to the CTA of the same parity in the other pair (bulk copies, async proxy)
+            //   land(u):  once our rows are done and the other pair's rows have landed, arrive on the pair's kv_ready_sh
+            const uint32_t peer_smem = mapa_u32(smem_u32(smem), (uint32_t)(rank ^ 2));
+            const uint32_t peer_full0 = mapa_u32(smem_u32(&bars->peer_full[0]), (uint32_t)(rank ^ 2));
+            const uint32_t ready0 = mapa_u32(smem_u32(&bars->kv_ready_sh[0]), (uint32_t)(rank & ~1));
+            const uint32_t nbox = precise == 0 ? 2u : 4u;            // 4 KB pieces: the K'hi boxes (+ the two cross-term boxes)
+            const int nsh = plan.nv - plan.n_local;                  // shared (remote) visits
+            int lv = 0, cu = 0, du = 0;
+            bool go = false;
+            while (lv < plan.nv || cu < nsh || du < nsh) {
+                if (lv < plan.nv && (lv < NS || mbar_test(&bars->kv_empty[lv % NS], ((lv / NS) - 1) & 1))) {
+                    const Visit x = plan.at(lv, bifocal);
+                    const int s = lv % NS;
+                    if (x.mode == 2) {
+                        const int u = lv - plan.n_local;
+                        mbar_arrive_expect_tx(&bars->peer_full[u % NS], nbox * 4096u);
+                        mbar_arrive_expect_tx(&bars->kv_full[s], KH_BYTES / 2 + VH_BYTES);
+                        tma_load_3d(sK(s) + pr * 4096, &tmK32, &bars->kv_full[s], 0, kvh, x.kt * BN + 64 * cta + 32 * pr);
+                        tma_load_3d(sK(s) + KBOX + pr * 4096, &tmK32, &bars->kv_full[s], 64, kvh, x.kt * BN + 64 * cta + 32 * pr);
+                    } else {
+                        mbar_arrive_expect_tx(&bars->kv_full[s], KH_BYTES + VH_BYTES);
+                        tma_load_3d(sK(s), &tmK, &bars->kv_full[s], 0, kvh, x.kt * BN + 64 * cta);
+                        tma_load_3d(sK(s) + KBOX, &tmK, &bars->kv_full[s], 64, kvh, x.kt * BN + 64 * cta);
+                    }
+                    tma_load_3d(sV(s), &tmV, &bars->kv_full[s], 64 * cta, kvh, x.kt * BN);
+                    ++lv;
+                }
+                if (cu < nsh && mbar_test(&bars->rows_done[cu % NS], (cu / NS) & 1)) {
+                    const int vp = n_local_peer + cu, sp = vp % NS;  // the other pair's visit number and stage
+                    if (!go) go = mbar_test(&bars->peer_go, 0);  // its local visits are over: all its stages are free
+                    if (go && (cu < NS || mbar_test(&bars->peer_empty[sp], ((vp / NS) - 1) & 1))) {
+                        const int s = (plan.n_local + cu) % NS;
+                        const uint32_t src = smem_u32(smem) + (uint32_t)s * STAGE_BYTES + (uint32_t)pr * 4096u;
+                        const uint32_t dst = peer_smem + (uint32_t)sp * STAGE_BYTES + (uint32_t)pr * 4096u;
+                        const uint32_t mb = peer_full0 + 8u * (uint32_t)(cu % NS);
+                        for (uint32_t b = 0; b < nbox; ++b) bulk_copy_to_peer(dst + b * KBOX, src + b * KBOX, 4096u, mb);
+                        ++cu;
+                    }
+                }
+                if (du < cu && mbar_test(&bars->peer_full[du % NS], (du / NS) & 1)) {
+                    mbar_arrive_cluster_addr(ready0 + 8u * (uint32_t)(du % NS));
+                    ++du;
+                }
+            }
+        } else if (lane == 0) {
             for (int v = 0; v < plan.nv; ++v) {
                 const Visit x = plan.at(v, bifocal);
                 const int s = v % NS;
@@ -274,11 +325,6 @@ __device__ __forceinline__ void prefill_body(const CUtensorMap& tmK, const CUten
                     tma_load_3d(sK(s) + KBOX, &tmKh, &bars->kv_full[s], 64, kvh, x.kt * BN + 64 * cta);
                     if (precise >= 2) tma_load_3d(sKl(s), &tmKe, &bars->kv_full[s], 0, kvh, x.kt * BN + 64 * cta);
                     if (precise == 2) tma_load_3d(sKl(s) + KBOX, &tmKl, &bars->kv_full[s], 0, kvh, x.kt * BN + 64 * cta);
-                } else if (SHARE && x.mode == 2) {
-                    // shared remote visit: only the 32 rows this CTA rotates; the other 32 arrive rotated from the other pair
-                    mbar_arrive_expect_tx(&bars->kv_full[s], KH_BYTES / 2 + VH_BYTES);
-                    tma_load_3d(sK(s) + pr * 4096, &tmK32, &bars->kv_full[s], 0, kvh, x.kt * BN + 64 * cta + 32 * pr);
-                    tma_load_3d(sK(s) + KBOX + pr * 4096, &tmK32, &bars->kv_full[s], 64, kvh, x.kt * BN + 64 * cta + 32 * pr);
                 } else {
                     mbar_arrive_expect_tx(&bars->kv_full[s], KH_BYTES + VH_BYTES);
                     tma_load_3d(sK(s), &tmK, &bars->kv_full[s], 0, kvh, x.kt * BN + 64 * cta);
@@ -357,7 +403,14 @@ __device__ __forceinline__ void prefill_body(const CUtensorMap& tmK, const CUten
             };
             // operands of visit v are in place: local visits (and every visit without SHARE) count the two rotate groups of
             // the pair on kv_ready (in a shared visit each group arrives once the other pair's rows have landed too)
-            auto wait_ready = [&](int v) { mbar_wait(&bars->kv_ready[v % NS], (v / NS) & 1); };
+            auto wait_ready = [&](int v) {
+                if (SHARE && v >= plan.n_local) {                     // shared visit: one arrival per CTA of the pair
+                    const int u = v - plan.n_local;
+                    mbar_wait(&bars->kv_ready_sh[u % NS], (u / NS) & 1);
+                } else {
+                    mbar_wait(&bars->kv_ready[v % NS], (v / NS) & 1);
+                }
+            };
             if (SHARE && plan.n_local == 0 && elect_one()) umma2_commit_mask(&bars->peer_go, peer_mask);   // no local visit: all stages free
             __syncwarp();
             mbar_wait(&bars->q_ready, 0);
@@ -409,28 +462,9 @@ __device__ __forceinline__ void prefill_body(const CUtensorMap& tmK, const CUten
             rot.init(p.lo, p.hi, t, p.G, SHARE ? 32 * pr : 0);
             rot.prefetch((unsigned)(plan.kt_hi * BN + 64 * cta));     // first remote visit
         }
-        // SHARE: the CTA of the same parity in the other pair receives a copy of the rows rotated here (bulk copy
-        // through the async proxy, counted on ITS peer_full barrier), and sends us the other 32 rows of each stage
-        const uint32_t peer_smem = SHARE ? mapa_u32(smem_u32(smem), (uint32_t)(rank ^ 2)) : 0u;
-        const uint32_t peer_full0 = SHARE ? mapa_u32(smem_u32(&bars->peer_full[0]), (uint32_t)(rank ^ 2)) : 0u;
-        // SHARE: the hand-over of a shared visit (wait for the other pair's rows, then arrive on kv_ready) is deferred to
-        // the start of the next iteration, so the rotation of visit u+1 never waits for the bulk copy of visit u
-        int pend_v = -1;
-        auto flush_pending = [&]() {
-            if (pend_v < 0) return;
-            const int u = pend_v - plan.n_local;
-            mbar_wait(&bars->peer_full[u % NS], (u / NS) & 1);       // the other 32 rows of that stage have landed
-            __syncwarp();
-            if (lane == 0) {
-                if (pend_v == plan.n_local) arrive_leader(&bars->q_rot_done);
-                arrive_leader(&bars->kv_ready[pend_v % NS]);
-            }
-            pend_v = -1;
-        };
         for (int v = 0; v < plan.nv; ++v) {
             const Visit x = plan.at(v, bifocal);
             const int s = v % NS;
-            if (SHARE) flush_pending();
             mbar_wait(&bars->kv_full[s], (v / NS) & 1);
             if (x.mode == 2) {
                 if (v == plan.n_local) {                              // first remote visit: Q -> Q' = R(Delta q) Q
@@ -441,28 +475,17 @@ __device__ __forceinline__ void prefill_body(const CUtensorMap& tmK, const CUten
                     tc_fence_before();
                 }
                 if (SHARE) {
-                    const int u = v - plan.n_local;                   // index of the shared remote visit
-                    const int vp = n_local_peer + u, sp = vp % NS;    // the other pair's visit number and stage
-                    const uint32_t nbox = precise == 0 ? 2u : 4u;     // 4 KB pieces: K'hi boxes (+ the two cross-term boxes)
-                    if (t == 0) mbar_arrive_expect_tx(&bars->peer_full[u % NS], nbox * 4096u);
+                    // shared visit: rotate our 32 rows, fence, tell the producer thread (it sends them to the other pair and
+                    // hands the stage to the MMA warp once the other pair's rows have landed)
+                    const int u = v - plan.n_local;
                     rotate_k_rows<RR, KBOX>(smem_u32(sK(s)), smem_u32(sKl(s)), (unsigned)(x.kt * BN + 64 * cta), rot, precise);
                     fence_proxy_async_smem();
-                    named_bar_sync(8, 128);                           // every rotate thread has written and fenced its rows
-                    if (t < 32) {
-                        // the whole first warp waits (a lone lane would share its issue slots with 31 lanes spinning on
-                        // peer_full below: measured 1 k cycles for this block), one lane issues the copies
-                        if (u == 0) mbar_wait(&bars->peer_go, 0);     // its local visits are over: all its stages are free
-                        if (u >= NS) mbar_wait(&bars->peer_empty[sp], ((vp / NS) - 1) & 1);
-                        if (lane == 0) {
-                            const uint32_t src = smem_u32(smem) + (uint32_t)s * STAGE_BYTES + (uint32_t)pr * 4096u;
-                            const uint32_t dst = peer_smem + (uint32_t)sp * STAGE_BYTES + (uint32_t)pr * 4096u;
-                            const uint32_t mb = peer_full0 + 8u * (uint32_t)(u % NS);
-                            for (uint32_t b = 0; b < nbox; ++b) bulk_copy_to_peer(dst + b * KBOX, src + b * KBOX, 4096u, mb);
-                        }
-                        __syncwarp();
-                    }
                     if (x.kt > 0) rot.prefetch((unsigned)((x.kt - 1) * BN + 64 * cta));
-                    pend_v = v;
+                    __syncwarp();
+                    if (lane == 0) {
+                        mbar_arrive(&bars->rows_done[u % NS]);
+                        if (v == plan.n_local) arrive_leader(&bars->q_rot_done);
+                    }
                     continue;
                 }
                 if (!p.prerot) {
@@ -477,7 +500,6 @@ __device__ __forceinline__ void prefill_body(const CUtensorMap& tmK, const CUten
                 arrive_leader(&bars->kv_ready[s]);
             }
         }
-        if (SHARE) flush_pending();
     } else if (warp >= 6) {
         // ===================== softmax groups (steps a6-a8) =====================
         // Two threads per query row: warps w and w+4 hold the same 32 rows, column half `half` (64 keys) each.
