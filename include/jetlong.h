@@ -134,10 +134,13 @@ const char* jetlong_status_string(int status);
 /* Number of kernels this process has launched through the library (for bench accounting). */
 int64_t jetlong_launch_count(void);
 
-/* Which prefill implementation a bf16 call uses: 0 = SIMT fp32-FMA tiles, 1 = tcgen05 UMMA in CTA pairs (the default
- * where supported), 2 = tcgen05 UMMA with the on-the-fly bifocal prefill run in clusters of four CTAs (two pairs on
- * adjacent query blocks share every rotated K tile through distributed shared memory; experimental: same results,
- * not faster yet).  jetlong_set_prefill_impl(-1) restores the default.  Returns the previous value. */
+/* Which prefill implementation a bf16 call uses.  -1 (default): tcgen05 UMMA where supported; the on-the-fly bifocal
+ * prefill of >= 64 query blocks runs as clusters of four CTAs (two CTA pairs on adjacent query blocks share every rotated K
+ * tile through distributed shared memory) on an internal high-priority stream, forked from and joined to `stream` by
+ * events, while CTA pairs take the lightest query blocks on the SMs that cannot hold such a cluster.
+ * 0 = SIMT fp32-FMA tiles; 1 = tcgen05 UMMA, CTA pairs only; 2 = clusters of four for every query block;
+ * 3 = clusters of four + CTA pairs regardless of size.  All give the same results up to rounding.
+ * Returns the previous value. */
 int jetlong_set_prefill_impl(int impl);
 
 /* Operand precision of the REMOTE Q'K'^T on the tcgen05 prefill path.  Rotated operands must be

@@ -232,7 +232,7 @@ const char* jetlong_status_string(int status) {
 int64_t jetlong_launch_count(void) { return g_launches.load(); }
 
 int jetlong_set_prefill_impl(int impl) {
-    g_share_clusters = impl == 2 ? 1 : 0;
+    g_share_clusters = impl == 2 ? 1 : impl == 3 ? 2 : impl == 1 ? 0 : 3;   // see prefill_umma.cu; -1 (default) = auto
     return g_prefill_impl.exchange(impl);
 }
 

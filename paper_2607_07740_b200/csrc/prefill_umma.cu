@@ -25,6 +25,7 @@
 // outlier-channel inputs; it is opt-in (jetlong_set_prefill_precision).
 #include <cuda.h>
 #include <math.h>
+#include <mutex>
 
 #include "common.cuh"
 #include "umma.cuh"
@@ -84,6 +85,7 @@ struct Params {
     int prerot;                                       // remote K tiles come pre-rotated from the workspace (8(f)-1)
     int window_only;                                  // only the local band 0 <= q-k <= w0 (calls A and C of the unfused path)
     int qk_f16;                                       // Q and K hold fp16 (pre-rotated operands of calls B and C), not bf16
+    int qb_top, qb_lo;                                // this launch covers query blocks [qb_lo, qb_top), heaviest first
     const float2* lo;
     const float2* hi;
     const uint32_t* selinfo;                          // [H_kv][16]: 8 PRMT selectors (two pairs per 8-pair chunk), full-mode flag
@@ -215,11 +217,11 @@ __device__ __forceinline__ void prefill_body(const CUtensorMap& tmK, const CUten
     const int rank = (int)cluster_ctarank();
     const int cta = rank & 1;                                      // position in the CTA pair (0 = leader)
     const int pr = SHARE ? (rank >> 1) : 0;                        // which pair of the cluster
-    const int n_qb = (int)((p.L + BM - 1) / BM);
     const int pairs = p.H_q / 2;
     const int unit = SHARE ? (int)(blockIdx.x >> 2) : (int)(blockIdx.x >> 1);
-    const int qbA = SHARE ? n_qb - 1 - 2 * (unit / pairs) : n_qb - 1 - unit / pairs;   // heaviest row blocks first
-    const int qb = qbA - pr;                                       // SHARE: pair 1 takes the block below (-1 = none)
+    const int qbA = SHARE ? p.qb_top - 1 - 2 * (unit / pairs) : p.qb_top - 1 - unit / pairs;   // heaviest row blocks first
+    const int qbB = (qbA - 1 >= p.qb_lo) ? qbA - 1 : -1;           // SHARE: pair 1 takes the block below (-1 = none)
+    const int qb = pr == 0 ? qbA : qbB;
     const int h0 = 2 * (unit % pairs);
     const int head = h0 + cta;
     const int kvh = h0 / p.g;
@@ -232,7 +234,7 @@ __device__ __forceinline__ void prefill_body(const CUtensorMap& tmK, const CUten
     Plan plan(qb, p.w0, bifocal, p.window_only != 0);
     int n_local_peer = 0;                                          // SHARE: local visits of the other pair
     if (SHARE) {
-        const Plan pa(qbA, p.w0, bifocal), pb(qbA - 1, p.w0, bifocal);
+        const Plan pa(qbA, p.w0, bifocal), pb(qbB, p.w0, bifocal);
         if (pr == 1) plan.adopt_remote(pa.kt_hi);
         n_local_peer = pr == 0 ? pb.n_local : pa.n_local;
     }
@@ -835,9 +837,13 @@ size_t umma_prefill_unfused_workspace_bytes(long long L, int H_q, int H_kv, int 
     return two_level_bytes(L + 256, d) + 3 * align256(2 * nq) + align256(2 * nk) + 2 * align256((size_t)L * H_q * 4);
 }
 
-// 1: the on-the-fly bifocal prefill runs in clusters of four CTAs that share rotated K tiles (experimental, opt-in through
-// jetlong_set_prefill_impl(2): parity-green but not faster yet); 0: CTA pairs only (default)
-int g_share_clusters = 0;
+// How the on-the-fly bifocal prefill is launched (jetlong_set_prefill_impl):
+//   0  CTA pairs only (impl 1)
+//   1  clusters of four CTAs that share rotated K tiles, every query block (impl 2)
+//   2  clusters of four on an internal high-priority stream + CTA pairs for the lightest query blocks on the SMs that
+//      cannot hold a cluster (impl 3)
+//   3  default: as 2 when there are at least 64 query blocks, CTA pairs otherwise
+int g_share_clusters = 3;
 
 bool umma_prefill_supported(long long L, int H_q, int H_kv, int d, int dtype) {
     if (dtype != JETLONG_BF16 || d != 128 || H_kv < 1 || H_q % H_kv) return false;
@@ -872,6 +878,8 @@ int launch_prefill_umma(const void* Q, const void* K, const void* V, void* out, 
     p.window_only = 0;
     p.qk_f16 = 0;
     p.selinfo = nullptr;
+    p.qb_top = (int)((L + BM - 1) / BM);
+    p.qb_lo = 0;
     CUtensorMap tmKh = tmK, tmKe = tmK, tmKl = tmK;
     p.lo = nullptr; p.hi = nullptr;
     if (bifocal) {
@@ -925,7 +933,11 @@ int launch_prefill_umma(const void* Q, const void* K, const void* V, void* out, 
         attr_set = true;
     }
     const int n_qb = (int)((L + BM - 1) / BM);
-    if (bifocal && !p.prerot && g_share_clusters) {
+    const bool capturing = [&] {
+        cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+        return cudaStreamIsCapturing(st, &cs) == cudaSuccess && cs != cudaStreamCaptureStatusNone;
+    }();
+    if (bifocal && !p.prerot && g_share_clusters && !(g_share_clusters == 3 && (n_qb < 64 || capturing))) {
         // on the fly: clusters of four CTAs, two query blocks per cluster share each rotated K tile
         CUtensorMap tmK32;
         if (!make_kv_tensor_map(&tmK32, K, L, H_kv, 32)) return JETLONG_UNSUPPORTED;
@@ -936,10 +948,53 @@ int launch_prefill_umma(const void* Q, const void* K, const void* V, void* out, 
                 return check_launch("prefill_umma_share attr");
             attr4_set = true;
         }
-        const unsigned grid4 = 4u * (unsigned)((n_qb + 1) / 2) * (unsigned)(H_q / 2);
-        prefill_umma_share_kernel<<<grid4, NTHREADS, SMEM_BYTES, st>>>(tmK, tmV, tmK32, p);
+        // Only 132 of the 148 SMs can hold a 4-CTA cluster of this size.  With g_share_clusters == 2 the lightest query
+        // blocks [0, qb_lo) -- about the share of the work 16 SMs can do -- go to the CTA-pair kernel on the caller's
+        // stream, while the clusters run on an internal high-priority stream (fork / join through events): the block
+        // scheduler places clusters first and fills the SMs they cannot use with CTA pairs.
+        int qb_lo = 0;
+        if (g_share_clusters >= 2 && n_qb >= 64 && !capturing) {
+            qb_lo = (int)(0.30 * n_qb);                              // ~9 % of the visits; measured flat from 0.2 to 0.5
+            qb_lo -= (n_qb - qb_lo) & 1;                             // an even number of blocks for the clusters
+        }
+        struct Fork { cudaStream_t hs = nullptr; cudaEvent_t ev_fork = nullptr, ev_join = nullptr; };
+        static Fork forks[64];                                       // per device
+        static std::mutex fork_mu;
+        std::lock_guard<std::mutex> lock(fork_mu);                   // the events are reused from call to call
+        int dev = 0;
+        cudaGetDevice(&dev);
+        Fork& fk = forks[dev & 63];
+        cudaStream_t& hs = fk.hs;
+        cudaEvent_t &ev_fork = fk.ev_fork, &ev_join = fk.ev_join;
+        cudaStream_t s4 = st;
+        if (qb_lo > 0) {
+            if (!hs) {
+                int lo_pri = 0, hi_pri = 0;
+                cudaDeviceGetStreamPriorityRange(&lo_pri, &hi_pri);
+                if (cudaStreamCreateWithPriority(&hs, cudaStreamNonBlocking, hi_pri) != cudaSuccess ||
+                    cudaEventCreateWithFlags(&ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+                    cudaEventCreateWithFlags(&ev_join, cudaEventDisableTiming) != cudaSuccess)
+                    return check_launch("prefill_umma_share stream");
+            }
+            cudaEventRecord(ev_fork, st);
+            cudaStreamWaitEvent(hs, ev_fork, 0);
+            s4 = hs;
+        }
+        Params p4 = p;
+        p4.qb_top = n_qb; p4.qb_lo = qb_lo;
+        const unsigned grid4 = 4u * (unsigned)((n_qb - qb_lo + 1) / 2) * (unsigned)(H_q / 2);
+        prefill_umma_share_kernel<<<grid4, NTHREADS, SMEM_BYTES, s4>>>(tmK, tmV, tmK32, p4);
         note_launch();
-        return check_launch("prefill_umma_share_kernel");
+        int rc4 = check_launch("prefill_umma_share_kernel");
+        if (rc4 != JETLONG_OK || qb_lo == 0) return rc4;
+        cudaEventRecord(ev_join, hs);
+        Params p2 = p;
+        p2.qb_top = qb_lo; p2.qb_lo = 0;
+        prefill_umma_kernel<<<2u * (unsigned)qb_lo * (unsigned)(H_q / 2), NTHREADS, SMEM_BYTES, st>>>(tmK, tmV, tmKh, tmKe, tmKl, p2);
+        note_launch();
+        rc4 = check_launch("prefill_umma_kernel");
+        cudaStreamWaitEvent(st, ev_join, 0);
+        return rc4;
     }
     const unsigned grid = 2u * (unsigned)n_qb * (unsigned)(H_q / 2);
     prefill_umma_kernel<<<grid, NTHREADS, SMEM_BYTES, st>>>(tmK, tmV, tmKh, tmKe, tmKl, p);
@@ -968,6 +1023,8 @@ static int launch_plain(const void* Q, const void* K, const void* V, void* out, 
     p.prerot = 0;
     p.window_only = window_only ? 1 : 0;
     p.qk_f16 = qk_f16 ? 1 : 0;
+    p.qb_top = (int)((L + BM - 1) / BM);
+    p.qb_lo = 0;
     p.lo = nullptr; p.hi = nullptr; p.selinfo = nullptr;
     if (cudaFuncSetAttribute(prefill_umma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES) != cudaSuccess)
         return check_launch("prefill_umma attr");

@@ -245,17 +245,20 @@ def test_unfused_G1_is_the_control():
     assert torch.equal(out, outc) and torch.equal(lse, lsec)
 
 
-# ---- experimental: on-the-fly prefill in clusters of four CTAs sharing rotated K tiles (jetlong_set_prefill_impl(2)) ----
-@pytest.mark.parametrize("L,H_q,H_kv,w_pre,w0", [
-    (777, 4, 2, 200, 100),        # odd number of query blocks: one cluster has a block-less second pair
-    (640, 8, 2, 320, 128),        # G=2, g=4
-    (1300, 2, 1, 300, 0),         # G=5, w0=0
-    (4096, 4, 2, 1024, 128),      # 32 query blocks, long shared phases
+# ---- on-the-fly prefill in clusters of four CTAs sharing rotated K tiles (jetlong_set_prefill_impl 2 / 3; 3 is what the
+# default does from 64 query blocks on) and the CTA-pair kernel alone (impl 1) ---------------------------------------------
+@pytest.mark.parametrize("impl,L,H_q,H_kv,w_pre,w0", [
+    (2, 777, 4, 2, 200, 100),        # odd number of query blocks: one cluster has a block-less second pair
+    (2, 640, 8, 2, 320, 128),        # G=2, g=4
+    (2, 1300, 2, 1, 300, 0),         # G=5, w0=0
+    (2, 4096, 4, 2, 1024, 128),      # 32 query blocks, long shared phases
+    (3, 8320, 4, 2, 2048, 256),      # 65 query blocks: clusters for the top 46, CTA pairs for the lightest 19, G=5
+    (1, 8320, 4, 2, 2048, 256),      # the same through CTA pairs only
 ])
-def test_cluster_of_four_sharing_matches_oracle(L, H_q, H_kv, w_pre, w0):
+def test_cluster_of_four_sharing_matches_oracle(impl, L, H_q, H_kv, w_pre, w0):
     Q, K, V = W.make_qkv(L, H_q, H_kv, 128, 1e6, "bf16", 9753 + L, True, DEV)
     try:
-        J.jetlong_set_prefill_impl(2)
+        J.jetlong_set_prefill_impl(impl)
         out, lse = J.jetlong_prefill(Q, K, V, w_local=w0, w_pretrained=w_pre, rope_theta=1e6)
         torch.cuda.synchronize()
     finally:
@@ -264,5 +267,9 @@ def test_cluster_of_four_sharing_matches_oracle(L, H_q, H_kv, w_pre, w0):
     if L > 2000:
         pick = np.random.RandomState(2).choice(len(rows), 2048, replace=False)
         rows, heads = rows[pick], heads[pick]
+        edge = np.array([0, 127, 128, 19 * 128 - 1, 19 * 128, 20 * 128, L - 129, L - 128, L - 1])   # around the kernel split
+        edge = edge[edge < L]
+        rows = np.concatenate([rows, np.repeat(edge, H_q)])
+        heads = np.concatenate([heads, np.tile(np.arange(H_q, dtype=np.int32), len(edge))])
     ro, rl = oracle_rows(Q, K, V, rows, heads, w_local=w0, w_pretrained=w_pre, rope_theta=1e6)
-    check(*gather(out, lse, rows, heads), ro, rl, Q.dtype, "cluster-of-four L=%d" % L)
+    check(*gather(out, lse, rows, heads), ro, rl, Q.dtype, "impl %d L=%d" % (impl, L))
