@@ -297,7 +297,7 @@ def main():
     if rank == 0 and not args.no_extras:
         # ---- roofline of the dominant kernel (the prefill kernel is >99.9% of a step, profiles/) ----------
         impl = "tcgen05 UMMA" if _umma_active(B, cfg) else "SIMT fp32 FMA"
-        kern_ms = sum(per) / len(per)                             # the step is one prefill kernel + 2 table kernels (~10 us)
+        kern_ms = sum(per) / len(per)                             # the step is the two overlapped prefill kernels + the table check (~10 us)
         ach = fl / (kern_ms * 1e-3) / 1e12
         traffic = None
         tp = os.path.join(ROOT, "profiles", "traffic.json")
@@ -309,7 +309,8 @@ def main():
         else:
             peak, bound, which = 148 * 128 * 2 * 1.965e9 / 1e12, "alu", "148 SM x 128 FMA lanes x 2 x 1965 MHz (derived)"
         line["roofline"] = {"bound": bound, "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
-                            "traffic": traffic, "kernel": "prefill_umma_kernel (" + impl + ")", "peak_source": which,
+                            "traffic": traffic, "kernel": "prefill_umma_share_kernel (clusters of four, 91 % of the step) + prefill_umma_kernel "
+                                                          "(CTA pairs on the SMs that cannot hold a cluster), " + impl, "peak_source": which,
                             "algorithmic_flops_per_launch": fl,
                             "frac_of_bf16_burst_peak": ach / pk["tflops_burst"], "bf16_burst_peak": pk["tflops_burst"],
                             "frac_of_nominal_2250": ach / 2250.0,
