@@ -150,7 +150,7 @@ int jetlong_set_prefill_impl(int impl);
  *                          (kind::f8f6f4, half the tensor cycles of fp16); lse error ~2e-4.
  *   COMPENSATED_F16:       the two cross terms in fp16 as well (three fp16 UMMA groups); lse error ~1e-5.
  *   FAST:                  Q'hi K'hi only; lse error up to ~3e-3 on such inputs (out still within tolerance).
- * Local tiles, the control and decode are unaffected (decode always uses the fp16 cross terms).
+ * Local tiles, the control and decode are unaffected (decode always compensates: fp16 K'hi [Q'hi; Q'lo] + e5m2 K'lo Q'hi).
  * Returns the previous mode; an unknown mode changes nothing. */
 enum { JETLONG_PRECISION_COMPENSATED = 0, JETLONG_PRECISION_FAST = 1, JETLONG_PRECISION_COMPENSATED_F16 = 2 };
 int jetlong_set_prefill_precision(int mode);
