@@ -36,6 +36,8 @@ struct TableHeader {          // first 256 bytes of a table region; lets decode 
     int pad;
 };
 
+constexpr unsigned long long kTableMagic = 0x4a45544c4f4e4732ull;  // "JETLONG2": header of a sealed two-level table
+
 constexpr size_t align256(size_t x) { return (x + 255) & ~size_t(255); }
 
 // prefill (SIMT): key table

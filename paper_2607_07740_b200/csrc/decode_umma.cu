@@ -65,6 +65,7 @@ struct Params {
     int H_q, H_kv, g, bifocal;
     const float2* lo;
     const float2* hi;
+    double theta;                                    // for the table-header check (see the prologue)
 };
 
 // byte offset of element (row n, k) in a [2 boxes][16 rows][128 B] SWIZZLE_128B K-major operand (16-bit elements)
@@ -143,6 +144,22 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
     // the query loads go out before the TMA streams start: behind ~14 MB of in-flight cache tiles they take microseconds
     const int rt = tid - 96;                                           // rotate-group thread index
     __nv_bfloat16 qv1[NH * 64 / RT], qv2[NH * 64 / RT];
+    float2 tqh[NH * 64 / RT], tql[NH * 64 / RT];                       // HI / LO table entries of the query position
+    KRot<RROWS> rot;
+    bool tab_early = false;
+    const long long nq = (p.L - 1) - (p.L - 1) / p.G;                  // -Delta(q) >= 0, Eq.(5)
+    auto load_tables = [&]() {
+#pragma unroll
+        for (int it = 0; it < NH * 64 / RT; ++it) {
+            const int idx = rt + it * RT;
+            if (idx < p.g * 64) {
+                tqh[it] = __ldg(&p.hi[(nq >> 8) * 64 + (idx & 63)]);
+                tql[it] = __ldg(&p.lo[(nq & 255) * 64 + (idx & 63)]);
+            }
+        }
+        rot.init(p.lo, p.hi, rt, p.G);
+        rot.prefetch((unsigned)(plan.kt(0) * BN));
+    };
     if (warp >= 3 && warp < 3 + RW) {
 #pragma unroll
         for (int it = 0; it < NH * 64 / RT; ++it) {
@@ -152,6 +169,16 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
                 qv1[it] = qh[idx & 63];
                 qv2[it] = qh[(idx & 63) + 64];
             }
+        }
+        // So do the table loads (Q' entries, the unit step, the first tile's first rows): once the streams run, an L2 hit
+        // takes microseconds (measured: 8.4 k cycles from the first TMA to the first rotation, 1.7 k in the control).
+        // The tables come from the preceding kernel, which rewrites them only when their header does not match (theta,
+        // n_hi, d); if it matches NOW that kernel will find the same and write nothing, so they can be read before it ends.
+        if (plan.nr > 0) {
+            const volatile TableHeader* hdr =
+                reinterpret_cast<const volatile TableHeader*>(reinterpret_cast<const unsigned char*>(p.lo) - 256);
+            tab_early = hdr->magic == kTableMagic && hdr->theta == p.theta && hdr->n_hi == (p.L + 255) / 256 + 1 && hdr->d == D;
+            if (tab_early) load_tables();
         }
     }
     griddep_launch_dependents();                                       // the merge kernel may queue up behind us
@@ -264,8 +291,10 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
         for (int i = t; i < (QBUF + QCBUF + QYBUF) / 4; i += RT) reinterpret_cast<uint32_t*>(sQ)[i] = 0u;
         for (int i = t; i < QBUF / 4; i += RT) reinterpret_cast<uint32_t*>(sP)[i] = 0u;
         named_bar_sync(1, RT);
-        const long long nq = qpos - qpos / p.G;                      // -Delta(q) >= 0, Eq.(5)
-        if (plan.nr > 0) griddep_wait();                             // the rotation tables come from the preceding kernel
+        if (plan.nr > 0 && !tab_early) {                             // header not sealed: wait for the table kernel
+            griddep_wait();
+            load_tables();
+        }
 #pragma unroll
         for (int it = 0; it < NH * 64 / RT; ++it) {
             const int idx = t + it * RT;
@@ -275,7 +304,7 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
             *reinterpret_cast<__nv_bfloat16*>(sQ + bop_off(h, i)) = b1;
             *reinterpret_cast<__nv_bfloat16*>(sQ + bop_off(h, i + 64)) = b2;
             if (plan.nr > 0) {
-                const float2 ch = __ldg(&p.hi[(nq >> 8) * 64 + i]), cl = __ldg(&p.lo[(nq & 255) * 64 + i]);
+                const float2 ch = tqh[it], cl = tql[it];
                 const float c = ch.x * cl.x - ch.y * cl.y, s = ch.y * cl.x + ch.x * cl.y;
                 const float x1 = __bfloat162float(b1), x2 = __bfloat162float(b2);
                 const float y1 = x1 * c - x2 * s, y2 = x1 * s + x2 * c;
@@ -293,11 +322,6 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
         fence_proxy_async_smem();
         __syncwarp();
         if (lane == 0) mbar_arrive(&bars->q_ready);
-        KRot<RROWS> rot;
-        if (plan.nr > 0) {
-            rot.init(p.lo, p.hi, t, p.G);
-            rot.prefetch((unsigned)(plan.kt(0) * BN));
-        }
         for (int v = 0; v < plan.nv; ++v) {
             const int s = v % KS;
             mbar_wait(&bars->k_full[s], (v / KS) & 1);
@@ -452,8 +476,8 @@ void umma_decode_plan(long long L, int H_kv, int* nsplit, long long* kps) {
 }
 
 int launch_decode_umma(const void* q, const void* K, const void* V, float* part, long long L, int H_q, int H_kv,
-                       long long w0, long long G, bool bifocal, const float2* lo, const float2* hi, int* nsplit_out,
-                       cudaStream_t st) {
+                       long long w0, long long G, double theta, bool bifocal, const float2* lo, const float2* hi,
+                       int* nsplit_out, cudaStream_t st) {
     CUtensorMap tmK, tmV;
     if (!make_kv_tensor_map(&tmK, K, L, H_kv, BN) || !make_kv_tensor_map(&tmV, V, L, H_kv, BN)) return JETLONG_UNSUPPORTED;
     Params p;
@@ -465,6 +489,7 @@ int launch_decode_umma(const void* q, const void* K, const void* V, float* part,
     p.H_q = H_q; p.H_kv = H_kv; p.g = H_q / H_kv;
     p.bifocal = bifocal ? 1 : 0;
     p.lo = lo; p.hi = hi;
+    p.theta = theta;
     auto kern = p.g <= 1 ? decode_umma_kernel<1> : p.g <= 2 ? decode_umma_kernel<2> : p.g <= 4 ? decode_umma_kernel<4>
               : p.g <= 8 ? decode_umma_kernel<8> : decode_umma_kernel<16>;
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES) != cudaSuccess)

@@ -39,7 +39,7 @@ int build_key_table(float2* tab, long long L, long long G, int d, double theta, 
 // Independent of G; depends on L only through n_hi = ceil(L/256)+1, so consecutive decode steps skip the
 // rebuild (header match) except once every 256 tokens.
 // Region layout: [TableHeader (256 B)] [LO: 256*half float2] [HI: n_hi*half float2]
-static constexpr unsigned long long kMagic = 0x4a45544c4f4e4732ull;  // "JETLONG2"
+static constexpr unsigned long long kMagic = kTableMagic;
 
 size_t two_level_bytes(long long L, int d) {
     long long n_hi = (L + 255) / 256 + 1;
