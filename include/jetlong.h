@@ -143,16 +143,22 @@ int64_t jetlong_launch_count(void);
  * Returns the previous value. */
 int jetlong_set_prefill_impl(int impl);
 
-/* Operand precision of the REMOTE Q'K'^T on the tcgen05 prefill path (DESIGN.md 5.2).  Rotated operands must be
+/* Operand precision of the REMOTE Q'K'^T on the tcgen05 prefill path (DESIGN.md 5.2, 5.5).  Rotated operands must be
  * re-rounded for the tensor core; with one fp16 rounding (11 bits) the lse error reaches ~3e-3 on outlier-channel
  * inputs (tolerance 1e-3).  With y = hi + lo (hi = fp16(y), lo = y - hi):
  *   COMPENSATED (default): S = Q'hi K'hi (fp16 UMMA) + Q' K'lo + Q'lo K' with the two cross terms in e5m2
- *                          (kind::f8f6f4, half the tensor cycles of fp16); lse error ~2e-4.
- *   COMPENSATED_F16:       the two cross terms in fp16 as well (three fp16 UMMA groups); lse error ~1e-5.
+ *                          (kind::f8f6f4) over the two highest-energy channel pairs of every 8-pair chunk (32 of the
+ *                          128 channels, chosen per KV head on the device from the pair energies of K and Q); a head
+ *                          whose remaining channels are too loud (predicted score noise > 3e-4) gets the full cross
+ *                          terms.  lse error 1e-4 (64K-128K) to 8e-4 (short, peaked rows).
+ *   COMPENSATED_E5M2:      the two e5m2 cross terms over all 128 channels for every head; lse error ~3e-4.
+ *   COMPENSATED_F16:       the two cross terms in fp16 (three fp16 UMMA groups); lse error ~1e-5.  The workspace variant
+ *                          serves this mode with COMPENSATED_E5M2.
  *   FAST:                  Q'hi K'hi only; lse error up to ~3e-3 on such inputs (out still within tolerance).
  * Local tiles, the control and decode are unaffected (decode always compensates: fp16 K'hi [Q'hi; Q'lo] + e5m2 K'lo Q'hi).
  * Returns the previous mode; an unknown mode changes nothing. */
-enum { JETLONG_PRECISION_COMPENSATED = 0, JETLONG_PRECISION_FAST = 1, JETLONG_PRECISION_COMPENSATED_F16 = 2 };
+enum { JETLONG_PRECISION_COMPENSATED = 0, JETLONG_PRECISION_FAST = 1, JETLONG_PRECISION_COMPENSATED_F16 = 2,
+       JETLONG_PRECISION_COMPENSATED_E5M2 = 3 };
 int jetlong_set_prefill_precision(int mode);
 
 /* 1 if a bf16 prefill of these shapes runs on the tcgen05 UMMA kernel under the current setting, else 0. */

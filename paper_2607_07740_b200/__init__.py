@@ -3,4 +3,5 @@ from .binding import (BF16, FP32, JetlongError, jetlong_causal_decode, jetlong_c
                       jetlong_decode, jetlong_group_size, jetlong_launch_count, jetlong_prefill,
                       jetlong_prefill_host, jetlong_prefill_prerotated, jetlong_prefill_unfused, jetlong_set_prefill_impl,
                       jetlong_set_prefill_precision,
-                      jetlong_workspace_bytes, PRECISION_COMPENSATED, PRECISION_COMPENSATED_F16, PRECISION_FAST)
+                      jetlong_workspace_bytes, PRECISION_COMPENSATED, PRECISION_COMPENSATED_E5M2,
+                      PRECISION_COMPENSATED_F16, PRECISION_FAST)

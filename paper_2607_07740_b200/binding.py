@@ -17,7 +17,7 @@ OK, INVALID_ARG, UNSUPPORTED, CUDA_ERROR = 0, 1, 2, 3
 BF16, FP32 = 0, 1
 OP_PREFILL, OP_DECODE, OP_CAUSAL_PREFILL, OP_CAUSAL_DECODE, OP_PREFILL_PREROTATED, OP_PREFILL_UNFUSED = \
     0, 1, 2, 3, 4, 5
-PRECISION_COMPENSATED, PRECISION_FAST, PRECISION_COMPENSATED_F16 = 0, 1, 2
+PRECISION_COMPENSATED, PRECISION_FAST, PRECISION_COMPENSATED_F16, PRECISION_COMPENSATED_E5M2 = 0, 1, 2, 3
 
 EXPORTS = ["jetlong_group_size", "jetlong_workspace_bytes", "jetlong_prefill", "jetlong_decode",
            "jetlong_causal_prefill", "jetlong_causal_decode", "jetlong_prefill_host", "jetlong_status_string",

@@ -86,7 +86,8 @@ static int prefill_common(const void* Q, const void* K, const void* V, void* out
     const int prec = g_prefill_precision.load();
     if (prerot || use_umma(L, H_q, H_kv, d, dtype))
         return launch_prefill_umma(Q, K, V, out, lse, L, H_q, H_kv, d, w0, G, theta, bifocal,
-                                   prec == JETLONG_PRECISION_FAST ? 0 : (prec == JETLONG_PRECISION_COMPENSATED_F16 ? 1 : 2), ws, ws_bytes, st,
+                                   prec == JETLONG_PRECISION_FAST ? 0 : prec == JETLONG_PRECISION_COMPENSATED_F16 ? 1 : prec == JETLONG_PRECISION_COMPENSATED_E5M2 ? 6 : 2,
+                                   ws, ws_bytes, st,
                                    prerot && bifocal);
     const float2* tab = nullptr;
     if (bifocal) {
@@ -237,7 +238,8 @@ int jetlong_set_prefill_impl(int impl) {
 }
 
 int jetlong_set_prefill_precision(int mode) {
-    if (mode != JETLONG_PRECISION_COMPENSATED && mode != JETLONG_PRECISION_FAST && mode != JETLONG_PRECISION_COMPENSATED_F16)
+    if (mode != JETLONG_PRECISION_COMPENSATED && mode != JETLONG_PRECISION_FAST && mode != JETLONG_PRECISION_COMPENSATED_F16 &&
+        mode != JETLONG_PRECISION_COMPENSATED_E5M2)
         return g_prefill_precision.load();
     return g_prefill_precision.exchange(mode);
 }

@@ -276,7 +276,7 @@ __device__ __forceinline__ void prefill_body(const CUtensorMap& tmK, const CUten
             const uint32_t peer_smem = mapa_u32(smem_u32(smem), (uint32_t)(rank ^ 2));
             const uint32_t peer_full0 = mapa_u32(smem_u32(&bars->peer_full[0]), (uint32_t)(rank ^ 2));
             const uint32_t ready0 = mapa_u32(smem_u32(&bars->kv_ready_sh[0]), (uint32_t)(rank & ~1));
-            const uint32_t nbox = precise == 0 ? 2u : 4u;            // 4 KB pieces: the K'hi boxes (+ the two cross-term boxes)
+            const uint32_t nbox = precise == 0 ? 2u : precise == 3 ? 3u : 4u;   // 4 KB pieces: K'hi boxes (+ cross-term boxes)
             const int nsh = plan.nv - plan.n_local;                  // shared (remote) visits
             int lv = 0, cu = 0, du = 0;
             bool go = false;
@@ -462,6 +462,7 @@ __device__ __forceinline__ void prefill_body(const CUtensorMap& tmK, const CUten
         KRot<RR> rot;
         if (plan.n_remote > 0 && !p.prerot) {
             rot.init(p.lo, p.hi, t, p.G, SHARE ? 32 * pr : 0);
+            rot.selw = p.selinfo ? __ldg(p.selinfo + kvh * 16 + (t & 7)) : 0u;
             rot.prefetch((unsigned)(plan.kt_hi * BN + 64 * cta));     // first remote visit
         }
         for (int v = 0; v < plan.nv; ++v) {
@@ -480,7 +481,7 @@ __device__ __forceinline__ void prefill_body(const CUtensorMap& tmK, const CUten
                     // shared visit: rotate our 32 rows, fence, tell the producer thread (it sends them to the other pair and
                     // hands the stage to the MMA warp once the other pair's rows have landed)
                     const int u = v - plan.n_local;
-                    rotate_k_rows<RR, KBOX>(smem_u32(sK(s)), smem_u32(sKl(s)), (unsigned)(x.kt * BN + 64 * cta), rot, precise);
+                    rotate_k_rows<RR, KBOX>(smem_u32(sK(s)), smem_u32(sKl(s)), (unsigned)(x.kt * BN + 64 * cta), rot, precise == 3 ? 4 : precise);
                     fence_proxy_async_smem();
                     if (x.kt > 0) rot.prefetch((unsigned)((x.kt - 1) * BN + 64 * cta));
                     __syncwarp();
@@ -491,7 +492,7 @@ __device__ __forceinline__ void prefill_body(const CUtensorMap& tmK, const CUten
                     continue;
                 }
                 if (!p.prerot) {
-                    rotate_k_rows<RR, KBOX>(smem_u32(sK(s)), smem_u32(sKl(s)), (unsigned)(x.kt * BN + 64 * cta), rot, precise);
+                    rotate_k_rows<RR, KBOX>(smem_u32(sK(s)), smem_u32(sKl(s)), (unsigned)(x.kt * BN + 64 * cta), rot, precise == 3 ? 4 : precise);
                     fence_proxy_async_smem();
                     if (x.kt > 0) rot.prefetch((unsigned)((x.kt - 1) * BN + 64 * cta));   // next remote visit's first row
                 }
@@ -827,6 +828,26 @@ static bool make_tensor_map(CUtensorMap* m, const void* base, long long L, int H
               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
+// pair energies of K (every row) and Q (every 8th row) and the per-head selection table (selective compensation);
+// scratch: eK [H_kv][64] | eQ [H_kv][64] floats, then selinfo [H_kv][16] uint32
+static size_t selection_bytes(int H_kv) { return align256((size_t)H_kv * 64 * 4 * 2) + align256((size_t)H_kv * 16 * 4); }
+static int run_selection(const void* Q, const void* K, long long L, int H_q, int H_kv, unsigned char* scratch,
+                         cudaStream_t st, uint32_t** selinfo_out) {
+    float* eK = reinterpret_cast<float*>(scratch);
+    float* eQ = eK + (size_t)H_kv * 64;
+    uint32_t* selinfo = reinterpret_cast<uint32_t*>(scratch + align256((size_t)H_kv * 64 * 4 * 2));
+    if (cudaMemsetAsync(eK, 0, (size_t)H_kv * 64 * 4 * 2, st) != cudaSuccess) return check_launch("memset");
+    const int sk = 1, sq = 8;
+    const unsigned bk = (unsigned)((L / sk + 255) / 256), bq = (unsigned)((L / sq + 255) / 256);
+    pair_energy_kernel<<<dim3(bk ? bk : 1, H_kv), 256, 0, st>>>((const __nv_bfloat16*)K, eK, L, H_kv, 1, sk);
+    pair_energy_kernel<<<dim3(bq ? bq : 1, H_q), 256, 0, st>>>((const __nv_bfloat16*)Q, eQ, L, H_q, H_q / H_kv, sq);
+    const double nk = (double)((L + sk - 1) / sk), nq = (double)((L + sq - 1) / sq) * (H_q / H_kv);
+    select_pairs_kernel<<<H_kv, 64, 0, st>>>(eK, eQ, selinfo, (float)(1.0 / nk), (float)(1.0 / nq));
+    note_launch(3);
+    *selinfo_out = selinfo;
+    return check_launch("select_pairs_kernel");
+}
+
 bool make_kv_tensor_map(CUtensorMap* m, const void* base, long long L, int H, int rows) {
     return make_tensor_map(m, base, L, H, rows, 2);
 }
@@ -844,6 +865,8 @@ size_t umma_prefill_unfused_workspace_bytes(long long L, int H_q, int H_kv, int 
 //      cannot hold a cluster (impl 3)
 //   3  default: as 2 when there are at least 64 query blocks, CTA pairs otherwise
 int g_share_clusters = 3;
+// 1: the default precision of the on-the-fly kernel uses the selective e5m2 compensation; 0: the full cross terms
+int g_otf_selective = 1;
 
 bool umma_prefill_supported(long long L, int H_q, int H_kv, int d, int dtype) {
     if (dtype != JETLONG_BF16 || d != 128 || H_kv < 1 || H_q % H_kv) return false;
@@ -851,13 +874,12 @@ bool umma_prefill_supported(long long L, int H_q, int H_kv, int d, int dtype) {
     return (g % 2) == 0 && L >= 1 && L < (1ll << 30);
 }
 
-size_t umma_prefill_workspace_bytes(long long L, int, int, int d) { return two_level_bytes(L + 256, d); }
+size_t umma_prefill_workspace_bytes(long long L, int, int H_kv, int d) { return two_level_bytes(L + 256, d) + selection_bytes(H_kv); }
 
 // pre-rotated variant: tables, then K'hi (fp16), K' (e5m2), K'lo (e5m2), each [L, H_kv, 128]
 size_t umma_prefill_prerot_workspace_bytes(long long L, int H_kv, int d) {
     const size_t n = (size_t)L * H_kv * d;
-    return two_level_bytes(L + 256, d) + align256(2 * n) + 2 * align256(n) + align256((size_t)H_kv * 64 * 4 * 2) +
-           align256((size_t)H_kv * 16 * 4);       // + pair energies of K and Q, selection table
+    return two_level_bytes(L + 256, d) + align256(2 * n) + 2 * align256(n) + selection_bytes(H_kv);
 }
 
 int launch_prefill_umma(const void* Q, const void* K, const void* V, void* out, float* lse, long long L, int H_q,
@@ -873,6 +895,8 @@ int launch_prefill_umma(const void* Q, const void* K, const void* V, void* out, 
     p.L = L; p.w0 = w0; p.G = G;
     p.H_q = H_q; p.H_kv = H_kv; p.g = H_q / H_kv;
     p.bifocal = bifocal ? 1 : 0;
+    const bool full_e5m2 = precise == 6;                           // JETLONG_PRECISION_COMPENSATED_E5M2: never the selective form
+    if (full_e5m2) precise = 2;
     p.precise = precise;
     p.prerot = 0;
     p.window_only = 0;
@@ -890,7 +914,7 @@ int launch_prefill_umma(const void* Q, const void* K, const void* V, void* out, 
         if (prerot) {
             // the scratch holds e5m2 cross-term operands only: the fp16 mode is served by the full e5m2 terms (2),
             // the default by the selective e5m2 terms (3) with a per-head fallback to 2
-            precise = p.precise = (precise == 0 ? 0 : precise == 1 ? 2 : 3);
+            precise = p.precise = (precise == 0 ? 0 : (precise == 1 || full_e5m2) ? 2 : 3);
             const size_t n = (size_t)L * H_kv * d;
             unsigned char* base = (unsigned char*)ws + two_level_bytes(L + 256, d);
             __half* Kh = reinterpret_cast<__half*>(base);
@@ -898,18 +922,7 @@ int launch_prefill_umma(const void* Q, const void* K, const void* V, void* out, 
             unsigned char* Kl = Ke + align256(n);
             uint32_t* selinfo = nullptr;
             if (precise == 3) {
-                float* eK = reinterpret_cast<float*>(Kl + align256(n));
-                float* eQ = eK + (size_t)H_kv * 64;
-                selinfo = reinterpret_cast<uint32_t*>(reinterpret_cast<unsigned char*>(eK) + align256((size_t)H_kv * 64 * 4 * 2));
-                if (cudaMemsetAsync(eK, 0, (size_t)H_kv * 64 * 4 * 2, st) != cudaSuccess) return check_launch("memset");
-                const int sk = 1, sq = 8;                              // every key row, every 8th query row
-                const unsigned bk = (unsigned)((L / sk + 255) / 256), bq = (unsigned)((L / sq + 255) / 256);
-                pair_energy_kernel<<<dim3(bk ? bk : 1, H_kv), 256, 0, st>>>((const __nv_bfloat16*)K, eK, L, H_kv, 1, sk);
-                pair_energy_kernel<<<dim3(bq ? bq : 1, H_q), 256, 0, st>>>((const __nv_bfloat16*)Q, eQ, L, H_q, H_q / H_kv, sq);
-                const double nk = (double)((L + sk - 1) / sk), nq = (double)((L + sq - 1) / sq) * (H_q / H_kv);
-                select_pairs_kernel<<<H_kv, 64, 0, st>>>(eK, eQ, selinfo, (float)(1.0 / nk), (float)(1.0 / nq));
-                note_launch(3);
-                rc = check_launch("select_pairs_kernel");
+                rc = run_selection(Q, K, L, H_q, H_kv, Kl + align256(n), st, &selinfo);
                 if (rc != JETLONG_OK) return rc;
                 p.selinfo = selinfo;
             }
@@ -923,6 +936,14 @@ int launch_prefill_umma(const void* Q, const void* K, const void* V, void* out, 
                 !make_tensor_map(&tmKl, Kl, L, H_kv, 64, 1))
                 return JETLONG_UNSUPPORTED;
             p.prerot = 1;
+        } else if (precise == 2 && g_otf_selective && !full_e5m2) {
+            // on the fly, default precision: selective e5m2 compensation as in the workspace variant (per-head fallback
+            // to the full cross terms inside the kernel)
+            uint32_t* selinfo = nullptr;
+            rc = run_selection(Q, K, L, H_q, H_kv, (unsigned char*)ws + two_level_bytes(L + 256, d), st, &selinfo);
+            if (rc != JETLONG_OK) return rc;
+            p.selinfo = selinfo;
+            precise = p.precise = 3;
         }
     }
     static bool attr_set = false;

@@ -131,6 +131,7 @@ template <int ROWS> struct KRot {
     const float2* lo; const float2* hi;
     int c, r0;
     unsigned G;
+    uint32_t selw;                  // mode 4: PRMT selector of the two compensated pairs of this thread's chunk
     __device__ __forceinline__ void init(const float2* lo_, const float2* hi_, int t, long long G_, int rbase = 0) {
         lo = lo_; hi = hi_; c = t & 7; r0 = rbase + ROWS * (t >> 3); G = (unsigned)G_;
         const float4* p1 = reinterpret_cast<const float4*>(lo + 64 + 8 * c);       // LO[1][8c..]
@@ -179,6 +180,9 @@ __device__ __forceinline__ void split_hi_lo(uint64_t y, uint32_t& h, uint32_t& l
 __device__ __forceinline__ uint32_t e5m2x4(uint32_t w0, uint32_t w1) {
     return __byte_perm(w0 + 0x00800080u, w1 + 0x00800080u, 0x7531);
 }
+__device__ __forceinline__ void sts16s(uint32_t a, uint32_t v) {           // low 16 bits of v
+    asm volatile("st.shared.u16 [%0], %1;" ::"r"(a), "h"((uint16_t)v) : "memory");
+}
 __device__ __forceinline__ void sts64(uint32_t a, uint32_t x, uint32_t y) {
     asm volatile("st.shared.v2.u32 [%0], {%1,%2};" ::"r"(a), "r"(x), "r"(y) : "memory");
 }
@@ -198,7 +202,9 @@ __device__ __forceinline__ void sts128(uint32_t a, uint32_t x, uint32_t y, uint3
 template <int ROWS, int KBOX, bool REMOTE = false>
 __device__ __forceinline__ void rotate_k_rows(uint32_t kh, uint32_t kl, unsigned pos0, KRot<ROWS>& R,
                                               int precise, uint32_t rkh = 0, uint32_t rkl = 0) {   // kh, kl: shared-space addresses
-    // precise: 0 = hi only; 1 = fp16 lo at kl (same layout as kh); 2 = e5m2 copies for the cross terms at kl:
+    // precise: 4 = selective e5m2 compensation: one 128-byte row per key at kl = [lo1 | lo2 | hi1 | hi2] (16 B each: the two
+    //          pairs R.selw picks from each 8-pair chunk, as e5m2) | unused, SWIZZLE_128B;
+    //          0 = hi only; 1 = fp16 lo at kl (same layout as kh); 2 = e5m2 copies for the cross terms at kl:
     //          [box of KBOX bytes: K' as e5m2, rows x 128 channels][box: K' lo as e5m2], SWIZZLE_128B;
     //          3 = only K' lo as e5m2 at kl (one box)
     // first-row (cos, sin) from the prefetched table entries: HI * LO as complex numbers
@@ -266,6 +272,12 @@ __device__ __forceinline__ void rotate_k_rows(uint32_t kh, uint32_t kl, unsigned
                 ptx::sts64_cluster(rkl + KBOX + o1, c0, c1);
                 ptx::sts64_cluster(rkl + KBOX + o2, d0, d1);
             }
+        } else if (precise == 4) {
+            const uint32_t rb = kl + r * 128 + 2 * R.c, x = (uint32_t)(r & 7);
+            sts16s(rb + ((0u ^ x) << 4), __byte_perm(e5m2x4(l1[0], l1[1]), e5m2x4(l1[2], l1[3]), R.selw));
+            sts16s(rb + ((1u ^ x) << 4), __byte_perm(e5m2x4(l2[0], l2[1]), e5m2x4(l2[2], l2[3]), R.selw));
+            sts16s(rb + ((2u ^ x) << 4), __byte_perm(e5m2x4(h1[0], h1[1]), e5m2x4(h1[2], h1[3]), R.selw));
+            sts16s(rb + ((3u ^ x) << 4), __byte_perm(e5m2x4(h2[0], h2[1]), e5m2x4(h2[2], h2[3]), R.selw));
         } else if (precise == 3) {
             const uint32_t o1 = r * 128 + ((((R.c >> 1)) ^ (r & 7)) << 4) + (R.c & 1) * 8;
             const uint32_t o2 = r * 128 + (((4 + (R.c >> 1)) ^ (r & 7)) << 4) + (R.c & 1) * 8;

@@ -120,7 +120,7 @@ def test_config4_layers_sampled_rows(w0, layer):
 
 
 def test_precision_modes_of_the_remote_scores():
-    """the default (e5m2 cross terms) and the fp16-compensated mode meet the lse tolerance on
+    """the default (selective e5m2 cross terms), the full e5m2 and the fp16-compensated modes meet the lse tolerance on
     outlier-channel inputs; the opt-in fast mode keeps out within tolerance but not lse."""
     from paper_2607_07740_b200 import binding as B
     L, H_q, H_kv, d, theta, w_pre, w0 = 4096, 4, 2, 128, 1e6, 1024, 128
@@ -131,7 +131,8 @@ def test_precision_modes_of_the_remote_scores():
     ro, rl = oracle_rows(Q, K, V, rows, heads, w_local=w0, w_pretrained=w_pre, rope_theta=theta)
     errs = {}
     try:
-        for name, mode in (("default", B.PRECISION_COMPENSATED), ("f16", B.PRECISION_COMPENSATED_F16), ("fast", B.PRECISION_FAST)):
+        for name, mode in (("default", B.PRECISION_COMPENSATED), ("e5m2", B.PRECISION_COMPENSATED_E5M2),
+                           ("f16", B.PRECISION_COMPENSATED_F16), ("fast", B.PRECISION_FAST)):
             J.jetlong_set_prefill_precision(mode)
             out, lse = J.jetlong_prefill(Q, K, V, w_local=w0, w_pretrained=w_pre, rope_theta=theta)
             torch.cuda.synchronize()
@@ -139,7 +140,7 @@ def test_precision_modes_of_the_remote_scores():
             errs[name] = (np.abs(og.double().cpu().numpy() - ro).max(), np.abs(lg.double().cpu().numpy() - rl).max())
     finally:
         J.jetlong_set_prefill_precision(B.PRECISION_COMPENSATED)
-    assert errs["default"][1] <= 1e-3 and errs["f16"][1] <= 1e-4, errs
+    assert errs["default"][1] <= 1e-3 and errs["e5m2"][1] <= 5e-4 and errs["f16"][1] <= 1e-4, errs
     assert all(e[0] <= 2e-2 for e in errs.values()), errs
     assert errs["fast"][1] <= 1e-2, errs                           # bounded, but it is NOT within the 1e-3 tolerance
 
