@@ -39,12 +39,17 @@ using namespace ptx;
 using namespace dev;
 
 constexpr int D = 128, BM = 128, BN = 128;
-constexpr int NS = 4;                                 // K/V ring depth
+// Two rings: K stages are released as soon as Q K^T of their visit has completed, V stages after P V -- so the K side
+// (TMA load -> rotate -> cluster exchange -> MMA) runs several visits ahead of the softmax (r1: one ring of four K|Klo|V
+// stages held every K tile until its P V, the K side had ~2 visits of slack and the MMA warp waited ~1.1 k cycles per
+// visit for operands).
+constexpr int NV = 4;                                 // V ring depth
+constexpr int NKMAX = 8;                              // K ring depth = min(NKMAX, K_RING_BYTES / K stage size)
 constexpr int KH_BYTES = 64 * D * 2;                  // this CTA's 64 keys: two 8 KB SWIZZLE_128B boxes (ch 0-63 | 64-127)
 constexpr int KBOX = 64 * 128;                        // one K box: 64 rows x 128 B
 constexpr int VH_BYTES = BN * 64 * 2;                 // this CTA's 64 channels of 128 keys: one 16 KB box
-constexpr int STAGE_BYTES = 2 * KH_BYTES + VH_BYTES;  // K (hi in place) | K lo | V
-constexpr int NTHREADS = 448;
+constexpr int K_RING_BYTES = 9 * KH_BYTES;            // 144 KB: 8 stages of K alone, 6 of K | compact lo rows, 4 of K | K lo
+constexpr int NTHREADS = 512;
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr int POLY_OF_4 = 0;                          // of every 4 exponential pairs, this many use the FMA-pipe polynomial.
 // Measured on C2 (same box, back to back): 0 -> 25.5 ms, 1 -> 25.4 ms, 2 -> 27.2 ms (default precision); the kernel runs
@@ -53,9 +58,12 @@ constexpr uint32_t TM_S = 0, TM_O = 256, TM_QA = 384, TM_QB = 448;
 constexpr uint32_t TM_QY = 448, TM_QR = 480;         // precision mode 2: Q' and Q' lo as e5m2 (32 columns each) in place of Qb
 
 struct Bars {
-    uint64_t kv_full[NS];      // local: TMA bytes of this CTA's K/V halves landed
-    uint64_t kv_ready[NS];     // leader: both rotate groups are done with stage s (8 warp arrivals)
-    uint64_t kv_empty[NS];     // both: MMAs reading stage s have completed (multicast commit)
+    uint64_t k_full[NKMAX];    // local: TMA bytes of this CTA's K half landed
+    uint64_t k_ready[NKMAX];   // leader: both rotate groups are done with K stage s (8 warp arrivals)
+    uint64_t k_empty[NKMAX];   // both: Q K^T reading K stage s has completed (multicast commit)
+    uint64_t v_full[NV];       // local: TMA bytes of this CTA's V half landed
+    uint64_t v_ready[NV];      // leader: the other CTA's V half has landed (its forwarding warp)
+    uint64_t v_empty[NV];      // both: P V reading V stage s has completed (multicast commit)
     uint64_t s_full[2];        // both: S_b holds Q K^T of a visit
     uint64_t p_full[2];        // leader: both softmax groups wrote P_b and are done reading S_b (8 warp arrivals)
     uint64_t pv_done;          // both: O += P V of a visit has completed
@@ -64,16 +72,26 @@ struct Bars {
     uint64_t q_local_done;     // both: the last local Q K^T has completed, Qa may be overwritten
     uint64_t q_rot_done;       // leader: Q' (hi, lo) staged in TMEM
     // cluster of four (SHARE): the other CTA pair rotates half of our rows and writes them into our stages
-    uint64_t peer_full[NS];    // local: the rows rotated by the other pair have landed in our stage (bulk copy, complete_tx)
-    uint64_t rows_done[NS];    // local: our four rotate warps have rotated and fenced their 32 rows of a shared visit
-    uint64_t kv_ready_sh[NS];  // leader: a shared visit is complete in a CTA of the pair (its own rows + the other pair's), 2 arrivals
-    uint64_t peer_empty[NS];   // both: the OTHER pair's MMAs reading ITS stage s have completed (its commit, multicast to us)
-    uint64_t peer_go;          // both: the other pair's last local visit has completed (all its stages are free)
+    uint64_t peer_full[NKMAX];   // local: the rows rotated by the other pair have landed in our stage (bulk copy, complete_tx)
+    uint64_t rows_done[NKMAX];   // local: our four rotate warps have rotated and fenced their 32 rows of a shared visit
+    uint64_t kv_ready_sh[NKMAX]; // leader: a shared visit is complete in a CTA of the pair (its own rows + the other pair's), 2 arrivals
+    uint64_t peer_empty[NKMAX];  // both: the OTHER pair's Q K^T reading ITS K stage s has completed (its commit, multicast to us)
+    uint64_t peer_go;            // both: the other pair's last local Q K^T has completed (all its K stages are free)
     uint32_t tmem_base;
     float xchg[4 * BM];        // row-max / row-sum exchange between the two column halves of a row
 };
 
-constexpr size_t SMEM_BYTES = 1024 /*align slack*/ + (size_t)NS * STAGE_BYTES + 4096 /*Bars*/;
+constexpr size_t SMEM_BYTES = 1024 /*align slack*/ + (size_t)NV * VH_BYTES + K_RING_BYTES + 4096 /*Bars*/;
+static_assert(SMEM_BYTES <= 232448, "shared memory budget");
+static_assert(sizeof(Bars) <= 4096, "Bars");
+
+// position in a ring of n stages: stage s, phase parity ph of the current use
+struct Ring {
+    int n, s;
+    uint32_t ph;
+    __device__ Ring(int n_, int start = 0) : n(n_), s(start % n_), ph((uint32_t)(start / n_) & 1u) {}
+    __device__ __forceinline__ void next() { if (++s == n) { s = 0; ph ^= 1u; } }
+};
 
 struct Params {
     const __nv_bfloat16* Q;
@@ -208,10 +226,8 @@ __device__ __forceinline__ void prefill_body(const CUtensorMap& tmK, const CUten
                                              const Params& p) {
     extern __shared__ unsigned char smem_raw[];
     unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-    Bars* bars = reinterpret_cast<Bars*>(smem + NS * STAGE_BYTES);
-    auto sK = [&](int s) { return smem + s * STAGE_BYTES; };
-    auto sKl = [&](int s) { return smem + s * STAGE_BYTES + KH_BYTES; };
-    auto sV = [&](int s) { return smem + s * STAGE_BYTES + 2 * KH_BYTES; };
+    unsigned char* kring = smem + NV * VH_BYTES;
+    Bars* bars = reinterpret_cast<Bars*>(kring + K_RING_BYTES);
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int rank = (int)cluster_ctarank();
@@ -227,8 +243,8 @@ __device__ __forceinline__ void prefill_body(const CUtensorMap& tmK, const CUten
     const int kvh = h0 / p.g;
     const long long q0 = (long long)qb * BM;
     const bool bifocal = p.bifocal != 0;
-    // 0 fast, 1 fp16 cross terms, 2 e5m2 cross terms, 3 (pre-rotated variant only) e5m2 cross terms over the two
-    // highest-energy pairs of every 8-pair chunk; a KV head whose other channels are too loud falls back to 2
+    // 0 fast, 1 fp16 cross terms, 2 e5m2 cross terms, 3 e5m2 cross terms over the two highest-energy pairs of every
+    // 8-pair chunk; a KV head whose other channels are too loud falls back to 2
     int precise = p.precise;
     if (precise == 3 && __ldg(p.selinfo + kvh * 16 + 8) != 0u) precise = 2;
     Plan plan(qb, p.w0, bifocal, p.window_only != 0);
@@ -239,14 +255,21 @@ __device__ __forceinline__ void prefill_body(const CUtensorMap& tmK, const CUten
         n_local_peer = pr == 0 ? pb.n_local : pa.n_local;
     }
     const uint32_t own_mask = 3u << (2 * pr), peer_mask = 3u << (2 * (pr ^ 1));
+    // K stage = K (hi in place) | cross-term operands; the same for every CTA of the cluster (one KV head)
+    const int KST = KH_BYTES + ((!bifocal || p.window_only || precise == 0) ? 0 : precise == 3 ? KBOX : 2 * KBOX);
+    const int NK = (K_RING_BYTES / KST) < NKMAX ? (K_RING_BYTES / KST) : NKMAX;
+    auto sK = [&](int st) { return kring + st * KST; };
+    auto sKl = [&](int st) { return kring + st * KST + KH_BYTES; };
+    auto sV = [&](int st) { return smem + st * VH_BYTES; };
 
     if (tid == 0) {
-        for (int i = 0; i < NS; ++i) { mbar_init(&bars->kv_full[i], 1); mbar_init(&bars->kv_ready[i], 8); mbar_init(&bars->kv_empty[i], 1); }
+        for (int i = 0; i < NKMAX; ++i) { mbar_init(&bars->k_full[i], 1); mbar_init(&bars->k_ready[i], 8); mbar_init(&bars->k_empty[i], 1); }
+        for (int i = 0; i < NV; ++i) { mbar_init(&bars->v_full[i], 1); mbar_init(&bars->v_ready[i], 1); mbar_init(&bars->v_empty[i], 1); }
         for (int i = 0; i < 2; ++i) { mbar_init(&bars->s_full[i], 1); mbar_init(&bars->p_full[i], 16); }
         mbar_init(&bars->pv_done, 1); mbar_init(&bars->o_full, 1); mbar_init(&bars->q_ready, 8);
         mbar_init(&bars->q_local_done, 1); mbar_init(&bars->q_rot_done, 8);
-        for (int i = 0; i < NS; ++i) { mbar_init(&bars->peer_full[i], 1); mbar_init(&bars->peer_empty[i], 1);
-                                       mbar_init(&bars->rows_done[i], 4); mbar_init(&bars->kv_ready_sh[i], 2); }
+        for (int i = 0; i < NKMAX; ++i) { mbar_init(&bars->peer_full[i], 1); mbar_init(&bars->peer_empty[i], 1);
+                                          mbar_init(&bars->rows_done[i], 4); mbar_init(&bars->kv_ready_sh[i], 2); }
         mbar_init(&bars->peer_go, 1);
         fence_barrier_init();
         prefetch_tmap(&tmK); prefetch_tmap(&tmV);
@@ -264,88 +287,93 @@ __device__ __forceinline__ void prefill_body(const CUtensorMap& tmK, const CUten
         if (SHARE) mbar_arrive_cluster_addr(mapa_u32(smem_u32(bar), (uint32_t)(rank & ~1)));
         else mbar_arrive_leader(bar);
     };
+    // 4 KB pieces a CTA sends per shared visit: its 32 rows of the two K'hi boxes (+ of the cross-term boxes)
+    const uint32_t nbox = precise == 0 ? 2u : precise == 3 ? 3u : 4u;
 
     if (warp == 0) {
-        // ===================== TMA producer (each CTA loads its halves) =====================
-        if (SHARE && lane == 0) {
-            // One thread, three duties, none of which may block the others (an event loop over non-blocking barrier tests):
-            //   load(v):  TMA of visit v once its stage is free; for a shared visit also arm peer_full with the incoming bytes
-            //   copy(u):  once our rotate warps have fenced their 32 rows of shared visit u and the other pair's stage is
-            //             free, send the rows to the CTA of the same parity in the other pair (bulk copies, async proxy)
-            //   land(u):  once our rows are done and the other pair's rows have landed, arrive on the pair's kv_ready_sh
-            const uint32_t peer_smem = mapa_u32(smem_u32(smem), (uint32_t)(rank ^ 2));
-            const uint32_t peer_full0 = mapa_u32(smem_u32(&bars->peer_full[0]), (uint32_t)(rank ^ 2));
-            const uint32_t ready0 = mapa_u32(smem_u32(&bars->kv_ready_sh[0]), (uint32_t)(rank & ~1));
-            const uint32_t nbox = precise == 0 ? 2u : precise == 3 ? 3u : 4u;   // 4 KB pieces: K'hi boxes (+ cross-term boxes)
-            const int nsh = plan.nv - plan.n_local;                  // shared (remote) visits
-            int lv = 0, cu = 0, du = 0;
-            bool go = false;
-            while (lv < plan.nv || cu < nsh || du < nsh) {
-                if (lv < plan.nv && (lv < NS || mbar_test(&bars->kv_empty[lv % NS], ((lv / NS) - 1) & 1))) {
-                    const Visit x = plan.at(lv, bifocal);
-                    const int s = lv % NS;
-                    if (x.mode == 2) {
-                        const int u = lv - plan.n_local;
-                        mbar_arrive_expect_tx(&bars->peer_full[u % NS], nbox * 4096u);
-                        mbar_arrive_expect_tx(&bars->kv_full[s], KH_BYTES / 2 + VH_BYTES);
-                        tma_load_3d(sK(s) + pr * 4096, &tmK32, &bars->kv_full[s], 0, kvh, x.kt * BN + 64 * cta + 32 * pr);
-                        tma_load_3d(sK(s) + KBOX + pr * 4096, &tmK32, &bars->kv_full[s], 64, kvh, x.kt * BN + 64 * cta + 32 * pr);
-                    } else {
-                        mbar_arrive_expect_tx(&bars->kv_full[s], KH_BYTES + VH_BYTES);
-                        tma_load_3d(sK(s), &tmK, &bars->kv_full[s], 0, kvh, x.kt * BN + 64 * cta);
-                        tma_load_3d(sK(s) + KBOX, &tmK, &bars->kv_full[s], 64, kvh, x.kt * BN + 64 * cta);
-                    }
-                    tma_load_3d(sV(s), &tmV, &bars->kv_full[s], 64 * cta, kvh, x.kt * BN);
-                    ++lv;
-                }
-                if (cu < nsh && mbar_test(&bars->rows_done[cu % NS], (cu / NS) & 1)) {
-                    const int vp = n_local_peer + cu, sp = vp % NS;  // the other pair's visit number and stage
-                    if (!go) go = mbar_test(&bars->peer_go, 0);  // its local visits are over: all its stages are free
-                    if (go && (cu < NS || mbar_test(&bars->peer_empty[sp], ((vp / NS) - 1) & 1))) {
-                        const int s = (plan.n_local + cu) % NS;
-                        const uint32_t src = smem_u32(smem) + (uint32_t)s * STAGE_BYTES + (uint32_t)pr * 4096u;
-                        const uint32_t dst = peer_smem + (uint32_t)sp * STAGE_BYTES + (uint32_t)pr * 4096u;
-                        const uint32_t mb = peer_full0 + 8u * (uint32_t)(cu % NS);
-                        for (uint32_t b = 0; b < nbox; ++b) bulk_copy_to_peer(dst + b * KBOX, src + b * KBOX, 4096u, mb);
-                        ++cu;
-                    }
-                }
-                if (du < cu && mbar_test(&bars->peer_full[du % NS], (du / NS) & 1)) {
-                    mbar_arrive_cluster_addr(ready0 + 8u * (uint32_t)(du % NS));
-                    ++du;
+        // ===================== K producer (each CTA loads its 64 keys; 32 in a shared visit) =====================
+        if (lane == 0) {
+            Ring rk(NK), ru(NK);
+            for (int v = 0; v < plan.nv; ++v, rk.next()) {
+                const Visit x = plan.at(v, bifocal);
+                const int st = rk.s;
+                if (v >= NK) mbar_wait(&bars->k_empty[st], rk.ph ^ 1u);
+                if (SHARE && x.mode == 2) {
+                    mbar_arrive_expect_tx(&bars->peer_full[ru.s], nbox * 4096u);   // the other pair's rows will land here
+                    ru.next();
+                    mbar_arrive_expect_tx(&bars->k_full[st], KH_BYTES / 2);
+                    tma_load_3d(sK(st) + pr * 4096, &tmK32, &bars->k_full[st], 0, kvh, x.kt * BN + 64 * cta + 32 * pr);
+                    tma_load_3d(sK(st) + KBOX + pr * 4096, &tmK32, &bars->k_full[st], 64, kvh, x.kt * BN + 64 * cta + 32 * pr);
+                } else if (p.prerot && x.mode == 2) {
+                    // pre-rotated variant: K' hi (fp16) and the e5m2 copies of K' and K' lo come from the workspace
+                    mbar_arrive_expect_tx(&bars->k_full[st], KH_BYTES + (precise == 2 ? 2 * KBOX : precise == 3 ? KBOX : 0));
+                    tma_load_3d(sK(st), &tmKh, &bars->k_full[st], 0, kvh, x.kt * BN + 64 * cta);
+                    tma_load_3d(sK(st) + KBOX, &tmKh, &bars->k_full[st], 64, kvh, x.kt * BN + 64 * cta);
+                    if (precise >= 2) tma_load_3d(sKl(st), &tmKe, &bars->k_full[st], 0, kvh, x.kt * BN + 64 * cta);
+                    if (precise == 2) tma_load_3d(sKl(st) + KBOX, &tmKl, &bars->k_full[st], 0, kvh, x.kt * BN + 64 * cta);
+                } else {
+                    mbar_arrive_expect_tx(&bars->k_full[st], KH_BYTES);
+                    tma_load_3d(sK(st), &tmK, &bars->k_full[st], 0, kvh, x.kt * BN + 64 * cta);
+                    tma_load_3d(sK(st) + KBOX, &tmK, &bars->k_full[st], 64, kvh, x.kt * BN + 64 * cta);
                 }
             }
-        } else if (lane == 0) {
-            for (int v = 0; v < plan.nv; ++v) {
+        }
+    } else if (warp == 2) {
+        // ===================== V producer (each CTA loads its 64 channels of the tile) =====================
+        if (lane == 0) {
+            Ring rv(NV);
+            for (int v = 0; v < plan.nv; ++v, rv.next()) {
                 const Visit x = plan.at(v, bifocal);
-                const int s = v % NS;
-                if (v >= NS) mbar_wait(&bars->kv_empty[s], ((v / NS) - 1) & 1);
-                if (p.prerot && x.mode == 2) {
-                    // pre-rotated variant: K' hi (fp16) and the e5m2 copies of K' and K' lo come from the workspace
-                    mbar_arrive_expect_tx(&bars->kv_full[s], KH_BYTES + VH_BYTES + (precise == 2 ? 2 * KBOX : precise == 3 ? KBOX : 0));
-                    tma_load_3d(sK(s), &tmKh, &bars->kv_full[s], 0, kvh, x.kt * BN + 64 * cta);
-                    tma_load_3d(sK(s) + KBOX, &tmKh, &bars->kv_full[s], 64, kvh, x.kt * BN + 64 * cta);
-                    if (precise >= 2) tma_load_3d(sKl(s), &tmKe, &bars->kv_full[s], 0, kvh, x.kt * BN + 64 * cta);
-                    if (precise == 2) tma_load_3d(sKl(s) + KBOX, &tmKl, &bars->kv_full[s], 0, kvh, x.kt * BN + 64 * cta);
-                } else {
-                    mbar_arrive_expect_tx(&bars->kv_full[s], KH_BYTES + VH_BYTES);
-                    tma_load_3d(sK(s), &tmK, &bars->kv_full[s], 0, kvh, x.kt * BN + 64 * cta);
-                    tma_load_3d(sK(s) + KBOX, &tmK, &bars->kv_full[s], 64, kvh, x.kt * BN + 64 * cta);
-                }
-                tma_load_3d(sV(s), &tmV, &bars->kv_full[s], 64 * cta, kvh, x.kt * BN);
+                if (v >= NV) mbar_wait(&bars->v_empty[rv.s], rv.ph ^ 1u);
+                mbar_arrive_expect_tx(&bars->v_full[rv.s], VH_BYTES);
+                tma_load_3d(sV(rv.s), &tmV, &bars->v_full[rv.s], 64 * cta, kvh, x.kt * BN);
+            }
+        }
+    } else if (warp == 3) {
+        // ===================== SHARE: exchange of rotated rows between the two pairs of the cluster =====================
+        // per shared visit u: once our rotate warps have fenced their 32 rows and the other pair's K stage is free, send the
+        // rows to the CTA of the same parity in the other pair (bulk copies, async proxy, complete_tx on ITS peer_full);
+        // once the other pair's rows have landed here, arrive on our pair's kv_ready_sh.
+        if (SHARE && lane == 0) {
+            const int nsh = plan.nv - plan.n_local;                  // shared (remote) visits
+            const uint32_t peer_k = mapa_u32(smem_u32(kring), (uint32_t)(rank ^ 2));
+            const uint32_t peer_full0 = mapa_u32(smem_u32(&bars->peer_full[0]), (uint32_t)(rank ^ 2));
+            const uint32_t ready0 = mapa_u32(smem_u32(&bars->kv_ready_sh[0]), (uint32_t)(rank & ~1));
+            Ring rs(NK, plan.n_local), rp(NK, n_local_peer), ru(NK);
+            if (nsh > 0) mbar_wait(&bars->peer_go, 0);               // the other pair's local visits are over: its K stages are free
+            for (int u = 0; u < nsh; ++u, rs.next(), rp.next(), ru.next()) {
+                mbar_wait(&bars->rows_done[ru.s], ru.ph);
+                if (u >= NK) mbar_wait(&bars->peer_empty[rp.s], rp.ph ^ 1u);
+                const uint32_t src = smem_u32(kring) + (uint32_t)(rs.s * KST) + (uint32_t)pr * 4096u;
+                const uint32_t dst = peer_k + (uint32_t)(rp.s * KST) + (uint32_t)pr * 4096u;
+                const uint32_t mb = peer_full0 + 8u * (uint32_t)ru.s;
+                for (uint32_t b = 0; b < nbox; ++b) bulk_copy_to_peer(dst + b * KBOX, src + b * KBOX, 4096u, mb);
+                mbar_wait(&bars->peer_full[ru.s], ru.ph);
+                mbar_arrive_cluster_addr(ready0 + 8u * (uint32_t)ru.s);
             }
         }
     } else if (warp == 1) {
+        if (cta == 1) {
+            // ===================== non-leader CTA: tell the leader when our V half has landed =====================
+            if (lane == 0) {
+                Ring rv(NV);
+                for (int v = 0; v < plan.nv; ++v, rv.next()) {
+                    mbar_wait(&bars->v_full[rv.s], rv.ph);
+                    arrive_leader(&bars->v_ready[rv.s]);
+                }
+            }
+        } else {
         // ===================== MMA issuer (warp 1 of the leader CTA; one elected lane issues) =====================
         // The whole warp runs the loop convergently so that descriptors and TMEM addresses stay in uniform
         // registers; a divergent single-lane issuer costs ~100 cycles of R2UR/ELECT waterfall per MMA (measured).
-        if (cta == 0) {
             const uint32_t tm = __shfl_sync(0xffffffffu, tmem, 0);
-            const uint32_t smem0 = __shfl_sync(0xffffffffu, smem_u32(smem), 0);
+            const uint32_t kring0 = __shfl_sync(0xffffffffu, smem_u32(kring), 0);
+            const uint32_t vring0 = __shfl_sync(0xffffffffu, smem_u32(smem), 0);
+            Ring rq(NK), ruq(NK), rvp(NV);                           // K stage / shared-visit slot of the next Q K^T, V stage of the next P V
             auto issue_qk = [&](int v) {
                 const Visit x = plan.at(v, bifocal);
                 const uint32_t dS = tm + TM_S + (v & 1) * 128;
-                const uint32_t kb = smem0 + (v % NS) * STAGE_BYTES, klb = kb + KH_BYTES;
+                const uint32_t kb = kring0 + (uint32_t)(rq.s * KST), klb = kb + KH_BYTES;
                 if (elect_one()) {
                     if (x.mode != 2) {
                         const uint32_t idesc = p.qk_f16 ? IDESC_QK_F16 : IDESC_QK_BF16;
@@ -383,34 +411,39 @@ __device__ __forceinline__ void prefill_body(const CUtensorMap& tmK, const CUten
                         }
                     }
                     umma2_commit_mask(&bars->s_full[v & 1], own_mask);
+                    umma2_commit_mask(&bars->k_empty[rq.s], own_mask);   // the K stage is free again
+                    if (SHARE) {                                     // ... and the other pair may write ITS rows of our next use of it
+                        umma2_commit_mask(&bars->peer_empty[rq.s], peer_mask);
+                        if (v == plan.n_local - 1) umma2_commit_mask(&bars->peer_go, peer_mask);
+                    }
                     if (plan.n_remote > 0 && v == plan.n_local - 1) umma2_commit_mask(&bars->q_local_done, own_mask);
                 }
                 __syncwarp();
+                rq.next();
             };
             auto issue_pv = [&](int v) {
-                const uint32_t vb = smem0 + (v % NS) * STAGE_BYTES + 2 * KH_BYTES;
+                mbar_wait(&bars->v_full[rvp.s], rvp.ph);             // our V half ...
+                mbar_wait(&bars->v_ready[rvp.s], rvp.ph);            // ... and the other CTA's
+                const uint32_t vb = vring0 + (uint32_t)(rvp.s * VH_BYTES);
                 if (elect_one()) {
 #pragma unroll
                     for (int ks = 0; ks < BN / 16; ++ks)
                         umma2_ts(tm + TM_O, tm + TM_S + (v & 1) * 128 + ks * 8,
                                  smem_desc_sw128(vb + ks * 2048, VH_BYTES, 1024), IDESC_PV, (v > 0 || ks > 0) ? 1u : 0u);
-                    umma2_commit_mask(&bars->kv_empty[v % NS], own_mask);
-                    if (SHARE) {                                      // the other pair may now overwrite ITS rows of our next use of the stage
-                        umma2_commit_mask(&bars->peer_empty[v % NS], peer_mask);
-                        if (v == plan.n_local - 1) umma2_commit_mask(&bars->peer_go, peer_mask);
-                    }
+                    umma2_commit_mask(&bars->v_empty[rvp.s], own_mask);
                     umma2_commit_mask(&bars->pv_done, own_mask);
                 }
                 __syncwarp();
+                rvp.next();
             };
             // operands of visit v are in place: local visits (and every visit without SHARE) count the two rotate groups of
-            // the pair on kv_ready (in a shared visit each group arrives once the other pair's rows have landed too)
+            // the pair on k_ready (in a shared visit each CTA arrives once the other pair's rows have landed too)
             auto wait_ready = [&](int v) {
                 if (SHARE && v >= plan.n_local) {                     // shared visit: one arrival per CTA of the pair
-                    const int u = v - plan.n_local;
-                    mbar_wait(&bars->kv_ready_sh[u % NS], (u / NS) & 1);
+                    mbar_wait(&bars->kv_ready_sh[ruq.s], ruq.ph);
+                    ruq.next();
                 } else {
-                    mbar_wait(&bars->kv_ready[v % NS], (v / NS) & 1);
+                    mbar_wait(&bars->k_ready[rq.s], rq.ph);
                 }
             };
             if (SHARE && plan.n_local == 0 && elect_one()) umma2_commit_mask(&bars->peer_go, peer_mask);   // no local visit: all stages free
@@ -423,32 +456,22 @@ __device__ __forceinline__ void prefill_body(const CUtensorMap& tmK, const CUten
                 issue_qk(0);
             }
             for (int v = 0; v < plan.nv; ++v) {
-                // SHARE: the first shared visit can only become ready after OUR peer_go, which the P V of the last local
-                // visit commits -- so that one P V is issued before, not after, waiting for the next visit's operands
-                const bool pv_first = SHARE && v + 1 == plan.n_local;
-                if (pv_first) {
-                    mbar_wait(&bars->p_full[v & 1], (v >> 1) & 1);
-                    tc_fence_after();
-                    issue_pv(v);
-                }
                 if (v + 1 < plan.nv) {
                     if (plan.n_remote > 0 && v + 1 == plan.n_local) mbar_wait(&bars->q_rot_done, 0);
                     wait_ready(v + 1);
                     tc_fence_after();
                     issue_qk(v + 1);
                 }
-                if (!pv_first) {
-                    mbar_wait(&bars->p_full[v & 1], (v >> 1) & 1);
-                    tc_fence_after();
-                    issue_pv(v);
-                }
+                mbar_wait(&bars->p_full[v & 1], (v >> 1) & 1);
+                tc_fence_after();
+                issue_pv(v);
             }
             if (elect_one()) umma2_commit_mask(&bars->o_full, own_mask);
             __syncwarp();
         }
-    } else if (warp >= 2 && warp < 6) {
+    } else if (warp >= 4 && warp < 8) {
         // ===================== rotate group (steps a4, a5) =====================
-        const int t = tid - 64;                                       // work index for the K rotation
+        const int t = tid - 128;                                      // work index for the K rotation
         const uint32_t lane_base = (uint32_t)((warp & 3) << 5) << 16; // TMEM lanes a warp may touch: 32 (warp % 4) ..
         const long long q = q0 + (((warp & 3) << 5) | lane);
         const bool valid = q >= 0 && q < p.L;
@@ -465,10 +488,11 @@ __device__ __forceinline__ void prefill_body(const CUtensorMap& tmK, const CUten
             rot.selw = p.selinfo ? __ldg(p.selinfo + kvh * 16 + (t & 7)) : 0u;
             rot.prefetch((unsigned)(plan.kt_hi * BN + 64 * cta));     // first remote visit
         }
-        for (int v = 0; v < plan.nv; ++v) {
+        Ring rk(NK), ru(NK);
+        for (int v = 0; v < plan.nv; ++v, rk.next()) {
             const Visit x = plan.at(v, bifocal);
-            const int s = v % NS;
-            mbar_wait(&bars->kv_full[s], (v / NS) & 1);
+            const int st = rk.s;
+            mbar_wait(&bars->k_full[st], rk.ph);
             if (x.mode == 2) {
                 if (v == plan.n_local) {                              // first remote visit: Q -> Q' = R(Delta q) Q
                     if (plan.n_local > 0) mbar_wait(&bars->q_local_done, 0);
@@ -478,21 +502,21 @@ __device__ __forceinline__ void prefill_body(const CUtensorMap& tmK, const CUten
                     tc_fence_before();
                 }
                 if (SHARE) {
-                    // shared visit: rotate our 32 rows, fence, tell the producer thread (it sends them to the other pair and
+                    // shared visit: rotate our 32 rows, fence, tell the exchange thread (it sends them to the other pair and
                     // hands the stage to the MMA warp once the other pair's rows have landed)
-                    const int u = v - plan.n_local;
-                    rotate_k_rows<RR, KBOX>(smem_u32(sK(s)), smem_u32(sKl(s)), (unsigned)(x.kt * BN + 64 * cta), rot, precise == 3 ? 4 : precise);
+                    rotate_k_rows<RR, KBOX>(smem_u32(sK(st)), smem_u32(sKl(st)), (unsigned)(x.kt * BN + 64 * cta), rot, precise == 3 ? 4 : precise);
                     fence_proxy_async_smem();
                     if (x.kt > 0) rot.prefetch((unsigned)((x.kt - 1) * BN + 64 * cta));
                     __syncwarp();
                     if (lane == 0) {
-                        mbar_arrive(&bars->rows_done[u % NS]);
+                        mbar_arrive(&bars->rows_done[ru.s]);
                         if (v == plan.n_local) arrive_leader(&bars->q_rot_done);
                     }
+                    ru.next();
                     continue;
                 }
                 if (!p.prerot) {
-                    rotate_k_rows<RR, KBOX>(smem_u32(sK(s)), smem_u32(sKl(s)), (unsigned)(x.kt * BN + 64 * cta), rot, precise == 3 ? 4 : precise);
+                    rotate_k_rows<RR, KBOX>(smem_u32(sK(st)), smem_u32(sKl(st)), (unsigned)(x.kt * BN + 64 * cta), rot, precise == 3 ? 4 : precise);
                     fence_proxy_async_smem();
                     if (x.kt > 0) rot.prefetch((unsigned)((x.kt - 1) * BN + 64 * cta));   // next remote visit's first row
                 }
@@ -500,14 +524,14 @@ __device__ __forceinline__ void prefill_body(const CUtensorMap& tmK, const CUten
             __syncwarp();
             if (lane == 0) {
                 if (x.mode == 2 && v == plan.n_local) arrive_leader(&bars->q_rot_done);
-                arrive_leader(&bars->kv_ready[s]);
+                arrive_leader(&bars->k_ready[st]);
             }
         }
-    } else if (warp >= 6) {
+    } else if (warp >= 8) {
         // ===================== softmax groups (steps a6-a8) =====================
         // Two threads per query row: warps w and w+4 hold the same 32 rows, column half `half` (64 keys) each.
         // The S values are loaded ONCE into registers; the row max is combined through shared memory.
-        const int half = (warp - 6) >> 2;
+        const int half = (warp - 8) >> 2;
         const int quad = warp & 3;
         const int r = (quad << 5) | lane;
         const uint32_t lane_base = (uint32_t)(quad << 5) << 16;

@@ -78,6 +78,10 @@ template <int N> __device__ __forceinline__ void reg_inc() { asm volatile("setma
 __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
+// producer side of a named barrier: counts this thread in and goes on (the consumer side is named_bar_sync)
+__device__ __forceinline__ void named_bar_arrive(int id, int nthreads) {
+    asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
 
 // (cos, sin)(Delta(pos) theta_i) for 8 consecutive frequencies i = i0 .. i0+7 from the two-level table
 // (HI[n >> 8] * LO[n & 255] as complex numbers, n = -Delta(pos) >= 0, Eq.(5))
