@@ -54,6 +54,9 @@ constexpr float kLog2e = 1.4426950408889634f;
 constexpr int POLY_OF_4 = 0;                          // of every 4 exponential pairs, this many use the FMA-pipe polynomial.
 // Measured on C2 (same box, back to back): 0 -> 25.5 ms, 1 -> 25.4 ms, 2 -> 27.2 ms (default precision); the kernel runs
 // under the power cap (~1.45 GHz), where extra FMA instructions cost more clock than the freed MUFU cycles return.
+// warp roles.  The scheduler of an SM sub-partition prefers the highest warp id: the MMA issuer and the producers (few
+// instructions, all on the critical path) sit above the softmax warps, the rotate group (which runs visits ahead) below.
+constexpr int W_KLOAD = 12, W_VLOAD = 13, W_XCHG = 14, W_MMA = 15;   // warps 0-3 rotate, 4-11 softmax
 constexpr uint32_t TM_S = 0, TM_O = 256, TM_QA = 384, TM_QB = 448;
 constexpr uint32_t TM_QY = 448, TM_QR = 480;         // precision mode 2: Q' and Q' lo as e5m2 (32 columns each) in place of Qb
 
@@ -276,7 +279,7 @@ __device__ __forceinline__ void prefill_body(const CUtensorMap& tmK, const CUten
         if (SHARE) prefetch_tmap(&tmK32);
         if (p.prerot) { prefetch_tmap(&tmKh); prefetch_tmap(&tmKe); prefetch_tmap(&tmKl); }
     }
-    if (warp == 1) tmem_alloc2<512>(&bars->tmem_base);
+    if (warp == W_MMA) tmem_alloc2<512>(&bars->tmem_base);
     tc_fence_before();
     cluster_sync_all();                                            // barriers of both CTAs initialised, TMEM allocated
     tc_fence_after();
@@ -290,7 +293,7 @@ __device__ __forceinline__ void prefill_body(const CUtensorMap& tmK, const CUten
     // 4 KB pieces a CTA sends per shared visit: its 32 rows of the two K'hi boxes (+ of the cross-term boxes)
     const uint32_t nbox = precise == 0 ? 2u : precise == 3 ? 3u : 4u;
 
-    if (warp == 0) {
+    if (warp == W_KLOAD) {
         // ===================== K producer (each CTA loads its 64 keys; 32 in a shared visit) =====================
         if (lane == 0) {
             Ring rk(NK), ru(NK);
@@ -318,7 +321,7 @@ __device__ __forceinline__ void prefill_body(const CUtensorMap& tmK, const CUten
                 }
             }
         }
-    } else if (warp == 2) {
+    } else if (warp == W_VLOAD) {
         // ===================== V producer (each CTA loads its 64 channels of the tile) =====================
         if (lane == 0) {
             Ring rv(NV);
@@ -329,7 +332,7 @@ __device__ __forceinline__ void prefill_body(const CUtensorMap& tmK, const CUten
                 tma_load_3d(sV(rv.s), &tmV, &bars->v_full[rv.s], 64 * cta, kvh, x.kt * BN);
             }
         }
-    } else if (warp == 3) {
+    } else if (warp == W_XCHG) {
         // ===================== SHARE: exchange of rotated rows between the two pairs of the cluster =====================
         // per shared visit u: once our rotate warps have fenced their 32 rows and the other pair's K stage is free, send the
         // rows to the CTA of the same parity in the other pair (bulk copies, async proxy, complete_tx on ITS peer_full);
@@ -352,7 +355,7 @@ __device__ __forceinline__ void prefill_body(const CUtensorMap& tmK, const CUten
                 mbar_arrive_cluster_addr(ready0 + 8u * (uint32_t)ru.s);
             }
         }
-    } else if (warp == 1) {
+    } else if (warp == W_MMA) {
         if (cta == 1) {
             // ===================== non-leader CTA: tell the leader when our V half has landed =====================
             if (lane == 0) {
@@ -469,9 +472,9 @@ __device__ __forceinline__ void prefill_body(const CUtensorMap& tmK, const CUten
             if (elect_one()) umma2_commit_mask(&bars->o_full, own_mask);
             __syncwarp();
         }
-    } else if (warp >= 4 && warp < 8) {
+    } else if (warp < 4) {
         // ===================== rotate group (steps a4, a5) =====================
-        const int t = tid - 128;                                      // work index for the K rotation
+        const int t = tid;                                            // work index for the K rotation
         const uint32_t lane_base = (uint32_t)((warp & 3) << 5) << 16; // TMEM lanes a warp may touch: 32 (warp % 4) ..
         const long long q = q0 + (((warp & 3) << 5) | lane);
         const bool valid = q >= 0 && q < p.L;
@@ -527,11 +530,11 @@ __device__ __forceinline__ void prefill_body(const CUtensorMap& tmK, const CUten
                 arrive_leader(&bars->k_ready[st]);
             }
         }
-    } else if (warp >= 8) {
+    } else if (warp >= 4 && warp < 12) {
         // ===================== softmax groups (steps a6-a8) =====================
         // Two threads per query row: warps w and w+4 hold the same 32 rows, column half `half` (64 keys) each.
         // The S values are loaded ONCE into registers; the row max is combined through shared memory.
-        const int half = (warp - 8) >> 2;
+        const int half = (warp - 4) >> 2;
         const int quad = warp & 3;
         const int r = (quad << 5) | lane;
         const uint32_t lane_base = (uint32_t)(quad << 5) << 16;
@@ -657,7 +660,7 @@ __device__ __forceinline__ void prefill_body(const CUtensorMap& tmK, const CUten
     }
     tc_fence_before();
     cluster_sync_all();                                            // the peer may still be reading our smem / TMEM
-    if (warp == 1) tmem_dealloc2<512>(tmem);
+    if (warp == W_MMA) tmem_dealloc2<512>(tmem);
 }
 
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1)
