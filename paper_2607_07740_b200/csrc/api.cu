@@ -33,6 +33,7 @@ int launch_prefill_umma(const void* Q, const void* K, const void* V, void* out, 
                         size_t ws_bytes, cudaStream_t st, bool prerot);
 
 extern int g_share_clusters;   // prefill_umma.cu
+extern int g_two_tile;         // prefill_umma.cu
 
 static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; }
 
@@ -234,6 +235,7 @@ int64_t jetlong_launch_count(void) { return g_launches.load(); }
 
 int jetlong_set_prefill_impl(int impl) {
     g_share_clusters = impl == 2 ? 1 : impl == 3 ? 2 : impl == 1 ? 0 : 3;   // see prefill_umma.cu; -1 (default) = auto
+    g_two_tile = (impl == 1 || impl == 2 || impl == 3) ? 0 : 1;             // 1 / 2 / 3: the one-tile kernels
     return g_prefill_impl.exchange(impl);
 }
 

@@ -30,6 +30,7 @@
 #include "common.cuh"
 #include "umma.cuh"
 #include "rot.cuh"
+#include "prefill_v2.cuh"
 
 namespace jetlong {
 
@@ -892,6 +893,9 @@ size_t umma_prefill_unfused_workspace_bytes(long long L, int H_q, int H_kv, int 
 //      cannot hold a cluster (impl 3)
 //   3  default: as 2 when there are at least 64 query blocks, CTA pairs otherwise
 int g_share_clusters = 3;
+// 1 (default): the two-tile kernel of prefill_umma2.cu serves every precision it supports; 0: the one-tile kernels of this
+// file (jetlong_set_prefill_impl 1 / 2 / 3)
+int g_two_tile = 1;
 // 1: the default precision of the on-the-fly kernel uses the selective e5m2 compensation; 0: the full cross terms
 int g_otf_selective = 1;
 
@@ -972,6 +976,15 @@ int launch_prefill_umma(const void* Q, const void* K, const void* V, void* out, 
             p.selinfo = selinfo;
             precise = p.precise = 3;
         }
+    }
+    if (g_two_tile && prefill_v2_serves(precise)) {
+        PrefillV2Args a;
+        if (!make_kv_tensor_map(&a.tmQ, Q, L, H_q, 128)) return JETLONG_UNSUPPORTED;
+        a.tmK = tmK; a.tmV = tmV; a.tmKh = tmKh; a.tmKe = tmKe; a.tmKl = tmKl;
+        a.out = p.out; a.lse = lse; a.L = L; a.w0 = w0; a.G = G; a.H_q = H_q; a.H_kv = H_kv;
+        a.bifocal = p.bifocal; a.precise = precise; a.prerot = p.prerot; a.window_only = 0; a.qk_f16 = 0;
+        a.lo = p.lo; a.hi = p.hi; a.selinfo = p.selinfo;
+        return launch_prefill_v2(a, st);
     }
     static bool attr_set = false;
     if (!attr_set) {
@@ -1074,6 +1087,15 @@ static int launch_plain(const void* Q, const void* K, const void* V, void* out, 
     p.qb_top = (int)((L + BM - 1) / BM);
     p.qb_lo = 0;
     p.lo = nullptr; p.hi = nullptr; p.selinfo = nullptr;
+    if (g_two_tile) {
+        PrefillV2Args a;
+        if (!make_kv_tensor_map(&a.tmQ, Q, L, H_q, 128)) return JETLONG_UNSUPPORTED;
+        a.tmK = tmK; a.tmV = tmV; a.tmKh = tmK; a.tmKe = tmK; a.tmKl = tmK;
+        a.out = p.out; a.lse = lse; a.L = L; a.w0 = w0; a.G = 1; a.H_q = H_q; a.H_kv = H_kv;
+        a.bifocal = p.bifocal; a.precise = 0; a.prerot = 0; a.window_only = p.window_only; a.qk_f16 = p.qk_f16;
+        a.lo = nullptr; a.hi = nullptr; a.selinfo = nullptr;
+        return launch_prefill_v2(a, st);
+    }
     if (cudaFuncSetAttribute(prefill_umma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES) != cudaSuccess)
         return check_launch("prefill_umma attr");
     const int n_qb = (int)((L + BM - 1) / BM);

@@ -1,0 +1,664 @@
+// prefill_umma2.cu -- tcgen05 UMMA bifocal / causal prefill, two query tiles per CTA (bf16, head_dim 128; steps a3-a8, a10).
+//
+// One CTA PAIR (cluster of 2, tcgen05 cta_group::2) owns 256 query rows (two 128-row tiles) x 2 query heads of one KV
+// group: CTA c owns head h0 + c, every UMMA is M = 256 across the pair, and each CTA stages -- and on remote visits
+// rotates (Eq.(6)) -- only its half of every K tile.  Each staged / rotated K tile feeds BOTH query tiles, so a
+// rotated key serves 512 (row, head) pairs with no exchange between CTAs beyond the pair's shared B operand, and the
+// rotation per unit of tensor work is half that of one tile per CTA (prefill_umma.cu).
+//   warps 0-3    rotate group: forwards local K stages; on remote visits rotates its K half in shared memory between the
+//                TMA load and the MMA; once per CTA it replaces Q in shared memory by Q' = R(Delta q) Q (Eq.(6)), in place
+//   warps 4-7    softmax group of tile 0, warps 8-11 of tile 1: ONE thread per query row (no row-max exchange), S loaded once
+//                into registers, online softmax with lazy rescaling, epilogue
+//   warp 12      K (and Q) TMA producer, warp 13 V TMA producer, warp 15 MMA issuer (leader CTA) / V forwarder (peer CTA)
+// TMEM (512 columns): S0 | S1 | O0 | O1.  P_t (bf16) aliases columns 0..63 of S_t.  Tensor-pipe order in steady state:
+// P0 V(m), Q0 K(m+1), P1 V(m), Q1 K(m+1): the softmax of one tile runs under the two MMAs of the other.
+// Q lives in shared memory (UMMA A operand, SWIZZLE_128B), so the register file is split with setmaxnreg:
+// softmax groups 176, rotate group 112, producers / issuer 48.
+//
+// Visit order per pair: the local visits of either tile (from the upper tile's diagonal down to the lower tile's
+// window edge), then the Q -> Q' switch, then the remote visits.  A tile takes part in a visit only when the key tile is
+// in its own list (Plan); the straddle tile is visited twice with complementary masks.  All visits of a tile feed ONE
+// running (m, l, O) per row: the additive form of the Eq.(7) merge.
+#include <cuda.h>
+#include <math.h>
+
+#include "common.cuh"
+#include "umma.cuh"
+#include "rot.cuh"
+#include "prefill_v2.cuh"
+
+namespace jetlong {
+
+namespace {
+
+using namespace ptx;
+using namespace dev;
+
+constexpr int D = 128, BM = 128, BN = 128;
+constexpr int NKMAX = 6, NVMAX = 6;
+constexpr int KH_BYTES = 64 * D * 2;                  // this CTA's 64 keys: two 8 KB SWIZZLE_128B boxes (ch 0-63 | 64-127)
+constexpr int KBOX = 64 * 128;
+constexpr int VH_BYTES = BN * 64 * 2;                 // this CTA's 64 channels of 128 keys
+constexpr int QBOX = BM * 128;                        // one Q box: 128 rows x 64 channels
+constexpr int QT_BYTES = 2 * QBOX;                    // one Q tile
+constexpr int Q_BYTES = 2 * QT_BYTES;                 // both tiles
+constexpr int BARS_BYTES = 2048;
+constexpr int SMEM_BYTES = 232448;                    // the 227 KB opt-in maximum
+constexpr int RING_BYTES = SMEM_BYTES - 1024 /*align slack*/ - Q_BYTES - BARS_BYTES;   // cross-term Q operands + K ring + V ring
+constexpr int NTHREADS = 512;
+constexpr float kLog2e = 1.4426950408889634f;
+constexpr int POLY_OF_4 = 0;                          // of every 4 exponential pairs, this many use the FMA-pipe polynomial
+constexpr int W_SOFTMAX = 4, W_KLOAD = 12, W_VLOAD = 13, W_MMA = 15;   // warps 0-3 rotate, 4-7 / 8-11 softmax of tile 0 / 1
+constexpr uint32_t TM_S = 0, TM_O = 256;
+// setmaxnreg.inc draws only on what other warps of the CTA released (registers left unallocated at launch are not in the
+// pool): the split must balance against 4 warpgroups x 128, or the last group to grow waits forever
+constexpr int REGS_ROT = 128, REGS_SOFTMAX = 160, REGS_MISC = 64;
+static_assert(REGS_ROT + 2 * REGS_SOFTMAX + REGS_MISC == 512, "register file split");
+
+// ---- optional cycle trace of one CTA (build with -DJL_TRACE; read back with jetlong_debug_trace) ----------------
+#ifdef JL_TRACE
+constexpr int TR_M = 192, TR_SLOTS = 8, TR_ROLES = 5;     // roles: 0 MMA, 1 softmax tile 0, 2 softmax tile 1, 3 rotate, 4 K producer
+__device__ long long g_trace[TR_ROLES * TR_M * TR_SLOTS];
+__device__ int g_trace_block = 0;
+#define TR(role, m, slot)                                                                                      \
+    do {                                                                                                       \
+        if (blockIdx.x == g_trace_block && (threadIdx.x & 31) == 0 && (m) >= 0 && (m) < TR_M)                  \
+            g_trace[((role) * TR_M + (m)) * TR_SLOTS + (slot)] = clock64();                                    \
+    } while (0)
+#else
+#define TR(role, m, slot) do {} while (0)
+#endif
+
+struct Bars {
+    uint64_t k_full[NKMAX];    // local: TMA bytes of this CTA's K half landed
+    uint64_t k_ready[NKMAX];   // leader: both rotate groups are done with K stage s (8 warp arrivals)
+    uint64_t k_empty[NKMAX];   // both: every Q K^T reading K stage s has completed (multicast commit)
+    uint64_t v_full[NVMAX];    // local: TMA bytes of this CTA's V half landed
+    uint64_t v_ready[NVMAX];   // leader: the other CTA's V half has landed (its forwarding warp)
+    uint64_t v_empty[NVMAX];   // both: every P V reading V stage s has completed
+    uint64_t s_full[2];        // both: S_t holds Q_t K^T of a visit
+    uint64_t p_half[2];        // leader: the first 64 columns of P_t are written (8 warp arrivals): the first half of P V may start
+    uint64_t p_full[2];        // leader: both softmax groups of tile t wrote P_t and are done reading S_t (8 warp arrivals)
+    uint64_t pv_done[2];       // both: O_t += P_t V of a visit has completed
+    uint64_t o_full;           // both: all MMAs done
+    uint64_t q_full;           // local: TMA bytes of this CTA's Q tiles landed
+    uint64_t q_ready;          // leader: Q landed in both CTAs (8 warp arrivals)
+    uint64_t q_local_done;     // both: the last local Q K^T has completed, Q may be overwritten by Q'
+    uint64_t q_rot_done;       // leader: Q' staged in both CTAs (8 warp arrivals)
+    uint32_t tmem_base;
+};
+static_assert(sizeof(Bars) <= BARS_BYTES, "Bars");
+
+struct Ring {
+    int n, s;
+    uint32_t ph;
+    __device__ Ring(int n_) : n(n_), s(0), ph(0) {}
+    __device__ __forceinline__ void next() { if (++s == n) { s = 0; ph ^= 1u; } }
+};
+
+struct Params {
+    __nv_bfloat16* out;
+    float* lse;
+    long long L, w0, G;
+    int H_q, H_kv, g;
+    int bifocal, precise, prerot, window_only, qk_f16;
+    int n_qb, n_sb;
+    const float2* lo;
+    const float2* hi;
+    const uint32_t* selinfo;
+};
+
+struct Visit { int kt; int mode; };                   // mode 0 = causal/control, 1 = local, 2 = remote
+
+// visit list of ONE 128-row query tile qb (step a3): local key tiles [kt_lo, qb] descending, then remote [0, kt_hi] descending
+struct Plan {
+    int qb, kt_lo, kt_hi, n_local, n_remote, nv;
+    __device__ Plan() : qb(0), kt_lo(1), kt_hi(-1), n_local(0), n_remote(0), nv(0) {}
+    __device__ Plan(int qb_, long long w0, bool bifocal, bool window_only) : qb(qb_) {
+        const long long q0 = (long long)qb * BM;
+        if (!bifocal) { kt_lo = 0; n_local = qb + 1; n_remote = 0; kt_hi = -1; nv = n_local; return; }
+        long long t = q0 - w0 - (BN - 1);                              // local iff k0 >= t
+        kt_lo = t <= 0 ? 0 : (int)((t + BN - 1) / BN);
+        n_local = qb - kt_lo + 1;
+        long long u = q0 + (BM - 1) - 1 - w0;                          // remote iff k0 <= u  (q0+127-k0 > w0)
+        kt_hi = u < 0 ? -1 : (int)(u / BN);
+        if (kt_hi > qb) kt_hi = qb;
+        if (window_only) kt_hi = -1;
+        n_remote = kt_hi + 1;
+        nv = n_local + n_remote;
+    }
+    __device__ Visit at(int v, bool bifocal) const {
+        Visit x;
+        if (v < n_local) { x.kt = qb - v; x.mode = bifocal ? 1 : 0; }
+        else { x.kt = kt_hi - (v - n_local); x.mode = 2; }
+        return x;
+    }
+};
+
+// the pair's merged visit list: K tiles needed by either query tile (plain scalars: the issuer warp runs on 72 registers)
+struct MPlan {
+    int qb0, lo0, hi0, lo1, hi1;                      // tile i = query block qb0 + i: local key tiles [lo_i, qb0 + i], remote [0, hi_i]
+    int lo_m, top_m, hi_m, n_loc, n_rem, nm;
+    bool bifocal, valid1;
+    __device__ MPlan(int qb0_, bool valid1_, long long w0, bool bifocal_, bool window_only)
+        : qb0(qb0_), bifocal(bifocal_), valid1(valid1_) {
+        const Plan a(qb0, w0, bifocal, window_only);
+        lo0 = a.kt_lo; hi0 = a.kt_hi; lo1 = 1 << 30; hi1 = -1;
+        if (valid1) { const Plan b(qb0 + 1, w0, bifocal, window_only); lo1 = b.kt_lo; hi1 = b.kt_hi; }
+        lo_m = lo0;                                                    // lo1 >= lo0
+        top_m = valid1 ? qb0 + 1 : qb0;
+        hi_m = hi1 > hi0 ? hi1 : hi0;
+        n_loc = top_m - lo_m + 1;
+        n_rem = hi_m + 1;
+        nm = n_loc + n_rem;
+    }
+    __device__ __forceinline__ Visit at(int m) const {
+        Visit x;
+        if (m < n_loc) { x.kt = top_m - m; x.mode = bifocal ? 1 : 0; }
+        else { x.kt = hi_m - (m - n_loc); x.mode = 2; }
+        return x;
+    }
+    __device__ __forceinline__ bool part(int i, const Visit& x) const {
+        const int lo = i ? lo1 : lo0, hi = i ? hi1 : hi0;
+        return x.mode == 2 ? x.kt <= hi : (x.kt >= lo && x.kt <= qb0 + i);
+    }
+    __device__ __forceinline__ Plan tile(int i) const {
+        Plan t;
+        if (i && !valid1) return t;
+        t.qb = qb0 + i; t.kt_lo = i ? lo1 : lo0; t.kt_hi = i ? hi1 : hi0;
+        t.n_local = t.qb - t.kt_lo + 1; t.n_remote = t.kt_hi + 1; t.nv = t.n_local + t.n_remote;
+        return t;
+    }
+};
+
+// Softmax exponentials of one row, 32 columns per block, software-pipelined by hand: ptxas puts the FADD2 / F2FP that
+// consume an exponential directly behind its MUFU.EX2, and the in-order warp then stalls one MUFU latency per pair
+// (measured: 1.7-1.9 k cycles for 128 columns).  Here a block's scores first become exp2 arguments (exp_args), then its
+// exponentials are issued while the sums and bf16 packs of the PREVIOUS block are interleaved (exp_issue_consume).
+__device__ __forceinline__ void exp_args(uint32_t (&sx)[32], uint64_t sl2x2, uint64_t mneg2) {
+#pragma unroll
+    for (int j = 0; j < 32; j += 2) {
+        const uint64_t xx = ffma2(pack2(__uint_as_float(sx[j]), __uint_as_float(sx[j + 1])), sl2x2, mneg2);
+        float x0, x1;
+        unpack2(xx, x0, x1);
+        sx[j] = __float_as_uint(x0); sx[j + 1] = __float_as_uint(x1);
+    }
+}
+__device__ __forceinline__ float ex2v(float x) {                      // volatile: keeps the issue order written here
+    float y;
+    asm volatile("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+// volatile as well: ptxas otherwise hoists these consumers back up to their MUFU.EX2
+__device__ __forceinline__ uint64_t fadd2v(uint64_t a, uint64_t b) {
+    uint64_t y;
+    asm volatile("add.rn.f32x2 %0, %1, %2;" : "=l"(y) : "l"(a), "l"(b));
+    return y;
+}
+__device__ __forceinline__ uint32_t bf16x2v(float lo, float hi) {
+    uint32_t y;
+    asm volatile("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(y) : "f"(hi), "f"(lo));
+    return y;
+}
+__device__ __forceinline__ void consume_pair(const uint32_t (&pp)[32], int j, uint64_t& l2a, uint64_t& l2b, uint32_t (&pk)[16]) {
+    const float p0 = __uint_as_float(pp[j]), p1 = __uint_as_float(pp[j + 1]);
+    if (j & 2) l2b = fadd2v(l2b, pack2(p0, p1)); else l2a = fadd2v(l2a, pack2(p0, p1));
+    pk[j >> 1] = bf16x2v(p0, p1);
+}
+// exponentials of block `cur` (in place); the row sums and P words of block `prev` (already exponentiated) in between
+template <bool HAS_PREV>
+__device__ __forceinline__ void exp_issue_consume(uint32_t (&cur)[32], const uint32_t (&prev)[32], uint64_t& l2a, uint64_t& l2b,
+                                                  uint32_t (&pk)[16]) {
+#pragma unroll
+    for (int j = 0; j < 32; j += 2) {
+        cur[j] = __float_as_uint(ex2v(__uint_as_float(cur[j])));
+        cur[j + 1] = __float_as_uint(ex2v(__uint_as_float(cur[j + 1])));
+        if (HAS_PREV) consume_pair(prev, j, l2a, l2b, pk);
+    }
+}
+__device__ __forceinline__ void consume_block(const uint32_t (&pp)[32], uint64_t& l2a, uint64_t& l2b, uint32_t (&pk)[16]) {
+#pragma unroll
+    for (int j = 0; j < 32; j += 2) consume_pair(pp, j, l2a, l2b, pk);
+}
+
+__device__ __forceinline__ float max32(const uint32_t (&s)[32], float m) {
+    float a = m, b = -INFINITY, c = -INFINITY, d = -INFINITY;
+#pragma unroll
+    for (int j = 0; j < 32; j += 8) {
+        a = max3(a, __uint_as_float(s[j]), __uint_as_float(s[j + 1]));
+        b = max3(b, __uint_as_float(s[j + 2]), __uint_as_float(s[j + 3]));
+        c = max3(c, __uint_as_float(s[j + 4]), __uint_as_float(s[j + 5]));
+        d = max3(d, __uint_as_float(s[j + 6]), __uint_as_float(s[j + 7]));
+    }
+    return fmaxf(fmaxf(a, b), fmaxf(c, d));
+}
+
+__device__ __forceinline__ void mask32(uint32_t (&s)[32], int lo, int hi) {   // keep columns lo..hi of this 32-column block
+#pragma unroll
+    for (int j = 0; j < 32; ++j)
+        if (j < lo || j > hi) s[j] = 0xff800000u;                      // -inf: exp2 -> 0, never wins the max
+}
+
+constexpr uint32_t IDESC_QK_BF16 = idesc_f16(1, 1, 0, 0, 2 * BM, BN);
+constexpr uint32_t IDESC_QK_F16 = idesc_f16(0, 0, 0, 0, 2 * BM, BN);
+constexpr uint32_t IDESC_QK_E5M2 = idesc_f16(1, 1, 0, 0, 2 * BM, BN);   // kind::f8f6f4: format code 1 = e5m2
+constexpr uint32_t IDESC_PV = idesc_f16(1, 1, 0, 1, 2 * BM, D);         // A = P (TMEM, bf16), B = V (smem, MN-major)
+
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1)
+prefill_umma2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
+                     const __grid_constant__ CUtensorMap tmV, const __grid_constant__ CUtensorMap tmKh,
+                     const __grid_constant__ CUtensorMap tmKe, const __grid_constant__ CUtensorMap tmKl, const Params p) {
+    extern __shared__ unsigned char smem_raw[];
+    unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int cta = (int)cluster_ctarank();
+    const int pairs = p.H_q / 2;
+    const int unit = (int)(blockIdx.x >> 1);
+    const int sb = p.n_sb - 1 - unit / pairs;                      // heaviest 256-row blocks first
+    const int h0 = 2 * (unit % pairs);
+    const int head = h0 + cta;
+    const int kvh = h0 / p.g;
+    const int qb0 = 2 * sb;
+    const bool valid1 = qb0 + 1 < p.n_qb;
+    const bool bifocal = p.bifocal != 0;
+    const MPlan mp(qb0, valid1, p.w0, bifocal, p.window_only != 0);
+    // 0 fast, 2 e5m2 cross terms, 3 e5m2 cross terms over the two highest-energy pairs of every 8-pair chunk; a KV head
+    // whose other channels are too loud falls back from 3 to 2
+    int precise = (bifocal && mp.n_rem > 0) ? p.precise : 0;
+    if (precise == 3 && __ldg(p.selinfo + kvh * 16 + 8) != 0u) precise = 2;
+    // shared memory: Q tiles | cross-term Q' operands | K ring | V ring | barriers
+    const int QX_BYTES = precise == 3 ? QBOX : precise == 2 ? 4 * QBOX : 0;
+    const int KST = KH_BYTES + (precise == 3 ? KBOX : precise == 2 ? 2 * KBOX : 0);
+    const int NK = precise == 3 ? 4 : precise == 2 ? 2 : 5;
+    const int NV = precise == 3 ? 3 : precise == 2 ? 2 : 5;
+    unsigned char* sQ = smem;
+    unsigned char* sQX = smem + Q_BYTES;
+    unsigned char* kring = sQX + QX_BYTES;
+    unsigned char* vring = kring + NK * KST;
+    Bars* bars = reinterpret_cast<Bars*>(smem + Q_BYTES + RING_BYTES);
+    auto sK = [&](int st) { return kring + st * KST; };
+    auto sKl = [&](int st) { return kring + st * KST + KH_BYTES; };
+    auto sV = [&](int st) { return vring + st * VH_BYTES; };
+
+    if (tid == 0) {
+        for (int i = 0; i < NKMAX; ++i) { mbar_init(&bars->k_full[i], 1); mbar_init(&bars->k_ready[i], 8); mbar_init(&bars->k_empty[i], 1); }
+        for (int i = 0; i < NVMAX; ++i) { mbar_init(&bars->v_full[i], 1); mbar_init(&bars->v_ready[i], 1); mbar_init(&bars->v_empty[i], 1); }
+        for (int i = 0; i < 2; ++i) { mbar_init(&bars->s_full[i], 1); mbar_init(&bars->p_full[i], 8); mbar_init(&bars->p_half[i], 8); mbar_init(&bars->pv_done[i], 1); }
+        mbar_init(&bars->o_full, 1); mbar_init(&bars->q_full, 1); mbar_init(&bars->q_ready, 8);
+        mbar_init(&bars->q_local_done, 1); mbar_init(&bars->q_rot_done, 8);
+        fence_barrier_init();
+        prefetch_tmap(&tmQ); prefetch_tmap(&tmK); prefetch_tmap(&tmV);
+        if (p.prerot) { prefetch_tmap(&tmKh); prefetch_tmap(&tmKe); prefetch_tmap(&tmKl); }
+    }
+    if (warp == W_MMA) tmem_alloc2<512>(&bars->tmem_base);
+    tc_fence_before();
+    cluster_sync_all();                                            // barriers of both CTAs initialised, TMEM allocated
+    tc_fence_after();
+    const uint32_t tmem = bars->tmem_base;
+
+    if (warp >= 12) {
+        reg_dec<REGS_MISC>();
+        if (warp == W_KLOAD) {
+            // ===================== Q and K producer (each CTA loads its head's Q tiles and its 64 keys of every K tile) =====
+            if (lane == 0) {
+                mbar_arrive_expect_tx(&bars->q_full, valid1 ? Q_BYTES : QT_BYTES);
+                for (int i = 0; i < (valid1 ? 2 : 1); ++i) {
+                    tma_load_3d(sQ + i * QT_BYTES, &tmQ, &bars->q_full, 0, head, (qb0 + i) * BM);
+                    tma_load_3d(sQ + i * QT_BYTES + QBOX, &tmQ, &bars->q_full, 64, head, (qb0 + i) * BM);
+                }
+                Ring rk(NK);
+                for (int m = 0; m < mp.nm; ++m, rk.next()) {
+                    const Visit x = mp.at(m);
+                    const int st = rk.s;
+                    TR(4, m, 0);
+                    if (m >= NK) mbar_wait_sleep(&bars->k_empty[st], rk.ph ^ 1u);
+                    TR(4, m, 1);
+                    if (p.prerot && x.mode == 2) {
+                        // workspace variant: K' hi (fp16) and the e5m2 cross-term operands come from the scratch
+                        mbar_arrive_expect_tx(&bars->k_full[st], KH_BYTES + (precise == 2 ? 2 * KBOX : precise == 3 ? KBOX : 0));
+                        tma_load_3d(sK(st), &tmKh, &bars->k_full[st], 0, kvh, x.kt * BN + 64 * cta);
+                        tma_load_3d(sK(st) + KBOX, &tmKh, &bars->k_full[st], 64, kvh, x.kt * BN + 64 * cta);
+                        if (precise >= 2) tma_load_3d(sKl(st), &tmKe, &bars->k_full[st], 0, kvh, x.kt * BN + 64 * cta);
+                        if (precise == 2) tma_load_3d(sKl(st) + KBOX, &tmKl, &bars->k_full[st], 0, kvh, x.kt * BN + 64 * cta);
+                    } else {
+                        mbar_arrive_expect_tx(&bars->k_full[st], KH_BYTES);
+                        tma_load_3d(sK(st), &tmK, &bars->k_full[st], 0, kvh, x.kt * BN + 64 * cta);
+                        tma_load_3d(sK(st) + KBOX, &tmK, &bars->k_full[st], 64, kvh, x.kt * BN + 64 * cta);
+                    }
+                }
+            }
+        } else if (warp == W_VLOAD) {
+            // ===================== V producer (each CTA loads its 64 channels of the tile) =====================
+            if (lane == 0) {
+                Ring rv(NV);
+                for (int m = 0; m < mp.nm; ++m, rv.next()) {
+                    const Visit x = mp.at(m);
+                    if (m >= NV) mbar_wait_sleep(&bars->v_empty[rv.s], rv.ph ^ 1u);
+                    mbar_arrive_expect_tx(&bars->v_full[rv.s], VH_BYTES);
+                    tma_load_3d(sV(rv.s), &tmV, &bars->v_full[rv.s], 64 * cta, kvh, x.kt * BN);
+                }
+            }
+        } else if (warp == W_MMA && cta == 1) {
+            // ===================== non-leader CTA: tell the leader when our V half has landed =====================
+            if (lane == 0) {
+                Ring rv(NV);
+                for (int m = 0; m < mp.nm; ++m, rv.next()) {
+                    mbar_wait_sleep(&bars->v_full[rv.s], rv.ph);
+                    mbar_arrive_leader(&bars->v_ready[rv.s]);
+                }
+            }
+        } else if (warp == W_MMA) {
+            // ===================== MMA issuer (leader CTA; the warp runs convergently, one elected lane issues) ===========
+            const uint32_t tm = __shfl_sync(0xffffffffu, tmem, 0);
+            const uint32_t q0a = __shfl_sync(0xffffffffu, smem_u32(sQ), 0);
+            const uint32_t qxa = __shfl_sync(0xffffffffu, smem_u32(sQX), 0);
+            const uint32_t kring0 = __shfl_sync(0xffffffffu, smem_u32(kring), 0);
+            const uint32_t vring0 = __shfl_sync(0xffffffffu, smem_u32(vring), 0);
+            Ring rk(NK), rv(NV);
+            const uint32_t el = elect_one() ? 1u : 0u;               // the issuing lane; every lane runs the uniform arithmetic
+            const uint32_t HI_K = desc_hi_sw128(1024), HI_V = desc_hi_sw128(1024);
+            const uint32_t q_lo0 = desc_lo(q0a, 16), qx_lo0 = desc_lo(qxa, 16);
+            const uint32_t k_lo0 = desc_lo(kring0, 16), v_lo0 = desc_lo(vring0, VH_BYTES);
+            // S_i = Q_i K^T of one visit (K stage kst), then the arrival for the tile's softmax group
+            auto qk = [&](int i, int mode, int kst) {
+                const uint32_t dS = tm + TM_S + i * 128;
+                const uint32_t qa = q_lo0 + (uint32_t)(i * (QT_BYTES >> 4));
+                const uint32_t kb = k_lo0 + (uint32_t)((kst * KST) >> 4), klb = kb + (KH_BYTES >> 4);
+                const uint32_t idesc = (mode == 2 || p.qk_f16) ? IDESC_QK_F16 : IDESC_QK_BF16;
+#pragma unroll
+                for (int ks = 0; ks < D / 16; ++ks)
+                    umma2_ss_e(dS, qa + (((ks >> 2) * QBOX + (ks & 3) * 32) >> 4), HI_K,
+                               kb + (((ks >> 2) * KBOX + (ks & 3) * 32) >> 4), HI_K, idesc, ks > 0 ? 1u : 0u, el);
+                if (mode == 2 && precise == 3) {
+                    // compact operands: Q' row = [hi1 | hi2 | lo1 | lo2] (tile i at byte 64 i), K' row = [lo1 | lo2 | hi1 | hi2]
+                    umma2_ss_f8_e(dS, qx_lo0 + 4 * i, HI_K, klb, HI_K, IDESC_QK_E5M2, 1u, el);
+                    umma2_ss_f8_e(dS, qx_lo0 + 4 * i + 2, HI_K, klb + 2, HI_K, IDESC_QK_E5M2, 1u, el);
+                } else if (mode == 2 && precise == 2) {
+                    const uint32_t qe = qx_lo0 + (uint32_t)(i * ((2 * QBOX) >> 4));   // [Q' e5m2 | Q' lo e5m2] of tile i
+#pragma unroll
+                    for (int ks = 0; ks < D / 32; ++ks)              // Q' (e5m2) . K' lo (e5m2)
+                        umma2_ss_f8_e(dS, qe + 2 * ks, HI_K, klb + (KBOX >> 4) + 2 * ks, HI_K, IDESC_QK_E5M2, 1u, el);
+#pragma unroll
+                    for (int ks = 0; ks < D / 32; ++ks)              // Q' lo (e5m2) . K' (e5m2)
+                        umma2_ss_f8_e(dS, qe + (QBOX >> 4) + 2 * ks, HI_K, klb + 2 * ks, HI_K, IDESC_QK_E5M2, 1u, el);
+                }
+                umma2_commit_e(&bars->s_full[i], el);
+            };
+            // the K stage of visit m is free once its Q K^T (of both tiles) have completed
+            auto qk_finish = [&](int m) {
+                umma2_commit_e(&bars->k_empty[rk.s], el);
+                if (mp.n_rem > 0 && m == mp.n_loc - 1) umma2_commit_e(&bars->q_local_done, el);
+                rk.next();
+            };
+            // O_i += P_i V over keys [64 half, 64 half + 64) of the tile
+            auto pv = [&](int i, int vst, bool first, int half) {
+                const uint32_t vb = v_lo0 + (uint32_t)((vst * VH_BYTES) >> 4);
+#pragma unroll
+                for (int k4 = 0; k4 < 4; ++k4) {
+                    const int ks = 4 * half + k4;
+                    umma2_ts_e(tm + TM_O + i * 128, tm + TM_S + i * 128 + ks * 8, vb + ((ks * 2048) >> 4), HI_V, IDESC_PV,
+                               (!first || ks > 0) ? 1u : 0u, el);
+                }
+                if (half) umma2_commit_e(&bars->pv_done[i], el);
+            };
+            mbar_wait_sleep(&bars->q_ready, 0);
+            uint32_t jp = 0, started = 0;                            // per tile (bit i): parity of the next P V, any P V issued
+            // step m issues P_i V of visit m and Q_i K^T of visit m + 1, tile by tile (m = -1: only the first Q K^T).  When
+            // visit m + 1 is the first remote one, the P V go first and the Q K^T wait for Q' (second pass).
+            for (int m = -1; m < mp.nm; ++m) {
+                const bool has_pv = m >= 0, has_next = m + 1 < mp.nm;
+                const Visit x = mp.at(has_pv ? m : 0);
+                const Visit y = mp.at(has_next ? m + 1 : 0);
+                const bool sw = has_next && y.mode == 2 && m + 1 == mp.n_loc;
+                if (has_pv) {
+                    TR(0, m, 6);
+                    mbar_wait_sleep(&bars->v_full[rv.s], rv.ph);           // our V half ...
+                    mbar_wait_sleep(&bars->v_ready[rv.s], rv.ph);          // ... and the other CTA's
+                    TR(0, m, 7);
+                }
+                bool kw = false;
+#pragma unroll 1
+                for (int pass = 0; pass < (sw ? 2 : 1); ++pass) {
+                    if (pass == 1) mbar_wait_sleep(&bars->q_rot_done, 0);
+#pragma unroll 1
+                    for (int i = 0; i < 2; ++i) {
+                        if (pass == 0 && has_pv && mp.part(i, x)) {
+                            TR(0, m, 2 * i);
+                            mbar_wait_sleep(&bars->p_half[i], (jp >> i) & 1u);
+                            tc_fence_after();
+                            pv(i, rv.s, !((started >> i) & 1u), 0);
+                            mbar_wait_sleep(&bars->p_full[i], (jp >> i) & 1u);
+                            TR(0, m, 2 * i + 1);
+                            tc_fence_after();
+                            pv(i, rv.s, !((started >> i) & 1u), 1);
+                            jp ^= 1u << i;
+                            started |= 1u << i;
+                        }
+                        if (pass == (sw ? 1 : 0) && has_next && mp.part(i, y)) {
+                            if (!kw) { TR(0, m, 4); mbar_wait_sleep(&bars->k_ready[rk.s], rk.ph); TR(0, m, 5); tc_fence_after(); kw = true; }
+                            qk(i, y.mode, rk.s);
+                        }
+                    }
+                }
+                if (has_pv) {
+                    umma2_commit_e(&bars->v_empty[rv.s], el);
+                    rv.next();
+                }
+                if (has_next) qk_finish(m + 1);
+            }
+            umma2_commit_e(&bars->o_full, el);
+        }
+    } else if (warp < 4) {
+        // ===================== rotate group (steps a4, a5) =====================
+        mbar_wait_sleep(&bars->q_full, 0);
+        if (lane == 0) mbar_arrive_leader(&bars->q_ready);
+        KRot<4> rot;
+        const bool rotating = mp.n_rem > 0 && !p.prerot;
+        if (mp.n_rem > 0) {
+            rot.init(p.lo, p.hi, tid, p.G, 0);
+            rot.selw = p.selinfo ? __ldg(p.selinfo + kvh * 16 + (tid & 7)) : 0u;
+            if (rotating) rot.prefetch((unsigned)(mp.hi_m * BN + 64 * cta));     // first remote visit
+        }
+        const int kmode = precise == 3 ? 4 : precise;
+        Ring rk(NK);
+        for (int m = 0; m < mp.nm; ++m, rk.next()) {
+            const Visit x = mp.at(m);
+            const int st = rk.s;
+            TR(3, m, 0);
+            mbar_wait_sleep(&bars->k_full[st], rk.ph);
+            TR(3, m, 1);
+            if (x.mode == 2) {
+                if (rotating) {
+                    rotate_k_rows<4, KBOX>(smem_u32(sK(st)), smem_u32(sKl(st)), (unsigned)(x.kt * BN + 64 * cta), rot, kmode);
+                    fence_proxy_async_smem();
+                    if (x.kt > 0) rot.prefetch((unsigned)((x.kt - 1) * BN + 64 * cta));   // next remote visit's first row
+                }
+                if (m == mp.n_loc) {
+                    // first remote visit: Q -> Q' = R(Delta q) Q, in place in shared memory (both tiles, 64 rows per pass)
+                    if (mp.n_loc > 0) mbar_wait_sleep(&bars->q_local_done, 0);
+                    for (int i = 0; i < (valid1 ? 2 : 1); ++i) {
+#pragma unroll 1
+                        for (int half = 0; half < 2; ++half) {
+                            KRot<4> qr;
+                            qr.init(p.lo, p.hi, tid, p.G, 64 * half);
+                            qr.selw = rot.selw;
+                            qr.prefetch((unsigned)((qb0 + i) * BM));
+                            const uint32_t qx = precise == 2 ? smem_u32(sQX) + (uint32_t)(i * 2 * QBOX) : smem_u32(sQX);
+                            const uint32_t c4 = (uint32_t)(((4 * i + 1) << 12) | ((4 * i) << 8) | ((4 * i + 3) << 4) | (4 * i + 2));
+                            rotate_k_rows<4, QBOX>(smem_u32(sQ + i * QT_BYTES), qx, (unsigned)((qb0 + i) * BM), qr, kmode, 0, 0, c4);
+                        }
+                    }
+                    fence_proxy_async_smem();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive_leader(&bars->q_rot_done);
+                }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive_leader(&bars->k_ready[st]);
+            TR(3, m, 2);
+        }
+    } else {
+        // ===================== softmax groups (steps a6-a8): one thread per query row =====================
+        reg_inc<REGS_SOFTMAX>();
+        const int i = (warp - W_SOFTMAX) >> 2;                         // query tile of this group
+        const int quad = warp & 3;
+        const int r = (quad << 5) | lane;
+        const Plan plan = mp.tile(i);
+        const int qb = qb0 + i;
+        const long long q0 = (long long)qb * BM;
+        const uint32_t lane_base = (uint32_t)(quad << 5) << 16;
+        const uint32_t tS = tmem + lane_base + TM_S + i * 128;
+        const uint32_t tO = tmem + lane_base + TM_O + i * 128;
+        const float sl2 = (1.0f / sqrtf((float)D)) * kLog2e;
+        const uint64_t sl2x2 = pack2(sl2, sl2);
+        float m_ref = -INFINITY;
+        uint64_t l2a = 0, l2b = 0;                                     // packed fp32x2 partial row sums
+        for (int v = 0; v < plan.nv; ++v) {
+            const Visit x = plan.at(v, bifocal);
+            const long long k0 = (long long)x.kt * BN;
+            const long long qrel = q0 + r - k0;
+            int lo = 0, hi = BN - 1;
+            bool masked = false;
+            if (x.mode != 2 && k0 + BN - 1 > q0) {                                               // causal diagonal
+                hi = qrel < hi ? (int)qrel : hi;
+                masked = true;
+            }
+            if (x.mode == 1 && (q0 + BM - 1 - k0 > p.w0)) {                                      // q-k <= w0 (R1)
+                const long long a = qrel - p.w0;
+                lo = a > 0 ? (int)a : 0;
+                masked = true;
+            }
+            if (x.mode == 2 && (q0 - (k0 + BN - 1) <= p.w0)) {                                   // q-k > w0
+                const long long a = qrel - p.w0 - 1;
+                hi = a < hi ? (int)a : hi;
+                masked = true;
+            }
+            TR(1 + i, v, 0);
+            mbar_wait_sleep(&bars->s_full[i], (uint32_t)v & 1u);
+            TR(1 + i, v, 1);
+            tc_fence_after();
+            uint32_t s0[32], s1[32], s2[32], s3[32];
+            tmem_ld32(tS, s0);
+            tmem_ld32(tS + 32, s1);
+            tmem_ld_wait();
+            tmem_ld32(tS + 64, s2);                                    // in flight under the maxima of the first half
+            tmem_ld32(tS + 96, s3);
+            if (masked) { mask32(s0, lo, hi); mask32(s1, lo - 32, hi - 32); }
+            const float mxa = fmaxf(max32(s0, -INFINITY), max32(s1, -INFINITY));
+            tmem_ld_wait();
+            if (masked) { mask32(s2, lo - 64, hi - 64); mask32(s3, lo - 96, hi - 96); }
+            const float mx = fmaxf(mxa, fmaxf(max32(s2, -INFINITY), max32(s3, -INFINITY)));
+            const float mnew = mx * sl2;
+            TR(1 + i, v, 2);
+            if (v == 0) {
+                m_ref = mnew;
+            } else {
+                const bool need = mnew > m_ref + 8.0f;                 // lazy rescale: only on a jump of 2^8
+                if (__any_sync(0xffffffffu, need)) {
+                    mbar_wait_sleep(&bars->pv_done[i], (uint32_t)(v - 1) & 1u);   // O += P V of visit v-1 must have landed
+                    tc_fence_after();
+                    const float alpha = need ? ex2(m_ref - mnew) : 1.0f;
+                    if (need) m_ref = mnew;
+                    const uint64_t al2 = pack2(alpha, alpha);
+                    l2a = fmul2(l2a, al2); l2b = fmul2(l2b, al2);
+                    uint32_t rg[16];
+#pragma unroll 1
+                    for (int ch = 0; ch < 8; ++ch) {
+                        tmem_ld16(tO + ch * 16, rg);
+                        tmem_ld_wait();
+#pragma unroll
+                        for (int j = 0; j < 16; ++j) rg[j] = __float_as_uint(__uint_as_float(rg[j]) * alpha);
+                        tmem_st16(tO + ch * 16, rg);
+                    }
+                }
+            }
+            // a row whose every key so far is masked has m_ref = -inf: keep exp2 arguments finite (-> p = 0)
+            const float mneg = (m_ref == -INFINITY) ? 0.f : -m_ref;
+            const uint64_t mneg2 = pack2(mneg, mneg);
+            uint32_t pk[16];
+            // P (bf16, columns 0..63 of S_i) overwrites S values that are already in registers
+            exp_args(s0, sl2x2, mneg2);
+            exp_args(s1, sl2x2, mneg2);
+            exp_issue_consume<false>(s0, s0, l2a, l2b, pk);
+            exp_args(s2, sl2x2, mneg2);
+            exp_issue_consume<true>(s1, s0, l2a, l2b, pk); tmem_st16(tS, pk);
+            exp_args(s3, sl2x2, mneg2);
+            exp_issue_consume<true>(s2, s1, l2a, l2b, pk); tmem_st16(tS + 16, pk);
+            tmem_st_wait();                                            // the first 64 columns of P are in TMEM
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive_leader(&bars->p_half[i]);
+            exp_issue_consume<true>(s3, s2, l2a, l2b, pk); tmem_st16(tS + 32, pk);
+            consume_block(s3, l2a, l2b, pk); tmem_st16(tS + 48, pk);
+            TR(1 + i, v, 3);
+            tmem_st_wait();
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive_leader(&bars->p_full[i]);
+            TR(1 + i, v, 4);
+        }
+        // ---- epilogue (step a8) ----
+        if (plan.nv > 0) {
+            float la, lb, lc, ld;
+            unpack2(l2a, la, lb); unpack2(l2b, lc, ld);
+            const float l = (la + lb) + (lc + ld);
+            mbar_wait_sleep(&bars->o_full, 0);
+            tc_fence_after();
+            const long long q = q0 + r;
+            const float inv = 1.0f / l;
+            const bool qok = q < p.L;
+            __nv_bfloat16* orow = p.out + ((size_t)(qok ? q : 0) * p.H_q + head) * D;
+#pragma unroll 1
+            for (int ch = 0; ch < 4; ++ch) {
+                uint32_t rg[32];
+                tmem_ld32(tO + ch * 32, rg);
+                tmem_ld_wait();
+                if (qok) {
+#pragma unroll
+                    for (int j = 0; j < 32; j += 8) {
+                        uint32_t w[4];
+#pragma unroll
+                        for (int e = 0; e < 4; ++e)
+                            w[e] = bf16x2(__uint_as_float(rg[j + 2 * e]) * inv, __uint_as_float(rg[j + 2 * e + 1]) * inv);
+                        *reinterpret_cast<uint4*>(orow + ch * 32 + j) = make_uint4(w[0], w[1], w[2], w[3]);
+                    }
+                }
+            }
+            if (qok) p.lse[(size_t)head * p.L + q] = (m_ref + log2f(l)) * 0.6931471805599453f;
+        }
+    }
+    tc_fence_before();
+    cluster_sync_all();                                            // the peer may still be reading our smem / TMEM
+    if (warp == W_MMA) tmem_dealloc2<512>(tmem);
+}
+
+}  // namespace
+
+#ifdef JL_TRACE
+extern "C" int jetlong_debug_trace(long long* dst, int n, int block) {
+    const int total = TR_ROLES * TR_M * TR_SLOTS;
+    if (dst && cudaMemcpyFromSymbol(dst, g_trace, sizeof(long long) * (n < total ? n : total)) != cudaSuccess) return -1;
+    if (cudaMemcpyToSymbol(g_trace_block, &block, sizeof(int)) != cudaSuccess) return -1;
+    return total;
+}
+#endif
+
+int launch_prefill_v2(const PrefillV2Args& a, cudaStream_t st) {
+    Params p;
+    p.out = a.out; p.lse = a.lse;
+    p.L = a.L; p.w0 = a.w0; p.G = a.G;
+    p.H_q = a.H_q; p.H_kv = a.H_kv; p.g = a.H_q / a.H_kv;
+    p.bifocal = a.bifocal; p.precise = a.precise; p.prerot = a.prerot; p.window_only = a.window_only; p.qk_f16 = a.qk_f16;
+    p.n_qb = (int)((a.L + BM - 1) / BM);
+    p.n_sb = (p.n_qb + 1) / 2;
+    p.lo = a.lo; p.hi = a.hi; p.selinfo = a.selinfo;
+    if (cudaFuncSetAttribute(prefill_umma2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES) != cudaSuccess)
+        return check_launch("prefill_umma2 attr");
+    const unsigned grid = 2u * (unsigned)p.n_sb * (unsigned)(a.H_q / 2);
+    prefill_umma2_kernel<<<grid, NTHREADS, SMEM_BYTES, st>>>(a.tmQ, a.tmK, a.tmV, a.tmKh, a.tmKe, a.tmKl, p);
+    note_launch();
+    return check_launch("prefill_umma2_kernel");
+}
+
+}  // namespace jetlong

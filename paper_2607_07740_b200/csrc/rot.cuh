@@ -205,7 +205,8 @@ __device__ __forceinline__ void sts128(uint32_t a, uint32_t x, uint32_t y, uint3
 // cluster (the CTA pair working on the adjacent query block, which needs the same rotated rows).
 template <int ROWS, int KBOX, bool REMOTE = false>
 __device__ __forceinline__ void rotate_k_rows(uint32_t kh, uint32_t kl, unsigned pos0, KRot<ROWS>& R,
-                                              int precise, uint32_t rkh = 0, uint32_t rkl = 0) {   // kh, kl: shared-space addresses
+                                              int precise, uint32_t rkh = 0, uint32_t rkl = 0,      // kh, kl: shared-space addresses
+                                              uint32_t c4 = 0x3210u) {   // mode 4: 16-byte chunk of lo1 | lo2 << 4 | hi1 << 8 | hi2 << 12
     // precise: 4 = selective e5m2 compensation: one 128-byte row per key at kl = [lo1 | lo2 | hi1 | hi2] (16 B each: the two
     //          pairs R.selw picks from each 8-pair chunk, as e5m2) | unused, SWIZZLE_128B;
     //          0 = hi only; 1 = fp16 lo at kl (same layout as kh); 2 = e5m2 copies for the cross terms at kl:
@@ -278,10 +279,10 @@ __device__ __forceinline__ void rotate_k_rows(uint32_t kh, uint32_t kl, unsigned
             }
         } else if (precise == 4) {
             const uint32_t rb = kl + r * 128 + 2 * R.c, x = (uint32_t)(r & 7);
-            sts16s(rb + ((0u ^ x) << 4), __byte_perm(e5m2x4(l1[0], l1[1]), e5m2x4(l1[2], l1[3]), R.selw));
-            sts16s(rb + ((1u ^ x) << 4), __byte_perm(e5m2x4(l2[0], l2[1]), e5m2x4(l2[2], l2[3]), R.selw));
-            sts16s(rb + ((2u ^ x) << 4), __byte_perm(e5m2x4(h1[0], h1[1]), e5m2x4(h1[2], h1[3]), R.selw));
-            sts16s(rb + ((3u ^ x) << 4), __byte_perm(e5m2x4(h2[0], h2[1]), e5m2x4(h2[2], h2[3]), R.selw));
+            sts16s(rb + (((c4 & 15u) ^ x) << 4), __byte_perm(e5m2x4(l1[0], l1[1]), e5m2x4(l1[2], l1[3]), R.selw));
+            sts16s(rb + ((((c4 >> 4) & 15u) ^ x) << 4), __byte_perm(e5m2x4(l2[0], l2[1]), e5m2x4(l2[2], l2[3]), R.selw));
+            sts16s(rb + ((((c4 >> 8) & 15u) ^ x) << 4), __byte_perm(e5m2x4(h1[0], h1[1]), e5m2x4(h1[2], h1[3]), R.selw));
+            sts16s(rb + ((((c4 >> 12) & 15u) ^ x) << 4), __byte_perm(e5m2x4(h2[0], h2[1]), e5m2x4(h2[2], h2[3]), R.selw));
         } else if (precise == 3) {
             const uint32_t o1 = r * 128 + ((((R.c >> 1)) ^ (r & 7)) << 4) + (R.c & 1) * 8;
             const uint32_t o2 = r * 128 + (((4 + (R.c >> 1)) ^ (r & 7)) << 4) + (R.c & 1) * 8;

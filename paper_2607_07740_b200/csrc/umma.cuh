@@ -47,6 +47,20 @@ __device__ __forceinline__ bool mbar_test(uint64_t* bar, uint32_t parity) {
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
     while (!mbar_try_wait(bar, parity)) {}
 }
+// wait with a suspend-time hint: the thread sleeps in hardware until the phase completes (or the hint expires) instead
+// of re-issuing the poll every few cycles -- measured with ncu: half of all issued instructions of the two-tile prefill
+// were polls (SYNCS / BRA / address arithmetic) of warps waiting on s_full / k_full
+__device__ __forceinline__ void mbar_wait_sleep(uint64_t* bar, uint32_t parity) {
+    const uint32_t a = smem_u32(bar);
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "WAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n\t"
+        "@p bra DONE_%=;\n\t"
+        "bra WAIT_%=;\n\t"
+        "DONE_%=:\n\t}"
+        ::"r"(a), "r"(parity), "r"(0x989680u) : "memory");
+}
 
 // ---- proxies / fences -----------------------------------------------------------------------------------
 // generic-proxy smem writes -> visible to the async proxy (TMA, tcgen05.mma operand reads)
@@ -211,11 +225,69 @@ __device__ __forceinline__ void umma2_ts_f8(uint32_t d_tmem, uint32_t a_tmem, ui
         "tcgen05.mma.cta_group::2.kind::f8f6f4 [%0], [%1], %2, %3, p;\n\t}"
         ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(acc) : "memory");
 }
+// D[tmem] (+)= A[smem] * B[smem] across the CTA pair: M = 256 (each CTA supplies its 128 rows of A and N/2 of B from
+// the same shared-memory offsets)
+__device__ __forceinline__ void umma2_ss(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t acc) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n\t}"
+        ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(acc) : "memory");
+}
+__device__ __forceinline__ void umma2_ss_f8(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t acc) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::2.kind::f8f6f4 [%0], %1, %2, %3, p;\n\t}"
+        ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(acc) : "memory");
+}
 // arrive on `bar` (same offset) in both CTAs of the pair when all prior MMAs of this thread have completed
 __device__ __forceinline__ void umma2_commit(uint64_t* bar) {
     asm volatile(
         "tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
         ::"r"(smem_u32(bar)), "h"((uint16_t)3) : "memory");
+}
+// ---- branch-free issue: every lane runs the (warp-uniform) descriptor arithmetic, the instruction itself is predicated
+// on `elect` (1 in one lane).  With the descriptor math inside an `if (elect_one())` block ptxas computes it in vector
+// registers and moves each operand to a uniform register (R2UR) per MMA: ~25 dependent instructions, ~90 cycles per
+// UMMA issue (measured with a clock64 trace) -- more than the 64 cycles the tensor pipe needs to execute it.
+// Descriptors are passed as (low word, high word): the high word of a SWIZZLE_128B K-major descriptor is a constant,
+// the low word is ((addr >> 4) & 0x3fff) | (LBO >> 4) << 16, so stepping along K or to another stage is one 32-bit add.
+constexpr uint32_t kDescHiSw128 = (uint32_t)((1024u >> 4) | (1u << 14) | (2u << 29));   // SBO = 1024, version 1, SWIZZLE_128B
+__host__ __device__ constexpr uint32_t desc_hi_sw128(uint32_t sbo_bytes) { return (sbo_bytes >> 4) | (1u << 14) | (2u << 29); }
+__device__ __forceinline__ uint32_t desc_lo(uint32_t saddr, uint32_t lbo_bytes) {
+    return ((saddr >> 4) & 0x3fffu) | ((lbo_bytes >> 4) << 16);
+}
+__device__ __forceinline__ void umma2_ss_e(uint32_t d_tmem, uint32_t a_lo, uint32_t a_hi, uint32_t b_lo, uint32_t b_hi,
+                                           uint32_t idesc, uint32_t acc, uint32_t elect) {
+    asm volatile(
+        "{\n\t.reg .pred pe, pa;\n\t.reg .b64 da, db;\n\t"
+        "setp.ne.b32 pe, %7, 0;\n\tsetp.ne.b32 pa, %6, 0;\n\t"
+        "mov.b64 da, {%1, %2};\n\tmov.b64 db, {%3, %4};\n\t"
+        "@pe tcgen05.mma.cta_group::2.kind::f16 [%0], da, db, %5, pa;\n\t}"
+        ::"r"(d_tmem), "r"(a_lo), "r"(a_hi), "r"(b_lo), "r"(b_hi), "r"(idesc), "r"(acc), "r"(elect) : "memory");
+}
+__device__ __forceinline__ void umma2_ss_f8_e(uint32_t d_tmem, uint32_t a_lo, uint32_t a_hi, uint32_t b_lo, uint32_t b_hi,
+                                              uint32_t idesc, uint32_t acc, uint32_t elect) {
+    asm volatile(
+        "{\n\t.reg .pred pe, pa;\n\t.reg .b64 da, db;\n\t"
+        "setp.ne.b32 pe, %7, 0;\n\tsetp.ne.b32 pa, %6, 0;\n\t"
+        "mov.b64 da, {%1, %2};\n\tmov.b64 db, {%3, %4};\n\t"
+        "@pe tcgen05.mma.cta_group::2.kind::f8f6f4 [%0], da, db, %5, pa;\n\t}"
+        ::"r"(d_tmem), "r"(a_lo), "r"(a_hi), "r"(b_lo), "r"(b_hi), "r"(idesc), "r"(acc), "r"(elect) : "memory");
+}
+__device__ __forceinline__ void umma2_ts_e(uint32_t d_tmem, uint32_t a_tmem, uint32_t b_lo, uint32_t b_hi, uint32_t idesc,
+                                           uint32_t acc, uint32_t elect) {
+    asm volatile(
+        "{\n\t.reg .pred pe, pa;\n\t.reg .b64 db;\n\t"
+        "setp.ne.b32 pe, %6, 0;\n\tsetp.ne.b32 pa, %5, 0;\n\t"
+        "mov.b64 db, {%2, %3};\n\t"
+        "@pe tcgen05.mma.cta_group::2.kind::f16 [%0], [%1], db, %4, pa;\n\t}"
+        ::"r"(d_tmem), "r"(a_tmem), "r"(b_lo), "r"(b_hi), "r"(idesc), "r"(acc), "r"(elect) : "memory");
+}
+__device__ __forceinline__ void umma2_commit_e(uint64_t* bar, uint32_t elect) {
+    asm volatile(
+        "{\n\t.reg .pred pe;\n\tsetp.ne.b32 pe, %1, 0;\n\t"
+        "@pe tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %2;\n\t}"
+        ::"r"(smem_u32(bar)), "r"(elect), "h"((uint16_t)3) : "memory");
 }
 // ---- cluster of four (two CTA pairs sharing rotated K tiles): addresses in another CTA of the cluster ----------
 __device__ __forceinline__ uint32_t mapa_u32(uint32_t cta_addr, uint32_t rank) {
