@@ -753,13 +753,12 @@ __global__ void __launch_bounds__(256) prerotate_k_kernel(const __nv_bfloat16* _
     const uint2 el1 = make_uint2(e5m2x4(l1[0], l1[1]), e5m2x4(l1[2], l1[3])), el2 = make_uint2(e5m2x4(l2[0], l2[1]), e5m2x4(l2[2], l2[3]));
     const int kvh = (int)(row - k * H_kv);
     if (selinfo != nullptr && selinfo[kvh * 16 + 8] == 0u) {
-        // selective mode: one 128-byte row per key = [lo1 | lo2 | hi1 | hi2] (16 B each: two pairs per chunk) | unused
+        // selective mode: one 128-byte row per key = region LO (32 B) | region HI (32 B) | unused; chunk c of a region is
+        // [x1(f0) x1(f1) x2(f0) x2(f1)], the layout rotate_rows2 (rot.cuh) writes on the fly
         const uint32_t sj = selinfo[kvh * 16 + c];
-        unsigned short* dst = reinterpret_cast<unsigned short*>(Ke + row * D);
-        dst[c] = (unsigned short)__byte_perm(el1.x, el1.y, sj);
-        dst[8 + c] = (unsigned short)__byte_perm(el2.x, el2.y, sj);
-        dst[16 + c] = (unsigned short)__byte_perm(eh1.x, eh1.y, sj);
-        dst[24 + c] = (unsigned short)__byte_perm(eh2.x, eh2.y, sj);
+        uint32_t* dst = reinterpret_cast<uint32_t*>(Ke + row * D);
+        dst[c] = (__byte_perm(el1.x, el1.y, sj) & 0xffffu) | (__byte_perm(el2.x, el2.y, sj) << 16);
+        dst[8 + c] = (__byte_perm(eh1.x, eh1.y, sj) & 0xffffu) | (__byte_perm(eh2.x, eh2.y, sj) << 16);
     } else {
         reinterpret_cast<uint2*>(Ke + row * D)[c] = eh1;
         reinterpret_cast<uint2*>(Ke + row * D)[8 + c] = eh2;
@@ -945,7 +944,8 @@ int launch_prefill_umma(const void* Q, const void* K, const void* V, void* out, 
         if (prerot) {
             // the scratch holds e5m2 cross-term operands only: the fp16 mode is served by the full e5m2 terms (2),
             // the default by the selective e5m2 terms (3) with a per-head fallback to 2
-            precise = p.precise = (precise == 0 ? 0 : (precise == 1 || full_e5m2) ? 2 : 3);
+            // (the one-tile kernels of this file read the full e5m2 operands only)
+            precise = p.precise = (precise == 0 ? 0 : (precise == 1 || full_e5m2 || !g_two_tile) ? 2 : 3);
             const size_t n = (size_t)L * H_kv * d;
             unsigned char* base = (unsigned char*)ws + two_level_bytes(L + 256, d);
             __half* Kh = reinterpret_cast<__half*>(base);
@@ -967,7 +967,7 @@ int launch_prefill_umma(const void* Q, const void* K, const void* V, void* out, 
                 !make_tensor_map(&tmKl, Kl, L, H_kv, 64, 1))
                 return JETLONG_UNSUPPORTED;
             p.prerot = 1;
-        } else if (precise == 2 && g_otf_selective && !full_e5m2) {
+        } else if (precise == 2 && g_otf_selective && !full_e5m2 && g_two_tile) {
             // on the fly, default precision: selective e5m2 compensation as in the workspace variant (per-head fallback
             // to the full cross terms inside the kernel)
             uint32_t* selinfo = nullptr;

@@ -21,6 +21,7 @@
 // running (m, l, O) per row: the additive form of the Eq.(7) merge.
 #include <cuda.h>
 #include <math.h>
+#include <type_traits>
 
 #include "common.cuh"
 #include "umma.cuh"
@@ -243,6 +244,8 @@ constexpr uint32_t IDESC_QK_BF16 = idesc_f16(1, 1, 0, 0, 2 * BM, BN);
 constexpr uint32_t IDESC_QK_F16 = idesc_f16(0, 0, 0, 0, 2 * BM, BN);
 constexpr uint32_t IDESC_QK_E5M2 = idesc_f16(1, 1, 0, 0, 2 * BM, BN);   // kind::f8f6f4: format code 1 = e5m2
 constexpr uint32_t IDESC_PV = idesc_f16(1, 1, 0, 1, 2 * BM, D);         // A = P (TMEM, bf16), B = V (smem, MN-major)
+// the lean rotation (rot.cuh: rotate_rows2) stores -lo; the negate-A / negate-B bits of the descriptor undo the sign
+constexpr uint32_t IDESC_NEG_A = 1u << 13, IDESC_NEG_B = 1u << 14;
 
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1)
 prefill_umma2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
@@ -370,18 +373,20 @@ prefill_umma2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_const
                 for (int ks = 0; ks < D / 16; ++ks)
                     umma2_ss_e(dS, qa + (((ks >> 2) * QBOX + (ks & 3) * 32) >> 4), HI_K,
                                kb + (((ks >> 2) * KBOX + (ks & 3) * 32) >> 4), HI_K, idesc, ks > 0 ? 1u : 0u, el);
+                // cross terms: Q' lo (written by this kernel) is stored negated; so is K' lo unless it comes from the workspace
+                const uint32_t id_hl = IDESC_QK_E5M2 | (p.prerot ? 0u : IDESC_NEG_B), id_lh = IDESC_QK_E5M2 | IDESC_NEG_A;
                 if (mode == 2 && precise == 3) {
-                    // compact operands: Q' row = [hi1 | hi2 | lo1 | lo2] (tile i at byte 64 i), K' row = [lo1 | lo2 | hi1 | hi2]
-                    umma2_ss_f8_e(dS, qx_lo0 + 4 * i, HI_K, klb, HI_K, IDESC_QK_E5M2, 1u, el);
-                    umma2_ss_f8_e(dS, qx_lo0 + 4 * i + 2, HI_K, klb + 2, HI_K, IDESC_QK_E5M2, 1u, el);
+                    // compact operands: Q' row = [HI | LO] regions of 32 bytes (tile i at byte 64 i), K' row = [LO | HI]
+                    umma2_ss_f8_e(dS, qx_lo0 + 4 * i, HI_K, klb, HI_K, id_hl, 1u, el);
+                    umma2_ss_f8_e(dS, qx_lo0 + 4 * i + 2, HI_K, klb + 2, HI_K, id_lh, 1u, el);
                 } else if (mode == 2 && precise == 2) {
                     const uint32_t qe = qx_lo0 + (uint32_t)(i * ((2 * QBOX) >> 4));   // [Q' e5m2 | Q' lo e5m2] of tile i
 #pragma unroll
                     for (int ks = 0; ks < D / 32; ++ks)              // Q' (e5m2) . K' lo (e5m2)
-                        umma2_ss_f8_e(dS, qe + 2 * ks, HI_K, klb + (KBOX >> 4) + 2 * ks, HI_K, IDESC_QK_E5M2, 1u, el);
+                        umma2_ss_f8_e(dS, qe + 2 * ks, HI_K, klb + (KBOX >> 4) + 2 * ks, HI_K, id_hl, 1u, el);
 #pragma unroll
                     for (int ks = 0; ks < D / 32; ++ks)              // Q' lo (e5m2) . K' (e5m2)
-                        umma2_ss_f8_e(dS, qe + (QBOX >> 4) + 2 * ks, HI_K, klb + 2 * ks, HI_K, IDESC_QK_E5M2, 1u, el);
+                        umma2_ss_f8_e(dS, qe + (QBOX >> 4) + 2 * ks, HI_K, klb + 2 * ks, HI_K, id_lh, 1u, el);
                 }
                 umma2_commit_e(&bars->s_full[i], el);
             };
@@ -453,51 +458,58 @@ prefill_umma2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_const
         // ===================== rotate group (steps a4, a5) =====================
         mbar_wait_sleep(&bars->q_full, 0);
         if (lane == 0) mbar_arrive_leader(&bars->q_ready);
-        KRot<4> rot;
         const bool rotating = mp.n_rem > 0 && !p.prerot;
-        if (mp.n_rem > 0) {
-            rot.init(p.lo, p.hi, tid, p.G, 0);
-            rot.selw = p.selinfo ? __ldg(p.selinfo + kvh * 16 + (tid & 7)) : 0u;
-            if (rotating) rot.prefetch((unsigned)(mp.hi_m * BN + 64 * cta));     // first remote visit
-        }
-        const int kmode = precise == 3 ? 4 : precise;
-        Ring rk(NK);
-        for (int m = 0; m < mp.nm; ++m, rk.next()) {
-            const Visit x = mp.at(m);
-            const int st = rk.s;
-            TR(3, m, 0);
-            mbar_wait_sleep(&bars->k_full[st], rk.ph);
-            TR(3, m, 1);
-            if (x.mode == 2) {
-                if (rotating) {
-                    rotate_k_rows<4, KBOX>(smem_u32(sK(st)), smem_u32(sKl(st)), (unsigned)(x.kt * BN + 64 * cta), rot, kmode);
-                    fence_proxy_async_smem();
-                    if (x.kt > 0) rot.prefetch((unsigned)((x.kt - 1) * BN + 64 * cta));   // next remote visit's first row
-                }
-                if (m == mp.n_loc) {
-                    // first remote visit: Q -> Q' = R(Delta q) Q, in place in shared memory (both tiles, 64 rows per pass)
-                    if (mp.n_loc > 0) mbar_wait_sleep(&bars->q_local_done, 0);
-                    for (int i = 0; i < (valid1 ? 2 : 1); ++i) {
+        const uint32_t selw = (mp.n_rem > 0 && p.selinfo) ? __ldg(p.selinfo + kvh * 16 + (tid & 7)) : 0u;
+        // one visit loop per operand mode, chosen once per CTA, so the hot loop carries no mode switches (code size)
+        auto visit_loop = [&](auto mode_tag) {
+            constexpr int KM = decltype(mode_tag)::value;             // 0 hi only, 2 full e5m2 copies, 5 compact selective rows
+            KRot<4> rot;
+            SelTree sel;
+            sel.init(selw);
+            if (mp.n_rem > 0) {
+                rot.init(p.lo, p.hi, tid, p.G, 0);
+                if (rotating) rot.prefetch((unsigned)(mp.hi_m * BN + 64 * cta));     // first remote visit
+            }
+            Ring rk(NK);
 #pragma unroll 1
-                        for (int half = 0; half < 2; ++half) {
+            for (int m = 0; m < mp.nm; ++m, rk.next()) {
+                const Visit x = mp.at(m);
+                const int st = rk.s;
+                TR(3, m, 0);
+                mbar_wait_sleep(&bars->k_full[st], rk.ph);
+                TR(3, m, 1);
+                if (x.mode == 2) {
+                    if (rotating) {
+                        rotate_rows2<4, KBOX, KM>(smem_u32(sK(st)), smem_u32(sKl(st)), (unsigned)(x.kt * BN + 64 * cta), rot, sel, 0u, 32u);
+                        fence_proxy_async_smem();
+                        if (x.kt > 0) rot.prefetch((unsigned)((x.kt - 1) * BN + 64 * cta));   // next remote visit's first row
+                    }
+                    if (m == mp.n_loc) {
+                        // first remote visit: Q -> Q' = R(Delta q) Q, in place in shared memory (both tiles, 64 rows per pass)
+                        if (mp.n_loc > 0) mbar_wait_sleep(&bars->q_local_done, 0);
+#pragma unroll 1
+                        for (int pass = 0; pass < (valid1 ? 4 : 2); ++pass) {
+                            const int i = pass >> 1, half = pass & 1;
                             KRot<4> qr;
                             qr.init(p.lo, p.hi, tid, p.G, 64 * half);
-                            qr.selw = rot.selw;
                             qr.prefetch((unsigned)((qb0 + i) * BM));
-                            const uint32_t qx = precise == 2 ? smem_u32(sQX) + (uint32_t)(i * 2 * QBOX) : smem_u32(sQX);
-                            const uint32_t c4 = (uint32_t)(((4 * i + 1) << 12) | ((4 * i) << 8) | ((4 * i + 3) << 4) | (4 * i + 2));
-                            rotate_k_rows<4, QBOX>(smem_u32(sQ + i * QT_BYTES), qx, (unsigned)((qb0 + i) * BM), qr, kmode, 0, 0, c4);
+                            const uint32_t qx = KM == 2 ? smem_u32(sQX) + (uint32_t)(i * 2 * QBOX) : smem_u32(sQX);
+                            rotate_rows2<4, QBOX, KM>(smem_u32(sQ + i * QT_BYTES), qx, (unsigned)((qb0 + i) * BM), qr, sel,
+                                                      64u * i + 32u, 64u * i);
                         }
+                        fence_proxy_async_smem();
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive_leader(&bars->q_rot_done);
                     }
-                    fence_proxy_async_smem();
-                    __syncwarp();
-                    if (lane == 0) mbar_arrive_leader(&bars->q_rot_done);
                 }
+                __syncwarp();
+                if (lane == 0) mbar_arrive_leader(&bars->k_ready[st]);
+                TR(3, m, 2);
             }
-            __syncwarp();
-            if (lane == 0) mbar_arrive_leader(&bars->k_ready[st]);
-            TR(3, m, 2);
-        }
+        };
+        if (precise == 3) visit_loop(std::integral_constant<int, 5>{});
+        else if (precise == 2) visit_loop(std::integral_constant<int, 2>{});
+        else visit_loop(std::integral_constant<int, 0>{});
     } else {
         // ===================== softmax groups (steps a6-a8): one thread per query row =====================
         reg_inc<REGS_SOFTMAX>();

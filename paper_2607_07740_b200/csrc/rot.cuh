@@ -292,5 +292,120 @@ __device__ __forceinline__ void rotate_k_rows(uint32_t kh, uint32_t kl, unsigned
     }
 }
 
+// ---- lean form of the correction rotation (two-tile prefill) ---------------------------------------------------
+// Same arithmetic as rotate_k_rows, about half the instructions per key row (measured with ncu: 250 -> ~125):
+//   * (cos, sin, -sin) are all carried, so neither the rotation nor the recurrence negates a packed operand per use;
+//   * the residual is one mixed-precision FHADD per value (sub.f32.f16: hi - y = -lo) instead of two conversions and a
+//     packed subtract; the consumer undoes the sign with the negate bit of the UMMA instruction descriptor;
+//   * MODE 5 (selective compensation): the two selected pairs of the chunk are picked from the fp16 words with a
+//     three-PRMT tree BEFORE the e5m2 rounding, and each thread stores one 32-bit word per region:
+//       compact row = region LO at byte b_lo: 8 chunks x [lo1(f0) lo1(f1) lo2(f0) lo2(f1)], region HI at b_hi: the same of hi
+//     (position j of the 32-byte contraction slice means the same (chunk, pair, half) in Q' and K' rows, which is all the
+//     UMMA needs);
+//   * the next row's shared-memory loads are issued before the current row's arithmetic.
+// MODE 0: hi only.  MODE 2: full e5m2 copies at kl (as rotate_k_rows mode 2, lo negated).  MODE 5 as above.
+__device__ __forceinline__ float fhsub_lo(uint32_t h, float y) {     // (low fp16 of h) - y
+    float r;
+    unsigned short hs;
+    asm("{.reg .b16 t; mov.b32 {%0, t}, %1;}" : "=h"(hs) : "r"(h));
+    asm("sub.rn.f32.f16 %0, %1, %2;" : "=f"(r) : "h"(hs), "f"(y));
+    return r;
+}
+__device__ __forceinline__ float fhsub_hi(uint32_t h, float y) {     // (high fp16 of h) - y
+    float r;
+    unsigned short hs;
+    asm("{.reg .b16 t; mov.b32 {t, %0}, %1;}" : "=h"(hs) : "r"(h));
+    asm("sub.rn.f32.f16 %0, %1, %2;" : "=f"(r) : "h"(hs), "f"(y));
+    return r;
+}
+// selectors of the PRMT tree for the two compensated pairs f0 < f1 (0..7) of a chunk, from selw = f0 | f1 << 4
+struct SelTree {
+    uint32_t s_pool, s_top;
+    __device__ __forceinline__ void init(uint32_t selw) {
+        const uint32_t f0 = selw & 7u, f1 = (selw >> 4) & 7u;
+        const uint32_t h0 = 2u * (f0 & 3u), h1 = 2u * (f1 & 3u);
+        s_pool = h0 | ((h0 + 1u) << 4) | (h1 << 8) | ((h1 + 1u) << 12);           // the same selector serves both pools
+        const uint32_t a = f0 < 4u ? 0u : 4u, b = f1 < 4u ? 2u : 6u;
+        s_top = a | ((a + 1u) << 4) | (b << 8) | ((b + 1u) << 12);
+    }
+    // [half f0 | half f1] of the eight fp16 halves in w[0..3]
+    __device__ __forceinline__ uint32_t pick(const uint32_t (&w)[4]) const {
+        return __byte_perm(__byte_perm(w[0], w[1], s_pool), __byte_perm(w[2], w[3], s_pool), s_top);
+    }
+};
+
+template <int ROWS, int KBOX, int MODE>
+__device__ __forceinline__ void rotate_rows2(uint32_t kh, uint32_t kl, unsigned pos0, KRot<ROWS>& R, const SelTree& T,
+                                             uint32_t b_lo, uint32_t b_hi) {
+    uint64_t cc[4], cs[4], ncs[4], nss[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const float4 h = R.nh[j], l = R.nl[j];
+        cc[j] = pack2(h.x * l.x - h.y * l.y, h.z * l.z - h.w * l.w);
+        cs[j] = pack2(h.y * l.x + h.x * l.y, h.w * l.z + h.z * l.w);
+        ncs[j] = neg2(cs[j]);
+        nss[j] = neg2(R.ss[j]);
+    }
+    unsigned rem = (pos0 + R.r0) % R.G;
+    int off = R.r0 * 128 + ((R.c ^ (R.r0 & 7)) << 4);
+    uint4 u1 = lds128(kh + off), u2 = lds128(kh + KBOX + off);
+    // rolled on purpose: the SM's instruction caches are small (L0 ~6 KB, L1.5 32 KB) and four roles run different loops;
+    // unrolled, this loop alone was 16 KB and its warps spent most samples in stall_no_inst (ncu)
+#pragma unroll 1
+    for (int m = 0; m < ROWS; ++m) {
+        const int r = R.r0 + m;
+        const int off_n = (r + 1) * 128 + ((R.c ^ ((r + 1) & 7)) << 4);
+        uint4 n1 = u1, n2 = u2;
+        if (m + 1 < ROWS) { n1 = lds128(kh + off_n); n2 = lds128(kh + KBOX + off_n); }
+        const uint32_t a[4] = {u1.x, u1.y, u1.z, u1.w}, b[4] = {u2.x, u2.y, u2.z, u2.w};
+        uint32_t h1[4], h2[4], l1[4], l2[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const uint64_t x1 = bf16x2_to_f32x2(a[j]), x2 = bf16x2_to_f32x2(b[j]);
+            const uint64_t y1 = ffma2(x2, ncs[j], fmul2(x1, cc[j]));           // x1 c - x2 s
+            const uint64_t y2 = ffma2(x1, cs[j], fmul2(x2, cc[j]));            // x1 s + x2 c
+            float y1a, y1b, y2a, y2b;
+            unpack2(y1, y1a, y1b);
+            unpack2(y2, y2a, y2b);
+            h1[j] = f16x2_rn(y1a, y1b);
+            h2[j] = f16x2_rn(y2a, y2b);
+            if (MODE != 0) {                                                   // -lo = hi - y
+                l1[j] = f16x2_rn(fhsub_lo(h1[j], y1a), fhsub_hi(h1[j], y1b));
+                l2[j] = f16x2_rn(fhsub_lo(h2[j], y2a), fhsub_hi(h2[j], y2b));
+            }
+        }
+        sts128(kh + off, h1[0], h1[1], h1[2], h1[3]);
+        sts128(kh + KBOX + off, h2[0], h2[1], h2[2], h2[3]);
+        if (MODE == 2) {
+            // byte b of an e5m2 row is channel b: channels 8c.. sit in 16-byte chunk c/2, channels 64+8c.. in chunk 4+c/2
+            const uint32_t o1 = r * 128 + ((((R.c >> 1)) ^ (r & 7)) << 4) + (R.c & 1) * 8;
+            const uint32_t o2 = r * 128 + (((4 + (R.c >> 1)) ^ (r & 7)) << 4) + (R.c & 1) * 8;
+            sts64(kl + o1, e5m2x4(h1[0], h1[1]), e5m2x4(h1[2], h1[3]));
+            sts64(kl + o2, e5m2x4(h2[0], h2[1]), e5m2x4(h2[2], h2[3]));
+            sts64(kl + KBOX + o1, e5m2x4(l1[0], l1[1]), e5m2x4(l1[2], l1[3]));
+            sts64(kl + KBOX + o2, e5m2x4(l2[0], l2[1]), e5m2x4(l2[2], l2[3]));
+        } else if (MODE == 5) {
+            const uint32_t x = (uint32_t)(r & 7), cw = (uint32_t)(R.c >> 2), cb = (uint32_t)(R.c & 3) * 4u;
+            const uint32_t wl = __byte_perm(T.pick(l1) + 0x00800080u, T.pick(l2) + 0x00800080u, 0x7531);
+            const uint32_t wh = __byte_perm(T.pick(h1) + 0x00800080u, T.pick(h2) + 0x00800080u, 0x7531);
+            asm volatile("st.shared.u32 [%0], %1;" ::"r"(kl + r * 128 + ((((b_lo >> 4) + cw) ^ x) << 4) + cb), "r"(wl) : "memory");
+            asm volatile("st.shared.u32 [%0], %1;" ::"r"(kl + r * 128 + ((((b_hi >> 4) + cw) ^ x) << 4) + cb), "r"(wh) : "memory");
+        }
+        if (m + 1 < ROWS) {
+            rem = (rem + 1 == R.G) ? 0u : rem + 1;
+            if (rem != 0) {                                           // n grows by one: advance by the unit step
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const uint64_t c2 = ffma2(cs[j], nss[j], fmul2(cc[j], R.sc[j]));
+                    cs[j] = ffma2(cc[j], R.ss[j], fmul2(cs[j], R.sc[j]));
+                    cc[j] = c2;
+                    ncs[j] = neg2(cs[j]);
+                }
+            }
+        }
+        off = off_n; u1 = n1; u2 = n2;
+    }
+}
+
 }  // namespace dev
 }  // namespace jetlong
