@@ -18,7 +18,10 @@
  *   - dtype: JETLONG_BF16 (bf16 Q/K/V/out, fp32 accumulation) or JETLONG_FP32 (fp32 everything).
  *   - Return value: a jetlong_status.  Arguments are validated before any launch; on a non-OK
  *     status nothing has been written.  There is no CPU fallback: without a compute-capability
- *     10.x device the compute entry points return JETLONG_UNSUPPORTED.
+ *     10.0 device (B200, sm_100a) the compute entry points return JETLONG_UNSUPPORTED.
+ *   - Value range (bf16 path): rotated remote operands are re-rounded to fp16 and e5m2 for the tensor core, so
+ *     |Q|, |K| elements must stay below 2^15 (a rotated pair can grow by sqrt 2; fp16 overflows at 65504, e5m2 at
+ *     61440).  Larger magnitudes give inf / NaN remote scores; activations of the models in scope are < 2^10.
  *   - INVALID_ARG: null pointer, L < 1, H_q % H_kv != 0, head_dim not in {64, 128}, w_local < 0,
  *     w_pretrained < 1, rope_theta <= 0, unknown dtype, a pointer not 16-byte aligned, or a
  *     workspace smaller than jetlong_workspace_bytes() reports.
@@ -51,7 +54,11 @@ enum { JETLONG_OP_PREFILL = 0, JETLONG_OP_DECODE = 1, JETLONG_OP_CAUSAL_PREFILL 
 int64_t jetlong_group_size(int64_t L, int64_t w_pretrained);
 
 /* Bytes of caller-allocated device workspace the op needs for these shapes (0 is possible).
- * Holds rotation tables (Eq.(5)-(6)) and split-KV partial states (decode).  16-byte aligned. */
+ * Holds rotation tables (Eq.(5)-(6)) and split-KV partial states (decode).  16-byte aligned.
+ * Contract: the first 256 bytes are a table header.  A workspace must be ZERO-FILLED before its first use (at least
+ * its first 256 bytes); between calls that reuse it the caller must not write into it.  A sealed header
+ * (magic, rope_theta, table length, head_dim, checksum of the table's first and last rows) lets consecutive calls
+ * skip the table rebuild; a header that does not verify is rebuilt, never trusted. */
 size_t jetlong_workspace_bytes(int op, int64_t L, int H_q, int H_kv, int head_dim, int dtype);
 
 /*
@@ -121,12 +128,17 @@ int jetlong_causal_decode(const void* q, const void* Kcache, const void* Vcache,
 
 /*
  * Host-buffer convenience wrappers (used for end-to-end timing): same arguments, but Q, K, V, out,
- * lse are HOST pointers (pinned or pageable).  The call allocates device buffers, copies in, runs
- * the op on the default stream, copies out/lse back and synchronises before returning.
+ * lse are HOST pointers (pinned or pageable).  The call copies in, runs the op, copies out / lse back and synchronises
+ * before returning.  Device staging memory is taken from an arena the library keeps per device and reuses from call
+ * to call (grown on demand, released by jetlong_host_release or at process exit); calls are serialised per device.
+ * Every copy's status is checked (JETLONG_CUDA_ERROR).
  */
 int jetlong_prefill_host(const void* Q, const void* K, const void* V, void* out, float* lse,
                          int64_t L, int H_q, int H_kv, int head_dim,
                          int64_t w_local, int64_t w_pretrained, double rope_theta, int dtype);
+
+/* Frees the staging arenas of jetlong_prefill_host (all devices).  Safe to call at any time between calls. */
+void jetlong_host_release(void);
 
 /* Text for a status; for JETLONG_CUDA_ERROR the text of the last CUDA error seen by this thread. */
 const char* jetlong_status_string(int status);
@@ -134,13 +146,37 @@ const char* jetlong_status_string(int status);
 /* Number of kernels this process has launched through the library (for bench accounting). */
 int64_t jetlong_launch_count(void);
 
-/* Which prefill implementation a bf16 call uses.  -1 (default): tcgen05 UMMA where supported; the on-the-fly bifocal
- * prefill of >= 64 query blocks runs as clusters of four CTAs (two CTA pairs on adjacent query blocks share every rotated K
- * tile through distributed shared memory) on an internal high-priority stream, forked from and joined to `stream` by
- * events, while CTA pairs take the lightest query blocks on the SMs that cannot hold such a cluster.
- * 0 = SIMT fp32-FMA tiles; 1 = tcgen05 UMMA, CTA pairs only; 2 = clusters of four for every query block;
- * 3 = clusters of four + CTA pairs regardless of size.  All give the same results up to rounding.
- * Returns the previous value. */
+/*
+ * Per-call options of the prefill entry points (precision of the remote scores, implementation).  Pass NULL for the
+ * defaults.  struct_bytes = sizeof(jetlong_options) (checked: a smaller value is JETLONG_INVALID_ARG); a field set to
+ * JETLONG_DEFAULT takes the calling thread's default (see the two deprecated setters below).  Nothing in the library's
+ * launch path is process-global: two host threads may call with different options on different streams.
+ */
+#define JETLONG_DEFAULT (-2)
+typedef struct {
+    uint32_t struct_bytes;
+    int precision;      /* a JETLONG_PRECISION_* value or JETLONG_DEFAULT */
+    int prefill_impl;   /* -1 / 4: tcgen05 two-tile kernel (default); 1: tcgen05 one-tile CTA pairs; 0: SIMT fp32; or JETLONG_DEFAULT */
+} jetlong_options;
+
+/* jetlong_prefill / jetlong_prefill_prerotated with explicit options; identical otherwise. */
+int jetlong_prefill_opt(const void* Q, const void* K, const void* V, void* out, float* lse,
+                        int64_t L, int H_q, int H_kv, int head_dim,
+                        int64_t w_local, int64_t w_pretrained, double rope_theta,
+                        int dtype, void* workspace, size_t workspace_bytes, void* stream,
+                        const jetlong_options* options);
+int jetlong_prefill_prerotated_opt(const void* Q, const void* K, const void* V, void* out, float* lse,
+                                   int64_t L, int H_q, int H_kv, int head_dim,
+                                   int64_t w_local, int64_t w_pretrained, double rope_theta,
+                                   int dtype, void* workspace, size_t workspace_bytes, void* stream,
+                                   const jetlong_options* options);
+
+/* DEPRECATED (kept as shims): set the CALLING THREAD's default prefill implementation.
+ * -1 or 4 (default): tcgen05 UMMA where supported (bf16, head_dim 128, even H_q / H_kv): the two-tile kernel, in which a
+ * CTA pair owns 256 query rows x 2 heads and every staged / rotated K tile feeds both 128-row tiles (prefill_umma2.cu).
+ * 1 = the one-tile CTA-pair kernel of round 1 (prefill_umma.cu; also serves JETLONG_PRECISION_COMPENSATED_F16);
+ * 0 = SIMT fp32-FMA tiles.  2 and 3 (round 1's cluster-of-four launches, superseded by the two-tile kernel and
+ * removed) are accepted and mean 1.  All give the same results up to rounding.  Returns the previous value. */
 int jetlong_set_prefill_impl(int impl);
 
 /* Operand precision of the REMOTE Q'K'^T on the tcgen05 prefill path.  Rotated operands must be
@@ -152,10 +188,11 @@ int jetlong_set_prefill_impl(int impl);
  *                          whose remaining channels are too loud (predicted score noise > 3e-4) gets the full cross
  *                          terms.  lse error 1e-4 (64K-128K) to 8e-4 (short, peaked rows).
  *   COMPENSATED_E5M2:      the two e5m2 cross terms over all 128 channels for every head; lse error ~3e-4.
- *   COMPENSATED_F16:       the two cross terms in fp16 (three fp16 UMMA groups); lse error ~1e-5.  The workspace variant
- *                          serves this mode with COMPENSATED_E5M2.
+ *   COMPENSATED_F16:       the two cross terms in fp16 (three fp16 UMMA groups, one-tile kernel); lse error ~1e-5.  The
+ *                          workspace variant serves this mode with COMPENSATED_E5M2.
  *   FAST:                  Q'hi K'hi only; lse error up to ~3e-3 on such inputs (out still within tolerance).
  * Local tiles, the control and decode are unaffected (decode always compensates: fp16 K'hi [Q'hi; Q'lo] + e5m2 K'lo Q'hi).
+ * DEPRECATED setter (a shim): sets the CALLING THREAD's default; prefer jetlong_options.precision.
  * Returns the previous mode; an unknown mode changes nothing. */
 enum { JETLONG_PRECISION_COMPENSATED = 0, JETLONG_PRECISION_FAST = 1, JETLONG_PRECISION_COMPENSATED_F16 = 2,
        JETLONG_PRECISION_COMPENSATED_E5M2 = 3 };

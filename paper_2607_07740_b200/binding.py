@@ -22,7 +22,21 @@ PRECISION_COMPENSATED, PRECISION_FAST, PRECISION_COMPENSATED_F16, PRECISION_COMP
 EXPORTS = ["jetlong_group_size", "jetlong_workspace_bytes", "jetlong_prefill", "jetlong_decode",
            "jetlong_causal_prefill", "jetlong_causal_decode", "jetlong_prefill_host", "jetlong_status_string",
            "jetlong_launch_count", "jetlong_set_prefill_impl", "jetlong_prefill_uses_umma",
-           "jetlong_set_prefill_precision", "jetlong_prefill_prerotated", "jetlong_prefill_unfused"]
+           "jetlong_set_prefill_precision", "jetlong_prefill_prerotated", "jetlong_prefill_unfused",
+           "jetlong_prefill_opt", "jetlong_prefill_prerotated_opt", "jetlong_host_release"]
+DEFAULT = -2                                              # JETLONG_DEFAULT: take the calling thread's default
+
+
+class Options(ctypes.Structure):
+    """jetlong_options (include/jetlong.h): per-call precision / implementation."""
+    _fields_ = [("struct_bytes", ctypes.c_uint32), ("precision", ctypes.c_int), ("prefill_impl", ctypes.c_int)]
+
+
+def _options(precision, impl):
+    if precision is None and impl is None:
+        return None
+    o = Options(ctypes.sizeof(Options), DEFAULT if precision is None else int(precision), DEFAULT if impl is None else int(impl))
+    return ctypes.byref(o)
 
 
 class JetlongError(RuntimeError):
@@ -51,6 +65,11 @@ def lib():
         L.jetlong_prefill_prerotated.argtypes = [vp] * 5 + tail
         L.jetlong_prefill_unfused.restype = i32
         L.jetlong_prefill_unfused.argtypes = [vp] * 5 + tail
+        L.jetlong_prefill_opt.restype = i32
+        L.jetlong_prefill_opt.argtypes = [vp] * 5 + tail + [vp]
+        L.jetlong_prefill_prerotated_opt.restype = i32
+        L.jetlong_prefill_prerotated_opt.argtypes = [vp] * 5 + tail + [vp]
+        L.jetlong_host_release.restype = None
         L.jetlong_decode.restype = i32
         L.jetlong_decode.argtypes = [vp] * 5 + tail
         ctail = [i64, i32, i32, i32, i32, vp, sz, vp]
@@ -127,27 +146,31 @@ def _prefill_args(Q, K, V, out, lse):
     return L, H_q, H_kv, d, out, lse
 
 
-def jetlong_prefill(Q, K, V, *, w_local, w_pretrained, rope_theta, out=None, lse=None, workspace=None):
-    """Bifocal prefill.  Q [L,H_q,d], K/V [L,H_kv,d] (bf16 or fp32, RoPE'd at true positions).  Returns out, lse."""
+def jetlong_prefill(Q, K, V, *, w_local, w_pretrained, rope_theta, out=None, lse=None, workspace=None, precision=None,
+                    impl=None):
+    """Bifocal prefill.  Q [L,H_q,d], K/V [L,H_kv,d] (bf16 or fp32, RoPE'd at true positions).  Returns out, lse.
+    precision / impl: per-call jetlong_options (None = the thread's default)."""
     L, H_q, H_kv, d, out, lse = _prefill_args(Q, K, V, out, lse)
     dt = _dt(Q)
     if workspace is None:
         workspace = alloc_workspace(OP_PREFILL, L, H_q, H_kv, d, dt, Q.device)
-    _check(lib().jetlong_prefill(Q.data_ptr(), K.data_ptr(), V.data_ptr(), out.data_ptr(), lse.data_ptr(), L, H_q,
-                                 H_kv, d, int(w_local), int(w_pretrained), float(rope_theta), dt,
-                                 workspace.data_ptr(), workspace.numel(), _stream()))
+    _check(lib().jetlong_prefill_opt(Q.data_ptr(), K.data_ptr(), V.data_ptr(), out.data_ptr(), lse.data_ptr(), L, H_q,
+                                     H_kv, d, int(w_local), int(w_pretrained), float(rope_theta), dt,
+                                     workspace.data_ptr(), workspace.numel(), _stream(), _options(precision, impl)))
     return out, lse
 
 
-def jetlong_prefill_prerotated(Q, K, V, *, w_local, w_pretrained, rope_theta, out=None, lse=None, workspace=None):
+def jetlong_prefill_prerotated(Q, K, V, *, w_local, w_pretrained, rope_theta, out=None, lse=None, workspace=None,
+                               precision=None, impl=None):
     """Workspace variant of the bifocal prefill: K is correction-rotated once into a scratch in the workspace."""
     L, H_q, H_kv, d, out, lse = _prefill_args(Q, K, V, out, lse)
     dt = _dt(Q)
     if workspace is None:
         workspace = alloc_workspace(OP_PREFILL_PREROTATED, L, H_q, H_kv, d, dt, Q.device)
-    _check(lib().jetlong_prefill_prerotated(Q.data_ptr(), K.data_ptr(), V.data_ptr(), out.data_ptr(), lse.data_ptr(),
-                                            L, H_q, H_kv, d, int(w_local), int(w_pretrained), float(rope_theta), dt,
-                                            workspace.data_ptr(), workspace.numel(), _stream()))
+    _check(lib().jetlong_prefill_prerotated_opt(Q.data_ptr(), K.data_ptr(), V.data_ptr(), out.data_ptr(), lse.data_ptr(),
+                                                L, H_q, H_kv, d, int(w_local), int(w_pretrained), float(rope_theta), dt,
+                                                workspace.data_ptr(), workspace.numel(), _stream(),
+                                                _options(precision, impl)))
     return out, lse
 
 

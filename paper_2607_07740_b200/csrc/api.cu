@@ -1,5 +1,6 @@
 // api.cu -- the C ABI of libjetlong (include/jetlong.h): validation, dispatch, workspace layout.
 #include <atomic>
+#include <mutex>
 #include <stdio.h>
 #include <string.h>
 
@@ -9,8 +10,25 @@ namespace jetlong {
 
 static std::atomic<long long> g_launches{0};
 static thread_local char g_err[256] = "no CUDA error recorded";
-static std::atomic<int> g_prefill_impl{-1};
-static std::atomic<int> g_prefill_precision{JETLONG_PRECISION_COMPENSATED};
+// per-thread defaults behind the deprecated setters; a call's jetlong_options override them
+static thread_local int t_prefill_impl = -1;
+static thread_local int t_prefill_precision = JETLONG_PRECISION_COMPENSATED;
+
+static bool precision_known(int m) {
+    return m == JETLONG_PRECISION_COMPENSATED || m == JETLONG_PRECISION_FAST || m == JETLONG_PRECISION_COMPENSATED_F16 ||
+           m == JETLONG_PRECISION_COMPENSATED_E5M2;
+}
+struct Resolved { int precision, impl; bool ok; };
+static Resolved resolve(const jetlong_options* opt) {
+    Resolved r{t_prefill_precision, t_prefill_impl, true};
+    if (opt) {
+        if (opt->struct_bytes < sizeof(jetlong_options)) { r.ok = false; return r; }
+        if (opt->precision != JETLONG_DEFAULT) r.precision = opt->precision;
+        if (opt->prefill_impl != JETLONG_DEFAULT) r.impl = opt->prefill_impl;
+    }
+    r.ok = precision_known(r.precision) && r.impl >= -1 && r.impl <= 4;
+    return r;
+}
 
 void note_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
 
@@ -30,10 +48,7 @@ int launch_prefill_unfused(const void* Q, const void* K, const void* V, void* ou
                            int H_kv, int d, long long w0, long long G, double theta, void* ws, cudaStream_t st);
 int launch_prefill_umma(const void* Q, const void* K, const void* V, void* out, float* lse, long long L, int H_q,
                         int H_kv, int d, long long w0, long long G, double theta, bool bifocal, int precise, void* ws,
-                        size_t ws_bytes, cudaStream_t st, bool prerot);
-
-extern int g_share_clusters;   // prefill_umma.cu
-extern int g_two_tile;         // prefill_umma.cu
+                        size_t ws_bytes, cudaStream_t st, bool prerot, bool two_tile);
 
 static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; }
 
@@ -51,16 +66,16 @@ static int validate(const void* a, const void* b, const void* c, const void* o, 
 static int device_ok() {
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return JETLONG_UNSUPPORTED; }
-    int major = 0;
-    if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) {
+    int major = 0, minor = 0;
+    if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&minor, cudaDevAttrComputeCapabilityMinor, dev) != cudaSuccess) {
         cudaGetLastError();
         return JETLONG_UNSUPPORTED;
     }
-    return major == 10 ? JETLONG_OK : JETLONG_UNSUPPORTED;
+    return (major == 10 && minor == 0) ? JETLONG_OK : JETLONG_UNSUPPORTED;   // the library carries sm_100a code only
 }
 
-static bool use_umma(long long L, int H_q, int H_kv, int d, int dtype) {
-    const int impl = g_prefill_impl.load();
+static bool use_umma(int impl, long long L, int H_q, int H_kv, int d, int dtype) {
     if (impl == 0) return false;
     return umma_prefill_supported(L, H_q, H_kv, d, dtype);
 }
@@ -73,9 +88,12 @@ static size_t prefill_ws(long long L, int H_q, int H_kv, int d, int dtype, bool 
 
 static int prefill_common(const void* Q, const void* K, const void* V, void* out, float* lse, long long L, int H_q,
                           int H_kv, int d, long long w0, long long w_pre, double theta, int dtype, void* ws,
-                          size_t ws_bytes, void* stream, bool bifocal, bool prerot = false) {
+                          size_t ws_bytes, void* stream, bool bifocal, bool prerot = false,
+                          const jetlong_options* opt = nullptr) {
     int rc = validate(Q, K, V, out, lse, L, H_q, H_kv, d, w0, w_pre, theta, dtype);
     if (rc != JETLONG_OK) return rc;
+    const Resolved o = resolve(opt);
+    if (!o.ok) return JETLONG_INVALID_ARG;
     if (prerot && !umma_prefill_supported(L, H_q, H_kv, d, dtype)) return JETLONG_UNSUPPORTED;
     long long G = bifocal ? jetlong_group_size(L, w_pre) : 1;
     if (G == 1 || w0 >= L - 1) bifocal = false;          // step a2: G = 1 (or an all-covering window) is the control
@@ -84,12 +102,12 @@ static int prefill_common(const void* Q, const void* K, const void* V, void* out
     rc = device_ok();
     if (rc != JETLONG_OK) return rc;
     cudaStream_t st = (cudaStream_t)stream;
-    const int prec = g_prefill_precision.load();
-    if (prerot || use_umma(L, H_q, H_kv, d, dtype))
+    const int prec = o.precision;
+    if (prerot || use_umma(o.impl, L, H_q, H_kv, d, dtype))
         return launch_prefill_umma(Q, K, V, out, lse, L, H_q, H_kv, d, w0, G, theta, bifocal,
                                    prec == JETLONG_PRECISION_FAST ? 0 : prec == JETLONG_PRECISION_COMPENSATED_F16 ? 1 : prec == JETLONG_PRECISION_COMPENSATED_E5M2 ? 6 : 2,
                                    ws, ws_bytes, st,
-                                   prerot && bifocal);
+                                   prerot && bifocal, /*two_tile=*/o.impl != 1);
     const float2* tab = nullptr;
     if (bifocal) {
         rc = build_key_table((float2*)ws, L, G, d, theta, st);
@@ -155,6 +173,21 @@ int jetlong_prefill_prerotated(const void* Q, const void* K, const void* V, void
                           workspace, workspace_bytes, stream, true, true);
 }
 
+int jetlong_prefill_opt(const void* Q, const void* K, const void* V, void* out, float* lse, int64_t L, int H_q, int H_kv,
+                        int head_dim, int64_t w_local, int64_t w_pretrained, double rope_theta, int dtype, void* workspace,
+                        size_t workspace_bytes, void* stream, const jetlong_options* options) {
+    return prefill_common(Q, K, V, out, lse, L, H_q, H_kv, head_dim, w_local, w_pretrained, rope_theta, dtype,
+                          workspace, workspace_bytes, stream, true, false, options);
+}
+
+int jetlong_prefill_prerotated_opt(const void* Q, const void* K, const void* V, void* out, float* lse, int64_t L, int H_q,
+                                   int H_kv, int head_dim, int64_t w_local, int64_t w_pretrained, double rope_theta,
+                                   int dtype, void* workspace, size_t workspace_bytes, void* stream,
+                                   const jetlong_options* options) {
+    return prefill_common(Q, K, V, out, lse, L, H_q, H_kv, head_dim, w_local, w_pretrained, rope_theta, dtype,
+                          workspace, workspace_bytes, stream, true, true, options);
+}
+
 int jetlong_prefill_unfused(const void* Q, const void* K, const void* V, void* out, float* lse, int64_t L, int H_q,
                             int H_kv, int head_dim, int64_t w_local, int64_t w_pretrained, double rope_theta, int dtype,
                             void* workspace, size_t workspace_bytes, void* stream) {
@@ -193,6 +226,27 @@ int jetlong_causal_decode(const void* q, const void* Kcache, const void* Vcache,
                          workspace_bytes, stream, false);
 }
 
+// staging arena of jetlong_prefill_host: one per device, grown on demand, reused from call to call
+struct HostArena { unsigned char* base = nullptr; size_t bytes = 0; cudaStream_t st = nullptr; };
+static HostArena g_arena[64];
+static std::mutex g_arena_mu;
+
+void jetlong_host_release(void) {
+    std::lock_guard<std::mutex> lock(g_arena_mu);
+    int cur = 0;
+    cudaGetDevice(&cur);
+    for (int d = 0; d < 64; ++d) {
+        HostArena& a = g_arena[d];
+        if (!a.base && !a.st) continue;
+        cudaSetDevice(d);
+        if (a.base) cudaFree(a.base);
+        if (a.st) cudaStreamDestroy(a.st);
+        a = HostArena();
+    }
+    cudaSetDevice(cur);
+    cudaGetLastError();
+}
+
 int jetlong_prefill_host(const void* Q, const void* K, const void* V, void* out, float* lse, int64_t L, int H_q,
                          int H_kv, int head_dim, int64_t w_local, int64_t w_pretrained, double rope_theta, int dtype) {
     int rc = validate(Q, K, V, out, lse, L, H_q, H_kv, head_dim, w_local, w_pretrained, rope_theta, dtype);
@@ -203,29 +257,41 @@ int jetlong_prefill_host(const void* Q, const void* K, const void* V, void* out,
     const size_t nq = (size_t)L * H_q * head_dim * es, nk = (size_t)L * H_kv * head_dim * es;
     const size_t nl = (size_t)L * H_q * sizeof(float);
     const size_t nws = jetlong_workspace_bytes(JETLONG_OP_PREFILL, L, H_q, H_kv, head_dim, dtype);
-    unsigned char* dev = nullptr;
     const size_t oq = 0, ok = align256(nq), ov = ok + align256(nk), oo = ov + align256(nk), ol = oo + align256(nq),
                  ow = ol + align256(nl), total = ow + align256(nws) + 256;
-    if (cudaMalloc(&dev, total) != cudaSuccess) return check_launch("cudaMalloc");
-    cudaMemcpyAsync(dev + oq, Q, nq, cudaMemcpyHostToDevice, 0);
-    cudaMemcpyAsync(dev + ok, K, nk, cudaMemcpyHostToDevice, 0);
-    cudaMemcpyAsync(dev + ov, V, nk, cudaMemcpyHostToDevice, 0);
-    rc = jetlong_prefill(dev + oq, dev + ok, dev + ov, dev + oo, (float*)(dev + ol), L, H_q, H_kv, head_dim, w_local,
-                         w_pretrained, rope_theta, dtype, dev + ow, align256(nws) + 256, nullptr);
-    if (rc == JETLONG_OK) {
-        cudaMemcpyAsync(out, dev + oo, nq, cudaMemcpyDeviceToHost, 0);
-        cudaMemcpyAsync(lse, dev + ol, nl, cudaMemcpyDeviceToHost, 0);
-        if (cudaStreamSynchronize(0) != cudaSuccess) rc = check_launch("jetlong_prefill_host");
+    int devid = 0;
+    if (cudaGetDevice(&devid) != cudaSuccess || devid < 0 || devid >= 64) return check_launch("cudaGetDevice");
+    std::lock_guard<std::mutex> lock(g_arena_mu);               // calls are serialised: they share the arena
+    HostArena& a = g_arena[devid];
+    if (!a.st && cudaStreamCreateWithFlags(&a.st, cudaStreamNonBlocking) != cudaSuccess) return check_launch("cudaStreamCreate");
+    if (a.bytes < total) {
+        if (a.base && cudaFree(a.base) != cudaSuccess) return check_launch("cudaFree");
+        a.base = nullptr; a.bytes = 0;
+        if (cudaMalloc(&a.base, total) != cudaSuccess) return check_launch("cudaMalloc");
+        a.bytes = total;
+        // the table header must start zeroed (jetlong_workspace_bytes contract); afterwards the sealed tables are reused
+        if (cudaMemsetAsync(a.base + ow, 0, 256, a.st) != cudaSuccess) return check_launch("cudaMemsetAsync");
     }
-    cudaFree(dev);
-    return rc;
+    unsigned char* dev = a.base;
+    if (cudaMemcpyAsync(dev + ok, K, nk, cudaMemcpyHostToDevice, a.st) != cudaSuccess ||
+        cudaMemcpyAsync(dev + ov, V, nk, cudaMemcpyHostToDevice, a.st) != cudaSuccess ||
+        cudaMemcpyAsync(dev + oq, Q, nq, cudaMemcpyHostToDevice, a.st) != cudaSuccess)
+        return check_launch("jetlong_prefill_host H2D");
+    rc = jetlong_prefill(dev + oq, dev + ok, dev + ov, dev + oo, (float*)(dev + ol), L, H_q, H_kv, head_dim, w_local,
+                         w_pretrained, rope_theta, dtype, dev + ow, align256(nws) + 256, a.st);
+    if (rc != JETLONG_OK) { cudaStreamSynchronize(a.st); return rc; }
+    if (cudaMemcpyAsync(out, dev + oo, nq, cudaMemcpyDeviceToHost, a.st) != cudaSuccess ||
+        cudaMemcpyAsync(lse, dev + ol, nl, cudaMemcpyDeviceToHost, a.st) != cudaSuccess)
+        return check_launch("jetlong_prefill_host D2H");
+    if (cudaStreamSynchronize(a.st) != cudaSuccess) return check_launch("jetlong_prefill_host");
+    return JETLONG_OK;
 }
 
 const char* jetlong_status_string(int status) {
     switch (status) {
         case JETLONG_OK: return "ok";
         case JETLONG_INVALID_ARG: return "invalid argument";
-        case JETLONG_UNSUPPORTED: return "unsupported device or configuration (needs compute capability 10.x)";
+        case JETLONG_UNSUPPORTED: return "unsupported device or configuration (needs compute capability 10.0, sm_100a)";
         case JETLONG_CUDA_ERROR: return g_err;
         default: return "unknown status";
     }
@@ -234,20 +300,19 @@ const char* jetlong_status_string(int status) {
 int64_t jetlong_launch_count(void) { return g_launches.load(); }
 
 int jetlong_set_prefill_impl(int impl) {
-    g_share_clusters = impl == 2 ? 1 : impl == 3 ? 2 : impl == 1 ? 0 : 3;   // see prefill_umma.cu; -1 (default) = auto
-    g_two_tile = (impl == 1 || impl == 2 || impl == 3) ? 0 : 1;             // 1 / 2 / 3: the one-tile kernels
-    return g_prefill_impl.exchange(impl);
+    const int prev = t_prefill_impl;
+    if (impl >= -1 && impl <= 4) t_prefill_impl = (impl == 2 || impl == 3) ? 1 : impl;   // 2, 3: the removed cluster launches
+    return prev;
 }
 
 int jetlong_set_prefill_precision(int mode) {
-    if (mode != JETLONG_PRECISION_COMPENSATED && mode != JETLONG_PRECISION_FAST && mode != JETLONG_PRECISION_COMPENSATED_F16 &&
-        mode != JETLONG_PRECISION_COMPENSATED_E5M2)
-        return g_prefill_precision.load();
-    return g_prefill_precision.exchange(mode);
+    const int prev = t_prefill_precision;
+    if (precision_known(mode)) t_prefill_precision = mode;
+    return prev;
 }
 
 int jetlong_prefill_uses_umma(int64_t L, int H_q, int H_kv, int head_dim) {
-    return use_umma(L, H_q, H_kv, head_dim, JETLONG_BF16) ? 1 : 0;
+    return use_umma(t_prefill_impl, L, H_q, H_kv, head_dim, JETLONG_BF16) ? 1 : 0;
 }
 
 }  // extern "C"

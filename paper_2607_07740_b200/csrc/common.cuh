@@ -33,7 +33,8 @@ struct TableHeader {          // first 256 bytes of a table region; lets decode 
     double theta;
     long long n_hi;
     int d;
-    int pad;
+    unsigned check;           // hash of LO[1][*] and HI[n_hi-1][*]: a header whose body was overwritten does not verify
+    unsigned gen;             // incremented by every rebuild: a reader that loaded entries early re-reads them if it moved
 };
 
 constexpr unsigned long long kTableMagic = 0x4a45544c4f4e4732ull;  // "JETLONG2": header of a sealed two-level table
@@ -45,6 +46,9 @@ int build_key_table(float2* tab, long long L, long long G, int d, double theta, 
 // decode / UMMA prefill: two-level table; returns bytes via two_level_bytes
 size_t two_level_bytes(long long L, int d);
 int build_two_level(void* region, long long L, int d, double theta, cudaStream_t st);
+
+// multiprocessor count of the current device (cached per device)
+int sm_count();
 
 // kernels' host launchers (defined in the respective .cu files)
 int launch_prefill_simt(const void* Q, const void* K, const void* V, void* out, float* lse, long long L, int H_q,

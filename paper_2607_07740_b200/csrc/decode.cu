@@ -361,7 +361,7 @@ Plan make_plan(long long L, int H_q, int H_kv) {
     const int g = H_q / H_kv;
     pl.GQ = (g % 4 == 0) ? 4 : ((g % 2 == 0) ? 2 : 1);
     pl.gz = g / pl.GQ;
-    const int target = 148 * 2;
+    const int target = sm_count() * 2;
     int ns = target / (pl.gy * pl.gz);
     if (ns < 1) ns = 1;
     if (ns > 1024) ns = 1024;

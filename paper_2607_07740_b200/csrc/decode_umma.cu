@@ -141,12 +141,19 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
     const DPlan plan(p, split);
     const float sl2 = (1.0f / sqrtf((float)D)) * kLog2e;
 
+    // Launched with programmatic stream serialization.  When the kernel in front of us on the stream is the library's own
+    // table kernel (bifocal), that kernel was launched normally, so everything the caller enqueued before the call --
+    // the kernel that wrote q or appended KV row L-1 -- has completed before we run.  In the control (and G = 1) there is
+    // no table kernel: wait for the predecessor here, before q or the cache are read (the prologue up to here still
+    // overlaps its tail).
+    if (!p.bifocal) griddep_wait();
     // the query loads go out before the TMA streams start: behind ~14 MB of in-flight cache tiles they take microseconds
     const int rt = tid - 96;                                           // rotate-group thread index
     __nv_bfloat16 qv1[NH * 64 / RT], qv2[NH * 64 / RT];
     float2 tqh[NH * 64 / RT], tql[NH * 64 / RT];                       // HI / LO table entries of the query position
     KRot<RROWS> rot;
     bool tab_early = false;
+    unsigned tab_gen = 0;                                               // generation of the table the early loads saw
     const long long nq = (p.L - 1) - (p.L - 1) / p.G;                  // -Delta(q) >= 0, Eq.(5)
     auto load_tables = [&]() {
 #pragma unroll
@@ -178,6 +185,7 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
             const volatile TableHeader* hdr =
                 reinterpret_cast<const volatile TableHeader*>(reinterpret_cast<const unsigned char*>(p.lo) - 256);
             tab_early = hdr->magic == kTableMagic && hdr->theta == p.theta && hdr->n_hi == (p.L + 255) / 256 + 1 && hdr->d == D;
+            tab_gen = hdr->gen;
             if (tab_early) load_tables();
         }
     }
@@ -245,7 +253,7 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
 #pragma unroll
                     for (int ks = 0; ks < D / 32; ++ks)        // K'lo (e5m2) Q'hi (e5m2) into columns 0-15
                         umma_ss_f8(dS, smem_desc_sw128(kla + ks * 32, 16, 1024),
-                                   smem_desc_sw128(qc + QCBUF + ks * 32, 16, 1024), IDESC_S_E5M2, 1);
+                                   smem_desc_sw128(qc + QCBUF + ks * 32, 16, 1024), IDESC_S_E5M2 | (1u << 13), 1);   // K' lo is stored negated (rotate_rows2): negate A
                 }
                 umma_commit(&bars->s_full[v & 1]);
                 umma_commit(&bars->k_empty[v % KS]);
@@ -286,14 +294,17 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
     } else if (warp >= 3 && warp < 3 + RW) {
         // ===================== rotate group (steps a4, a5) =====================
         const int t = tid - 96;
-        const long long qpos = p.L - 1;
         // Q operands [16 heads][128 ch]: raw bf16 for local tiles; Q' = R(Delta q) Q as fp16 hi / lo for remote tiles
         for (int i = t; i < (QBUF + QCBUF + QYBUF) / 4; i += RT) reinterpret_cast<uint32_t*>(sQ)[i] = 0u;
         for (int i = t; i < QBUF / 4; i += RT) reinterpret_cast<uint32_t*>(sP)[i] = 0u;
         named_bar_sync(1, RT);
-        if (plan.nr > 0 && !tab_early) {                             // header not sealed: wait for the table kernel
+        if (plan.nr > 0) {
+            // the table kernel has finished by now (it returns at once when the table verifies against its header); if it
+            // rebuilt the table -- header not sealed at the early read, or a body that failed the check -- load again
             griddep_wait();
-            load_tables();
+            const volatile TableHeader* hdr =
+                reinterpret_cast<const volatile TableHeader*>(reinterpret_cast<const unsigned char*>(p.lo) - 256);
+            if (!tab_early || hdr->gen != tab_gen) load_tables();
         }
 #pragma unroll
         for (int it = 0; it < NH * 64 / RT; ++it) {
@@ -326,7 +337,7 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
             const int s = v % KS;
             mbar_wait(&bars->k_full[s], (v / KS) & 1);
             if (plan.remote(v)) {
-                rotate_k_rows<RROWS, BOXB>(smem_u32(sK(s)), smem_u32(sK(s)) + TILE, (unsigned)(plan.kt(v) * BN), rot, 3);
+                rotate_rows2<RROWS, BOXB, 3>(smem_u32(sK(s)), smem_u32(sK(s)) + TILE, (unsigned)(plan.kt(v) * BN), rot, SelTree(), 0u, 0u);
                 fence_proxy_async_smem();
                 if (plan.remote(v + 1)) rot.prefetch((unsigned)(plan.kt(v + 1) * BN));
             }
@@ -466,7 +477,7 @@ bool umma_decode_supported(int H_q, int H_kv, int d, int dtype) {
 // split plan: one CTA per SM (the kernel needs ~215 KB of shared memory), key ranges are multiples of the 128-key tile
 void umma_decode_plan(long long L, int H_kv, int* nsplit, long long* kps) {
     const long long ntiles = (L + BN - 1) / BN;
-    long long ns = 148 / H_kv;
+    long long ns = sm_count() / H_kv;
     if (ns < 1) ns = 1;
     if (ns > ntiles) ns = ntiles;
     if (ns > 1024) ns = 1024;

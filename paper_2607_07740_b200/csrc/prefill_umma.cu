@@ -671,62 +671,70 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_consta
     prefill_body<false>(tmK, tmV, tmKh, tmKe, tmKl, tmK, p);
 }
 
-// on-the-fly bifocal prefill: clusters of four CTAs (two pairs on adjacent query blocks) share every rotated K tile
-__global__ void __cluster_dims__(4, 1, 1) __launch_bounds__(NTHREADS, 1)
-prefill_umma_share_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV,
-                          const __grid_constant__ CUtensorMap tmK32, const Params p) {
-    prefill_body<true>(tmK, tmV, tmK, tmK, tmK, tmK32, p);
-}
-
 // ---- 8(f)-1: rotate K once into a scratch (the workspace variant) -------------------------------------------
 // K'hi [L, H_kv, 128] fp16, K'e5 [L, H_kv, 128] e5m2 (K' rounded), K'lo [L, H_kv, 128] e5m2 (K' - K'hi): exactly the
 // three operands the rotate group otherwise produces per visit.  Thread = (key k, KV head, 16-byte chunk c).
-// Mean pair energies for the selective compensation: e[(h / gdiv) * 64 + i] += x_i^2 + x_{i+64}^2 over the sampled rows
-// of head h.  grid (blocks, H), 256 threads: pair i = t & 63, row lane t >> 6.
+// Pair energies for the selective compensation.  The sequence is cut into gridDim.x contiguous blocks of rows; a CTA
+// measures the MEAN energy x_i^2 + x_{i+64}^2 of every pair i over (a sample of) its block and head h, and the table keeps
+// the MAXIMUM over blocks (and over the query heads of a KV group): e[(h / gdiv) * 64 + i] = max_blocks mean_rows(...).
+// A global mean (round 1) cannot see a channel that is loud in only part of the sequence; the block maximum can, and
+// for stationary inputs it equals the mean up to sampling noise (blocks hold >= 1024 rows).
+// grid (blocks, H), 256 threads: pair i = t & 63, row lane t >> 6.  Energies are >= 0, so their bit patterns order as ints.
 __global__ void __launch_bounds__(256) pair_energy_kernel(const __nv_bfloat16* __restrict__ X, float* __restrict__ e,
                                                           long long L, int H, int gdiv, int stride) {
     __shared__ float red[256];
     const int i = threadIdx.x & 63, sub = threadIdx.x >> 6, h = blockIdx.y;
+    const long long R = (L + gridDim.x - 1) / gridDim.x;
+    const long long r0 = (long long)blockIdx.x * R, r1 = r0 + R < L ? r0 + R : L;
     float acc = 0.f;
-    for (long long k = ((long long)blockIdx.x * 4 + sub) * stride; k < L; k += (long long)gridDim.x * 4 * stride) {
+    for (long long k = r0 + (long long)sub * stride; k < r1; k += 4ll * stride) {
         const __nv_bfloat16* r = X + ((size_t)k * H + h) * D;
         const float x1 = __bfloat162float(r[i]), x2 = __bfloat162float(r[i + 64]);
         acc += x1 * x1 + x2 * x2;
     }
     red[threadIdx.x] = acc;
     __syncthreads();
-    if (sub == 0) atomicAdd(&e[(h / gdiv) * 64 + i], red[i] + red[64 + i] + red[128 + i] + red[192 + i]);
+    if (sub == 0 && r1 > r0) {
+        const float n = (float)((r1 - r0 + stride - 1) / stride);
+        const float m = (red[i] + red[64 + i] + red[128 + i] + red[192 + i]) / n;
+        atomicMax(reinterpret_cast<int*>(&e[(h / gdiv) * 64 + i]), __float_as_int(m));
+    }
 }
 
-// Per KV head: weight w_i = mean pair energy of K times that of Q; in every chunk of 8 pairs the two heaviest are
+// Per KV head: weight w_i = (block-max pair energy of K) x (of Q); in every chunk of 8 pairs the two heaviest are
 // compensated (PRMT selector j0 | j1 << 4).  The pairs left out add rounding noise of about
-// sigma = scale * 2^-10 / (1.44 sqrt(12)) * sqrt(sum of their w_i) to a remote score; above
-// SEL_SIGMA_MAX the head falls back to the full e5m2 cross terms (flag at [8]).
+// sigma = scale * 2^-10 / (1.44 sqrt(12)) * sqrt(sum of their w_i) to a remote score.  The head falls back to
+// the full e5m2 cross terms (flag at [8]) when sigma > SEL_SIGMA_MAX, or when a pair that was left out is LOUD -- more
+// than SEL_LOUD times the mean weight of the pairs left out (three outlier pairs in one chunk; measured: one such pair
+// alone puts the lse error at 2e-3).
 constexpr float SEL_SIGMA_MAX = 3.0e-4f;
+constexpr float SEL_LOUD = 4.0f;
 __global__ void __launch_bounds__(64) select_pairs_kernel(const float* __restrict__ eK, const float* __restrict__ eQ,
-                                                          uint32_t* __restrict__ selinfo, float inv_nk, float inv_nq) {
+                                                          uint32_t* __restrict__ selinfo) {
     __shared__ float w[64];
-    __shared__ float resid[8];
+    __shared__ float resid[8], loud[8];
     const int kvh = blockIdx.x, t = threadIdx.x;
-    w[t] = (eK[kvh * 64 + t] * inv_nk) * (eQ[kvh * 64 + t] * inv_nq);
+    w[t] = eK[kvh * 64 + t] * eQ[kvh * 64 + t];
     __syncthreads();
     if (t < 8) {
         int j0 = 0;
         for (int j = 1; j < 8; ++j) if (w[8 * t + j] > w[8 * t + j0]) j0 = j;
         int j1 = j0 == 0 ? 1 : 0;
         for (int j = 0; j < 8; ++j) if (j != j0 && w[8 * t + j] > w[8 * t + j1]) j1 = j;
-        float r = 0.f;
-        for (int j = 0; j < 8; ++j) if (j != j0 && j != j1) r += w[8 * t + j];
+        float r = 0.f, mx = 0.f;
+        for (int j = 0; j < 8; ++j) if (j != j0 && j != j1) { r += w[8 * t + j]; mx = fmaxf(mx, w[8 * t + j]); }
         resid[t] = r;
+        loud[t] = mx;
         const int a = j0 < j1 ? j0 : j1, b = j0 < j1 ? j1 : j0;
         selinfo[kvh * 16 + t] = (uint32_t)(a | (b << 4));
     }
     __syncthreads();
     if (t == 0) {
-        float r = 0.f;
-        for (int c = 0; c < 8; ++c) r += resid[c];
+        float r = 0.f, mx = 0.f;
+        for (int c = 0; c < 8; ++c) { r += resid[c]; mx = fmaxf(mx, loud[c]); }
         const float sigma = rsqrtf((float)D) * 1.96e-4f * sqrtf(r);
-        selinfo[kvh * 16 + 8] = (sigma > SEL_SIGMA_MAX || !(sigma == sigma)) ? 1u : 0u;
+        const bool full = sigma > SEL_SIGMA_MAX || !(sigma == sigma) || mx > SEL_LOUD * (r / 48.0f);
+        selinfo[kvh * 16 + 8] = full ? 1u : 0u;
     }
 }
 
@@ -864,12 +872,14 @@ static int run_selection(const void* Q, const void* K, long long L, int H_q, int
     float* eQ = eK + (size_t)H_kv * 64;
     uint32_t* selinfo = reinterpret_cast<uint32_t*>(scratch + align256((size_t)H_kv * 64 * 4 * 2));
     if (cudaMemsetAsync(eK, 0, (size_t)H_kv * 64 * 4 * 2, st) != cudaSuccess) return check_launch("memset");
+    // blocks of >= 1024 rows (at most 64 of them): the block mean then carries ~3 % of sampling noise, so the maximum over
+    // blocks of a stationary input stays within ~10 % of its mean; K is read in full, Q every 8th row
     const int sk = 1, sq = 8;
-    const unsigned bk = (unsigned)((L / sk + 255) / 256), bq = (unsigned)((L / sq + 255) / 256);
-    pair_energy_kernel<<<dim3(bk ? bk : 1, H_kv), 256, 0, st>>>((const __nv_bfloat16*)K, eK, L, H_kv, 1, sk);
-    pair_energy_kernel<<<dim3(bq ? bq : 1, H_q), 256, 0, st>>>((const __nv_bfloat16*)Q, eQ, L, H_q, H_q / H_kv, sq);
-    const double nk = (double)((L + sk - 1) / sk), nq = (double)((L + sq - 1) / sq) * (H_q / H_kv);
-    select_pairs_kernel<<<H_kv, 64, 0, st>>>(eK, eQ, selinfo, (float)(1.0 / nk), (float)(1.0 / nq));
+    long long nb = L / 1024;
+    nb = nb < 1 ? 1 : nb > 64 ? 64 : nb;
+    pair_energy_kernel<<<dim3((unsigned)nb, H_kv), 256, 0, st>>>((const __nv_bfloat16*)K, eK, L, H_kv, 1, sk);
+    pair_energy_kernel<<<dim3((unsigned)nb, H_q), 256, 0, st>>>((const __nv_bfloat16*)Q, eQ, L, H_q, H_q / H_kv, sq);
+    select_pairs_kernel<<<H_kv, 64, 0, st>>>(eK, eQ, selinfo);
     note_launch(3);
     *selinfo_out = selinfo;
     return check_launch("select_pairs_kernel");
@@ -885,18 +895,8 @@ size_t umma_prefill_unfused_workspace_bytes(long long L, int H_q, int H_kv, int 
     return two_level_bytes(L + 256, d) + 3 * align256(2 * nq) + align256(2 * nk) + 2 * align256((size_t)L * H_q * 4);
 }
 
-// How the on-the-fly bifocal prefill is launched (jetlong_set_prefill_impl):
-//   0  CTA pairs only (impl 1)
-//   1  clusters of four CTAs that share rotated K tiles, every query block (impl 2)
-//   2  clusters of four on an internal high-priority stream + CTA pairs for the lightest query blocks on the SMs that
-//      cannot hold a cluster (impl 3)
-//   3  default: as 2 when there are at least 64 query blocks, CTA pairs otherwise
-int g_share_clusters = 3;
-// 1 (default): the two-tile kernel of prefill_umma2.cu serves every precision it supports; 0: the one-tile kernels of this
-// file (jetlong_set_prefill_impl 1 / 2 / 3)
-int g_two_tile = 1;
-// 1: the default precision of the on-the-fly kernel uses the selective e5m2 compensation; 0: the full cross terms
-int g_otf_selective = 1;
+// 1: the default precision of the on-the-fly two-tile kernel uses the selective e5m2 compensation; 0: the full cross terms
+constexpr int g_otf_selective = 1;
 
 bool umma_prefill_supported(long long L, int H_q, int H_kv, int d, int dtype) {
     if (dtype != JETLONG_BF16 || d != 128 || H_kv < 1 || H_q % H_kv) return false;
@@ -914,7 +914,7 @@ size_t umma_prefill_prerot_workspace_bytes(long long L, int H_kv, int d) {
 
 int launch_prefill_umma(const void* Q, const void* K, const void* V, void* out, float* lse, long long L, int H_q,
                         int H_kv, int d, long long w0, long long G, double theta, bool bifocal, int precise, void* ws,
-                        size_t ws_bytes, cudaStream_t st, bool prerot) {
+                        size_t ws_bytes, cudaStream_t st, bool prerot, bool g_two_tile) {
     (void)ws_bytes;
     CUtensorMap tmK, tmV;
     if (!make_kv_tensor_map(&tmK, K, L, H_kv, 64) || !make_kv_tensor_map(&tmV, V, L, H_kv, 128)) return JETLONG_UNSUPPORTED;
@@ -986,77 +986,9 @@ int launch_prefill_umma(const void* Q, const void* K, const void* V, void* out, 
         a.lo = p.lo; a.hi = p.hi; a.selinfo = p.selinfo;
         return launch_prefill_v2(a, st);
     }
-    static bool attr_set = false;
-    if (!attr_set) {
-        if (cudaFuncSetAttribute(prefill_umma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES) !=
-            cudaSuccess)
-            return check_launch("prefill_umma attr");
-        attr_set = true;
-    }
+    if (cudaFuncSetAttribute(prefill_umma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES) != cudaSuccess)
+        return check_launch("prefill_umma attr");
     const int n_qb = (int)((L + BM - 1) / BM);
-    const bool capturing = [&] {
-        cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
-        return cudaStreamIsCapturing(st, &cs) == cudaSuccess && cs != cudaStreamCaptureStatusNone;
-    }();
-    if (bifocal && !p.prerot && g_share_clusters && !(g_share_clusters == 3 && (n_qb < 64 || capturing))) {
-        // on the fly: clusters of four CTAs, two query blocks per cluster share each rotated K tile
-        CUtensorMap tmK32;
-        if (!make_kv_tensor_map(&tmK32, K, L, H_kv, 32)) return JETLONG_UNSUPPORTED;
-        static bool attr4_set = false;
-        if (!attr4_set) {
-            if (cudaFuncSetAttribute(prefill_umma_share_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES) !=
-                cudaSuccess)
-                return check_launch("prefill_umma_share attr");
-            attr4_set = true;
-        }
-        // Only 132 of the 148 SMs can hold a 4-CTA cluster of this size.  With g_share_clusters == 2 the lightest query
-        // blocks [0, qb_lo) -- about the share of the work 16 SMs can do -- go to the CTA-pair kernel on the caller's
-        // stream, while the clusters run on an internal high-priority stream (fork / join through events): the block
-        // scheduler places clusters first and fills the SMs they cannot use with CTA pairs.
-        int qb_lo = 0;
-        if (g_share_clusters >= 2 && n_qb >= 64 && !capturing) {
-            qb_lo = (int)(0.30 * n_qb);                              // ~9 % of the visits; measured flat from 0.2 to 0.5
-            qb_lo -= (n_qb - qb_lo) & 1;                             // an even number of blocks for the clusters
-        }
-        struct Fork { cudaStream_t hs = nullptr; cudaEvent_t ev_fork = nullptr, ev_join = nullptr; };
-        static Fork forks[64];                                       // per device
-        static std::mutex fork_mu;
-        std::lock_guard<std::mutex> lock(fork_mu);                   // the events are reused from call to call
-        int dev = 0;
-        cudaGetDevice(&dev);
-        Fork& fk = forks[dev & 63];
-        cudaStream_t& hs = fk.hs;
-        cudaEvent_t &ev_fork = fk.ev_fork, &ev_join = fk.ev_join;
-        cudaStream_t s4 = st;
-        if (qb_lo > 0) {
-            if (!hs) {
-                int lo_pri = 0, hi_pri = 0;
-                cudaDeviceGetStreamPriorityRange(&lo_pri, &hi_pri);
-                if (cudaStreamCreateWithPriority(&hs, cudaStreamNonBlocking, hi_pri) != cudaSuccess ||
-                    cudaEventCreateWithFlags(&ev_fork, cudaEventDisableTiming) != cudaSuccess ||
-                    cudaEventCreateWithFlags(&ev_join, cudaEventDisableTiming) != cudaSuccess)
-                    return check_launch("prefill_umma_share stream");
-            }
-            cudaEventRecord(ev_fork, st);
-            cudaStreamWaitEvent(hs, ev_fork, 0);
-            s4 = hs;
-        }
-        Params p4 = p;
-        p4.qb_top = n_qb; p4.qb_lo = qb_lo;
-        const unsigned grid4 = 4u * (unsigned)((n_qb - qb_lo + 1) / 2) * (unsigned)(H_q / 2);
-        prefill_umma_share_kernel<<<grid4, NTHREADS, SMEM_BYTES, s4>>>(tmK, tmV, tmK32, p4);
-        note_launch();
-        int rc4 = check_launch("prefill_umma_share_kernel");
-        if (rc4 != JETLONG_OK || qb_lo == 0) return rc4;
-        cudaEventRecord(ev_join, hs);
-        Params p2 = p;
-        p2.qb_top = qb_lo; p2.qb_lo = 0;
-        prefill_umma_kernel<<<2u * (unsigned)qb_lo * (unsigned)(H_q / 2), NTHREADS, SMEM_BYTES, st>>>(tmK, tmV, tmKh, tmKe, tmKl, p2);
-        note_launch();
-        rc4 = check_launch("prefill_umma_kernel");
-        cudaStreamWaitEvent(st, ev_join, 0);
-        return rc4;
-    }
     const unsigned grid = 2u * (unsigned)n_qb * (unsigned)(H_q / 2);
     prefill_umma_kernel<<<grid, NTHREADS, SMEM_BYTES, st>>>(tmK, tmV, tmKh, tmKe, tmKl, p);
     note_launch();
@@ -1071,37 +1003,15 @@ namespace jetlong {
 // One launch of the tcgen05 kernel on given operands: window_only = the local band only, qk_f16 = fp16 Q/K operands.
 static int launch_plain(const void* Q, const void* K, const void* V, void* out, float* lse, long long L, int H_q, int H_kv,
                         long long w0, bool window_only, bool qk_f16, cudaStream_t st) {
-    CUtensorMap tmK, tmV;
-    if (!make_kv_tensor_map(&tmK, K, L, H_kv, 64) || !make_kv_tensor_map(&tmV, V, L, H_kv, 128)) return JETLONG_UNSUPPORTED;
-    Params p;
-    p.Q = (const __nv_bfloat16*)Q;
-    p.out = (__nv_bfloat16*)out;
-    p.lse = lse;
-    p.L = L; p.w0 = w0; p.G = 1;
-    p.H_q = H_q; p.H_kv = H_kv; p.g = H_q / H_kv;
-    p.bifocal = window_only ? 1 : 0;
-    p.precise = 0;
-    p.prerot = 0;
-    p.window_only = window_only ? 1 : 0;
-    p.qk_f16 = qk_f16 ? 1 : 0;
-    p.qb_top = (int)((L + BM - 1) / BM);
-    p.qb_lo = 0;
-    p.lo = nullptr; p.hi = nullptr; p.selinfo = nullptr;
-    if (g_two_tile) {
-        PrefillV2Args a;
-        if (!make_kv_tensor_map(&a.tmQ, Q, L, H_q, 128)) return JETLONG_UNSUPPORTED;
-        a.tmK = tmK; a.tmV = tmV; a.tmKh = tmK; a.tmKe = tmK; a.tmKl = tmK;
-        a.out = p.out; a.lse = lse; a.L = L; a.w0 = w0; a.G = 1; a.H_q = H_q; a.H_kv = H_kv;
-        a.bifocal = p.bifocal; a.precise = 0; a.prerot = 0; a.window_only = p.window_only; a.qk_f16 = p.qk_f16;
-        a.lo = nullptr; a.hi = nullptr; a.selinfo = nullptr;
-        return launch_prefill_v2(a, st);
-    }
-    if (cudaFuncSetAttribute(prefill_umma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES) != cudaSuccess)
-        return check_launch("prefill_umma attr");
-    const int n_qb = (int)((L + BM - 1) / BM);
-    prefill_umma_kernel<<<2u * (unsigned)n_qb * (unsigned)(H_q / 2), NTHREADS, SMEM_BYTES, st>>>(tmK, tmV, tmK, tmK, tmK, p);
-    note_launch();
-    return check_launch("prefill_umma_kernel");
+    PrefillV2Args a;
+    if (!make_kv_tensor_map(&a.tmK, K, L, H_kv, 64) || !make_kv_tensor_map(&a.tmV, V, L, H_kv, 128) ||
+        !make_kv_tensor_map(&a.tmQ, Q, L, H_q, 128))
+        return JETLONG_UNSUPPORTED;
+    a.tmKh = a.tmK; a.tmKe = a.tmK; a.tmKl = a.tmK;
+    a.out = (__nv_bfloat16*)out; a.lse = lse; a.L = L; a.w0 = w0; a.G = 1; a.H_q = H_q; a.H_kv = H_kv;
+    a.bifocal = window_only ? 1 : 0; a.precise = 0; a.prerot = 0; a.window_only = window_only ? 1 : 0; a.qk_f16 = qk_f16 ? 1 : 0;
+    a.lo = nullptr; a.hi = nullptr; a.selinfo = nullptr;
+    return launch_prefill_v2(a, st);
 }
 
 // A = window attention on the stored Q, K; B = full causal attention at the remote positions; C = window attention at

@@ -212,8 +212,14 @@ __device__ __forceinline__ void exp_issue_consume(uint32_t (&cur)[32], const uin
                                                   uint32_t (&pk)[16]) {
 #pragma unroll
     for (int j = 0; j < 32; j += 2) {
-        cur[j] = __float_as_uint(ex2v(__uint_as_float(cur[j])));
-        cur[j + 1] = __float_as_uint(ex2v(__uint_as_float(cur[j + 1])));
+        if ((j & 6) < 2 * POLY_OF_4) {                                 // this pair on the FMA pipe (scores here are finite)
+            float r0, r1;
+            exp2_poly2(pack2(__uint_as_float(cur[j]), __uint_as_float(cur[j + 1])), r0, r1);
+            cur[j] = __float_as_uint(r0); cur[j + 1] = __float_as_uint(r1);
+        } else {
+            cur[j] = __float_as_uint(ex2v(__uint_as_float(cur[j])));
+            cur[j + 1] = __float_as_uint(ex2v(__uint_as_float(cur[j + 1])));
+        }
         if (HAS_PREV) consume_pair(prev, j, l2a, l2b, pk);
     }
 }

@@ -303,7 +303,8 @@ __device__ __forceinline__ void rotate_k_rows(uint32_t kh, uint32_t kl, unsigned
 //     (position j of the 32-byte contraction slice means the same (chunk, pair, half) in Q' and K' rows, which is all the
 //     UMMA needs);
 //   * the next row's shared-memory loads are issued before the current row's arithmetic.
-// MODE 0: hi only.  MODE 2: full e5m2 copies at kl (as rotate_k_rows mode 2, lo negated).  MODE 5 as above.
+// MODE 0: hi only.  MODE 2: full e5m2 copies at kl (as rotate_k_rows mode 2, lo negated).  MODE 3: only -lo as e5m2 at kl
+// (decode).  MODE 5 as above.
 __device__ __forceinline__ float fhsub_lo(uint32_t h, float y) {     // (low fp16 of h) - y
     float r;
     unsigned short hs;
@@ -384,6 +385,11 @@ __device__ __forceinline__ void rotate_rows2(uint32_t kh, uint32_t kl, unsigned 
             sts64(kl + o2, e5m2x4(h2[0], h2[1]), e5m2x4(h2[2], h2[3]));
             sts64(kl + KBOX + o1, e5m2x4(l1[0], l1[1]), e5m2x4(l1[2], l1[3]));
             sts64(kl + KBOX + o2, e5m2x4(l2[0], l2[1]), e5m2x4(l2[2], l2[3]));
+        } else if (MODE == 3) {                                        // decode: only K' lo as e5m2 at kl (one box)
+            const uint32_t o1 = r * 128 + ((((R.c >> 1)) ^ (r & 7)) << 4) + (R.c & 1) * 8;
+            const uint32_t o2 = r * 128 + (((4 + (R.c >> 1)) ^ (r & 7)) << 4) + (R.c & 1) * 8;
+            sts64(kl + o1, e5m2x4(l1[0], l1[1]), e5m2x4(l1[2], l1[3]));
+            sts64(kl + o2, e5m2x4(l2[0], l2[1]), e5m2x4(l2[2], l2[3]));
         } else if (MODE == 5) {
             const uint32_t x = (uint32_t)(r & 7), cw = (uint32_t)(R.c >> 2), cb = (uint32_t)(R.c & 3) * 4u;
             const uint32_t wl = __byte_perm(T.pick(l1) + 0x00800080u, T.pick(l2) + 0x00800080u, 0x7531);

@@ -41,20 +41,58 @@ int build_key_table(float2* tab, long long L, long long G, int d, double theta, 
 // Region layout: [TableHeader (256 B)] [LO: 256*half float2] [HI: n_hi*half float2]
 static constexpr unsigned long long kMagic = kTableMagic;
 
+int sm_count() {
+    static int cached[64] = {0};
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) { cudaGetLastError(); return 148; }
+    if (cached[dev] == 0) {
+        int n = 0;
+        if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n < 1) { cudaGetLastError(); n = 148; }
+        cached[dev] = n;
+    }
+    return cached[dev];
+}
+
 size_t two_level_bytes(long long L, int d) {
     long long n_hi = (L + 255) / 256 + 1;
     return 256 + align256((size_t)(256 + n_hi) * (d / 2) * sizeof(float2));
 }
 
-// One CTA.  Every call launches it; when the header already describes (theta, n_hi, d) it returns at once (decode
-// steps 1..n), otherwise it rebuilds the table and then seals the header.
+// hash of the 2 x 64 float2 entries of LO[1] and HI[n_hi-1] (the first row that is not all (1, 0) and the last row)
+__device__ __forceinline__ unsigned table_check(const float2* lo, const float2* hi, long long n_hi, int half, unsigned* red) {
+    const int t = threadIdx.x;
+    unsigned h = 0;
+    if (t < 2 * half) {
+        const float2 v = t < half ? lo[half + t] : hi[(n_hi - 1) * half + (t - half)];
+        h = (__float_as_uint(v.x) * 0x9E3779B1u) ^ (__float_as_uint(v.y) * 0x85EBCA77u) ^ ((unsigned)t * 0xC2B2AE3Du);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) h ^= __shfl_xor_sync(0xffffffffu, h, o);
+    if ((t & 31) == 0) red[t >> 5] = h;
+    __syncthreads();
+    unsigned r = 0;
+    for (int w = 0; w < (int)(blockDim.x >> 5); ++w) r ^= red[w];
+    __syncthreads();
+    return r | 1u;                                                    // never 0
+}
+
+// One CTA.  Every call launches it; when the header describes (theta, n_hi, d) AND the table verifies against the
+// header's check word it returns at once (decode steps 1..n); otherwise it un-seals the header, rebuilds the table
+// and seals it again with a new generation number.  The workspace must have been zero-filled before its first use
+// (include/jetlong.h), so an unsealed region never carries the magic by accident.
 __global__ void __launch_bounds__(1024) two_level_kernel(unsigned char* __restrict__ region, long long n_hi, int half,
                                                          double theta, double log2_theta, int d) {
+    __shared__ unsigned red[32];
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");   // a programmatically launched consumer (decode) may start
     TableHeader* hdr = reinterpret_cast<TableHeader*>(region);
-    if (hdr->magic == kMagic && hdr->theta == theta && hdr->n_hi == n_hi && hdr->d == d) return;   // uniform
     float2* lo = reinterpret_cast<float2*>(region + 256);
     float2* hi = lo + 256 * half;
+    const bool sealed = hdr->magic == kMagic && hdr->theta == theta && hdr->n_hi == n_hi && hdr->d == d;   // uniform
+    if (sealed && table_check(lo, hi, n_hi, half, red) == hdr->check) return;
+    const unsigned gen = hdr->gen;
+    __syncthreads();
+    if (threadIdx.x == 0) { hdr->magic = 0; __threadfence(); }        // un-seal before the body changes
+    __syncthreads();
     const long long total = (256 + n_hi) * half;
     for (long long idx = threadIdx.x; idx < total; idx += blockDim.x) {
         const long long row = idx / half;
@@ -67,11 +105,13 @@ __global__ void __launch_bounds__(1024) two_level_kernel(unsigned char* __restri
     }
     __threadfence();
     __syncthreads();
+    const unsigned chk = table_check(lo, hi, n_hi, half, red);
     if (threadIdx.x == 0) {
         hdr->theta = theta;
         hdr->n_hi = n_hi;
         hdr->d = d;
-        hdr->pad = 0;
+        hdr->check = chk;
+        hdr->gen = gen + 1u;
         __threadfence();
         hdr->magic = kMagic;
     }

@@ -70,12 +70,17 @@ def _rope_true_positions(x, pos0, theta, chunk=8192):
     return x
 
 
-def make_qkv(L, H_q, H_kv, d, rope_theta, dtype, seed, outliers=False, device="cpu", q_pos0=0, n_q=None, k_pos0=0):
+def make_qkv(L, H_q, H_kv, d, rope_theta, dtype, seed, outliers=False, device="cpu", q_pos0=0, n_q=None, k_pos0=0,
+             profile=None):
     """Q [n_q,H_q,d], K [L,H_kv,d], V [L,H_kv,d] in `dtype` on `device`.
 
     Q rows sit at absolute positions q_pos0 .. q_pos0+n_q-1 (default: 0..L-1); K rows at k_pos0 .. k_pos0+L-1
     (default 0..L-1; a non-zero k_pos0 is only used by the global-rotation invariance test).
     outliers: 4 seeded channel indices per KV head of the un-rotated x_k are scaled by 8.
+    profile (stress inputs for the precision-margin tests; value distributions only, no method arithmetic):
+      "switch"     the outlier channels change halfway through the sequence (4 channels x8 on rows < L/2, 4 others on the rest)
+      "q_outliers" the 4 loud channels are in the un-rotated x_q (per query head) instead of x_k
+      "loud"       every channel of x_k x1.5 on top of the standard outlier channels
     """
     n_q = L if n_q is None else n_q
     dev = torch.device(device)
@@ -85,10 +90,21 @@ def make_qkv(L, H_q, H_kv, d, rope_theta, dtype, seed, outliers=False, device="c
     xq = torch.randn((n_q, H_q, d), generator=gen, device=dev, dtype=torch.float32).double()
     xk = torch.randn((L, H_kv, d), generator=gen, device=dev, dtype=torch.float32).double()
     v = torch.randn((L, H_kv, d), generator=gen, device=dev, dtype=torch.float32)
-    if outliers:
+    if profile == "switch":
+        for kv in range(H_kv):
+            idx = torch.randperm(d, generator=gen, device=dev)[:8]
+            xk[: L // 2, kv, idx[:4]] *= 8.0
+            xk[L // 2:, kv, idx[4:]] *= 8.0
+    elif profile == "q_outliers":
+        for h in range(H_q):
+            idx = torch.randperm(d, generator=gen, device=dev)[:4]
+            xq[:, h, idx] *= 8.0
+    elif outliers or profile == "loud":
         for kv in range(H_kv):
             idx = torch.randperm(d, generator=gen, device=dev)[:4]
             xk[:, kv, idx] *= 8.0
+        if profile == "loud":
+            xk *= 1.5
     Q = _rope_true_positions(xq, q_pos0, rope_theta).to(td).contiguous()
     del xq
     K = _rope_true_positions(xk, k_pos0, rope_theta).to(td).contiguous()

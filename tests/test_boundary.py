@@ -116,7 +116,36 @@ def test_prefill_variants_validate_before_any_launch():
 
 
 def test_prefill_impl_switch_is_host_state():
-    prev = B.jetlong_set_prefill_impl(2)                  # experimental clusters of four
-    assert B.jetlong_set_prefill_impl(0) == 2
+    prev = B.jetlong_set_prefill_impl(1)                  # the one-tile CTA-pair kernel
+    assert B.jetlong_set_prefill_impl(0) == 1
     assert B.jetlong_set_prefill_impl(-1) == 0
-    assert B.jetlong_set_prefill_impl(prev) == -1
+    assert B.jetlong_set_prefill_impl(2) == -1            # 2, 3: the removed cluster launches, accepted and mean 1
+    assert B.jetlong_set_prefill_impl(prev) == 1
+
+
+def test_setters_are_per_thread_defaults():
+    """The deprecated setters change the CALLING thread's default only (include/jetlong.h: nothing process-global)."""
+    import threading
+    seen = {}
+    prev = B.jetlong_set_prefill_precision(B.PRECISION_FAST)
+
+    def other():
+        seen["before"] = B.jetlong_set_prefill_precision(B.PRECISION_COMPENSATED_E5M2)   # a fresh thread starts at the default
+        seen["after"] = B.jetlong_set_prefill_precision(B.PRECISION_COMPENSATED)
+    th = threading.Thread(target=other)
+    th.start()
+    th.join()
+    assert seen == {"before": B.PRECISION_COMPENSATED, "after": B.PRECISION_COMPENSATED_E5M2}
+    assert B.jetlong_set_prefill_precision(prev) == B.PRECISION_FAST                      # untouched by the other thread
+
+
+def test_options_are_validated_before_any_launch():
+    import ctypes
+    L = B.lib()
+    n0 = B.jetlong_launch_count()
+    bad = B.Options(4, B.DEFAULT, B.DEFAULT)              # struct_bytes too small
+    args = [1 << 12] * 5 + [64, 2, 2, 128, 8, 32, 1e4, B.BF16, 1 << 12, 1 << 20, None]
+    assert L.jetlong_prefill_opt(*args, ctypes.byref(bad)) == B.INVALID_ARG
+    unk = B.Options(ctypes.sizeof(B.Options), 17, B.DEFAULT)   # unknown precision
+    assert L.jetlong_prefill_opt(*args, ctypes.byref(unk)) == B.INVALID_ARG
+    assert B.jetlong_launch_count() == n0

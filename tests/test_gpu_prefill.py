@@ -110,7 +110,7 @@ def test_config2_sampled_rows():
 @pytest.mark.parametrize("L", W.C3_SWEEP_L)
 def test_config3_sweep_sampled_rows(L):
     c = W.C3
-    _sampled(c, L, c.w_local, 512 if L == c.L else 128, what="C3 L=%d" % L)
+    _sampled(c, L, c.w_local, 512, what="C3 L=%d" % L)             # north_star: 512 seeded (row, head) pairs per config
 
 
 @pytest.mark.parametrize("w0,layer", [(2048, 0), (8192, 35)])
@@ -130,16 +130,12 @@ def test_precision_modes_of_the_remote_scores():
     rows, heads = rows[sel], heads[sel]
     ro, rl = oracle_rows(Q, K, V, rows, heads, w_local=w0, w_pretrained=w_pre, rope_theta=theta)
     errs = {}
-    try:
-        for name, mode in (("default", B.PRECISION_COMPENSATED), ("e5m2", B.PRECISION_COMPENSATED_E5M2),
-                           ("f16", B.PRECISION_COMPENSATED_F16), ("fast", B.PRECISION_FAST)):
-            J.jetlong_set_prefill_precision(mode)
-            out, lse = J.jetlong_prefill(Q, K, V, w_local=w0, w_pretrained=w_pre, rope_theta=theta)
-            torch.cuda.synchronize()
-            og, lg = gather(out, lse, rows, heads)
-            errs[name] = (np.abs(og.double().cpu().numpy() - ro).max(), np.abs(lg.double().cpu().numpy() - rl).max())
-    finally:
-        J.jetlong_set_prefill_precision(B.PRECISION_COMPENSATED)
+    for name, mode in (("default", B.PRECISION_COMPENSATED), ("e5m2", B.PRECISION_COMPENSATED_E5M2),
+                       ("f16", B.PRECISION_COMPENSATED_F16), ("fast", B.PRECISION_FAST)):
+        out, lse = J.jetlong_prefill(Q, K, V, w_local=w0, w_pretrained=w_pre, rope_theta=theta, precision=mode)
+        torch.cuda.synchronize()
+        og, lg = gather(out, lse, rows, heads)
+        errs[name] = (np.abs(og.double().cpu().numpy() - ro).max(), np.abs(lg.double().cpu().numpy() - rl).max())
     assert errs["default"][1] <= 1e-3 and errs["e5m2"][1] <= 5e-4 and errs["f16"][1] <= 1e-4, errs
     assert all(e[0] <= 2e-2 for e in errs.values()), errs
     assert errs["fast"][1] <= 1e-2, errs                           # bounded, but it is NOT within the 1e-3 tolerance
@@ -246,24 +242,21 @@ def test_unfused_G1_is_the_control():
     assert torch.equal(out, outc) and torch.equal(lse, lsec)
 
 
-# ---- on-the-fly prefill in clusters of four CTAs sharing rotated K tiles (jetlong_set_prefill_impl 2 / 3; 3 is what the
-# default does from 64 query blocks on) and the CTA-pair kernel alone (impl 1) ---------------------------------------------
+# ---- the implementations behind jetlong_options.prefill_impl: 4 = the two-tile kernel (default), 1 = the one-tile CTA-pair
+# kernel of round 1, 0 = SIMT; shapes that stress the merged visit list of a CTA pair (odd block counts, w0 = 0, G = 5) ------
 @pytest.mark.parametrize("impl,L,H_q,H_kv,w_pre,w0", [
-    (2, 777, 4, 2, 200, 100),        # odd number of query blocks: one cluster has a block-less second pair
-    (2, 640, 8, 2, 320, 128),        # G=2, g=4
-    (2, 1300, 2, 1, 300, 0),         # G=5, w0=0
-    (2, 4096, 4, 2, 1024, 128),      # 32 query blocks, long shared phases
-    (3, 8320, 4, 2, 2048, 256),      # 65 query blocks: clusters for the top 46, CTA pairs for the lightest 19, G=5
-    (1, 8320, 4, 2, 2048, 256),      # the same through CTA pairs only
+    (4, 777, 4, 2, 200, 100),        # odd number of query blocks: the last CTA pair has no second tile
+    (4, 640, 8, 2, 320, 128),        # G=2, g=4
+    (4, 1300, 2, 1, 300, 0),         # G=5, w0=0
+    (4, 4096, 4, 2, 1024, 128),      # 32 query blocks, long remote phases
+    (4, 8320, 4, 2, 2048, 256),      # 65 query blocks, G=5
+    (1, 8320, 4, 2, 2048, 256),      # the same through the one-tile kernel
+    (0, 1300, 2, 1, 300, 0),         # and through the SIMT tiles
 ])
-def test_cluster_of_four_sharing_matches_oracle(impl, L, H_q, H_kv, w_pre, w0):
+def test_prefill_implementations_match_oracle(impl, L, H_q, H_kv, w_pre, w0):
     Q, K, V = W.make_qkv(L, H_q, H_kv, 128, 1e6, "bf16", 9753 + L, True, DEV)
-    try:
-        J.jetlong_set_prefill_impl(impl)
-        out, lse = J.jetlong_prefill(Q, K, V, w_local=w0, w_pretrained=w_pre, rope_theta=1e6)
-        torch.cuda.synchronize()
-    finally:
-        J.jetlong_set_prefill_impl(-1)
+    out, lse = J.jetlong_prefill(Q, K, V, w_local=w0, w_pretrained=w_pre, rope_theta=1e6, impl=impl)
+    torch.cuda.synchronize()
     rows, heads = all_pairs(L, H_q)
     if L > 2000:
         pick = np.random.RandomState(2).choice(len(rows), 2048, replace=False)
