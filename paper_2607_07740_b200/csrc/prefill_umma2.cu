@@ -53,7 +53,7 @@ constexpr int W_SOFTMAX = 4, W_KLOAD = 12, W_VLOAD = 13, W_MMA = 15;   // warps 
 constexpr uint32_t TM_S = 0, TM_O = 256;
 // setmaxnreg.inc draws only on what other warps of the CTA released (registers left unallocated at launch are not in the
 // pool): the split must balance against 4 warpgroups x 128, or the last group to grow waits forever
-constexpr int REGS_ROT = 128, REGS_SOFTMAX = 160, REGS_MISC = 64;
+constexpr int REGS_ROT = 112, REGS_SOFTMAX = 160, REGS_MISC = 80;
 static_assert(REGS_ROT + 2 * REGS_SOFTMAX + REGS_MISC == 512, "register file split");
 
 // ---- optional cycle trace of one CTA (build with -DJL_TRACE; read back with jetlong_debug_trace) ----------------
@@ -462,6 +462,7 @@ prefill_umma2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_const
         }
     } else if (warp < 4) {
         // ===================== rotate group (steps a4, a5) =====================
+        reg_dec<REGS_ROT>();
         mbar_wait_sleep(&bars->q_full, 0);
         if (lane == 0) mbar_arrive_leader(&bars->q_ready);
         const bool rotating = mp.n_rem > 0 && !p.prerot;
