@@ -44,6 +44,8 @@ def lib():
         L.jlo_attend_rows.argtypes = [vp, vp, vp, i64, i32, i32, i32, i64, i64, dbl, i32, i64, i64, vp, vp, vp, vp, vp]
         L.jlo_three_call_rows.restype = i32
         L.jlo_three_call_rows.argtypes = [vp, vp, vp, i64, i32, i32, i32, i64, i64, dbl, i64, vp, vp, vp, vp, vp]
+        L.jlo_attend_rows_freq.restype = i32
+        L.jlo_attend_rows_freq.argtypes = [vp, vp, vp, i64, i32, i32, i32, i64, i64, dbl, dbl, dbl, i64, i64, vp, vp, vp, vp]
         L.jlo_scores_row.restype = i32
         L.jlo_scores_row.argtypes = [vp, vp, i64, i32, i32, i32, i64, i64, dbl, i32, i64, vp]
         _lib = L
@@ -122,6 +124,30 @@ def attend_rows(Q, K, V, rows, heads, *, w_local, w_pretrained, rope_theta, mode
                                _p(rows), _p(heads), _p(Ls) if Ls is not None else None, _p(out), _p(lse))
     if rc != 0:
         raise ValueError("jlo_attend_rows: bad arguments")
+    return out, lse
+
+
+def attend_rows_freq(Q, K, V, rows, heads, *, w_local, w_pretrained, rope_theta, alpha=1.0, beta=32.0, pos_shift=0,
+                     q_is_compact=False):
+    """The frequency-interpolation remote map (R17): out[n,d], lse[n] (float64)."""
+    K = _f32(K)
+    V = _f32(V)
+    L, H_kv, d = K.shape
+    rows, heads = _rows_heads(rows, heads)
+    if q_is_compact:
+        Qrows, H_q = Q
+        Qrows = _f32(Qrows)
+    else:
+        H_q = Q.shape[1]
+        Qrows = _f32(np.asarray(Q)[rows, heads])
+    n = rows.shape[0]
+    out = np.empty((n, d), dtype=np.float64)
+    lse = np.empty((n,), dtype=np.float64)
+    rc = lib().jlo_attend_rows_freq(_p(Qrows), _p(K), _p(V), L, H_q, H_kv, d, int(w_local), int(w_pretrained),
+                                    float(rope_theta), float(alpha), float(beta), int(pos_shift), n, _p(rows), _p(heads),
+                                    _p(out), _p(lse))
+    if rc != 0:
+        raise ValueError("jlo_attend_rows_freq: bad arguments")
     return out, lse
 
 

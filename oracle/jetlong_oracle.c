@@ -23,6 +23,9 @@
  * closed-form cosine-sum scores for Eq.(1); Q=0 / constant-V softmax plumbing;
  * w0=0 and w0>=L-1 window edges; shift invariance; within-group aliasing
  * (P:220); brute force in pure Python on tiny inputs.
+ * jlo_attend_rows_freq (frequency-interpolation map, a DEFINITION of this repository, R17): pinned by G=1 == causal,
+ * gamma=1 == causal, gamma=0 == brute-force position interpolation, shift invariance for every shift, a from-scratch
+ * complex-number route from the un-rotated inputs; "parity unpinned" against the paper, which prints no formula for it.
  * Not pinned by the paper: absolute output values (none are printed) and the RoPE
  * pairing convention (R5) -- "parity unpinned" for those two points only.
  */
@@ -249,4 +252,76 @@ int jlo_scores_row(const float* Qrow, const float* K, int64_t L, int H_kv, int k
     }
     free(buf);
     return 0;
+}
+
+/*
+ * the "YaRN-style frequency interpolation" remote map "within the same bifocal
+ * construction".  The paper prints no formula; reading R17 fixes it as NTK-by-parts (YaRN) with scale s = G:
+ *   rotations of pair i inside the pretrained window   r_i = w_pre * theta_i / (2 pi)
+ *   ramp                                               gamma_i = clamp((r_i - alpha) / (beta - alpha), 0, 1)
+ *   remote frequency                                   theta'_i = theta_i * ((1 - gamma_i) / G + gamma_i)
+ * and the remote branch of Eq.(1) scores RoPE at the TRUE positions with theta' instead of theta:
+ *   s(q,k) = scale * <RoPE_theta'(x_q, q), RoPE_theta'(x_k, k)>                      if q-k > w0.
+ * On the stored operands (RoPE_theta at true positions, Eq.(4)) that is the correction rotation of pair i by the
+ * angle -x * phi_i, phi_i = theta_i - theta'_i = theta_i (1 - gamma_i)(1 - 1/G), x = the absolute position -- the analogue
+ * of Eq.(6) with a per-frequency, non-integer Delta_i(x) = -x (1 - gamma_i)(1 - 1/G).  No extra temperature (R10).
+ * G = 1 gives phi = 0 (the control); gamma = 1 everywhere gives the control; gamma = 0 everywhere is position
+ * interpolation x -> x / G, which agrees with aliasing (Eq.(3)) at multiples of G.
+ * Same layouts and conventions as jlo_attend_rows (mode is always bifocal).
+ */
+int jlo_attend_rows_freq(const float* Qrows, const float* K, const float* V,
+                         int64_t L, int H_q, int H_kv, int d,
+                         int64_t w0, int64_t w_pre, double theta, double alpha, double beta, int64_t pos_shift,
+                         int64_t n, const int64_t* rows, const int32_t* heads,
+                         double* out, double* lse) {
+    if (L < 1 || H_q < 1 || H_kv < 1 || H_q % H_kv || d < 2 || (d & 1) || w0 < 0 || w_pre < 1 ||
+        !(theta > 0.0) || n < 0 || !(beta > alpha) || d / 2 > 4096) return -1;
+    const int64_t G = jlo_group_size(L, w_pre);
+    const int g = H_q / H_kv, hd = d / 2;
+    const double scale = 1.0 / sqrt((double)d);
+    const double two_pi = 6.283185307179586476925286766559;
+    double phi[4096];
+    for (int i = 0; i < hd; ++i) {
+        const double th = freq(theta, d, i);
+        const double r = (double)w_pre * th / two_pi;
+        double gam = (r - alpha) / (beta - alpha);
+        gam = gam < 0.0 ? 0.0 : (gam > 1.0 ? 1.0 : gam);
+        phi[i] = th * (1.0 - gam) * (1.0 - 1.0 / (double)G);
+    }
+    int bad = 0;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t j = 0; j < n; ++j) {
+        const int64_t q = rows[j];
+        const int h = heads[j];
+        if (q < 0 || q >= L || h < 0 || h >= H_q) { bad = 1; continue; }
+        const int kv = h / g;
+        double* buf = (double*)malloc(sizeof(double) * d * 4);
+        double *qloc = buf, *qrem = buf + d, *kd = buf + 2 * d, *krem = buf + 3 * d;
+        double* s = (double*)malloc(sizeof(double) * (q + 1));
+        const float** vrow = (const float**)malloc(sizeof(float*) * (q + 1));
+        for (int c = 0; c < d; ++c) qloc[c] = (double)Qrows[j * d + c];
+        for (int i = 0; i < hd; ++i) {                                  /* correction of the query: angle -(q) phi_i */
+            const double a = -(double)(q + pos_shift) * phi[i], c = cos(a), sn = sin(a);
+            qrem[i] = qloc[i] * c - qloc[i + hd] * sn;
+            qrem[i + hd] = qloc[i] * sn + qloc[i + hd] * c;
+        }
+        for (int64_t k = 0; k <= q; ++k) {
+            const float* kp = K + ((size_t)k * H_kv + kv) * d;
+            for (int c = 0; c < d; ++c) kd[c] = (double)kp[c];
+            if (q - k <= w0) {
+                s[k] = scale * dotd(qloc, kd, d);                        /* Eq.(1), first case, unchanged */
+            } else {
+                for (int i = 0; i < hd; ++i) {                          /* correction of the key: angle -(k) phi_i */
+                    const double a = -(double)(k + pos_shift) * phi[i], c = cos(a), sn = sin(a);
+                    krem[i] = kd[i] * c - kd[i + hd] * sn;
+                    krem[i + hd] = kd[i] * sn + kd[i + hd] * c;
+                }
+                s[k] = scale * dotd(qrem, krem, d);
+            }
+            vrow[k] = V + ((size_t)k * H_kv + kv) * d;
+        }
+        softmax_pv(s, vrow, q + 1, d, out + j * d, lse + j);
+        free(buf); free(s); free((void*)vrow);
+    }
+    return bad ? -1 : 0;
 }

@@ -51,3 +51,23 @@ def test_llama3_shaped_G16_decode():
 def test_256k_native_512k_prefill(fn):
     assert J.jetlong_group_size(524288, 262144) == 2
     _sampled(fn, 524288, 4, 2, 1e6, 262144, 4096, 7740803, 48, "256K-native G=2 L=524288")
+
+
+def test_256k_native_1m_prefill_and_decode():
+    """Table 3: the 256K-native model at L = 1048576 -> G = 4, the longest length the paper reports.  One CTA pair walks
+    8192 key tiles; the rotation table reaches n = 786432.  Prefill on sampled rows, then one decode step at the same L."""
+    import numpy as np
+    L, H_q, H_kv, theta, w_pre, w0 = 1048576, 2, 1, 1e6, 262144, 4096
+    assert J.jetlong_group_size(L, w_pre) == 4
+    Q, K, V = W.make_qkv(L, H_q, H_kv, 128, theta, "bf16", 7740804, True, DEV)
+    out, lse = J.jetlong_prefill(Q, K, V, w_local=w0, w_pretrained=w_pre, rope_theta=theta)
+    torch.cuda.synchronize()
+    rows, heads = W.sample_pairs(L, H_q, 24, 7740804, w0, 4)
+    ro, rl = oracle_rows(Q, K, V, rows, heads, w_local=w0, w_pretrained=w_pre, rope_theta=theta)
+    check(*gather(out, lse, rows, heads), ro, rl, Q.dtype, "256K-native G=4 L=1048576")
+    od, ld = J.jetlong_decode(Q[L - 1].contiguous(), K, V, L, w_local=w0, w_pretrained=w_pre, rope_theta=theta)
+    torch.cuda.synchronize()
+    hh = np.arange(H_q, dtype=np.int32)
+    rr = np.full(H_q, L - 1, dtype=np.int64)
+    do, dl = oracle_rows(Q, K, V, rr, hh, w_local=w0, w_pretrained=w_pre, rope_theta=theta)
+    check(od, ld, do, dl, Q.dtype, "256K-native G=4 decode at L=1048576")

@@ -319,3 +319,90 @@ def test_bad_arguments_are_rejected():
         oracle.attend_rows(K, K, K, [1], [0], w_local=-1, w_pretrained=2, rope_theta=1e4)
     assert oracle.group_size(0, 5) == -1
     assert oracle.num_threads() >= 1
+
+
+# ---------------------------------------------------------------- frequency-interpolation remote map (R17)
+def _yarn_theta_prime(theta, d, w_pre, G, alpha=1.0, beta=32.0):
+    """theta'_i of the definition, written out independently of the C code."""
+    out = []
+    for i in range(d // 2):
+        th = theta ** (-2.0 * i / d)
+        r = w_pre * th / (2.0 * math.pi)
+        gam = min(1.0, max(0.0, (r - alpha) / (beta - alpha)))
+        out.append(th * ((1.0 - gam) / G + gam))
+    return out
+
+
+def test_freq_map_from_scratch_complex_bruteforce():
+    # the definition literally: remote scores = RoPE with theta' applied FROM SCRATCH to the content vectors at the TRUE
+    # positions; the oracle goes the other way (stored theta-rotated operands + per-frequency correction angle)
+    L, H_q, H_kv, d, theta, w_pre, w0 = 40, 4, 2, 8, 50.0, 9, 3
+    xq, xk, v = _raw_inputs(L, H_q, H_kv, d, 21)
+    Q = _rope_np(xq, np.arange(L), theta)
+    K = _rope_np(xk, np.arange(L), theta)
+    rows = np.repeat(np.arange(L), H_q)
+    heads = np.tile(np.arange(H_q, dtype=np.int32), L)
+    alpha, beta = 0.1, 0.9                     # a ramp that puts some of the 4 frequencies in each regime at this tiny size
+    out, lse = oracle.attend_rows_freq(Q, K, v, rows, heads, w_local=w0, w_pretrained=w_pre, rope_theta=theta,
+                                       alpha=alpha, beta=beta)
+    G = -(-L // w_pre)
+    h = d // 2
+    th = [theta ** (-2.0 * i / d) for i in range(h)]
+    thp = _yarn_theta_prime(theta, d, w_pre, G, alpha, beta)
+    assert any(abs(a - b) < 1e-15 for a, b in zip(th, thp)) and any(abs(a / G - b) < 1e-15 for a, b in zip(th, thp))
+    Q32, K32, V32 = Q.astype(np.float32), K.astype(np.float32), v.astype(np.float32)
+    for j, (q, hq) in enumerate(zip(rows, heads)):
+        kv = hq // (H_q // H_kv)
+        s = []
+        for k in range(q + 1):
+            acc = 0.0
+            for i in range(h):
+                zq = complex(Q32[q, hq, i], Q32[q, hq, i + h]) * cmath.exp(-1j * q * th[i])       # content vectors
+                zk = complex(K32[k, kv, i], K32[k, kv, i + h]) * cmath.exp(-1j * k * th[i])
+                f = th[i] if q - k <= w0 else thp[i]
+                acc += (zq * cmath.exp(1j * q * f) * (zk * cmath.exp(1j * k * f)).conjugate()).real
+            s.append(acc / math.sqrt(d))
+        m = max(s)
+        p = [math.exp(t - m) for t in s]
+        l = sum(p)
+        o = [sum(p[k] * float(V32[k, kv, c]) for k in range(q + 1)) / l for c in range(d)]
+        assert np.allclose(out[j], o, atol=1e-12)
+        assert abs(lse[j] - (m + math.log(l))) < 1e-12
+
+
+def test_freq_map_special_cases():
+    L, H_q, H_kv, d, theta, w0 = 60, 2, 1, 16, 1e4, 5
+    xq, xk, v = _raw_inputs(L, H_q, H_kv, d, 22)
+    Q = _rope_np(xq, np.arange(L), theta).astype(np.float32)
+    K = _rope_np(xk, np.arange(L), theta).astype(np.float32)
+    rows = np.repeat(np.arange(L), H_q)
+    heads = np.tile(np.arange(H_q, dtype=np.int32), L)
+    ctrl = oracle.attend_rows(Q, K, v, rows, heads, w_local=w0, w_pretrained=16, rope_theta=theta, mode="causal")
+    # G = 1: phi = 0, the map is the identity -> the control, bit for bit (cos 0 = 1, sin 0 = 0)
+    g1 = oracle.attend_rows_freq(Q, K, v, rows, heads, w_local=w0, w_pretrained=L, rope_theta=theta)
+    assert np.array_equal(g1[0], ctrl[0]) and np.array_equal(g1[1], ctrl[1])
+    # gamma = 1 for every frequency (ramp far below every r_i): nothing is interpolated -> the control
+    hi = oracle.attend_rows_freq(Q, K, v, rows, heads, w_local=w0, w_pretrained=16, rope_theta=theta, alpha=-2e9, beta=-1e9)
+    assert np.array_equal(hi[0], ctrl[0]) and np.array_equal(hi[1], ctrl[1])
+    # gamma = 0 for every frequency: position interpolation x -> x / G; with every pair of x_q, x_k equal to (1, 0) the
+    # remote score is the closed form sum_i cos((q - k) theta_i / G) / sqrt(d), the local one sum_i cos((q - k) theta_i)
+    ones = np.zeros((L, 1, d)); ones[..., : d // 2] = 1.0
+    Q1 = _rope_np(ones, np.arange(L), theta).astype(np.float32)
+    K1 = _rope_np(ones, np.arange(L), theta).astype(np.float32)
+    V1 = np.zeros((L, 1, d), dtype=np.float32)
+    q = L - 1
+    w_pre = 16
+    G = -(-L // w_pre)
+    o, lse = oracle.attend_rows_freq(Q1, K1, V1, [q], [0], w_local=w0, w_pretrained=w_pre, rope_theta=theta, alpha=1e30, beta=2e30)
+    th = theta ** (-2.0 * np.arange(d // 2) / d)
+    s = [(np.cos((q - k) * th).sum() if q - k <= w0 else np.cos((q - k) * th / G).sum()) / math.sqrt(d) for k in range(q + 1)]
+    assert abs(lse[0] - math.log(sum(math.exp(t) for t in s))) < 1e-5          # fp32 rounding of the generated inputs
+    # interpolation keeps RELATIVE positions: a global shift of every position by ANY c changes nothing
+    # (aliasing is invariant only for c divisible by G, test_shift_invariance)
+    base = oracle.attend_rows_freq(Q, K, v, rows, heads, w_local=w0, w_pretrained=16, rope_theta=theta)
+    for c in (1, 7, 1000):
+        sh = oracle.attend_rows_freq(Q, K, v, rows, heads, w_local=w0, w_pretrained=16, rope_theta=theta, pos_shift=c)
+        assert np.abs(sh[0] - base[0]).max() < 1e-9 and np.abs(sh[1] - base[1]).max() < 1e-9
+    # and it differs from aliasing and from the control on these inputs
+    ali = oracle.attend_rows(Q, K, v, rows, heads, w_local=w0, w_pretrained=16, rope_theta=theta)
+    assert np.abs(base[1] - ali[1]).max() > 1e-3 and np.abs(base[1] - ctrl[1]).max() > 1e-3
