@@ -157,7 +157,21 @@ typedef struct {
     uint32_t struct_bytes;
     int precision;      /* a JETLONG_PRECISION_* value or JETLONG_DEFAULT */
     int prefill_impl;   /* -1 / 4: tcgen05 two-tile kernel (default); 1: tcgen05 one-tile CTA pairs; 0: SIMT fp32; or JETLONG_DEFAULT */
+    int remote_map;     /* JETLONG_MAP_ALIAS (0, the paper's method and the default) or JETLONG_MAP_FREQ_INTERP */
+    double yarn_alpha;  /* ramp of JETLONG_MAP_FREQ_INTERP; 0, 0 = the YaRN defaults alpha = 1, beta = 32 */
+    double yarn_beta;
 } jetlong_options;
+
+/* Remote map (Section 4.7, Table 6: "position aliasing (default Jet-Long) vs. YaRN-style frequency interpolation
+ * within the same bifocal construction").  JETLONG_MAP_ALIAS is Eq.(3): remote position floor(x / G).
+ * JETLONG_MAP_FREQ_INTERP is this library's DEFINITION of the ablation (the paper prints no formula; R17):
+ * keys older than w_local score with RoPE at their TRUE positions but with the NTK-by-parts frequencies
+ *     theta'_i = theta_i ((1 - gamma_i) / G + gamma_i),   gamma_i = clamp((w_pretrained theta_i / 2 pi - alpha) / (beta - alpha), 0, 1),
+ * i.e. the stored operands are corrected by rotating pair i by -x (theta_i - theta'_i) at absolute position x; no extra
+ * attention temperature (R10).  G = 1 is still the control.  Everything else (window rule, one joint softmax, cache
+ * never written, precision modes) is unchanged.  Prefill (jetlong_prefill_opt, jetlong_prefill_prerotated_opt) and
+ * decode (jetlong_decode_opt) accept it; the unfused baseline is aliasing only. */
+enum { JETLONG_MAP_ALIAS = 0, JETLONG_MAP_FREQ_INTERP = 1 };
 
 /* jetlong_prefill / jetlong_prefill_prerotated with explicit options; identical otherwise. */
 int jetlong_prefill_opt(const void* Q, const void* K, const void* V, void* out, float* lse,
@@ -170,6 +184,13 @@ int jetlong_prefill_prerotated_opt(const void* Q, const void* K, const void* V, 
                                    int64_t w_local, int64_t w_pretrained, double rope_theta,
                                    int dtype, void* workspace, size_t workspace_bytes, void* stream,
                                    const jetlong_options* options);
+
+/* jetlong_decode with explicit options (only remote_map and the ramp are used). */
+int jetlong_decode_opt(const void* q, const void* Kcache, const void* Vcache, void* out, float* lse,
+                       int64_t L, int H_q, int H_kv, int head_dim,
+                       int64_t w_local, int64_t w_pretrained, double rope_theta,
+                       int dtype, void* workspace, size_t workspace_bytes, void* stream,
+                       const jetlong_options* options);
 
 /* DEPRECATED (kept as shims): set the CALLING THREAD's default prefill implementation.
  * -1 or 4 (default): tcgen05 UMMA where supported (bf16, head_dim 128, even H_q / H_kv): the two-tile kernel, in which a

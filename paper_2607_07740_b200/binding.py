@@ -23,19 +23,25 @@ EXPORTS = ["jetlong_group_size", "jetlong_workspace_bytes", "jetlong_prefill", "
            "jetlong_causal_prefill", "jetlong_causal_decode", "jetlong_prefill_host", "jetlong_status_string",
            "jetlong_launch_count", "jetlong_set_prefill_impl", "jetlong_prefill_uses_umma",
            "jetlong_set_prefill_precision", "jetlong_prefill_prerotated", "jetlong_prefill_unfused",
-           "jetlong_prefill_opt", "jetlong_prefill_prerotated_opt", "jetlong_host_release"]
+           "jetlong_prefill_opt", "jetlong_prefill_prerotated_opt", "jetlong_host_release", "jetlong_decode_opt"]
 DEFAULT = -2                                              # JETLONG_DEFAULT: take the calling thread's default
 
 
 class Options(ctypes.Structure):
     """jetlong_options (include/jetlong.h): per-call precision / implementation."""
-    _fields_ = [("struct_bytes", ctypes.c_uint32), ("precision", ctypes.c_int), ("prefill_impl", ctypes.c_int)]
+    _fields_ = [("struct_bytes", ctypes.c_uint32), ("precision", ctypes.c_int), ("prefill_impl", ctypes.c_int),
+                ("remote_map", ctypes.c_int), ("yarn_alpha", ctypes.c_double), ("yarn_beta", ctypes.c_double)]
 
 
-def _options(precision, impl):
-    if precision is None and impl is None:
+MAP_ALIAS, MAP_FREQ_INTERP = 0, 1
+
+
+def _options(precision=None, impl=None, remote_map=None, yarn=None):
+    if precision is None and impl is None and remote_map is None and yarn is None:
         return None
-    o = Options(ctypes.sizeof(Options), DEFAULT if precision is None else int(precision), DEFAULT if impl is None else int(impl))
+    a, b = (0.0, 0.0) if yarn is None else (float(yarn[0]), float(yarn[1]))
+    o = Options(ctypes.sizeof(Options), DEFAULT if precision is None else int(precision), DEFAULT if impl is None else int(impl),
+                DEFAULT if remote_map is None else int(remote_map), a, b)
     return ctypes.byref(o)
 
 
@@ -70,6 +76,8 @@ def lib():
         L.jetlong_prefill_prerotated_opt.restype = i32
         L.jetlong_prefill_prerotated_opt.argtypes = [vp] * 5 + tail + [vp]
         L.jetlong_host_release.restype = None
+        L.jetlong_decode_opt.restype = i32
+        L.jetlong_decode_opt.argtypes = [vp] * 5 + tail + [vp]
         L.jetlong_decode.restype = i32
         L.jetlong_decode.argtypes = [vp] * 5 + tail
         ctail = [i64, i32, i32, i32, i32, vp, sz, vp]
@@ -147,7 +155,7 @@ def _prefill_args(Q, K, V, out, lse):
 
 
 def jetlong_prefill(Q, K, V, *, w_local, w_pretrained, rope_theta, out=None, lse=None, workspace=None, precision=None,
-                    impl=None):
+                    impl=None, remote_map=None, yarn=None):
     """Bifocal prefill.  Q [L,H_q,d], K/V [L,H_kv,d] (bf16 or fp32, RoPE'd at true positions).  Returns out, lse.
     precision / impl: per-call jetlong_options (None = the thread's default)."""
     L, H_q, H_kv, d, out, lse = _prefill_args(Q, K, V, out, lse)
@@ -156,12 +164,13 @@ def jetlong_prefill(Q, K, V, *, w_local, w_pretrained, rope_theta, out=None, lse
         workspace = alloc_workspace(OP_PREFILL, L, H_q, H_kv, d, dt, Q.device)
     _check(lib().jetlong_prefill_opt(Q.data_ptr(), K.data_ptr(), V.data_ptr(), out.data_ptr(), lse.data_ptr(), L, H_q,
                                      H_kv, d, int(w_local), int(w_pretrained), float(rope_theta), dt,
-                                     workspace.data_ptr(), workspace.numel(), _stream(), _options(precision, impl)))
+                                     workspace.data_ptr(), workspace.numel(), _stream(),
+                                     _options(precision, impl, remote_map, yarn)))
     return out, lse
 
 
 def jetlong_prefill_prerotated(Q, K, V, *, w_local, w_pretrained, rope_theta, out=None, lse=None, workspace=None,
-                               precision=None, impl=None):
+                               precision=None, impl=None, remote_map=None, yarn=None):
     """Workspace variant of the bifocal prefill: K is correction-rotated once into a scratch in the workspace."""
     L, H_q, H_kv, d, out, lse = _prefill_args(Q, K, V, out, lse)
     dt = _dt(Q)
@@ -170,7 +179,7 @@ def jetlong_prefill_prerotated(Q, K, V, *, w_local, w_pretrained, rope_theta, ou
     _check(lib().jetlong_prefill_prerotated_opt(Q.data_ptr(), K.data_ptr(), V.data_ptr(), out.data_ptr(), lse.data_ptr(),
                                                 L, H_q, H_kv, d, int(w_local), int(w_pretrained), float(rope_theta), dt,
                                                 workspace.data_ptr(), workspace.numel(), _stream(),
-                                                _options(precision, impl)))
+                                                _options(precision, impl, remote_map, yarn)))
     return out, lse
 
 
@@ -209,15 +218,17 @@ def _decode_args(q, Kc, Vc, L, out, lse):
     return H_q, H_kv, d, out, lse
 
 
-def jetlong_decode(q, Kcache, Vcache, L, *, w_local, w_pretrained, rope_theta, out=None, lse=None, workspace=None):
+def jetlong_decode(q, Kcache, Vcache, L, *, w_local, w_pretrained, rope_theta, out=None, lse=None, workspace=None,
+                   remote_map=None, yarn=None):
     """Bifocal decode of the query at position L-1 against cache rows 0..L-1.  q [H_q,d]."""
     H_q, H_kv, d, out, lse = _decode_args(q, Kcache, Vcache, L, out, lse)
     dt = _dt(q)
     if workspace is None:
         workspace = alloc_workspace(OP_DECODE, L, H_q, H_kv, d, dt, q.device)
-    _check(lib().jetlong_decode(q.data_ptr(), Kcache.data_ptr(), Vcache.data_ptr(), out.data_ptr(), lse.data_ptr(),
-                                int(L), H_q, H_kv, d, int(w_local), int(w_pretrained), float(rope_theta), dt,
-                                workspace.data_ptr(), workspace.numel(), _stream()))
+    _check(lib().jetlong_decode_opt(q.data_ptr(), Kcache.data_ptr(), Vcache.data_ptr(), out.data_ptr(), lse.data_ptr(),
+                                    int(L), H_q, H_kv, d, int(w_local), int(w_pretrained), float(rope_theta), dt,
+                                    workspace.data_ptr(), workspace.numel(), _stream(),
+                                    _options(remote_map=remote_map, yarn=yarn)))
     return out, lse
 
 

@@ -18,16 +18,23 @@ static bool precision_known(int m) {
     return m == JETLONG_PRECISION_COMPENSATED || m == JETLONG_PRECISION_FAST || m == JETLONG_PRECISION_COMPENSATED_F16 ||
            m == JETLONG_PRECISION_COMPENSATED_E5M2;
 }
-struct Resolved { int precision, impl; bool ok; };
+struct Resolved { int precision, impl, map; double alpha, beta; bool ok; };
 static Resolved resolve(const jetlong_options* opt) {
-    Resolved r{t_prefill_precision, t_prefill_impl, true};
+    Resolved r{t_prefill_precision, t_prefill_impl, JETLONG_MAP_ALIAS, 1.0, 32.0, true};
     if (opt) {
         if (opt->struct_bytes < sizeof(jetlong_options)) { r.ok = false; return r; }
         if (opt->precision != JETLONG_DEFAULT) r.precision = opt->precision;
         if (opt->prefill_impl != JETLONG_DEFAULT) r.impl = opt->prefill_impl;
+        if (opt->remote_map != JETLONG_DEFAULT) r.map = opt->remote_map;
+        if (opt->yarn_alpha != 0.0 || opt->yarn_beta != 0.0) { r.alpha = opt->yarn_alpha; r.beta = opt->yarn_beta; }
     }
-    r.ok = precision_known(r.precision) && r.impl >= -1 && r.impl <= 4;
+    r.ok = precision_known(r.precision) && r.impl >= -1 && r.impl <= 4 &&
+           (r.map == JETLONG_MAP_ALIAS || r.map == JETLONG_MAP_FREQ_INTERP) && r.beta > r.alpha;
     return r;
+}
+static FreqMap make_map(const Resolved& o, long long G, long long w_pre) {
+    if (o.map != JETLONG_MAP_FREQ_INTERP) return alias_map();
+    return FreqMap{1, 1.0 - 1.0 / (double)G, (double)w_pre, o.alpha, o.beta};
 }
 
 void note_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
@@ -48,7 +55,7 @@ int launch_prefill_unfused(const void* Q, const void* K, const void* V, void* ou
                            int H_kv, int d, long long w0, long long G, double theta, void* ws, cudaStream_t st);
 int launch_prefill_umma(const void* Q, const void* K, const void* V, void* out, float* lse, long long L, int H_q,
                         int H_kv, int d, long long w0, long long G, double theta, bool bifocal, int precise, void* ws,
-                        size_t ws_bytes, cudaStream_t st, bool prerot, bool two_tile);
+                        size_t ws_bytes, cudaStream_t st, bool prerot, bool two_tile, FreqMap fm);
 
 static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; }
 
@@ -103,14 +110,16 @@ static int prefill_common(const void* Q, const void* K, const void* V, void* out
     if (rc != JETLONG_OK) return rc;
     cudaStream_t st = (cudaStream_t)stream;
     const int prec = o.precision;
+    const FreqMap fm = bifocal ? make_map(o, G, w_pre) : alias_map();
+    if (fm.interp) G = kInterpG;                         // the kernels' form of the map: n = -Delta = x (common.cuh)
     if (prerot || use_umma(o.impl, L, H_q, H_kv, d, dtype))
         return launch_prefill_umma(Q, K, V, out, lse, L, H_q, H_kv, d, w0, G, theta, bifocal,
                                    prec == JETLONG_PRECISION_FAST ? 0 : prec == JETLONG_PRECISION_COMPENSATED_F16 ? 1 : prec == JETLONG_PRECISION_COMPENSATED_E5M2 ? 6 : 2,
                                    ws, ws_bytes, st,
-                                   prerot && bifocal, /*two_tile=*/o.impl != 1);
+                                   prerot && bifocal, /*two_tile=*/o.impl != 1, fm);
     const float2* tab = nullptr;
     if (bifocal) {
-        rc = build_key_table((float2*)ws, L, G, d, theta, st);
+        rc = build_key_table((float2*)ws, L, G, d, theta, st, fm);
         if (rc != JETLONG_OK) return rc;
         tab = (const float2*)ws;
     }
@@ -119,17 +128,21 @@ static int prefill_common(const void* Q, const void* K, const void* V, void* out
 
 static int decode_common(const void* q, const void* K, const void* V, void* out, float* lse, long long L, int H_q,
                          int H_kv, int d, long long w0, long long w_pre, double theta, int dtype, void* ws,
-                         size_t ws_bytes, void* stream, bool bifocal) {
+                         size_t ws_bytes, void* stream, bool bifocal, const jetlong_options* opt = nullptr) {
     int rc = validate(q, K, V, out, lse, L, H_q, H_kv, d, w0, w_pre, theta, dtype);
     if (rc != JETLONG_OK) return rc;
+    const Resolved o = resolve(opt);
+    if (!o.ok) return JETLONG_INVALID_ARG;
     long long G = bifocal ? jetlong_group_size(L, w_pre) : 1;
     if (G == 1 || w0 >= L - 1) bifocal = false;
+    const FreqMap fm = bifocal ? make_map(o, G, w_pre) : alias_map();
+    if (fm.interp) G = kInterpG;
     const size_t need = decode_workspace_bytes(L, H_q, H_kv, d);
     if (!ws || ws_bytes < need || !aligned16(ws)) return JETLONG_INVALID_ARG;
     rc = device_ok();
     if (rc != JETLONG_OK) return rc;
     return launch_decode(q, K, V, out, lse, L, H_q, H_kv, d, w0, G, theta, dtype, bifocal, ws, ws_bytes,
-                         (cudaStream_t)stream);
+                         (cudaStream_t)stream, fm);
 }
 
 }  // namespace jetlong
@@ -217,6 +230,13 @@ int jetlong_decode(const void* q, const void* Kcache, const void* Vcache, void* 
                    void* workspace, size_t workspace_bytes, void* stream) {
     return decode_common(q, Kcache, Vcache, out, lse, L, H_q, H_kv, head_dim, w_local, w_pretrained, rope_theta, dtype,
                          workspace, workspace_bytes, stream, true);
+}
+
+int jetlong_decode_opt(const void* q, const void* Kcache, const void* Vcache, void* out, float* lse, int64_t L, int H_q,
+                       int H_kv, int head_dim, int64_t w_local, int64_t w_pretrained, double rope_theta, int dtype,
+                       void* workspace, size_t workspace_bytes, void* stream, const jetlong_options* options) {
+    return decode_common(q, Kcache, Vcache, out, lse, L, H_q, H_kv, head_dim, w_local, w_pretrained, rope_theta, dtype,
+                         workspace, workspace_bytes, stream, true, options);
 }
 
 int jetlong_causal_decode(const void* q, const void* Kcache, const void* Vcache, void* out, float* lse, int64_t L,

@@ -394,12 +394,12 @@ size_t decode_workspace_bytes(long long L, int H_q, int H_kv, int d) {
 template <typename T, int D>
 static int launch_decode_td(const void* q, const void* K, const void* V, void* out, float* lse, long long L,
                             int H_q, int H_kv, long long w0, long long G, double theta, bool bifocal, void* ws,
-                            cudaStream_t st) {
+                            cudaStream_t st, FreqMap fm) {
     Plan pl = make_plan(L, H_q, H_kv);
     unsigned char* base = (unsigned char*)ws;
     const size_t tb = two_level_bytes(L, D);
     if (bifocal) {
-        int rc = build_two_level(base, L, D, theta, st);
+        int rc = build_two_level(base, L, D, theta, st, fm);
         if (rc != JETLONG_OK) return rc;
     }
     DecodeParams p;
@@ -449,15 +449,15 @@ static int launch_decode_td(const void* q, const void* K, const void* V, void* o
 
 int launch_decode(const void* q, const void* K, const void* V, void* out, float* lse, long long L, int H_q, int H_kv,
                   int d, long long w0, long long G, double theta, int dtype, bool bifocal, void* ws, size_t ws_bytes,
-                  cudaStream_t st) {
+                  cudaStream_t st, FreqMap fm) {
     (void)ws_bytes;
     if (dtype == JETLONG_FP32) {
-        if (d == 64) return launch_decode_td<float, 64>(q, K, V, out, lse, L, H_q, H_kv, w0, G, theta, bifocal, ws, st);
-        return launch_decode_td<float, 128>(q, K, V, out, lse, L, H_q, H_kv, w0, G, theta, bifocal, ws, st);
+        if (d == 64) return launch_decode_td<float, 64>(q, K, V, out, lse, L, H_q, H_kv, w0, G, theta, bifocal, ws, st, fm);
+        return launch_decode_td<float, 128>(q, K, V, out, lse, L, H_q, H_kv, w0, G, theta, bifocal, ws, st, fm);
     }
     if (d == 64)
-        return launch_decode_td<__nv_bfloat16, 64>(q, K, V, out, lse, L, H_q, H_kv, w0, G, theta, bifocal, ws, st);
-    return launch_decode_td<__nv_bfloat16, 128>(q, K, V, out, lse, L, H_q, H_kv, w0, G, theta, bifocal, ws, st);
+        return launch_decode_td<__nv_bfloat16, 64>(q, K, V, out, lse, L, H_q, H_kv, w0, G, theta, bifocal, ws, st, fm);
+    return launch_decode_td<__nv_bfloat16, 128>(q, K, V, out, lse, L, H_q, H_kv, w0, G, theta, bifocal, ws, st, fm);
 }
 
 }  // namespace jetlong

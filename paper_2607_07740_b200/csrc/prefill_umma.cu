@@ -914,7 +914,7 @@ size_t umma_prefill_prerot_workspace_bytes(long long L, int H_kv, int d) {
 
 int launch_prefill_umma(const void* Q, const void* K, const void* V, void* out, float* lse, long long L, int H_q,
                         int H_kv, int d, long long w0, long long G, double theta, bool bifocal, int precise, void* ws,
-                        size_t ws_bytes, cudaStream_t st, bool prerot, bool g_two_tile) {
+                        size_t ws_bytes, cudaStream_t st, bool prerot, bool g_two_tile, FreqMap fm) {
     (void)ws_bytes;
     CUtensorMap tmK, tmV;
     if (!make_kv_tensor_map(&tmK, K, L, H_kv, 64) || !make_kv_tensor_map(&tmV, V, L, H_kv, 128)) return JETLONG_UNSUPPORTED;
@@ -937,7 +937,7 @@ int launch_prefill_umma(const void* Q, const void* K, const void* V, void* out, 
     CUtensorMap tmKh = tmK, tmKe = tmK, tmKl = tmK;
     p.lo = nullptr; p.hi = nullptr;
     if (bifocal) {
-        int rc = build_two_level(ws, L + 256, d, theta, st);
+        int rc = build_two_level(ws, L + 256, d, theta, st, fm);
         if (rc != JETLONG_OK) return rc;
         p.lo = reinterpret_cast<const float2*>((unsigned char*)ws + 256);
         p.hi = p.lo + 256 * (d / 2);

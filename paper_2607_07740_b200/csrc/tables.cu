@@ -9,26 +9,36 @@
 
 namespace jetlong {
 
+// frequency of pair i under the remote map: theta_i (aliasing) or phi_i = theta_i (1 - gamma_i)(1 - 1/G) (R17)
+__device__ __forceinline__ double map_freq(int i, int d, double log2_theta, const FreqMap& fm) {
+    const double th = exp2(-2.0 * (double)i / (double)d * log2_theta);
+    if (!fm.interp) return th;
+    const double r = fm.w_pre * th / 6.283185307179586476925286766559;
+    double gam = (r - fm.alpha) / (fm.beta - fm.alpha);
+    gam = gam < 0.0 ? 0.0 : (gam > 1.0 ? 1.0 : gam);
+    return th * (1.0 - gam) * fm.one_minus_inv_G;
+}
+
 // ---- per-key table: T[k][i] = (cos, sin)(Delta(k) theta_i) ------------------------------------------
 __global__ void key_table_kernel(float2* __restrict__ tab, long long L, long long G, int half, double log2_theta,
-                                 int d) {
+                                 int d, FreqMap fm) {
     long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= L * half) return;
     long long k = idx / half;
     int i = (int)(idx - k * half);
-    double th = exp2(-2.0 * (double)i / (double)d * log2_theta);
-    double a = (double)delta_pos(k, G) * th;
+    double th = map_freq(i, d, log2_theta, fm);
+    double a = (double)delta_pos(k, G) * th;                       // interpolation: G = 2^30, Delta(k) = -k
     double s, c;
     sincos(a, &s, &c);
     tab[idx] = make_float2((float)c, (float)s);
 }
 
-int build_key_table(float2* tab, long long L, long long G, int d, double theta, cudaStream_t st) {
+int build_key_table(float2* tab, long long L, long long G, int d, double theta, cudaStream_t st, FreqMap fm) {
     int half = d / 2;
     long long n = L * half;
     int threads = 256;
     long long blocks = (n + threads - 1) / threads;
-    key_table_kernel<<<(unsigned)blocks, threads, 0, st>>>(tab, L, G, half, log2(theta), d);
+    key_table_kernel<<<(unsigned)blocks, threads, 0, st>>>(tab, L, fm.interp ? kInterpG : G, half, log2(theta), d, fm);
     note_launch();
     return check_launch("key_table_kernel");
 }
@@ -81,13 +91,15 @@ __device__ __forceinline__ unsigned table_check(const float2* lo, const float2* 
 // and seals it again with a new generation number.  The workspace must have been zero-filled before its first use
 // (include/jetlong.h), so an unsealed region never carries the magic by accident.
 __global__ void __launch_bounds__(1024) two_level_kernel(unsigned char* __restrict__ region, long long n_hi, int half,
-                                                         double theta, double log2_theta, int d) {
+                                                         double theta, double log2_theta, int d, FreqMap fm) {
     __shared__ unsigned red[32];
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");   // a programmatically launched consumer (decode) may start
     TableHeader* hdr = reinterpret_cast<TableHeader*>(region);
     float2* lo = reinterpret_cast<float2*>(region + 256);
     float2* hi = lo + 256 * half;
-    const bool sealed = hdr->magic == kMagic && hdr->theta == theta && hdr->n_hi == n_hi && hdr->d == d;   // uniform
+    const bool same_map = hdr->interp == fm.interp && (!fm.interp || (hdr->omg == fm.one_minus_inv_G && hdr->w_pre == fm.w_pre &&
+                                                                         hdr->alpha == fm.alpha && hdr->beta == fm.beta));
+    const bool sealed = hdr->magic == kMagic && hdr->theta == theta && hdr->n_hi == n_hi && hdr->d == d && same_map;   // uniform
     if (sealed && table_check(lo, hi, n_hi, half, red) == hdr->check) return;
     const unsigned gen = hdr->gen;
     __syncthreads();
@@ -97,7 +109,7 @@ __global__ void __launch_bounds__(1024) two_level_kernel(unsigned char* __restri
     for (long long idx = threadIdx.x; idx < total; idx += blockDim.x) {
         const long long row = idx / half;
         const int i = (int)(idx - row * half);
-        const double th = exp2(-2.0 * (double)i / (double)d * log2_theta);
+        const double th = map_freq(i, d, log2_theta, fm);
         const double n = row < 256 ? (double)row : 256.0 * (double)(row - 256);
         double s, c;
         sincos(-n * th, &s, &c);
@@ -112,14 +124,15 @@ __global__ void __launch_bounds__(1024) two_level_kernel(unsigned char* __restri
         hdr->d = d;
         hdr->check = chk;
         hdr->gen = gen + 1u;
+        hdr->interp = fm.interp; hdr->omg = fm.one_minus_inv_G; hdr->w_pre = fm.w_pre; hdr->alpha = fm.alpha; hdr->beta = fm.beta;
         __threadfence();
         hdr->magic = kMagic;
     }
 }
 
-int build_two_level(void* region, long long L, int d, double theta, cudaStream_t st) {
+int build_two_level(void* region, long long L, int d, double theta, cudaStream_t st, FreqMap fm) {
     const long long n_hi = (L + 255) / 256 + 1;
-    two_level_kernel<<<1, 1024, 0, st>>>((unsigned char*)region, n_hi, d / 2, theta, log2(theta), d);
+    two_level_kernel<<<1, 1024, 0, st>>>((unsigned char*)region, n_hi, d / 2, theta, log2(theta), d, fm);
     note_launch(1);
     return check_launch("two_level_kernel");
 }

@@ -143,9 +143,13 @@ def test_options_are_validated_before_any_launch():
     import ctypes
     L = B.lib()
     n0 = B.jetlong_launch_count()
-    bad = B.Options(4, B.DEFAULT, B.DEFAULT)              # struct_bytes too small
+    bad = B.Options(4, B.DEFAULT, B.DEFAULT, B.DEFAULT, 0.0, 0.0)   # struct_bytes too small
     args = [1 << 12] * 5 + [64, 2, 2, 128, 8, 32, 1e4, B.BF16, 1 << 12, 1 << 20, None]
     assert L.jetlong_prefill_opt(*args, ctypes.byref(bad)) == B.INVALID_ARG
-    unk = B.Options(ctypes.sizeof(B.Options), 17, B.DEFAULT)   # unknown precision
+    unk = B.Options(ctypes.sizeof(B.Options), 17, B.DEFAULT, B.DEFAULT, 0.0, 0.0)   # unknown precision
     assert L.jetlong_prefill_opt(*args, ctypes.byref(unk)) == B.INVALID_ARG
+    bad_map = B.Options(ctypes.sizeof(B.Options), B.DEFAULT, B.DEFAULT, 9, 0.0, 0.0)
+    assert L.jetlong_prefill_opt(*args, ctypes.byref(bad_map)) == B.INVALID_ARG
+    bad_ramp = B.Options(ctypes.sizeof(B.Options), B.DEFAULT, B.DEFAULT, B.MAP_FREQ_INTERP, 4.0, 2.0)   # beta <= alpha
+    assert L.jetlong_prefill_opt(*args, ctypes.byref(bad_ramp)) == B.INVALID_ARG
     assert B.jetlong_launch_count() == n0
