@@ -116,6 +116,25 @@ int jetlong_decode(const void* q, const void* Kcache, const void* Vcache, void* 
                    int64_t w_local, int64_t w_pretrained, double rope_theta,
                    int dtype, void* workspace, size_t workspace_bytes, void* stream);
 
+/*
+ * Batched decode over a PAGED KV cache: `batch` independent sequences, one query token each
+ * (Eq.(1) per sequence), in one launch per 16 sequences.  Sequence b has its own current length seq_lens[b]
+ * (a HOST array; G_b = jetlong_group_size(seq_lens[b], w_pretrained) is computed on the host per sequence) and reads
+ * its keys through a page table: logical rows [128 t, 128 t + 127] of sequence b live in physical page
+ * page_table[b * max_pages_per_seq + t] of the pools Kpool, Vpool [pool_pages * 128, H_kv, d] (a page is the TMA tile
+ * of the scan, so paging costs one table read per tile).  page_table is a DEVICE array of int32.  q, out [batch, H_q, d];
+ * lse [batch, H_q].  Rows of a sequence's last page beyond its length are never used but must hold finite numbers.
+ * bf16, head_dim 128, H_q / H_kv <= 16 (JETLONG_UNSUPPORTED otherwise); remote map: aliasing.
+ * workspace >= jetlong_decode_paged_workspace_bytes(max over b of seq_lens[b], batch, ...), zero-filled before first use.
+ * INVALID_ARG additionally: batch < 1, a length < 1 or > 128 * max_pages_per_seq, pool_pages < 1.
+ */
+size_t jetlong_decode_paged_workspace_bytes(int64_t max_len, int batch, int H_q, int H_kv, int head_dim);
+int jetlong_decode_paged(const void* q, const void* Kpool, const void* Vpool, const int32_t* page_table,
+                         const int64_t* seq_lens, int batch, int max_pages_per_seq, int64_t pool_pages,
+                         void* out, float* lse, int H_q, int H_kv, int head_dim,
+                         int64_t w_local, int64_t w_pretrained, double rope_theta,
+                         int dtype, void* workspace, size_t workspace_bytes, void* stream);
+
 /* Matched control ("without bifocal attention"): plain causal attention on the given
  * (already RoPE'd) Q, K with the same kernels, no classifier and no rotation. */
 int jetlong_causal_prefill(const void* Q, const void* K, const void* V, void* out, float* lse,

@@ -23,7 +23,8 @@ EXPORTS = ["jetlong_group_size", "jetlong_workspace_bytes", "jetlong_prefill", "
            "jetlong_causal_prefill", "jetlong_causal_decode", "jetlong_prefill_host", "jetlong_status_string",
            "jetlong_launch_count", "jetlong_set_prefill_impl", "jetlong_prefill_uses_umma",
            "jetlong_set_prefill_precision", "jetlong_prefill_prerotated", "jetlong_prefill_unfused",
-           "jetlong_prefill_opt", "jetlong_prefill_prerotated_opt", "jetlong_host_release", "jetlong_decode_opt"]
+           "jetlong_prefill_opt", "jetlong_prefill_prerotated_opt", "jetlong_host_release", "jetlong_decode_opt",
+           "jetlong_decode_paged", "jetlong_decode_paged_workspace_bytes"]
 DEFAULT = -2                                              # JETLONG_DEFAULT: take the calling thread's default
 
 
@@ -76,6 +77,10 @@ def lib():
         L.jetlong_prefill_prerotated_opt.restype = i32
         L.jetlong_prefill_prerotated_opt.argtypes = [vp] * 5 + tail + [vp]
         L.jetlong_host_release.restype = None
+        L.jetlong_decode_paged_workspace_bytes.restype = sz
+        L.jetlong_decode_paged_workspace_bytes.argtypes = [i64, i32, i32, i32, i32]
+        L.jetlong_decode_paged.restype = i32
+        L.jetlong_decode_paged.argtypes = [vp, vp, vp, vp, vp, i32, i32, i64, vp, vp, i32, i32, i32, i64, i64, dbl, i32, vp, sz, vp]
         L.jetlong_decode_opt.restype = i32
         L.jetlong_decode_opt.argtypes = [vp] * 5 + tail + [vp]
         L.jetlong_decode.restype = i32
@@ -254,4 +259,28 @@ def jetlong_prefill_host(Q, K, V, *, w_local, w_pretrained, rope_theta, out=None
         lse = torch.empty((H_q, L), dtype=torch.float32)
     _check(lib().jetlong_prefill_host(Q.data_ptr(), K.data_ptr(), V.data_ptr(), out.data_ptr(), lse.data_ptr(), L, H_q,
                                       H_kv, d, int(w_local), int(w_pretrained), float(rope_theta), _dt(Q)))
+    return out, lse
+
+
+def jetlong_decode_paged(q, Kpool, Vpool, page_table, seq_lens, *, w_local, w_pretrained, rope_theta, out=None, lse=None,
+                         workspace=None):
+    """Batched decode over a paged cache.  q [B,H_q,d]; Kpool/Vpool [pages*128,H_kv,d]; page_table int32 [B,max_pages] on the
+    device; seq_lens: a sequence of B ints (host)."""
+    assert q.is_cuda and q.is_contiguous() and Kpool.is_contiguous() and Vpool.is_contiguous()
+    assert page_table.is_cuda and page_table.dtype == torch.int32 and page_table.is_contiguous()
+    Bn, H_q, d = q.shape
+    H_kv = Kpool.shape[1]
+    assert Kpool.shape == Vpool.shape and Kpool.shape[0] % 128 == 0 and page_table.shape[0] == Bn and len(seq_lens) == Bn
+    if out is None:
+        out = torch.empty_like(q)
+    if lse is None:
+        lse = torch.empty((Bn, H_q), dtype=torch.float32, device=q.device)
+    lens = (ctypes.c_int64 * Bn)(*[int(x) for x in seq_lens])
+    if workspace is None:
+        n = int(lib().jetlong_decode_paged_workspace_bytes(max(int(x) for x in seq_lens), Bn, H_q, H_kv, d))
+        workspace = torch.zeros(max(n, 256), dtype=torch.uint8, device=q.device)
+    _check(lib().jetlong_decode_paged(q.data_ptr(), Kpool.data_ptr(), Vpool.data_ptr(), page_table.data_ptr(), lens, Bn,
+                                      page_table.shape[1], Kpool.shape[0] // 128, out.data_ptr(), lse.data_ptr(), H_q, H_kv, d,
+                                      int(w_local), int(w_pretrained), float(rope_theta), _dt(q), workspace.data_ptr(),
+                                      workspace.numel(), _stream()))
     return out, lse

@@ -1,6 +1,7 @@
 // api.cu -- the C ABI of libjetlong (include/jetlong.h): validation, dispatch, workspace layout.
 #include <atomic>
 #include <mutex>
+#include <vector>
 #include <stdio.h>
 #include <string.h>
 
@@ -56,6 +57,13 @@ int launch_prefill_unfused(const void* Q, const void* K, const void* V, void* ou
 int launch_prefill_umma(const void* Q, const void* K, const void* V, void* out, float* lse, long long L, int H_q,
                         int H_kv, int d, long long w0, long long G, double theta, bool bifocal, int precise, void* ws,
                         size_t ws_bytes, cudaStream_t st, bool prerot, bool two_tile, FreqMap fm);
+
+// decode.cu / decode_umma.cu
+bool umma_decode_supported(int H_q, int H_kv, int d, int dtype);
+size_t decode_paged_workspace_bytes(long long Lmax, int batch, int H_q, int H_kv, int d);
+int launch_decode_paged(const void* q, const void* Kpool, const void* Vpool, const int* page_table, int max_pages,
+                        long long pool_pages, const long long* Ls, const long long* Gs, int batch, void* out, float* lse,
+                        int H_q, int H_kv, long long w0, double theta, void* ws, cudaStream_t st);
 
 static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; }
 
@@ -237,6 +245,35 @@ int jetlong_decode_opt(const void* q, const void* Kcache, const void* Vcache, vo
                        void* workspace, size_t workspace_bytes, void* stream, const jetlong_options* options) {
     return decode_common(q, Kcache, Vcache, out, lse, L, H_q, H_kv, head_dim, w_local, w_pretrained, rope_theta, dtype,
                          workspace, workspace_bytes, stream, true, options);
+}
+
+size_t jetlong_decode_paged_workspace_bytes(int64_t max_len, int batch, int H_q, int H_kv, int head_dim) {
+    if (max_len < 1 || batch < 1 || H_q < 1 || H_kv < 1 || (H_q % H_kv) || head_dim != 128) return 0;
+    return decode_paged_workspace_bytes(max_len, batch, H_q, H_kv, head_dim);
+}
+
+int jetlong_decode_paged(const void* q, const void* Kpool, const void* Vpool, const int32_t* page_table,
+                         const int64_t* seq_lens, int batch, int max_pages_per_seq, int64_t pool_pages, void* out, float* lse,
+                         int H_q, int H_kv, int head_dim, int64_t w_local, int64_t w_pretrained, double rope_theta, int dtype,
+                         void* workspace, size_t workspace_bytes, void* stream) {
+    if (!page_table || !seq_lens || batch < 1 || max_pages_per_seq < 1 || pool_pages < 1) return JETLONG_INVALID_ARG;
+    int rc = validate(q, Kpool, Vpool, out, lse, 1, H_q, H_kv, head_dim, w_local, w_pretrained, rope_theta, dtype);
+    if (rc != JETLONG_OK) return rc;
+    long long Lmax = 0;
+    std::vector<long long> Ls(batch), Gs(batch);
+    for (int b = 0; b < batch; ++b) {
+        if (seq_lens[b] < 1 || seq_lens[b] > 128ll * max_pages_per_seq) return JETLONG_INVALID_ARG;
+        Ls[b] = seq_lens[b];
+        Gs[b] = jetlong_group_size(seq_lens[b], w_pretrained);       // Eq.(2) per sequence, on the host
+        if (Ls[b] > Lmax) Lmax = Ls[b];
+    }
+    if (!umma_decode_supported(H_q, H_kv, head_dim, dtype)) return JETLONG_UNSUPPORTED;
+    const size_t need = decode_paged_workspace_bytes(Lmax, batch, H_q, H_kv, head_dim);
+    if (!workspace || workspace_bytes < need || !aligned16(workspace)) return JETLONG_INVALID_ARG;
+    rc = device_ok();
+    if (rc != JETLONG_OK) return rc;
+    return launch_decode_paged(q, Kpool, Vpool, page_table, max_pages_per_seq, pool_pages, Ls.data(), Gs.data(), batch, out,
+                               lse, H_q, H_kv, w_local, rope_theta, workspace, (cudaStream_t)stream);
 }
 
 int jetlong_causal_decode(const void* q, const void* Kcache, const void* Vcache, void* out, float* lse, int64_t L,

@@ -323,8 +323,12 @@ __global__ void __launch_bounds__(NW * 32) decode_kernel(DecodeParams p) {
 // ---- split merge: warp-shuffle log-sum-exp over the splits (step a7 (ii), a8) ---------------------------
 template <typename T, int D>
 __global__ void __launch_bounds__(D) decode_merge_kernel(const float* __restrict__ part, int nsplit, int H_q,
-                                                         T* __restrict__ out, float* __restrict__ lse) {
+                                                         T* __restrict__ out, float* __restrict__ lse,
+                                                         long long part_stride = 0) {
     constexpr int SS = D + 2;
+    part += (size_t)blockIdx.y * part_stride;                       // batched decode: grid y = sequence
+    out += (size_t)blockIdx.y * H_q * D;
+    lse += (size_t)blockIdx.y * H_q;
     __shared__ float w_s[1024];
     __shared__ float red[2];
     const int h = blockIdx.x, tid = threadIdx.x, lane = tid & 31;
@@ -422,7 +426,7 @@ static int launch_decode_td(const void* q, const void* K, const void* V, void* o
         at[0].val.programmaticStreamSerializationAllowed = 1;
         cfg.attrs = at;
         cfg.numAttrs = 1;
-        cudaLaunchKernelEx(&cfg, decode_merge_kernel<T, D>, (const float*)p.part, ns, H_q, (T*)out, lse);
+        cudaLaunchKernelEx(&cfg, decode_merge_kernel<T, D>, (const float*)p.part, ns, H_q, (T*)out, lse, 0ll);
         note_launch();
         return check_launch("decode_merge_kernel");
     }
@@ -445,6 +449,67 @@ static int launch_decode_td(const void* q, const void* K, const void* V, void* o
     decode_merge_kernel<T, D><<<H_q, D, 0, st>>>(p.part, pl.nsplit, H_q, (T*)out, lse);
     note_launch();
     return check_launch("decode_merge_kernel");
+}
+
+int launch_decode_umma_paged(const void* q, const void* Kpool, const void* Vpool, const int* page_table, int max_pages,
+                             long long pool_pages, const long long* Ls, const long long* Gs, int nb, float* part,
+                             long long part_stride, long long Lmax, int H_q, int H_kv, long long w0, double theta,
+                             const float2* lo, const float2* hi, int* nsplit_out, cudaStream_t st);
+
+size_t decode_paged_workspace_bytes(long long Lmax, int batch, int H_q, int H_kv, int d) {
+    int ns = 0;
+    long long kps = 0;
+    umma_decode_plan(Lmax, H_kv, &ns, &kps);                         // an upper bound of the splits of any launch
+    return two_level_bytes(Lmax, d) + (size_t)batch * align256((size_t)ns * H_q * (d + 2) * sizeof(float));
+}
+
+// batch > 1 over a paged cache (bf16, d = 128, tcgen05 path): chunks of up to 16 sequences per launch
+int launch_decode_paged(const void* q, const void* Kpool, const void* Vpool, const int* page_table, int max_pages,
+                        long long pool_pages, const long long* Ls, const long long* Gs, int batch, void* out, float* lse,
+                        int H_q, int H_kv, long long w0, double theta, void* ws, cudaStream_t st) {
+    constexpr int D = 128;
+    long long Lmax = 1;
+    bool any_bifocal = false;
+    for (int b = 0; b < batch; ++b) {
+        if (Ls[b] > Lmax) Lmax = Ls[b];
+        if (Gs[b] > 1 && w0 < Ls[b] - 1) any_bifocal = true;
+    }
+    unsigned char* base = (unsigned char*)ws;
+    const size_t tb = two_level_bytes(Lmax, D);
+    if (any_bifocal) {
+        int rc = build_two_level(base, Lmax, D, theta, st);          // the table does not depend on G: one for every sequence
+        if (rc != JETLONG_OK) return rc;
+    }
+    const float2* lo = reinterpret_cast<const float2*>(base + 256);
+    const float2* hi = lo + 256 * (D / 2);
+    int ns0 = 0;
+    long long kps0 = 0;
+    umma_decode_plan(Lmax, H_kv, &ns0, &kps0);
+    const long long part_stride = (long long)(align256((size_t)ns0 * H_q * (D + 2) * sizeof(float)) / sizeof(float));
+    float* part = reinterpret_cast<float*>(base + tb);
+    for (int b0 = 0; b0 < batch; b0 += 16) {
+        const int nb = batch - b0 < 16 ? batch - b0 : 16;
+        int ns = 0;
+        int rc = launch_decode_umma_paged((const __nv_bfloat16*)q + (size_t)b0 * H_q * D, Kpool, Vpool,
+                                          page_table + (size_t)b0 * max_pages, max_pages, pool_pages, Ls + b0, Gs + b0, nb,
+                                          part + (size_t)b0 * part_stride, part_stride, Lmax, H_q, H_kv, w0, theta, lo, hi, &ns, st);
+        if (rc != JETLONG_OK) return rc;
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(H_q, nb);
+        cfg.blockDim = dim3(D);
+        cfg.stream = st;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = at;
+        cfg.numAttrs = 1;
+        cudaLaunchKernelEx(&cfg, decode_merge_kernel<__nv_bfloat16, D>, (const float*)(part + (size_t)b0 * part_stride), ns, H_q,
+                           (__nv_bfloat16*)out + (size_t)b0 * H_q * D, lse + (size_t)b0 * H_q, part_stride);
+        note_launch();
+        rc = check_launch("decode_merge_kernel (paged)");
+        if (rc != JETLONG_OK) return rc;
+    }
+    return JETLONG_OK;
 }
 
 int launch_decode(const void* q, const void* K, const void* V, void* out, float* lse, long long L, int H_q, int H_kv,

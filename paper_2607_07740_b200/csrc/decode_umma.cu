@@ -66,7 +66,16 @@ struct Params {
     const float2* lo;
     const float2* hi;
     double theta;                                    // for the table-header check (see the prologue)
+    // batched / paged form: blockIdx.z = sequence b with its own length and group size; the cache is a pool
+    // of 128-row pages (= the TMA tile) addressed through a page table; the fields above are per sequence then
+    int batch;                                       // 0: the single-sequence call
+    const int* page_table;                           // [batch][max_pages] physical page of logical tile kt (device memory)
+    int max_pages;
+    long long part_stride;                           // floats between the partials of consecutive sequences
+    long long Ls[16];
+    int Gs[16];
 };
+constexpr int MAXB = 16;
 
 // byte offset of element (row n, k) in a [2 boxes][16 rows][128 B] SWIZZLE_128B K-major operand (16-bit elements)
 template <int ROWS = NH> __device__ __forceinline__ int bop_off(int n, int k) {
@@ -127,7 +136,20 @@ struct DPlan {
 
 template <int NG>                                    // NG = query heads per KV head, rounded up to a power of two
 __global__ void __launch_bounds__(NTHREADS, 1)
-decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV, const Params p) {
+decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV, const Params p0) {
+    Params p = p0;
+    const int* pages = nullptr;                                        // this sequence's row of the page table
+    if (p0.batch > 0) {
+        const int b = blockIdx.z;
+        p.L = p0.Ls[b];
+        p.G = p0.Gs[b];
+        p.bifocal = (p.G > 1 && p.w0 < p.L - 1) ? 1 : 0;               // step a2, per sequence
+        p.q = p0.q + (size_t)b * p0.H_q * D;
+        p.part = p0.part + (size_t)b * p0.part_stride;
+        const long long tiles = (p.L + BN - 1) / BN, tps = (tiles + gridDim.x - 1) / gridDim.x;
+        p.kps = tps * BN;
+        pages = p0.page_table + (size_t)b * p0.max_pages;
+    }
     extern __shared__ __align__(1024) unsigned char smem[];
     if ((smem_u32(smem) & 1023u) != 0) __trap();               // SWIZZLE_128B operands need the 1024-byte alignment
     unsigned char* sQ = smem + OFF_Q;                              // raw | hi | lo
@@ -207,8 +229,10 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
     if (warp == 0) {
         // ===================== TMA producer =====================
         if (lane == 0) {
+            int pg_next = (pages && plan.nv > 0) ? __ldg(pages + plan.kt(0)) : 0;
             for (int v = 0; v < plan.nv; ++v) {
-                const int row0 = plan.kt(v) * BN;
+                const int row0 = (pages ? pg_next : plan.kt(v)) * BN;  // paged: physical page of the logical tile
+                if (pages && v + 1 < plan.nv) pg_next = __ldg(pages + plan.kt(v + 1));   // in flight under the wait below
                 const int s = v % KS;
                 if (v >= KS) mbar_wait(&bars->k_empty[s], ((v / KS) - 1) & 1);
                 mbar_arrive_expect_tx(&bars->k_full[s], TILE);
@@ -220,8 +244,10 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
         // ===================== TMA producer for V (its own thread: a V stage lives until O += V^T P of its visit,
         // much longer than a K stage, and must not hold back the K loads) =====================
         if (lane == 0) {
+            int pg_next = (pages && plan.nv > 0) ? __ldg(pages + plan.kt(0)) : 0;
             for (int v = 0; v < plan.nv; ++v) {
-                const int row0 = plan.kt(v) * BN;
+                const int row0 = (pages ? pg_next : plan.kt(v)) * BN;
+                if (pages && v + 1 < plan.nv) pg_next = __ldg(pages + plan.kt(v + 1));
                 const int sv = v % VS;
                 if (v >= VS) mbar_wait(&bars->v_empty[sv], ((v / VS) - 1) & 1);
                 mbar_arrive_expect_tx(&bars->v_full[sv], TILE);
@@ -501,6 +527,7 @@ int launch_decode_umma(const void* q, const void* K, const void* V, float* part,
     p.bifocal = bifocal ? 1 : 0;
     p.lo = lo; p.hi = hi;
     p.theta = theta;
+    p.batch = 0; p.page_table = nullptr; p.max_pages = 0; p.part_stride = 0;
     auto kern = p.g <= 1 ? decode_umma_kernel<1> : p.g <= 2 ? decode_umma_kernel<2> : p.g <= 4 ? decode_umma_kernel<4>
               : p.g <= 8 ? decode_umma_kernel<8> : decode_umma_kernel<16>;
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES) != cudaSuccess)
@@ -519,6 +546,53 @@ int launch_decode_umma(const void* q, const void* K, const void* V, float* part,
     note_launch();
     *nsplit_out = ns;
     return check_launch("decode_umma_kernel");
+}
+
+// Batched decode over a paged cache: up to MAXB sequences per launch (grid z), each with its own length / group size.
+// Kpool, Vpool: [pool_pages * 128, H_kv, 128]; the split count follows the longest sequence.
+int launch_decode_umma_paged(const void* q, const void* Kpool, const void* Vpool, const int* page_table, int max_pages,
+                             long long pool_pages, const long long* Ls, const long long* Gs, int nb, float* part,
+                             long long part_stride, long long Lmax, int H_q, int H_kv, long long w0, double theta,
+                             const float2* lo, const float2* hi, int* nsplit_out, cudaStream_t st) {
+    CUtensorMap tmK, tmV;
+    if (!make_kv_tensor_map(&tmK, Kpool, pool_pages * BN, H_kv, BN) || !make_kv_tensor_map(&tmV, Vpool, pool_pages * BN, H_kv, BN))
+        return JETLONG_UNSUPPORTED;
+    if (nb < 1 || nb > MAXB) return JETLONG_INVALID_ARG;
+    Params p;
+    p.q = (const __nv_bfloat16*)q;
+    p.part = part;
+    p.L = Lmax; p.w0 = w0; p.G = 1;
+    int ns;
+    umma_decode_plan(Lmax, H_kv * nb, &ns, &p.kps);                    // one CTA per SM over all (sequence, KV head) pairs
+    p.H_q = H_q; p.H_kv = H_kv; p.g = H_q / H_kv;
+    p.bifocal = 0;
+    p.lo = lo; p.hi = hi;
+    p.theta = theta;
+    p.batch = nb; p.page_table = page_table; p.max_pages = max_pages; p.part_stride = part_stride;
+    bool any_bifocal = false;
+    for (int b = 0; b < MAXB; ++b) {
+        p.Ls[b] = b < nb ? Ls[b] : 1;
+        p.Gs[b] = b < nb ? (int)Gs[b] : 1;
+        if (b < nb && Gs[b] > 1 && w0 < Ls[b] - 1) any_bifocal = true;
+    }
+    auto kern = p.g <= 1 ? decode_umma_kernel<1> : p.g <= 2 ? decode_umma_kernel<2> : p.g <= 4 ? decode_umma_kernel<4>
+              : p.g <= 8 ? decode_umma_kernel<8> : decode_umma_kernel<16>;
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES) != cudaSuccess)
+        return check_launch("decode_umma attr");
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(ns, H_kv, nb);
+    cfg.blockDim = dim3(NTHREADS);
+    cfg.dynamicSmemBytes = SMEM_BYTES;
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = any_bifocal ? 1 : 0;                                // without the table kernel in front: a normal launch
+    cudaLaunchKernelEx(&cfg, kern, tmK, tmV, p);
+    note_launch();
+    *nsplit_out = ns;
+    return check_launch("decode_umma_kernel (paged)");
 }
 
 }  // namespace jetlong
