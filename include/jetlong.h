@@ -80,7 +80,7 @@ int jetlong_prefill(const void* Q, const void* K, const void* V, void* out, floa
  * rotation K' = R(Delta k) K (Eq.(5)-(6) P:101-106) is applied ONCE into a scratch inside the workspace
  * (K' as fp16 plus the two e5m2 cross-term operands: 4 bytes per key channel, e.g. 268 MB at L = 65536,
  * H_kv = 8) and the remote tiles are then TMA-loaded from it; the stored K is still never written.
- * bf16, head_dim 128, even H_q / H_kv only (JETLONG_UNSUPPORTED otherwise); the workspace must be at
+ * bf16, head_dim 128 only (JETLONG_UNSUPPORTED otherwise; any GQA group size); the workspace must be at
  * least jetlong_workspace_bytes(JETLONG_OP_PREFILL_PREROTATED, ...).  The fp16 cross-term precision
  * mode is served with the e5m2 cross terms.
  */
@@ -98,7 +98,7 @@ int jetlong_prefill_prerotated(const void* Q, const void* K, const void* V, void
  * each returning (O_X, l_X), then Eq.(7) WITH the minus sign: O = (W_A O_A + W_B O_B - W_C O_C) / (W_A + W_B - W_C).
  * The band is computed three times and the remote operands carry one fp16 rounding without compensation, so on
  * outlier-channel inputs lse is only good to ~3e-3 (the fused default: ~3e-4); out stays within the bf16 tolerance.
- * bf16, head_dim 128, even H_q / H_kv; workspace >= jetlong_workspace_bytes(JETLONG_OP_PREFILL_UNFUSED, ...)
+ * bf16, head_dim 128; workspace >= jetlong_workspace_bytes(JETLONG_OP_PREFILL_UNFUSED, ...)
  * (tables + Q', K', O_B, O_C, l_B, l_C: about 4.5x the size of Q).
  */
 int jetlong_prefill_unfused(const void* Q, const void* K, const void* V, void* out, float* lse,
@@ -212,9 +212,9 @@ int jetlong_decode_opt(const void* q, const void* Kcache, const void* Vcache, vo
                        const jetlong_options* options);
 
 /* DEPRECATED (kept as shims): set the CALLING THREAD's default prefill implementation.
- * -1 or 4 (default): tcgen05 UMMA where supported (bf16, head_dim 128, even H_q / H_kv): the two-tile kernel, in which a
+ * -1 or 4 (default): tcgen05 UMMA where supported (bf16, head_dim 128, any GQA group size): the two-tile kernel, in which a
  * CTA pair owns 256 query rows x 2 heads and every staged / rotated K tile feeds both 128-row tiles (prefill_umma2.cu).
- * 1 = the one-tile CTA-pair kernel of round 1 (prefill_umma.cu; also serves JETLONG_PRECISION_COMPENSATED_F16);
+ * 1 = the one-tile CTA-pair kernel of round 1 (prefill_umma.cu, even group sizes; also serves JETLONG_PRECISION_COMPENSATED_F16);
  * 0 = SIMT fp32-FMA tiles.  2 and 3 (round 1's cluster-of-four launches, superseded by the two-tile kernel and
  * removed) are accepted and mean 1.  All give the same results up to rounding.  Returns the previous value. */
 int jetlong_set_prefill_impl(int impl);

@@ -900,8 +900,7 @@ constexpr int g_otf_selective = 1;
 
 bool umma_prefill_supported(long long L, int H_q, int H_kv, int d, int dtype) {
     if (dtype != JETLONG_BF16 || d != 128 || H_kv < 1 || H_q % H_kv) return false;
-    const int g = H_q / H_kv;
-    return (g % 2) == 0 && L >= 1 && L < (1ll << 30);
+    return L >= 1 && L < (1ll << 30);                // any GQA group size: odd groups (MHA included) run a lone-head unit per group
 }
 
 size_t umma_prefill_workspace_bytes(long long L, int, int H_kv, int d) { return two_level_bytes(L + 256, d) + selection_bytes(H_kv); }
@@ -976,6 +975,10 @@ int launch_prefill_umma(const void* Q, const void* K, const void* V, void* out, 
             p.selinfo = selinfo;
             precise = p.precise = 3;
         }
+    }
+    if ((H_q / H_kv) & 1) {                          // odd group sizes exist only in the two-tile kernel
+        g_two_tile = true;
+        if (precise == 1) precise = p.precise = 2;
     }
     if (g_two_tile && prefill_v2_serves(precise)) {
         PrefillV2Args a;

@@ -103,7 +103,7 @@ struct Params {
     long long L, w0, G;
     int H_q, H_kv, g;
     int bifocal, precise, prerot, window_only, qk_f16;
-    int n_qb, n_sb;
+    int n_qb, n_sb, n_s4;
     const float2* lo;
     const float2* hi;
     const uint32_t* selinfo;
@@ -136,20 +136,35 @@ struct Plan {
     }
 };
 
-// the pair's merged visit list: K tiles needed by either query tile (plain scalars: the issuer warp runs on 72 registers)
+// The pair's merged visit list: the K tiles needed by ANY of its four query tiles.  UMMA "tile i" (i = 0, 1) is M = 256
+// across the pair: rows 0-127 are query block qbA + i of CTA 0, rows 128-255 query block qbB + i of CTA 1.  With an even
+// GQA group the two CTAs hold two heads on the SAME blocks (qbA = qbB); the lone head of an odd group (and every head
+// of MHA) is served by one pair on four consecutive blocks of that head (qbB = qbA + 2).  A tile takes part in a visit
+// when either CTA's block needs the key tile; the block that does not need it sees the visit fully masked (the masks in
+// the softmax are the exact per-row rule, whatever the tile), so no special case exists below this struct.
 struct MPlan {
-    int qb0, lo0, hi0, lo1, hi1;                      // tile i = query block qb0 + i: local key tiles [lo_i, qb0 + i], remote [0, hi_i]
+    int lo0, top0, hi0, lo1, top1, hi1;               // tile i: local key tiles [lo_i, top_i], remote [0, hi_i] (joint over the CTAs)
     int lo_m, top_m, hi_m, n_loc, n_rem, nm;
-    bool bifocal, valid1;
-    __device__ MPlan(int qb0_, bool valid1_, long long w0, bool bifocal_, bool window_only)
-        : qb0(qb0_), bifocal(bifocal_), valid1(valid1_) {
-        const Plan a(qb0, w0, bifocal, window_only);
-        lo0 = a.kt_lo; hi0 = a.kt_hi; lo1 = 1 << 30; hi1 = -1;
-        if (valid1) { const Plan b(qb0 + 1, w0, bifocal, window_only); lo1 = b.kt_lo; hi1 = b.kt_hi; }
-        lo_m = lo0;                                                    // lo1 >= lo0
-        top_m = valid1 ? qb0 + 1 : qb0;
-        hi_m = hi1 > hi0 ? hi1 : hi0;
-        n_loc = top_m - lo_m + 1;
+    bool bifocal;
+    __device__ MPlan(int qbA, int qbB, int n_qb, long long w0, bool bifocal_, bool window_only) : bifocal(bifocal_) {
+        lo0 = lo1 = 1 << 30; top0 = top1 = -1; hi0 = hi1 = -1;
+#pragma unroll
+        for (int c = 0; c < 2; ++c) {
+#pragma unroll
+            for (int i = 0; i < 2; ++i) {
+                const int qb = (c ? qbB : qbA) + i;
+                if (qb >= n_qb) continue;
+                const Plan t(qb, w0, bifocal, window_only);
+                int& lo = i ? lo1 : lo0; int& top = i ? top1 : top0; int& hi = i ? hi1 : hi0;
+                lo = t.kt_lo < lo ? t.kt_lo : lo;
+                top = qb > top ? qb : top;
+                hi = t.kt_hi > hi ? t.kt_hi : hi;
+            }
+        }
+        lo_m = lo0 < lo1 ? lo0 : lo1;
+        top_m = top0 > top1 ? top0 : top1;
+        hi_m = hi0 > hi1 ? hi0 : hi1;
+        n_loc = top_m >= lo_m ? top_m - lo_m + 1 : 0;
         n_rem = hi_m + 1;
         nm = n_loc + n_rem;
     }
@@ -160,15 +175,8 @@ struct MPlan {
         return x;
     }
     __device__ __forceinline__ bool part(int i, const Visit& x) const {
-        const int lo = i ? lo1 : lo0, hi = i ? hi1 : hi0;
-        return x.mode == 2 ? x.kt <= hi : (x.kt >= lo && x.kt <= qb0 + i);
-    }
-    __device__ __forceinline__ Plan tile(int i) const {
-        Plan t;
-        if (i && !valid1) return t;
-        t.qb = qb0 + i; t.kt_lo = i ? lo1 : lo0; t.kt_hi = i ? hi1 : hi0;
-        t.n_local = t.qb - t.kt_lo + 1; t.n_remote = t.kt_hi + 1; t.nv = t.n_local + t.n_remote;
-        return t;
+        const int lo = i ? lo1 : lo0, top = i ? top1 : top0, hi = i ? hi1 : hi0;
+        return x.mode == 2 ? x.kt <= hi : (x.kt >= lo && x.kt <= top);
     }
 };
 
@@ -262,16 +270,31 @@ prefill_umma2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_const
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int cta = (int)cluster_ctarank();
-    const int pairs = p.H_q / 2;
     const int unit = (int)(blockIdx.x >> 1);
-    const int sb = p.n_sb - 1 - unit / pairs;                      // heaviest 256-row blocks first
-    const int h0 = 2 * (unit % pairs);
-    const int head = h0 + cta;
-    const int kvh = h0 / p.g;
-    const int qb0 = 2 * sb;
-    const bool valid1 = qb0 + 1 < p.n_qb;
+    // work units, heaviest query blocks first.  Even GQA group: a unit = (256-row block sb, head pair).  Odd group (g = 2 pp + 1,
+    // MHA included): per 512-row block s4 and KV head, pp head pairs on each of its two 256-row blocks and one LONE-head
+    // unit that covers all four 128-row blocks of the last head of the group (CTA c takes blocks 4 s4 + 2 c, + 1).
+    int head, kvh, qbA, qbB;
+    if ((p.g & 1) == 0) {
+        const int pairs = p.H_q / 2;
+        const int sb = p.n_sb - 1 - unit / pairs;
+        const int h0 = 2 * (unit % pairs);
+        head = h0 + cta; kvh = h0 / p.g; qbA = qbB = 2 * sb;
+    } else {
+        const int pp = p.g / 2, npair = p.H_kv * pp;
+        const int s4 = p.n_s4 - 1 - unit / p.H_q, j = unit % p.H_q;
+        if (j < 2 * npair) {
+            const int pi = j < npair ? j : j - npair;
+            kvh = pi / pp; head = kvh * p.g + 2 * (pi % pp) + cta;
+            qbA = qbB = 2 * (2 * s4 + (j < npair ? 1 : 0));
+        } else {
+            kvh = j - 2 * npair; head = kvh * p.g + p.g - 1;
+            qbA = 4 * s4; qbB = 4 * s4 + 2;
+        }
+    }
+    const int qb0 = cta ? qbB : qbA;                               // this CTA's first query block
     const bool bifocal = p.bifocal != 0;
-    const MPlan mp(qb0, valid1, p.w0, bifocal, p.window_only != 0);
+    const MPlan mp(qbA, qbB, p.n_qb, p.w0, bifocal, p.window_only != 0);
     // 0 fast, 2 e5m2 cross terms, 3 e5m2 cross terms over the two highest-energy pairs of every 8-pair chunk; a KV head
     // whose other channels are too loud falls back from 3 to 2
     int precise = (bifocal && mp.n_rem > 0) ? p.precise : 0;
@@ -311,8 +334,8 @@ prefill_umma2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_const
         if (warp == W_KLOAD) {
             // ===================== Q and K producer (each CTA loads its head's Q tiles and its 64 keys of every K tile) =====
             if (lane == 0) {
-                mbar_arrive_expect_tx(&bars->q_full, valid1 ? Q_BYTES : QT_BYTES);
-                for (int i = 0; i < (valid1 ? 2 : 1); ++i) {
+                mbar_arrive_expect_tx(&bars->q_full, Q_BYTES);      // rows beyond L (a missing second tile) arrive as zeros
+                for (int i = 0; i < 2; ++i) {
                     tma_load_3d(sQ + i * QT_BYTES, &tmQ, &bars->q_full, 0, head, (qb0 + i) * BM);
                     tma_load_3d(sQ + i * QT_BYTES + QBOX, &tmQ, &bars->q_full, 64, head, (qb0 + i) * BM);
                 }
@@ -495,7 +518,7 @@ prefill_umma2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_const
                         // first remote visit: Q -> Q' = R(Delta q) Q, in place in shared memory (both tiles, 64 rows per pass)
                         if (mp.n_loc > 0) mbar_wait_sleep(&bars->q_local_done, 0);
 #pragma unroll 1
-                        for (int pass = 0; pass < (valid1 ? 4 : 2); ++pass) {
+                        for (int pass = 0; pass < 4; ++pass) {
                             const int i = pass >> 1, half = pass & 1;
                             KRot<4> qr;
                             qr.init(p.lo, p.hi, tid, p.G, 64 * half);
@@ -523,7 +546,6 @@ prefill_umma2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_const
         const int i = (warp - W_SOFTMAX) >> 2;                         // query tile of this group
         const int quad = warp & 3;
         const int r = (quad << 5) | lane;
-        const Plan plan = mp.tile(i);
         const int qb = qb0 + i;
         const long long q0 = (long long)qb * BM;
         const uint32_t lane_base = (uint32_t)(quad << 5) << 16;
@@ -533,8 +555,10 @@ prefill_umma2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_const
         const uint64_t sl2x2 = pack2(sl2, sl2);
         float m_ref = -INFINITY;
         uint64_t l2a = 0, l2b = 0;                                     // packed fp32x2 partial row sums
-        for (int v = 0; v < plan.nv; ++v) {
-            const Visit x = plan.at(v, bifocal);
+        int v = 0;                                                     // visits this tile has taken part in
+        for (int m = 0; m < mp.nm; ++m) {
+            const Visit x = mp.at(m);
+            if (!mp.part(i, x)) continue;
             const long long k0 = (long long)x.kt * BN;
             const long long qrel = q0 + r - k0;
             int lo = 0, hi = BN - 1;
@@ -616,9 +640,10 @@ prefill_umma2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_const
             __syncwarp();
             if (lane == 0) mbar_arrive_leader(&bars->p_full[i]);
             TR(1 + i, v, 4);
+            ++v;
         }
         // ---- epilogue (step a8) ----
-        if (plan.nv > 0) {
+        if (v > 0) {
             float la, lb, lc, ld;
             unpack2(l2a, la, lb); unpack2(l2b, lc, ld);
             const float l = (la + lb) + (lc + ld);
@@ -671,10 +696,11 @@ int launch_prefill_v2(const PrefillV2Args& a, cudaStream_t st) {
     p.bifocal = a.bifocal; p.precise = a.precise; p.prerot = a.prerot; p.window_only = a.window_only; p.qk_f16 = a.qk_f16;
     p.n_qb = (int)((a.L + BM - 1) / BM);
     p.n_sb = (p.n_qb + 1) / 2;
+    p.n_s4 = (p.n_qb + 3) / 4;
     p.lo = a.lo; p.hi = a.hi; p.selinfo = a.selinfo;
     if (cudaFuncSetAttribute(prefill_umma2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES) != cudaSuccess)
         return check_launch("prefill_umma2 attr");
-    const unsigned grid = 2u * (unsigned)p.n_sb * (unsigned)(a.H_q / 2);
+    const unsigned grid = (p.g & 1) ? 2u * (unsigned)p.n_s4 * (unsigned)a.H_q : 2u * (unsigned)p.n_sb * (unsigned)(a.H_q / 2);
     prefill_umma2_kernel<<<grid, NTHREADS, SMEM_BYTES, st>>>(a.tmQ, a.tmK, a.tmV, a.tmKh, a.tmKe, a.tmKl, p);
     note_launch();
     return check_launch("prefill_umma2_kernel");

@@ -101,7 +101,8 @@ def test_workspace_sizes_of_the_prefill_variants():
     assert 6 * nq + 2 * nk + 8 * L * H_q <= unf <= 6 * nq + 2 * nk + 8 * L * H_q + slack
     # shapes the tcgen05 kernel does not serve have no such variants
     assert B.jetlong_workspace_bytes(B.OP_PREFILL_PREROTATED, 1024, 4, 2, 64, B.FP32) == 0
-    assert B.jetlong_workspace_bytes(B.OP_PREFILL_UNFUSED, 1024, 3, 1, 128, B.BF16) == 0        # odd H_q / H_kv
+    assert B.jetlong_workspace_bytes(B.OP_PREFILL_UNFUSED, 1024, 3, 1, 64, B.BF16) == 0         # head_dim 64
+    assert B.jetlong_workspace_bytes(B.OP_PREFILL_UNFUSED, 1024, 3, 1, 128, B.BF16) > 0         # odd H_q / H_kv is served (round 2)
 
 
 def test_prefill_variants_validate_before_any_launch():

@@ -75,15 +75,29 @@ def test_default_precision_margin_on_config_rows():
         del Q, K, V
 
 
-# ---- shapes the tcgen05 kernels do not serve fall back to the SIMT tiles: they must still meet the bf16 tolerances ---------
-@pytest.mark.parametrize("H_q,H_kv", [(3, 1), (7, 1), (5, 5), (6, 2)])
-def test_bf16_d128_odd_group_sizes(H_q, H_kv):
-    L, w_pre, w0 = 700, 200, 64
-    Q, K, V = W.make_qkv(L, H_q, H_kv, 128, 1e6, "bf16", 4400 + H_q, True, DEV)
-    out, lse = J.jetlong_prefill(Q, K, V, w_local=w0, w_pretrained=w_pre, rope_theta=1e6)
+# ---- odd GQA groups and MHA run on the tcgen05 two-tile kernel too: the lone head of a group is served by one CTA pair on
+# four consecutive query blocks (prefill_umma2.cu); only fp32 and head_dim 64 use the SIMT tiles --------------------------
+@pytest.mark.parametrize("L,H_q,H_kv,w_pre,w0", [
+    (700, 3, 1, 200, 64),          # g = 3: one head pair + one lone head; 6 query blocks (ragged 512-row block)
+    (700, 7, 1, 200, 64),          # g = 7, as in 28 / 4-head models
+    (700, 5, 5, 200, 64),          # MHA: every head is a lone head
+    (2200, 7, 1, 512, 128),        # 18 query blocks, G = 5, longer remote phases
+    (1300, 4, 4, 300, 0),          # MHA, w0 = 0 (joint local ranges with gaps), 11 query blocks
+    (513, 1, 1, 128, 100),         # a single head
+    (700, 6, 2, 200, 64),          # g = 3 with two KV heads
+])
+def test_bf16_d128_odd_group_sizes(L, H_q, H_kv, w_pre, w0):
+    assert B.lib().jetlong_prefill_uses_umma(L, H_q, H_kv, 128) == 1
+    Q, K, V = W.make_qkv(L, H_q, H_kv, 128, 1e6, "bf16", 4400 + H_q + L, True, DEV)
     rows, heads = all_pairs(L, H_q)
-    ro, rl = oracle_rows(Q, K, V, rows, heads, w_local=w0, w_pretrained=w_pre, rope_theta=1e6)
-    check(*gather(out, lse, rows, heads), ro, rl, Q.dtype, "g=%d/%d" % (H_q, H_kv))
+    for name, fn in (("bifocal", lambda: J.jetlong_prefill(Q, K, V, w_local=w0, w_pretrained=w_pre, rope_theta=1e6)),
+                     ("workspace variant", lambda: J.jetlong_prefill_prerotated(Q, K, V, w_local=w0, w_pretrained=w_pre, rope_theta=1e6))):
+        out, lse = fn()
+        ro, rl = oracle_rows(Q, K, V, rows, heads, w_local=w0, w_pretrained=w_pre, rope_theta=1e6)
+        check(*gather(out, lse, rows, heads), ro, rl, Q.dtype, "%s g=%d/%d L=%d" % (name, H_q, H_kv, L))
+    out, lse = J.jetlong_causal_prefill(Q, K, V)
+    ro, rl = oracle_rows(Q, K, V, rows, heads, w_local=0, w_pretrained=1, rope_theta=1e6, mode="causal")
+    check(*gather(out, lse, rows, heads), ro, rl, Q.dtype, "control g=%d/%d L=%d" % (H_q, H_kv, L))
 
 
 # ---- determinism, repeats, capture, threads ---------------------------------------------------------------------------------
