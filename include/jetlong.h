@@ -93,13 +93,14 @@ int jetlong_prefill_prerotated(const void* Q, const void* K, const void* V, void
  * The paper's UNFUSED procedure on the GPU (Section 3.3, "Jet-Long (unfused)" of Table 7), a baseline
  * for the fused kernel, never the product path: three launches of the same tcgen05 attention kernel --
  *   A: sliding-window attention (0 <= q-k <= w_local) on the stored Q, K;
- *   B: full causal attention on Q' = R(Delta q) Q, K' = R(Delta k) K (both written once to the workspace as fp16);
- *   C: sliding-window attention on Q', K' --
- * each returning (O_X, l_X), then Eq.(7) WITH the minus sign: O = (W_A O_A + W_B O_B - W_C O_C) / (W_A + W_B - W_C).
- * The band is computed three times and the remote operands carry one fp16 rounding without compensation, so on
- * outlier-channel inputs lse is only good to ~3e-3 (the fused default: ~3e-4); out stays within the bf16 tolerance.
+ *   B: full causal attention at the remote positions, Q' = R(Delta q) Q, K' = R(Delta k) K;
+ *   C: sliding-window attention at the remote positions --
+ * each returning (O_X in fp32, l_X), then Eq.(7) WITH the minus sign in fp32:
+ *   O = (W_A O_A + W_B O_B - W_C O_C) / (W_A + W_B - W_C).
+ * K' is written once to the workspace (as in jetlong_prefill_prerotated); B and C score with the same compensated remote
+ * operands as the fused kernel, so the baseline meets the same tolerances; the band is computed three times.
  * bf16, head_dim 128; workspace >= jetlong_workspace_bytes(JETLONG_OP_PREFILL_UNFUSED, ...)
- * (tables + Q', K', O_B, O_C, l_B, l_C: about 4.5x the size of Q).
+ * (the workspace variant's region + O_A, O_B, O_C in fp32 + l_B, l_C: about 6.5x the size of Q).
  */
 int jetlong_prefill_unfused(const void* Q, const void* K, const void* V, void* out, float* lse,
                             int64_t L, int H_q, int H_kv, int head_dim,

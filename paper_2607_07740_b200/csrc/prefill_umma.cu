@@ -775,33 +775,13 @@ __global__ void __launch_bounds__(256) prerotate_k_kernel(const __nv_bfloat16* _
     }
 }
 
-// ---- 8(f)-2: the unfused three-call baseline ("Jet-Long (unfused)") ------------------------------
-// X' = R(Delta pos) X as fp16, one rounding: the remote-position operands of calls B and C.  Thread = (row, head, chunk).
-__global__ void __launch_bounds__(256) prerotate_hi_kernel(const __nv_bfloat16* __restrict__ X, __half* __restrict__ Xr,
-                                                           long long L, int H, long long G,
-                                                           const float2* __restrict__ lo, const float2* __restrict__ hi) {
-    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (idx >= L * H * 8) return;
-    const int c = (int)(idx & 7);
-    const long long row = idx >> 3;
-    const long long pos = row / H;
-    const uint4 u1 = __ldg(reinterpret_cast<const uint4*>(X + row * D) + c);
-    const uint4 u2 = __ldg(reinterpret_cast<const uint4*>(X + row * D) + 8 + c);
-    float cs_c[8], cs_s[8];
-    cs8(lo, hi, pos, G, 8 * c, cs_c, cs_s);
-    const uint32_t a[4] = {u1.x, u1.y, u1.z, u1.w}, b[4] = {u2.x, u2.y, u2.z, u2.w};
-    uint32_t h1[4], h2[4], l1[4], l2[4];
-    rot8(a, b, cs_c, cs_s, h1, h2, l1, l2);
-    reinterpret_cast<uint4*>(Xr + row * D)[c] = make_uint4(h1[0], h1[1], h1[2], h1[3]);
-    reinterpret_cast<uint4*>(Xr + row * D)[8 + c] = make_uint4(h2[0], h2[1], h2[2], h2[3]);
-}
-
-// Eq.(7) P:114 with the minus sign: O = (W_A O_A + W_B O_B - W_C O_C) / (W_A + W_B - W_C), W_X = exp(l_X - M).
-// A is read from and the result written to (out, lse).  Thread = (row q, head h, 8 channels).
+// Eq.(7) P:114 with the minus sign: O = (W_A O_A + W_B O_B - W_C O_C) / (W_A + W_B - W_C), W_X = exp(l_X - M); numerator and
+// denominator in fp32.  The partial outputs are fp32; the result is rounded once to bf16.  Thread = (row q, head h,
+// 8 channels); lA is read from and the merged lse written to `lse`.
 __global__ void __launch_bounds__(256) merge_abc_kernel(__nv_bfloat16* __restrict__ out, float* __restrict__ lse,
-                                                        const __nv_bfloat16* __restrict__ oB, const float* __restrict__ lB,
-                                                        const __nv_bfloat16* __restrict__ oC, const float* __restrict__ lC,
-                                                        long long L, int H_q) {
+                                                        const float* __restrict__ oA, const float* __restrict__ oB,
+                                                        const float* __restrict__ lB, const float* __restrict__ oC,
+                                                        const float* __restrict__ lC, long long L, int H_q) {
     const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= L * H_q * 16) return;
     const int c = (int)(idx & 15);
@@ -814,19 +794,19 @@ __global__ void __launch_bounds__(256) merge_abc_kernel(__nv_bfloat16* __restric
     const float wA = __expf(a - M), wB = __expf(b - M), wC = __expf(cc - M);
     const float den = wA + wB - wC;
     const float inv = 1.0f / den;
-    uint4 ua = reinterpret_cast<const uint4*>(out + row * D)[c];
-    const uint4 ub = reinterpret_cast<const uint4*>(oB + row * D)[c], uc = reinterpret_cast<const uint4*>(oC + row * D)[c];
-    uint32_t* pa = reinterpret_cast<uint32_t*>(&ua);
-    const uint32_t* pb = reinterpret_cast<const uint32_t*>(&ub);
-    const uint32_t* pc = reinterpret_cast<const uint32_t*>(&uc);
+    float va[8], vb[8], vc[8];
+    *reinterpret_cast<float4*>(va) = reinterpret_cast<const float4*>(oA + row * D)[2 * c];
+    *reinterpret_cast<float4*>(va + 4) = reinterpret_cast<const float4*>(oA + row * D)[2 * c + 1];
+    *reinterpret_cast<float4*>(vb) = reinterpret_cast<const float4*>(oB + row * D)[2 * c];
+    *reinterpret_cast<float4*>(vb + 4) = reinterpret_cast<const float4*>(oB + row * D)[2 * c + 1];
+    *reinterpret_cast<float4*>(vc) = reinterpret_cast<const float4*>(oC + row * D)[2 * c];
+    *reinterpret_cast<float4*>(vc + 4) = reinterpret_cast<const float4*>(oC + row * D)[2 * c + 1];
+    uint32_t w[4];
 #pragma unroll
-    for (int j = 0; j < 4; ++j) {
-        const float a0 = __uint_as_float(pa[j] << 16), a1 = __uint_as_float(pa[j] & 0xffff0000u);
-        const float b0 = __uint_as_float(pb[j] << 16), b1 = __uint_as_float(pb[j] & 0xffff0000u);
-        const float c0 = __uint_as_float(pc[j] << 16), c1 = __uint_as_float(pc[j] & 0xffff0000u);
-        pa[j] = bf16x2((wA * a0 + wB * b0 - wC * c0) * inv, (wA * a1 + wB * b1 - wC * c1) * inv);
-    }
-    reinterpret_cast<uint4*>(out + row * D)[c] = ua;
+    for (int j = 0; j < 4; ++j)
+        w[j] = bf16x2((wA * va[2 * j] + wB * vb[2 * j] - wC * vc[2 * j]) * inv,
+                      (wA * va[2 * j + 1] + wB * vb[2 * j + 1] - wC * vc[2 * j + 1]) * inv);
+    reinterpret_cast<uint4*>(out + row * D)[c] = make_uint4(w[0], w[1], w[2], w[3]);
     __syncwarp();                                                     // the 16 threads of a (q, h) all read lse first
     if (c == 0) lse[li] = M + __logf(den);
 }
@@ -889,10 +869,11 @@ bool make_kv_tensor_map(CUtensorMap* m, const void* base, long long L, int H, in
     return make_tensor_map(m, base, L, H, rows, 2);
 }
 
+size_t umma_prefill_prerot_workspace_bytes(long long L, int H_kv, int d);
 size_t umma_prefill_unfused_workspace_bytes(long long L, int H_q, int H_kv, int d) {
-    const size_t nq = (size_t)L * H_q * d, nk = (size_t)L * H_kv * d;
-    // tables | Q' fp16 | K' fp16 | out_B | out_C | lse_B | lse_C
-    return two_level_bytes(L + 256, d) + 3 * align256(2 * nq) + align256(2 * nk) + 2 * align256((size_t)L * H_q * 4);
+    const size_t nq = (size_t)L * H_q * d;
+    // the workspace variant's region (tables | K'hi fp16 | K' / K'lo e5m2 | selection) | O_A, O_B, O_C fp32 | lse_B | lse_C
+    return umma_prefill_prerot_workspace_bytes(L, H_kv, d) + 3 * align256(4 * nq) + 2 * align256((size_t)L * H_q * 4);
 }
 
 // 1: the default precision of the on-the-fly two-tile kernel uses the selective e5m2 compensation; 0: the full cross terms
@@ -985,7 +966,7 @@ int launch_prefill_umma(const void* Q, const void* K, const void* V, void* out, 
         if (!make_kv_tensor_map(&a.tmQ, Q, L, H_q, 128)) return JETLONG_UNSUPPORTED;
         a.tmK = tmK; a.tmV = tmV; a.tmKh = tmKh; a.tmKe = tmKe; a.tmKl = tmKl;
         a.out = p.out; a.lse = lse; a.L = L; a.w0 = w0; a.G = G; a.H_q = H_q; a.H_kv = H_kv;
-        a.bifocal = p.bifocal; a.precise = precise; a.prerot = p.prerot; a.window_only = 0; a.qk_f16 = 0;
+        a.bifocal = p.bifocal; a.precise = precise; a.prerot = p.prerot; a.window_only = 0; a.qk_f16 = 0; a.out_f32 = 0;
         a.lo = p.lo; a.hi = p.hi; a.selinfo = p.selinfo;
         return launch_prefill_v2(a, st);
     }
@@ -1003,22 +984,15 @@ int launch_prefill_umma(const void* Q, const void* K, const void* V, void* out, 
 
 namespace jetlong {
 
-// One launch of the tcgen05 kernel on given operands: window_only = the local band only, qk_f16 = fp16 Q/K operands.
-static int launch_plain(const void* Q, const void* K, const void* V, void* out, float* lse, long long L, int H_q, int H_kv,
-                        long long w0, bool window_only, bool qk_f16, cudaStream_t st) {
-    PrefillV2Args a;
-    if (!make_kv_tensor_map(&a.tmK, K, L, H_kv, 64) || !make_kv_tensor_map(&a.tmV, V, L, H_kv, 128) ||
-        !make_kv_tensor_map(&a.tmQ, Q, L, H_q, 128))
-        return JETLONG_UNSUPPORTED;
-    a.tmKh = a.tmK; a.tmKe = a.tmK; a.tmKl = a.tmK;
-    a.out = (__nv_bfloat16*)out; a.lse = lse; a.L = L; a.w0 = w0; a.G = 1; a.H_q = H_q; a.H_kv = H_kv;
-    a.bifocal = window_only ? 1 : 0; a.precise = 0; a.prerot = 0; a.window_only = window_only ? 1 : 0; a.qk_f16 = qk_f16 ? 1 : 0;
-    a.lo = nullptr; a.hi = nullptr; a.selinfo = nullptr;
-    return launch_prefill_v2(a, st);
-}
-
-// A = window attention on the stored Q, K; B = full causal attention at the remote positions; C = window attention at
-// the remote positions; then Eq.(7) with the minus sign.  Remote operands are rounded once to fp16.
+// ---- 8(f)-2: the unfused three-call baseline ("Jet-Long (unfused)") ---------------------------------------
+// Three launches of the two-tile kernel, each returning (O_X fp32, l_X), then Eq.(7) with the minus sign:
+//   A = the local band 0 <= q-k <= w0 on the stored Q, K;
+//   B = full causal attention at the remote positions: the bifocal kernel with an EMPTY local window (w0 = -1), remote
+//       operands from the workspace variant's scratch, compensated exactly as the fused product;
+//   C = the band scored with the remote operands (window_only = 2).
+// Round 1 ran B and C on once-rounded fp16 operands and stored O_B, O_C in bf16 (lse ~3e-3, out errors up to 0.9 from the
+// cancellation); with fp32 partials and the product's compensated operands the baseline is as accurate as the fused
+// kernel up to the cancellation Eq.(7) itself carries.
 int launch_prefill_unfused(const void* Q, const void* K, const void* V, void* out, float* lse, long long L, int H_q,
                            int H_kv, int d, long long w0, long long G, double theta, void* ws, cudaStream_t st) {
     int rc = build_two_level(ws, L + 256, d, theta, st);
@@ -1027,22 +1001,35 @@ int launch_prefill_unfused(const void* Q, const void* K, const void* V, void* ou
     const float2* hi = lo + 256 * (d / 2);
     const size_t nq = (size_t)L * H_q * d, nk = (size_t)L * H_kv * d;
     unsigned char* base = (unsigned char*)ws + two_level_bytes(L + 256, d);
-    __half* Qr = reinterpret_cast<__half*>(base);
-    __half* Kr = reinterpret_cast<__half*>(base + align256(2 * nq));
-    unsigned char* oB = base + align256(2 * nq) + align256(2 * nk);
-    unsigned char* oC = oB + align256(2 * nq);
-    float* lB = reinterpret_cast<float*>(oC + align256(2 * nq));
-    float* lC = reinterpret_cast<float*>(reinterpret_cast<unsigned char*>(lB) + align256((size_t)L * H_q * 4));
-    prerotate_hi_kernel<<<(unsigned)((L * H_q * 8 + 255) / 256), 256, 0, st>>>((const __nv_bfloat16*)Q, Qr, L, H_q, G, lo, hi);
-    prerotate_hi_kernel<<<(unsigned)((L * H_kv * 8 + 255) / 256), 256, 0, st>>>((const __nv_bfloat16*)K, Kr, L, H_kv, G, lo, hi);
-    note_launch(2);
-    rc = check_launch("prerotate_hi_kernel");
+    __half* Kh = reinterpret_cast<__half*>(base);
+    unsigned char* Ke = base + align256(2 * nk);
+    unsigned char* Kl = Ke + align256(nk);
+    uint32_t* selinfo = nullptr;
+    rc = run_selection(Q, K, L, H_q, H_kv, Kl + align256(nk), st, &selinfo);
     if (rc != JETLONG_OK) return rc;
-    if ((rc = launch_plain(Q, K, V, out, lse, L, H_q, H_kv, w0, true, false, st)) != JETLONG_OK) return rc;     // A
-    if ((rc = launch_plain(Qr, Kr, V, oB, lB, L, H_q, H_kv, w0, false, true, st)) != JETLONG_OK) return rc;     // B
-    if ((rc = launch_plain(Qr, Kr, V, oC, lC, L, H_q, H_kv, w0, true, true, st)) != JETLONG_OK) return rc;      // C
-    merge_abc_kernel<<<(unsigned)((L * H_q * 16 + 255) / 256), 256, 0, st>>>((__nv_bfloat16*)out, lse, (const __nv_bfloat16*)oB, lB,
-                                                                          (const __nv_bfloat16*)oC, lC, L, H_q);
+    prerotate_k_kernel<<<(unsigned)((L * H_kv * 8 + 255) / 256), 256, 0, st>>>((const __nv_bfloat16*)K, Kh, Ke, Kl, L, H_kv, G, lo, hi, selinfo);
+    note_launch();
+    if ((rc = check_launch("prerotate_k_kernel")) != JETLONG_OK) return rc;
+    unsigned char* part = (unsigned char*)ws + umma_prefill_prerot_workspace_bytes(L, H_kv, d);
+    float* oA = reinterpret_cast<float*>(part);
+    float* oB = reinterpret_cast<float*>(part + align256(4 * nq));
+    float* oC = reinterpret_cast<float*>(part + 2 * align256(4 * nq));
+    float* lB = reinterpret_cast<float*>(part + 3 * align256(4 * nq));
+    float* lC = reinterpret_cast<float*>(reinterpret_cast<unsigned char*>(lB) + align256((size_t)L * H_q * 4));
+    PrefillV2Args a;
+    if (!make_kv_tensor_map(&a.tmK, K, L, H_kv, 64) || !make_kv_tensor_map(&a.tmV, V, L, H_kv, 128) ||
+        !make_kv_tensor_map(&a.tmQ, Q, L, H_q, 128) || !make_tensor_map(&a.tmKh, Kh, L, H_kv, 64, 2) ||
+        !make_tensor_map(&a.tmKe, Ke, L, H_kv, 64, 1) || !make_tensor_map(&a.tmKl, Kl, L, H_kv, 64, 1))
+        return JETLONG_UNSUPPORTED;
+    a.L = L; a.G = G; a.H_q = H_q; a.H_kv = H_kv; a.bifocal = 1; a.precise = 3; a.qk_f16 = 0; a.out_f32 = 1;
+    a.lo = lo; a.hi = hi; a.selinfo = selinfo;
+    a.out = oA; a.lse = lse; a.w0 = w0; a.prerot = 0; a.window_only = 1;                         // A
+    if ((rc = launch_prefill_v2(a, st)) != JETLONG_OK) return rc;
+    a.out = oB; a.lse = lB; a.w0 = -1; a.prerot = 1; a.window_only = 0;                          // B
+    if ((rc = launch_prefill_v2(a, st)) != JETLONG_OK) return rc;
+    a.out = oC; a.lse = lC; a.w0 = w0; a.prerot = 1; a.window_only = 2;                          // C
+    if ((rc = launch_prefill_v2(a, st)) != JETLONG_OK) return rc;
+    merge_abc_kernel<<<(unsigned)((L * H_q * 16 + 255) / 256), 256, 0, st>>>((__nv_bfloat16*)out, lse, oA, oB, lB, oC, lC, L, H_q);
     note_launch();
     return check_launch("merge_abc_kernel");
 }

@@ -102,7 +102,7 @@ struct Params {
     float* lse;
     long long L, w0, G;
     int H_q, H_kv, g;
-    int bifocal, precise, prerot, window_only, qk_f16;
+    int bifocal, precise, prerot, window_only, qk_f16, out_f32;
     int n_qb, n_sb, n_s4;
     const float2* lo;
     const float2* hi;
@@ -112,10 +112,13 @@ struct Params {
 struct Visit { int kt; int mode; };                   // mode 0 = causal/control, 1 = local, 2 = remote
 
 // visit list of ONE 128-row query tile qb (step a3): local key tiles [kt_lo, qb] descending, then remote [0, kt_hi] descending
+// window_only: 0 = the full bifocal rule; 1 = only the local band 0 <= q-k <= w0 on the stored operands (call A of the
+// unfused baseline); 2 = the same band scored with the REMOTE operands (call C: "sliding window, remote q/k"):
+// no local visit, the remote list covers the band's key tiles and carries the band's mask
 struct Plan {
-    int qb, kt_lo, kt_hi, n_local, n_remote, nv;
-    __device__ Plan() : qb(0), kt_lo(1), kt_hi(-1), n_local(0), n_remote(0), nv(0) {}
-    __device__ Plan(int qb_, long long w0, bool bifocal, bool window_only) : qb(qb_) {
+    int qb, kt_lo, kt_hi, kt_rlo, n_local, n_remote, nv;
+    __device__ Plan() : qb(0), kt_lo(1), kt_hi(-1), kt_rlo(0), n_local(0), n_remote(0), nv(0) {}
+    __device__ Plan(int qb_, long long w0, bool bifocal, int window_only) : qb(qb_), kt_rlo(0) {
         const long long q0 = (long long)qb * BM;
         if (!bifocal) { kt_lo = 0; n_local = qb + 1; n_remote = 0; kt_hi = -1; nv = n_local; return; }
         long long t = q0 - w0 - (BN - 1);                              // local iff k0 >= t
@@ -124,8 +127,9 @@ struct Plan {
         long long u = q0 + (BM - 1) - 1 - w0;                          // remote iff k0 <= u  (q0+127-k0 > w0)
         kt_hi = u < 0 ? -1 : (int)(u / BN);
         if (kt_hi > qb) kt_hi = qb;
-        if (window_only) kt_hi = -1;
-        n_remote = kt_hi + 1;
+        if (window_only == 1) kt_hi = -1;
+        if (window_only == 2) { kt_rlo = kt_lo; kt_hi = qb; kt_lo = qb + 1; n_local = 0; }
+        n_remote = kt_hi - kt_rlo + 1;
         nv = n_local + n_remote;
     }
     __device__ Visit at(int v, bool bifocal) const {
@@ -143,11 +147,11 @@ struct Plan {
 // when either CTA's block needs the key tile; the block that does not need it sees the visit fully masked (the masks in
 // the softmax are the exact per-row rule, whatever the tile), so no special case exists below this struct.
 struct MPlan {
-    int lo0, top0, hi0, lo1, top1, hi1;               // tile i: local key tiles [lo_i, top_i], remote [0, hi_i] (joint over the CTAs)
-    int lo_m, top_m, hi_m, n_loc, n_rem, nm;
+    int lo0, top0, hi0, rlo0, lo1, top1, hi1, rlo1;   // tile i: local key tiles [lo_i, top_i], remote [rlo_i, hi_i] (joint over the CTAs)
+    int lo_m, top_m, hi_m, rlo_m, n_loc, n_rem, nm;
     bool bifocal;
-    __device__ MPlan(int qbA, int qbB, int n_qb, long long w0, bool bifocal_, bool window_only) : bifocal(bifocal_) {
-        lo0 = lo1 = 1 << 30; top0 = top1 = -1; hi0 = hi1 = -1;
+    __device__ MPlan(int qbA, int qbB, int n_qb, long long w0, bool bifocal_, int window_only) : bifocal(bifocal_) {
+        lo0 = lo1 = rlo0 = rlo1 = 1 << 30; top0 = top1 = -1; hi0 = hi1 = -1;
 #pragma unroll
         for (int c = 0; c < 2; ++c) {
 #pragma unroll
@@ -155,17 +159,17 @@ struct MPlan {
                 const int qb = (c ? qbB : qbA) + i;
                 if (qb >= n_qb) continue;
                 const Plan t(qb, w0, bifocal, window_only);
-                int& lo = i ? lo1 : lo0; int& top = i ? top1 : top0; int& hi = i ? hi1 : hi0;
-                lo = t.kt_lo < lo ? t.kt_lo : lo;
-                top = qb > top ? qb : top;
-                hi = t.kt_hi > hi ? t.kt_hi : hi;
+                int& lo = i ? lo1 : lo0; int& top = i ? top1 : top0; int& hi = i ? hi1 : hi0; int& rlo = i ? rlo1 : rlo0;
+                if (t.n_local > 0) { lo = t.kt_lo < lo ? t.kt_lo : lo; top = qb > top ? qb : top; }
+                if (t.n_remote > 0) { hi = t.kt_hi > hi ? t.kt_hi : hi; rlo = t.kt_rlo < rlo ? t.kt_rlo : rlo; }
             }
         }
         lo_m = lo0 < lo1 ? lo0 : lo1;
         top_m = top0 > top1 ? top0 : top1;
         hi_m = hi0 > hi1 ? hi0 : hi1;
+        rlo_m = rlo0 < rlo1 ? rlo0 : rlo1;
         n_loc = top_m >= lo_m ? top_m - lo_m + 1 : 0;
-        n_rem = hi_m + 1;
+        n_rem = hi_m >= rlo_m ? hi_m - rlo_m + 1 : 0;
         nm = n_loc + n_rem;
     }
     __device__ __forceinline__ Visit at(int m) const {
@@ -175,8 +179,8 @@ struct MPlan {
         return x;
     }
     __device__ __forceinline__ bool part(int i, const Visit& x) const {
-        const int lo = i ? lo1 : lo0, top = i ? top1 : top0, hi = i ? hi1 : hi0;
-        return x.mode == 2 ? x.kt <= hi : (x.kt >= lo && x.kt <= top);
+        const int lo = i ? lo1 : lo0, top = i ? top1 : top0, hi = i ? hi1 : hi0, rlo = i ? rlo1 : rlo0;
+        return x.mode == 2 ? (x.kt <= hi && x.kt >= rlo) : (x.kt >= lo && x.kt <= top);
     }
 };
 
@@ -294,7 +298,7 @@ prefill_umma2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_const
     }
     const int qb0 = cta ? qbB : qbA;                               // this CTA's first query block
     const bool bifocal = p.bifocal != 0;
-    const MPlan mp(qbA, qbB, p.n_qb, p.w0, bifocal, p.window_only != 0);
+    const MPlan mp(qbA, qbB, p.n_qb, p.w0, bifocal, p.window_only);
     // 0 fast, 2 e5m2 cross terms, 3 e5m2 cross terms over the two highest-energy pairs of every 8-pair chunk; a KV head
     // whose other channels are too loud falls back from 3 to 2
     int precise = (bifocal && mp.n_rem > 0) ? p.precise : 0;
@@ -572,10 +576,14 @@ prefill_umma2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_const
                 lo = a > 0 ? (int)a : 0;
                 masked = true;
             }
-            if (x.mode == 2 && (q0 - (k0 + BN - 1) <= p.w0)) {                                   // q-k > w0
+            if (x.mode == 2 && p.window_only != 2 && (q0 - (k0 + BN - 1) <= p.w0)) {             // q-k > w0
                 const long long a = qrel - p.w0 - 1;
                 hi = a < hi ? (int)a : hi;
                 masked = true;
+            }
+            if (x.mode == 2 && p.window_only == 2) {                                             // call C: 0 <= q-k <= w0
+                if (k0 + BN - 1 > q0) { hi = qrel < hi ? (int)qrel : hi; masked = true; }
+                if (q0 + BM - 1 - k0 > p.w0) { const long long a = qrel - p.w0; lo = a > 0 ? (int)a : 0; masked = true; }
             }
             TR(1 + i, v, 0);
             mbar_wait_sleep(&bars->s_full[i], (uint32_t)v & 1u);
@@ -653,12 +661,19 @@ prefill_umma2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_const
             const float inv = 1.0f / l;
             const bool qok = q < p.L;
             __nv_bfloat16* orow = p.out + ((size_t)(qok ? q : 0) * p.H_q + head) * D;
+            float* orow32 = reinterpret_cast<float*>(p.out) + ((size_t)(qok ? q : 0) * p.H_q + head) * D;   // out_f32 (unfused baseline)
 #pragma unroll 1
             for (int ch = 0; ch < 4; ++ch) {
                 uint32_t rg[32];
                 tmem_ld32(tO + ch * 32, rg);
                 tmem_ld_wait();
-                if (qok) {
+                if (qok && p.out_f32) {
+#pragma unroll
+                    for (int j = 0; j < 32; j += 4)
+                        *reinterpret_cast<float4*>(orow32 + ch * 32 + j) =
+                            make_float4(__uint_as_float(rg[j]) * inv, __uint_as_float(rg[j + 1]) * inv,
+                                        __uint_as_float(rg[j + 2]) * inv, __uint_as_float(rg[j + 3]) * inv);
+                } else if (qok) {
 #pragma unroll
                     for (int j = 0; j < 32; j += 8) {
                         uint32_t w[4];
@@ -690,10 +705,10 @@ extern "C" int jetlong_debug_trace(long long* dst, int n, int block) {
 
 int launch_prefill_v2(const PrefillV2Args& a, cudaStream_t st) {
     Params p;
-    p.out = a.out; p.lse = a.lse;
+    p.out = (__nv_bfloat16*)a.out; p.lse = a.lse;
     p.L = a.L; p.w0 = a.w0; p.G = a.G;
     p.H_q = a.H_q; p.H_kv = a.H_kv; p.g = a.H_q / a.H_kv;
-    p.bifocal = a.bifocal; p.precise = a.precise; p.prerot = a.prerot; p.window_only = a.window_only; p.qk_f16 = a.qk_f16;
+    p.bifocal = a.bifocal; p.precise = a.precise; p.prerot = a.prerot; p.window_only = a.window_only; p.qk_f16 = a.qk_f16; p.out_f32 = a.out_f32;
     p.n_qb = (int)((a.L + BM - 1) / BM);
     p.n_sb = (p.n_qb + 1) / 2;
     p.n_s4 = (p.n_qb + 3) / 4;

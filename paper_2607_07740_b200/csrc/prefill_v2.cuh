@@ -10,14 +10,15 @@ struct PrefillV2Args {
     CUtensorMap tmQ;                                  // Q (or Q' fp16) [L, H_q, 128], box 64 channels x 1 head x 128 rows
     CUtensorMap tmK, tmV;                             // stored K (box 64 x 1 x 64 rows), V (box 64 x 1 x 128 rows)
     CUtensorMap tmKh, tmKe, tmKl;                     // workspace variant: K'hi fp16, K' e5m2 / compact rows, K'lo e5m2
-    __nv_bfloat16* out;
+    void* out;                                        // bf16 [L, H_q, 128], or fp32 when out_f32
     float* lse;
     long long L, w0, G;
     int H_q, H_kv;
     int bifocal;                                      // 0: control (every visit multiplies the stored operands)
     int precise;                                      // 0 fast, 2 full e5m2 cross terms, 3 selective e5m2 cross terms
     int prerot;                                       // remote K tiles come pre-rotated from the workspace (8(f)-1)
-    int window_only;                                  // only the local band (calls A and C of the unfused baseline)
+    int window_only;                                  // 1: only the local band on the stored operands (call A); 2: the band on the remote operands (call C)
+    int out_f32;                                      // out holds fp32 (partial outputs of the unfused baseline)
     int qk_f16;                                       // Q and K hold fp16 (pre-rotated operands of calls B and C)
     const float2* lo;                                 // two-level (cos, sin) tables
     const float2* hi;

@@ -91,14 +91,14 @@ def test_prefill_precision_switch_is_host_state():
 
 def test_workspace_sizes_of_the_prefill_variants():
     """the workspace variant holds tables + K'hi (2 B) + two e5m2 buffers (1 B each) per key channel
-    + the selection scratch; the unfused baseline holds tables + Q', O_B, O_C (2 B per query channel) + K' + two lse."""
+    + the selection scratch; the unfused baseline holds the same region + O_A, O_B, O_C in fp32 (4 B per query channel) + two lse."""
     L, H_q, H_kv, d = 65536, 16, 8, 128
     pre = B.jetlong_workspace_bytes(B.OP_PREFILL_PREROTATED, L, H_q, H_kv, d, B.BF16)
     unf = B.jetlong_workspace_bytes(B.OP_PREFILL_UNFUSED, L, H_q, H_kv, d, B.BF16)
     nk, nq = L * H_kv * d, L * H_q * d
     slack = 1 << 20                                       # two-level rotation table (0.2 MB here) + alignment + selection scratch
     assert 4 * nk <= pre <= 4 * nk + slack
-    assert 6 * nq + 2 * nk + 8 * L * H_q <= unf <= 6 * nq + 2 * nk + 8 * L * H_q + slack
+    assert pre + 12 * nq + 8 * L * H_q <= unf <= pre + 12 * nq + 8 * L * H_q + slack
     # shapes the tcgen05 kernel does not serve have no such variants
     assert B.jetlong_workspace_bytes(B.OP_PREFILL_PREROTATED, 1024, 4, 2, 64, B.FP32) == 0
     assert B.jetlong_workspace_bytes(B.OP_PREFILL_UNFUSED, 1024, 3, 1, 64, B.BF16) == 0         # head_dim 64
