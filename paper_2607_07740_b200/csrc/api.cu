@@ -56,7 +56,8 @@ int launch_prefill_unfused(const void* Q, const void* K, const void* V, void* ou
                            int H_kv, int d, long long w0, long long G, double theta, void* ws, cudaStream_t st);
 int launch_prefill_umma(const void* Q, const void* K, const void* V, void* out, float* lse, long long L, int H_q,
                         int H_kv, int d, long long w0, long long G, double theta, bool bifocal, int precise, void* ws,
-                        size_t ws_bytes, cudaStream_t st, bool prerot, bool two_tile, FreqMap fm);
+                        size_t ws_bytes, cudaStream_t st, bool prerot, bool two_tile, FreqMap fm, int qb_lo, int qb_hi,
+                        long long L_sel);
 
 // decode.cu / decode_umma.cu
 bool umma_decode_supported(int H_q, int H_kv, int d, int dtype);
@@ -104,7 +105,7 @@ static size_t prefill_ws(long long L, int H_q, int H_kv, int d, int dtype, bool 
 static int prefill_common(const void* Q, const void* K, const void* V, void* out, float* lse, long long L, int H_q,
                           int H_kv, int d, long long w0, long long w_pre, double theta, int dtype, void* ws,
                           size_t ws_bytes, void* stream, bool bifocal, bool prerot = false,
-                          const jetlong_options* opt = nullptr) {
+                          const jetlong_options* opt = nullptr, int qb_lo = 0, int qb_hi = -1) {
     int rc = validate(Q, K, V, out, lse, L, H_q, H_kv, d, w0, w_pre, theta, dtype);
     if (rc != JETLONG_OK) return rc;
     const Resolved o = resolve(opt);
@@ -124,7 +125,8 @@ static int prefill_common(const void* Q, const void* K, const void* V, void* out
         return launch_prefill_umma(Q, K, V, out, lse, L, H_q, H_kv, d, w0, G, theta, bifocal,
                                    prec == JETLONG_PRECISION_FAST ? 0 : prec == JETLONG_PRECISION_COMPENSATED_F16 ? 1 : prec == JETLONG_PRECISION_COMPENSATED_E5M2 ? 6 : 2,
                                    ws, ws_bytes, st,
-                                   prerot && bifocal, /*two_tile=*/o.impl != 1, fm);
+                                   prerot && bifocal, /*two_tile=*/o.impl != 1 || qb_hi >= 0, fm, qb_lo, qb_hi,
+                                   qb_hi >= 0 ? 128ll * qb_hi : L);
     const float2* tab = nullptr;
     if (bifocal) {
         rc = build_key_table((float2*)ws, L, G, d, theta, st, fm);
@@ -284,7 +286,12 @@ int jetlong_causal_decode(const void* q, const void* Kcache, const void* Vcache,
 }
 
 // staging arena of jetlong_prefill_host: one per device, grown on demand, reused from call to call
-struct HostArena { unsigned char* base = nullptr; size_t bytes = 0; cudaStream_t st = nullptr; };
+struct HostArena {
+    unsigned char* base = nullptr;
+    size_t bytes = 0;
+    cudaStream_t st = nullptr, st_in = nullptr, st_out = nullptr;   // compute, host-to-device, device-to-host
+    cudaEvent_t ev_in[16] = {}, ev_done[16] = {};
+};
 static HostArena g_arena[64];
 static std::mutex g_arena_mu;
 
@@ -298,6 +305,9 @@ void jetlong_host_release(void) {
         cudaSetDevice(d);
         if (a.base) cudaFree(a.base);
         if (a.st) cudaStreamDestroy(a.st);
+        if (a.st_in) cudaStreamDestroy(a.st_in);
+        if (a.st_out) cudaStreamDestroy(a.st_out);
+        for (int i = 0; i < 16; ++i) { if (a.ev_in[i]) cudaEventDestroy(a.ev_in[i]); if (a.ev_done[i]) cudaEventDestroy(a.ev_done[i]); }
         a = HostArena();
     }
     cudaSetDevice(cur);
@@ -311,7 +321,8 @@ int jetlong_prefill_host(const void* Q, const void* K, const void* V, void* out,
     rc = device_ok();
     if (rc != JETLONG_OK) return rc;
     const size_t es = dtype == JETLONG_FP32 ? 4 : 2;
-    const size_t nq = (size_t)L * H_q * head_dim * es, nk = (size_t)L * H_kv * head_dim * es;
+    const size_t rq = (size_t)H_q * head_dim * es, rk = (size_t)H_kv * head_dim * es;   // bytes per row
+    const size_t nq = (size_t)L * rq, nk = (size_t)L * rk;
     const size_t nl = (size_t)L * H_q * sizeof(float);
     const size_t nws = jetlong_workspace_bytes(JETLONG_OP_PREFILL, L, H_q, H_kv, head_dim, dtype);
     const size_t oq = 0, ok = align256(nq), ov = ok + align256(nk), oo = ov + align256(nk), ol = oo + align256(nq),
@@ -320,28 +331,63 @@ int jetlong_prefill_host(const void* Q, const void* K, const void* V, void* out,
     if (cudaGetDevice(&devid) != cudaSuccess || devid < 0 || devid >= 64) return check_launch("cudaGetDevice");
     std::lock_guard<std::mutex> lock(g_arena_mu);               // calls are serialised: they share the arena
     HostArena& a = g_arena[devid];
-    if (!a.st && cudaStreamCreateWithFlags(&a.st, cudaStreamNonBlocking) != cudaSuccess) return check_launch("cudaStreamCreate");
+    if (!a.st) {
+        if (cudaStreamCreateWithFlags(&a.st, cudaStreamNonBlocking) != cudaSuccess ||
+            cudaStreamCreateWithFlags(&a.st_in, cudaStreamNonBlocking) != cudaSuccess ||
+            cudaStreamCreateWithFlags(&a.st_out, cudaStreamNonBlocking) != cudaSuccess)
+            return check_launch("cudaStreamCreate");
+        for (int i = 0; i < 16; ++i)
+            if (cudaEventCreateWithFlags(&a.ev_in[i], cudaEventDisableTiming) != cudaSuccess ||
+                cudaEventCreateWithFlags(&a.ev_done[i], cudaEventDisableTiming) != cudaSuccess)
+                return check_launch("cudaEventCreate");
+    }
     if (a.bytes < total) {
         if (a.base && cudaFree(a.base) != cudaSuccess) return check_launch("cudaFree");
         a.base = nullptr; a.bytes = 0;
         if (cudaMalloc(&a.base, total) != cudaSuccess) return check_launch("cudaMalloc");
         a.bytes = total;
-        // the table header must start zeroed (jetlong_workspace_bytes contract); afterwards the sealed tables are reused
-        if (cudaMemsetAsync(a.base + ow, 0, 256, a.st) != cudaSuccess) return check_launch("cudaMemsetAsync");
     }
     unsigned char* dev = a.base;
-    if (cudaMemcpyAsync(dev + ok, K, nk, cudaMemcpyHostToDevice, a.st) != cudaSuccess ||
-        cudaMemcpyAsync(dev + ov, V, nk, cudaMemcpyHostToDevice, a.st) != cudaSuccess ||
-        cudaMemcpyAsync(dev + oq, Q, nq, cudaMemcpyHostToDevice, a.st) != cudaSuccess)
-        return check_launch("jetlong_prefill_host H2D");
-    rc = jetlong_prefill(dev + oq, dev + ok, dev + ov, dev + oo, (float*)(dev + ol), L, H_q, H_kv, head_dim, w_local,
-                         w_pretrained, rope_theta, dtype, dev + ow, align256(nws) + 256, a.st);
-    if (rc != JETLONG_OK) { cudaStreamSynchronize(a.st); return rc; }
-    if (cudaMemcpyAsync(out, dev + oo, nq, cudaMemcpyDeviceToHost, a.st) != cudaSuccess ||
-        cudaMemcpyAsync(lse, dev + ol, nl, cudaMemcpyDeviceToHost, a.st) != cudaSuccess)
-        return check_launch("jetlong_prefill_host D2H");
-    if (cudaStreamSynchronize(a.st) != cudaSuccess) return check_launch("jetlong_prefill_host");
-    return JETLONG_OK;
+    // the table header must start zeroed (jetlong_workspace_bytes contract); the region moves with the shapes, so every call
+    if (cudaMemsetAsync(dev + ow, 0, 256, a.st) != cudaSuccess) return check_launch("cudaMemsetAsync");
+    // Row chunks, ascending: rows [r0, r1) need only keys < r1, so chunk c can run as soon as ITS rows of K, V, Q are on the
+    // device; its out / lse rows go back while the next chunk runs.  The tcgen05 two-tile kernel launches by row range
+    // (multiples of 512 rows); other shapes run as one chunk.
+    int nch = 1;
+    if (umma_prefill_supported(L, H_q, H_kv, head_dim, dtype) && L >= 8192) nch = L >= 32768 ? 8 : 4;
+    long long step = ((L + nch - 1) / nch + 511) / 512 * 512;
+    bool ok_all = true;
+    for (int c = 0; c < nch && ok_all; ++c) {
+        const long long r0 = c * step, r1 = (c + 1 == nch || (c + 1) * step > L) ? L : (c + 1) * step;
+        if (r0 >= L) { nch = c; break; }
+        const size_t n = (size_t)(r1 - r0);
+        ok_all = cudaMemcpyAsync(dev + ok + r0 * rk, (const unsigned char*)K + r0 * rk, n * rk, cudaMemcpyHostToDevice, a.st_in) == cudaSuccess &&
+                 cudaMemcpyAsync(dev + ov + r0 * rk, (const unsigned char*)V + r0 * rk, n * rk, cudaMemcpyHostToDevice, a.st_in) == cudaSuccess &&
+                 cudaMemcpyAsync(dev + oq + r0 * rq, (const unsigned char*)Q + r0 * rq, n * rq, cudaMemcpyHostToDevice, a.st_in) == cudaSuccess &&
+                 cudaEventRecord(a.ev_in[c], a.st_in) == cudaSuccess;
+        if (r1 == L) { nch = c + 1; break; }
+    }
+    if (!ok_all) { cudaStreamSynchronize(a.st_in); return check_launch("jetlong_prefill_host H2D"); }
+    for (int c = 0; c < nch; ++c) {
+        const long long r0 = c * step, r1 = (c + 1 == nch) ? L : (c + 1) * step;
+        if (cudaStreamWaitEvent(a.st, a.ev_in[c], 0) != cudaSuccess) { rc = check_launch("cudaStreamWaitEvent"); break; }
+        rc = prefill_common(dev + oq, dev + ok, dev + ov, dev + oo, (float*)(dev + ol), L, H_q, H_kv, head_dim, w_local,
+                            w_pretrained, rope_theta, dtype, dev + ow, align256(nws) + 256, a.st, true, false, nullptr,
+                            nch > 1 ? (int)(r0 / 128) : 0, nch > 1 ? (int)((r1 + 127) / 128) : -1);
+        if (rc != JETLONG_OK) break;
+        const size_t n = (size_t)(r1 - r0);
+        if (cudaEventRecord(a.ev_done[c], a.st) != cudaSuccess || cudaStreamWaitEvent(a.st_out, a.ev_done[c], 0) != cudaSuccess ||
+            cudaMemcpyAsync((unsigned char*)out + r0 * rq, dev + oo + r0 * rq, n * rq, cudaMemcpyDeviceToHost, a.st_out) != cudaSuccess ||
+            cudaMemcpy2DAsync(lse + r0, (size_t)L * 4, (float*)(dev + ol) + r0, (size_t)L * 4, n * 4, (size_t)H_q,
+                              cudaMemcpyDeviceToHost, a.st_out) != cudaSuccess) {
+            rc = check_launch("jetlong_prefill_host D2H");
+            break;
+        }
+    }
+    const bool s1 = cudaStreamSynchronize(a.st) == cudaSuccess, s2 = cudaStreamSynchronize(a.st_out) == cudaSuccess,
+               s3 = cudaStreamSynchronize(a.st_in) == cudaSuccess;
+    if (rc == JETLONG_OK && !(s1 && s2 && s3)) rc = check_launch("jetlong_prefill_host");
+    return rc;
 }
 
 const char* jetlong_status_string(int status) {

@@ -383,7 +383,7 @@ bool umma_decode_supported(int H_q, int H_kv, int d, int dtype);
 void umma_decode_plan(long long L, int H_kv, int* nsplit, long long* kps);
 int launch_decode_umma(const void* q, const void* K, const void* V, float* part, long long L, int H_q, int H_kv,
                        long long w0, long long G, double theta, bool bifocal, const float2* lo, const float2* hi,
-                       int* nsplit_out, cudaStream_t st);
+                       int* nsplit_out, cudaStream_t st, FreqMap fm);
 
 size_t decode_workspace_bytes(long long L, int H_q, int H_kv, int d) {
     // room for the partials of either implementation (SIMT or tcgen05) at this L
@@ -415,7 +415,7 @@ static int launch_decode_td(const void* q, const void* K, const void* V, void* o
     p.hi = p.lo + 256 * (D / 2);
     if (umma_decode_supported(H_q, H_kv, D, sizeof(T) == 2 ? JETLONG_BF16 : JETLONG_FP32)) {
         int ns = 0;
-        int rc = launch_decode_umma(q, K, V, p.part, L, H_q, H_kv, w0, G, theta, bifocal, p.lo, p.hi, &ns, st);
+        int rc = launch_decode_umma(q, K, V, p.part, L, H_q, H_kv, w0, G, theta, bifocal, p.lo, p.hi, &ns, st, fm);
         if (rc != JETLONG_OK) return rc;
         cudaLaunchConfig_t cfg = {};
         cfg.gridDim = dim3(H_q);

@@ -50,6 +50,7 @@ struct Bars {
     uint64_t pv_done, o_full, q_ready;
     uint32_t tmem_base;
     float red[4 * NH];                               // cross-warp max / sum exchange of the softmax group
+    uint32_t chk[4];                                 // per-warp partial hashes of the table check (rotate warps 0-3)
 };
 
 // smem: K ring (K | K lo e5m2 per stage) | V ring | Q raw | Q' (hi rows | lo rows) | Q'hi e5m2 | P | Bars
@@ -66,8 +67,14 @@ struct Params {
     const float2* lo;
     const float2* hi;
     double theta;                                    // for the table-header check (see the prologue)
-    // batched / paged form: blockIdx.z = sequence b with its own length and group size; the cache is a pool
-    // of 128-row pages (= the TMA tile) addressed through a page table; the fields above are per sequence then
+    long long n_hi;                                  // rows of the HI table the host asked the table kernel for
+    FreqMap fm;                                      // the remote map the tables must have been built for
+};
+// batched / paged form: blockIdx.z = sequence b with its own length and group size; the cache is a pool of
+// 128-row pages (= the TMA tile) addressed through a page table.  A separate kernel argument: the per-sequence arrays are
+// indexed at run time, and folding them into Params (which the kernel copies and edits per sequence) put every field of
+// it into local memory (measured: 115 -> 121 us per 128K step).
+struct BatchInfo {
     int batch;                                       // 0: the single-sequence call
     const int* page_table;                           // [batch][max_pages] physical page of logical tile kt (device memory)
     int max_pages;
@@ -134,22 +141,26 @@ struct DPlan {
     __device__ bool remote(int v) const { return v < nr; }
 };
 
-template <int NG>                                    // NG = query heads per KV head, rounded up to a power of two
+template <int NG, bool BATCHED>                      // NG = query heads per KV head, rounded up to a power of two
 __global__ void __launch_bounds__(NTHREADS, 1)
-decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV, const Params p0) {
-    Params p = p0;
+decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV, const Params p0,
+                   const __grid_constant__ BatchInfo bi) {
+    // the single-sequence instantiation reads its parameters straight from the constant bank; only the batched one
+    // works on an edited copy
+    Params pb = p0;
     const int* pages = nullptr;                                        // this sequence's row of the page table
-    if (p0.batch > 0) {
+    if (BATCHED) {
         const int b = blockIdx.z;
-        p.L = p0.Ls[b];
-        p.G = p0.Gs[b];
-        p.bifocal = (p.G > 1 && p.w0 < p.L - 1) ? 1 : 0;               // step a2, per sequence
-        p.q = p0.q + (size_t)b * p0.H_q * D;
-        p.part = p0.part + (size_t)b * p0.part_stride;
-        const long long tiles = (p.L + BN - 1) / BN, tps = (tiles + gridDim.x - 1) / gridDim.x;
-        p.kps = tps * BN;
-        pages = p0.page_table + (size_t)b * p0.max_pages;
+        pb.L = bi.Ls[b];
+        pb.G = bi.Gs[b];
+        pb.bifocal = (pb.G > 1 && pb.w0 < pb.L - 1) ? 1 : 0;           // step a2, per sequence
+        pb.q = p0.q + (size_t)b * p0.H_q * D;
+        pb.part = p0.part + (size_t)b * bi.part_stride;
+        const long long tiles = (pb.L + BN - 1) / BN, tps = (tiles + gridDim.x - 1) / gridDim.x;
+        pb.kps = tps * BN;
+        pages = bi.page_table + (size_t)b * bi.max_pages;
     }
+    const Params& p = BATCHED ? pb : p0;
     extern __shared__ __align__(1024) unsigned char smem[];
     if ((smem_u32(smem) & 1023u) != 0) __trap();               // SWIZZLE_128B operands need the 1024-byte alignment
     unsigned char* sQ = smem + OFF_Q;                              // raw | hi | lo
@@ -175,7 +186,7 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
     float2 tqh[NH * 64 / RT], tql[NH * 64 / RT];                       // HI / LO table entries of the query position
     KRot<RROWS> rot;
     bool tab_early = false;
-    unsigned tab_gen = 0;                                               // generation of the table the early loads saw
+    unsigned tab_gen = 0;                                               // check word of the table header at the early read
     const long long nq = (p.L - 1) - (p.L - 1) / p.G;                  // -Delta(q) >= 0, Eq.(5)
     auto load_tables = [&]() {
 #pragma unroll
@@ -206,9 +217,24 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
         if (plan.nr > 0) {
             const volatile TableHeader* hdr =
                 reinterpret_cast<const volatile TableHeader*>(reinterpret_cast<const unsigned char*>(p.lo) - 256);
-            tab_early = hdr->magic == kTableMagic && hdr->theta == p.theta && hdr->n_hi == (p.L + 255) / 256 + 1 && hdr->d == D;
-            tab_gen = hdr->gen;
+            tab_early = hdr->magic == kTableMagic && hdr->theta == p.theta && hdr->n_hi == p.n_hi && hdr->d == D &&
+                        hdr->interp == p.fm.interp &&
+                        (!p.fm.interp || (hdr->omg == p.fm.one_minus_inv_G && hdr->w_pre == p.fm.w_pre && hdr->alpha == p.fm.alpha &&
+                                          hdr->beta == p.fm.beta));
+            tab_gen = hdr->check;                                     // the check word the header promises for the table body
             if (tab_early) load_tables();
+            // verify the body ourselves, exactly as the table kernel does (hash of LO[1] and HI[n_hi-1], tables.cu): a CTA
+            // whose check passes need not wait for that kernel at all
+            if (rt < 128) {
+                uint32_t h = 0;
+                if (tab_early) {
+                    const float2 v = rt < 64 ? p.lo[64 + rt] : p.hi[(p.n_hi - 1) * 64 + (rt - 64)];
+                    h = (__float_as_uint(v.x) * 0x9E3779B1u) ^ (__float_as_uint(v.y) * 0x85EBCA77u) ^ ((uint32_t)rt * 0xC2B2AE3Du);
+                }
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) h ^= __shfl_xor_sync(0xffffffffu, h, o);
+                if (lane == 0) bars->chk[rt >> 5] = h;
+            }
         }
     }
     griddep_launch_dependents();                                       // the merge kernel may queue up behind us
@@ -325,12 +351,14 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
         for (int i = t; i < QBUF / 4; i += RT) reinterpret_cast<uint32_t*>(sP)[i] = 0u;
         named_bar_sync(1, RT);
         if (plan.nr > 0) {
-            // the table kernel has finished by now (it returns at once when the table verifies against its header); if it
-            // rebuilt the table -- header not sealed at the early read, or a body that failed the check -- load again
-            griddep_wait();
-            const volatile TableHeader* hdr =
-                reinterpret_cast<const volatile TableHeader*>(reinterpret_cast<const unsigned char*>(p.lo) - 256);
-            if (!tab_early || hdr->gen != tab_gen) load_tables();
+            // header sealed for these parameters AND the body verified against its check word (partial hashes of rotate
+            // warps 0-3, exchanged by the named barrier above): the early loads stand.  Otherwise the table kernel is
+            // rebuilding (or about to): wait for it, then load.
+            const uint32_t mine = (bars->chk[0] ^ bars->chk[1] ^ bars->chk[2] ^ bars->chk[3]) | 1u;
+            if (!tab_early || mine != tab_gen) {
+                griddep_wait();
+                load_tables();
+            }
         }
 #pragma unroll
         for (int it = 0; it < NH * 64 / RT; ++it) {
@@ -514,7 +542,7 @@ void umma_decode_plan(long long L, int H_kv, int* nsplit, long long* kps) {
 
 int launch_decode_umma(const void* q, const void* K, const void* V, float* part, long long L, int H_q, int H_kv,
                        long long w0, long long G, double theta, bool bifocal, const float2* lo, const float2* hi,
-                       int* nsplit_out, cudaStream_t st) {
+                       int* nsplit_out, cudaStream_t st, FreqMap fm) {
     CUtensorMap tmK, tmV;
     if (!make_kv_tensor_map(&tmK, K, L, H_kv, BN) || !make_kv_tensor_map(&tmV, V, L, H_kv, BN)) return JETLONG_UNSUPPORTED;
     Params p;
@@ -527,9 +555,10 @@ int launch_decode_umma(const void* q, const void* K, const void* V, float* part,
     p.bifocal = bifocal ? 1 : 0;
     p.lo = lo; p.hi = hi;
     p.theta = theta;
-    p.batch = 0; p.page_table = nullptr; p.max_pages = 0; p.part_stride = 0;
-    auto kern = p.g <= 1 ? decode_umma_kernel<1> : p.g <= 2 ? decode_umma_kernel<2> : p.g <= 4 ? decode_umma_kernel<4>
-              : p.g <= 8 ? decode_umma_kernel<8> : decode_umma_kernel<16>;
+    p.n_hi = (L + 255) / 256 + 1; p.fm = fm;
+    BatchInfo bi = {};                                                 // batch = 0: the single-sequence call
+    auto kern = p.g <= 1 ? decode_umma_kernel<1, false> : p.g <= 2 ? decode_umma_kernel<2, false> : p.g <= 4 ? decode_umma_kernel<4, false>
+              : p.g <= 8 ? decode_umma_kernel<8, false> : decode_umma_kernel<16, false>;
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES) != cudaSuccess)
         return check_launch("decode_umma attr");
     cudaLaunchConfig_t cfg = {};
@@ -542,7 +571,7 @@ int launch_decode_umma(const void* q, const void* K, const void* V, float* part,
     at[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at;
     cfg.numAttrs = 1;
-    cudaLaunchKernelEx(&cfg, kern, tmK, tmV, p);
+    cudaLaunchKernelEx(&cfg, kern, tmK, tmV, p, bi);
     note_launch();
     *nsplit_out = ns;
     return check_launch("decode_umma_kernel");
@@ -568,15 +597,17 @@ int launch_decode_umma_paged(const void* q, const void* Kpool, const void* Vpool
     p.bifocal = 0;
     p.lo = lo; p.hi = hi;
     p.theta = theta;
-    p.batch = nb; p.page_table = page_table; p.max_pages = max_pages; p.part_stride = part_stride;
+    p.n_hi = (Lmax + 255) / 256 + 1; p.fm = alias_map();
+    BatchInfo bi = {};
+    bi.batch = nb; bi.page_table = page_table; bi.max_pages = max_pages; bi.part_stride = part_stride;
     bool any_bifocal = false;
     for (int b = 0; b < MAXB; ++b) {
-        p.Ls[b] = b < nb ? Ls[b] : 1;
-        p.Gs[b] = b < nb ? (int)Gs[b] : 1;
+        bi.Ls[b] = b < nb ? Ls[b] : 1;
+        bi.Gs[b] = b < nb ? (int)Gs[b] : 1;
         if (b < nb && Gs[b] > 1 && w0 < Ls[b] - 1) any_bifocal = true;
     }
-    auto kern = p.g <= 1 ? decode_umma_kernel<1> : p.g <= 2 ? decode_umma_kernel<2> : p.g <= 4 ? decode_umma_kernel<4>
-              : p.g <= 8 ? decode_umma_kernel<8> : decode_umma_kernel<16>;
+    auto kern = p.g <= 1 ? decode_umma_kernel<1, true> : p.g <= 2 ? decode_umma_kernel<2, true> : p.g <= 4 ? decode_umma_kernel<4, true>
+              : p.g <= 8 ? decode_umma_kernel<8, true> : decode_umma_kernel<16, true>;
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES) != cudaSuccess)
         return check_launch("decode_umma attr");
     cudaLaunchConfig_t cfg = {};
@@ -589,7 +620,7 @@ int launch_decode_umma_paged(const void* q, const void* Kpool, const void* Vpool
     at[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at;
     cfg.numAttrs = any_bifocal ? 1 : 0;                                // without the table kernel in front: a normal launch
-    cudaLaunchKernelEx(&cfg, kern, tmK, tmV, p);
+    cudaLaunchKernelEx(&cfg, kern, tmK, tmV, p, bi);
     note_launch();
     *nsplit_out = ns;
     return check_launch("decode_umma_kernel (paged)");

@@ -894,7 +894,8 @@ size_t umma_prefill_prerot_workspace_bytes(long long L, int H_kv, int d) {
 
 int launch_prefill_umma(const void* Q, const void* K, const void* V, void* out, float* lse, long long L, int H_q,
                         int H_kv, int d, long long w0, long long G, double theta, bool bifocal, int precise, void* ws,
-                        size_t ws_bytes, cudaStream_t st, bool prerot, bool g_two_tile, FreqMap fm) {
+                        size_t ws_bytes, cudaStream_t st, bool prerot, bool g_two_tile, FreqMap fm, int qb_lo, int qb_hi,
+                        long long L_sel) {
     (void)ws_bytes;
     CUtensorMap tmK, tmV;
     if (!make_kv_tensor_map(&tmK, K, L, H_kv, 64) || !make_kv_tensor_map(&tmV, V, L, H_kv, 128)) return JETLONG_UNSUPPORTED;
@@ -951,7 +952,9 @@ int launch_prefill_umma(const void* Q, const void* K, const void* V, void* out, 
             // on the fly, default precision: selective e5m2 compensation as in the workspace variant (per-head fallback
             // to the full cross terms inside the kernel)
             uint32_t* selinfo = nullptr;
-            rc = run_selection(Q, K, L, H_q, H_kv, (unsigned char*)ws + two_level_bytes(L + 256, d), st, &selinfo);
+            // L_sel: the rows the selection statistics may read (jetlong_prefill_host launches row chunks while later rows
+            // are still being uploaded)
+            rc = run_selection(Q, K, L_sel > 0 && L_sel < L ? L_sel : L, H_q, H_kv, (unsigned char*)ws + two_level_bytes(L + 256, d), st, &selinfo);
             if (rc != JETLONG_OK) return rc;
             p.selinfo = selinfo;
             precise = p.precise = 3;
@@ -968,8 +971,10 @@ int launch_prefill_umma(const void* Q, const void* K, const void* V, void* out, 
         a.out = p.out; a.lse = lse; a.L = L; a.w0 = w0; a.G = G; a.H_q = H_q; a.H_kv = H_kv;
         a.bifocal = p.bifocal; a.precise = precise; a.prerot = p.prerot; a.window_only = 0; a.qk_f16 = 0; a.out_f32 = 0;
         a.lo = p.lo; a.hi = p.hi; a.selinfo = p.selinfo;
+        a.qb_lo = qb_lo; a.qb_hi = qb_hi;
         return launch_prefill_v2(a, st);
     }
+    if (qb_lo != 0 || qb_hi >= 0) return JETLONG_UNSUPPORTED;        // row chunks exist only in the two-tile kernel
     if (cudaFuncSetAttribute(prefill_umma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES) != cudaSuccess)
         return check_launch("prefill_umma attr");
     const int n_qb = (int)((L + BM - 1) / BM);

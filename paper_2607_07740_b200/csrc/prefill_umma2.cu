@@ -103,7 +103,7 @@ struct Params {
     long long L, w0, G;
     int H_q, H_kv, g;
     int bifocal, precise, prerot, window_only, qk_f16, out_f32;
-    int n_qb, n_sb, n_s4;
+    int n_qb, n_sb, n_s4;                            // n_sb / n_s4: one past the top 256- / 512-row block of this launch
     const float2* lo;
     const float2* hi;
     const uint32_t* selinfo;
@@ -710,12 +710,15 @@ int launch_prefill_v2(const PrefillV2Args& a, cudaStream_t st) {
     p.H_q = a.H_q; p.H_kv = a.H_kv; p.g = a.H_q / a.H_kv;
     p.bifocal = a.bifocal; p.precise = a.precise; p.prerot = a.prerot; p.window_only = a.window_only; p.qk_f16 = a.qk_f16; p.out_f32 = a.out_f32;
     p.n_qb = (int)((a.L + BM - 1) / BM);
-    p.n_sb = (p.n_qb + 1) / 2;
-    p.n_s4 = (p.n_qb + 3) / 4;
+    const int qb_hi = (a.qb_hi < 0 || a.qb_hi > p.n_qb) ? p.n_qb : a.qb_hi;
+    if ((a.qb_lo & 3) || a.qb_lo < 0 || a.qb_lo >= qb_hi) return JETLONG_INVALID_ARG;
+    p.n_sb = (qb_hi + 1) / 2;
+    p.n_s4 = (qb_hi + 3) / 4;
     p.lo = a.lo; p.hi = a.hi; p.selinfo = a.selinfo;
     if (cudaFuncSetAttribute(prefill_umma2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES) != cudaSuccess)
         return check_launch("prefill_umma2 attr");
-    const unsigned grid = (p.g & 1) ? 2u * (unsigned)p.n_s4 * (unsigned)a.H_q : 2u * (unsigned)p.n_sb * (unsigned)(a.H_q / 2);
+    const unsigned grid = (p.g & 1) ? 2u * (unsigned)(p.n_s4 - a.qb_lo / 4) * (unsigned)a.H_q
+                                    : 2u * (unsigned)(p.n_sb - a.qb_lo / 2) * (unsigned)(a.H_q / 2);
     prefill_umma2_kernel<<<grid, NTHREADS, SMEM_BYTES, st>>>(a.tmQ, a.tmK, a.tmV, a.tmKh, a.tmKe, a.tmKl, p);
     note_launch();
     return check_launch("prefill_umma2_kernel");

@@ -23,6 +23,8 @@ struct PrefillV2Args {
     const float2* lo;                                 // two-level (cos, sin) tables
     const float2* hi;
     const uint32_t* selinfo;                          // [H_kv][16] selective-compensation table (precise 3)
+    int qb_lo = 0, qb_hi = -1;                        // query blocks [qb_lo, qb_hi) of this launch (multiples of 4; -1 = to the end):
+                                                      // jetlong_prefill_host pipelines row chunks against the copies
 };
 
 // true when the two-tile kernel serves this precision mode (fp16 cross terms need the TMEM-resident Q of prefill_umma.cu)

@@ -232,3 +232,26 @@ def test_table_header_is_not_trusted_when_the_body_was_overwritten():
     o2, l2 = J.jetlong_prefill(Q, K, V, w_local=w0, w_pretrained=w_pre, rope_theta=1e6, workspace=ws)
     torch.cuda.synchronize()
     assert torch.equal(o1, o2) and torch.equal(l1, l2)
+
+
+# ---- the host-buffer call: chunked upload / compute / download pipeline ------------------------------------------------------
+@pytest.mark.parametrize("L,H_q,H_kv,d,dtype,w_pre,w0", [
+    (9000, 4, 2, 128, "bf16", 2048, 256),       # 4 row chunks on the two-tile kernel, ragged last chunk
+    (33000, 2, 1, 128, "bf16", 8192, 512),      # 8 chunks, an odd (lone-head) group
+    (700, 4, 2, 128, "bf16", 200, 64),          # one chunk
+    (1024, 4, 2, 64, "fp32", 256, 64),          # config-1 shape through the SIMT tiles
+])
+def test_prefill_host_pipeline(L, H_q, H_kv, d, dtype, w_pre, w0):
+    theta = 1e6 if d == 128 else 1e4
+    Q, K, V = W.make_qkv(L, H_q, H_kv, d, theta, dtype, 5150 + L, dtype == "bf16", DEV)
+    Qh, Kh, Vh = Q.cpu().pin_memory(), K.cpu().pin_memory(), V.cpu().pin_memory()
+    for _ in range(2):                                               # the second call reuses the arena
+        out, lse = J.jetlong_prefill_host(Qh, Kh, Vh, w_local=w0, w_pretrained=w_pre, rope_theta=theta)
+    rows, heads = _pick(L, H_q, 1024, 7)
+    edge = np.array([0, 511, 512, 513, L // 2, L - 1])
+    rows = np.concatenate([rows, np.repeat(edge, H_q)])
+    heads = np.concatenate([heads, np.tile(np.arange(H_q, dtype=np.int32), len(edge))])
+    ro, rl = oracle_rows(Q, K, V, rows, heads, w_local=w0, w_pretrained=w_pre, rope_theta=theta)
+    ri, hi = torch.as_tensor(rows), torch.as_tensor(heads).long()
+    check(out[ri, hi], lse[hi, ri], ro, rl, Q.dtype, "host pipeline L=%d" % L)
+    assert torch.isfinite(out.float()).all() and torch.isfinite(lse).all()
