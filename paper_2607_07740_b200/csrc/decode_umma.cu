@@ -391,7 +391,7 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
             const int s = v % KS;
             mbar_wait(&bars->k_full[s], (v / KS) & 1);
             if (plan.remote(v)) {
-                rotate_rows2<RROWS, BOXB, 3>(smem_u32(sK(s)), smem_u32(sK(s)) + TILE, (unsigned)(plan.kt(v) * BN), rot, SelTree(), 0u, 0u);
+                rotate_rows2<RROWS, BOXB, 3, true>(smem_u32(sK(s)), smem_u32(sK(s)) + TILE, (unsigned)(plan.kt(v) * BN), rot, SelTree(), 0u, 0u);
                 fence_proxy_async_smem();
                 if (plan.remote(v + 1)) rot.prefetch((unsigned)(plan.kt(v + 1) * BN));
             }

@@ -335,7 +335,7 @@ struct SelTree {
     }
 };
 
-template <int ROWS, int KBOX, int MODE>
+template <int ROWS, int KBOX, int MODE, bool UNROLL = false>
 __device__ __forceinline__ void rotate_rows2(uint32_t kh, uint32_t kl, unsigned pos0, KRot<ROWS>& R, const SelTree& T,
                                              uint32_t b_lo, uint32_t b_hi) {
     uint64_t cc[4], cs[4], ncs[4], nss[4];
@@ -352,7 +352,7 @@ __device__ __forceinline__ void rotate_rows2(uint32_t kh, uint32_t kl, unsigned 
     uint4 u1 = lds128(kh + off), u2 = lds128(kh + KBOX + off);
     // rolled on purpose: the SM's instruction caches are small (L0 ~6 KB, L1.5 32 KB) and four roles run different loops;
     // unrolled, this loop alone was 16 KB and its warps spent most samples in stall_no_inst (ncu)
-#pragma unroll 1
+#pragma unroll(UNROLL ? ROWS : 1)
     for (int m = 0; m < ROWS; ++m) {
         const int r = R.r0 + m;
         const int off_n = (r + 1) * 128 + ((R.c ^ ((r + 1) & 7)) << 4);

@@ -93,7 +93,12 @@ __device__ __forceinline__ unsigned table_check(const float2* lo, const float2* 
 __global__ void __launch_bounds__(1024) two_level_kernel(unsigned char* __restrict__ region, long long n_hi, int half,
                                                          double theta, double log2_theta, int d, FreqMap fm) {
     __shared__ unsigned red[32];
-    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");   // a programmatically launched consumer (decode) may start
+    // Launched with programmatic stream serialization itself: the CTA may become resident while the previous kernel on the
+    // stream (the previous decode step's merge, or any caller kernel) drains.  It first waits for that kernel to complete
+    // -- so everything the caller enqueued before this call is visible to us AND to our dependents -- and only then lets
+    // the programmatically launched consumer (the decode scan) start.
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     TableHeader* hdr = reinterpret_cast<TableHeader*>(region);
     float2* lo = reinterpret_cast<float2*>(region + 256);
     float2* hi = lo + 256 * half;
@@ -132,7 +137,16 @@ __global__ void __launch_bounds__(1024) two_level_kernel(unsigned char* __restri
 
 int build_two_level(void* region, long long L, int d, double theta, cudaStream_t st, FreqMap fm) {
     const long long n_hi = (L + 255) / 256 + 1;
-    two_level_kernel<<<1, 1024, 0, st>>>((unsigned char*)region, n_hi, d / 2, theta, log2(theta), d, fm);
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(1);
+    cfg.blockDim = dim3(1024);
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    cudaLaunchKernelEx(&cfg, two_level_kernel, (unsigned char*)region, n_hi, d / 2, theta, log2(theta), d, fm);
     note_launch(1);
     return check_launch("two_level_kernel");
 }
