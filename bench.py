@@ -330,9 +330,10 @@ def main():
                                                 "to a workspace scratch; the stored K is still never written")
             if "unfused" in others:
                 others["unfused"]["fused_speedup"] = others["unfused"]["ms"] / ms_per_step
-                others["unfused"]["note"] = ("SURVEY.md 8(f)-2: window(Q,K) + causal(Q',K') + window(Q',K') + merge with the minus "
-                                             "sign; the paper reports fused 1.43-1.56x faster than unfused on H100 (P:226); lse "
-                                             "only ~3e-3 here (one fp16 rounding, no compensation)")
+                others["unfused"]["note"] = ("SURVEY.md 8(f)-2: window(Q,K) + causal(Q',K') + window(Q',K') (fp32 partial outputs, the "
+                                             "product's compensated remote operands) + Eq.(7) merge with the minus sign; meets the "
+                                             "same tolerances as the fused kernel; the paper reports fused 1.43-1.56x faster than "
+                                             "unfused on H100 (P:226)")
         # ---- the same three kernels at 128K (BASELINE.json configs[2], Qwen3-4B-shaped) --------------------
         line["prefill_128k"] = bench_prefill_128k(J, B, W, dev, pk, timed, local)
         # ---- end to end through the host-buffer C-ABI call -----------------------------------------------

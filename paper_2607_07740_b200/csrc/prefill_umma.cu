@@ -57,7 +57,7 @@ constexpr int POLY_OF_4 = 0;                          // of every 4 exponential 
 // under the power cap (~1.45 GHz), where extra FMA instructions cost more clock than the freed MUFU cycles return.
 // warp roles.  The scheduler of an SM sub-partition prefers the highest warp id: the MMA issuer and the producers (few
 // instructions, all on the critical path) sit above the softmax warps, the rotate group (which runs visits ahead) below.
-constexpr int W_KLOAD = 12, W_VLOAD = 13, W_XCHG = 14, W_MMA = 15;   // warps 0-3 rotate, 4-11 softmax
+constexpr int W_KLOAD = 12, W_VLOAD = 13, W_MMA = 15;   // warps 0-3 rotate, 4-11 softmax
 constexpr uint32_t TM_S = 0, TM_O = 256, TM_QA = 384, TM_QB = 448;
 constexpr uint32_t TM_QY = 448, TM_QR = 480;         // precision mode 2: Q' and Q' lo as e5m2 (32 columns each) in place of Qb
 
@@ -75,12 +75,6 @@ struct Bars {
     uint64_t q_ready;          // leader: Q staged in TMEM by both rotate groups
     uint64_t q_local_done;     // both: the last local Q K^T has completed, Qa may be overwritten
     uint64_t q_rot_done;       // leader: Q' (hi, lo) staged in TMEM
-    // cluster of four (SHARE): the other CTA pair rotates half of our rows and writes them into our stages
-    uint64_t peer_full[NKMAX];   // local: the rows rotated by the other pair have landed in our stage (bulk copy, complete_tx)
-    uint64_t rows_done[NKMAX];   // local: our four rotate warps have rotated and fenced their 32 rows of a shared visit
-    uint64_t kv_ready_sh[NKMAX]; // leader: a shared visit is complete in a CTA of the pair (its own rows + the other pair's), 2 arrivals
-    uint64_t peer_empty[NKMAX];  // both: the OTHER pair's Q K^T reading ITS K stage s has completed (its commit, multicast to us)
-    uint64_t peer_go;            // both: the other pair's last local Q K^T has completed (all its K stages are free)
     uint32_t tmem_base;
     float xchg[4 * BM];        // row-max / row-sum exchange between the two column halves of a row
 };
@@ -130,8 +124,6 @@ struct Plan {
         if (window_only) { n_remote = 0; kt_hi = -1; }
         nv = n_local + n_remote;
     }
-    // SHARE: the pair on the earlier query block walks the remote list of the later one (its extra tile is fully masked)
-    __device__ void adopt_remote(int kt_hi_) { kt_hi = kt_hi_; n_remote = kt_hi + 1; nv = n_local + n_remote; }
     __device__ Visit at(int v, bool bifocal) const {
         Visit x;
         if (v < n_local) { x.kt = qb - v; x.mode = bifocal ? 1 : 0; }
@@ -221,13 +213,10 @@ constexpr uint32_t IDESC_QK_F16 = idesc_f16(0, 0, 0, 0, 2 * BM, BN);
 constexpr uint32_t IDESC_QK_E5M2 = idesc_f16(1, 1, 0, 0, 2 * BM, BN);   // kind::f8f6f4: format code 1 = e5m2
 constexpr uint32_t IDESC_PV = idesc_f16(1, 1, 0, 1, 2 * BM, D);  // A = P (TMEM, bf16), B = V (smem, MN-major)
 
-// SHARE = false: a cluster is one CTA pair.  SHARE = true (bifocal, on the fly): a cluster is TWO pairs on adjacent query
-// blocks of the same two heads; in a remote visit every CTA loads and rotates only 32 key rows and writes them to its
-// own stage and to the stage of the CTA with the same parity in the other pair, so a rotated row serves 512 query rows.
-template <bool SHARE>
+// A cluster is one CTA pair (round 1's clusters of four, which shared rotated K tiles through distributed shared memory,
+// were superseded by the two-tile kernel of prefill_umma2.cu and removed).
 __device__ __forceinline__ void prefill_body(const CUtensorMap& tmK, const CUtensorMap& tmV, const CUtensorMap& tmKh,
-                                             const CUtensorMap& tmKe, const CUtensorMap& tmKl, const CUtensorMap& tmK32,
-                                             const Params& p) {
+                                             const CUtensorMap& tmKe, const CUtensorMap& tmKl, const Params& p) {
     extern __shared__ unsigned char smem_raw[];
     unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
     unsigned char* kring = smem + NV * VH_BYTES;
@@ -236,12 +225,9 @@ __device__ __forceinline__ void prefill_body(const CUtensorMap& tmK, const CUten
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int rank = (int)cluster_ctarank();
     const int cta = rank & 1;                                      // position in the CTA pair (0 = leader)
-    const int pr = SHARE ? (rank >> 1) : 0;                        // which pair of the cluster
     const int pairs = p.H_q / 2;
-    const int unit = SHARE ? (int)(blockIdx.x >> 2) : (int)(blockIdx.x >> 1);
-    const int qbA = SHARE ? p.qb_top - 1 - 2 * (unit / pairs) : p.qb_top - 1 - unit / pairs;   // heaviest row blocks first
-    const int qbB = (qbA - 1 >= p.qb_lo) ? qbA - 1 : -1;           // SHARE: pair 1 takes the block below (-1 = none)
-    const int qb = pr == 0 ? qbA : qbB;
+    const int unit = (int)(blockIdx.x >> 1);
+    const int qb = p.qb_top - 1 - unit / pairs;                    // heaviest row blocks first
     const int h0 = 2 * (unit % pairs);
     const int head = h0 + cta;
     const int kvh = h0 / p.g;
@@ -252,13 +238,7 @@ __device__ __forceinline__ void prefill_body(const CUtensorMap& tmK, const CUten
     int precise = p.precise;
     if (precise == 3 && __ldg(p.selinfo + kvh * 16 + 8) != 0u) precise = 2;
     Plan plan(qb, p.w0, bifocal, p.window_only != 0);
-    int n_local_peer = 0;                                          // SHARE: local visits of the other pair
-    if (SHARE) {
-        const Plan pa(qbA, p.w0, bifocal), pb(qbB, p.w0, bifocal);
-        if (pr == 1) plan.adopt_remote(pa.kt_hi);
-        n_local_peer = pr == 0 ? pb.n_local : pa.n_local;
-    }
-    const uint32_t own_mask = 3u << (2 * pr), peer_mask = 3u << (2 * (pr ^ 1));
+    const uint32_t own_mask = 3u;
     // K stage = K (hi in place) | cross-term operands; the same for every CTA of the cluster (one KV head)
     const int KST = KH_BYTES + ((!bifocal || p.window_only || precise == 0) ? 0 : precise == 3 ? KBOX : 2 * KBOX);
     const int NK = (K_RING_BYTES / KST) < NKMAX ? (K_RING_BYTES / KST) : NKMAX;
@@ -272,12 +252,8 @@ __device__ __forceinline__ void prefill_body(const CUtensorMap& tmK, const CUten
         for (int i = 0; i < 2; ++i) { mbar_init(&bars->s_full[i], 1); mbar_init(&bars->p_full[i], 16); }
         mbar_init(&bars->pv_done, 1); mbar_init(&bars->o_full, 1); mbar_init(&bars->q_ready, 8);
         mbar_init(&bars->q_local_done, 1); mbar_init(&bars->q_rot_done, 8);
-        for (int i = 0; i < NKMAX; ++i) { mbar_init(&bars->peer_full[i], 1); mbar_init(&bars->peer_empty[i], 1);
-                                          mbar_init(&bars->rows_done[i], 4); mbar_init(&bars->kv_ready_sh[i], 2); }
-        mbar_init(&bars->peer_go, 1);
         fence_barrier_init();
         prefetch_tmap(&tmK); prefetch_tmap(&tmV);
-        if (SHARE) prefetch_tmap(&tmK32);
         if (p.prerot) { prefetch_tmap(&tmKh); prefetch_tmap(&tmKe); prefetch_tmap(&tmKl); }
     }
     if (warp == W_MMA) tmem_alloc2<512>(&bars->tmem_base);
@@ -288,27 +264,17 @@ __device__ __forceinline__ void prefill_body(const CUtensorMap& tmK, const CUten
     float* xchg = bars->xchg;
     // arrive on the pair leader's copy of a barrier (the leader is rank & ~1 of the cluster)
     auto arrive_leader = [&](uint64_t* bar) {
-        if (SHARE) mbar_arrive_cluster_addr(mapa_u32(smem_u32(bar), (uint32_t)(rank & ~1)));
-        else mbar_arrive_leader(bar);
+        mbar_arrive_leader(bar);
     };
-    // 4 KB pieces a CTA sends per shared visit: its 32 rows of the two K'hi boxes (+ of the cross-term boxes)
-    const uint32_t nbox = precise == 0 ? 2u : precise == 3 ? 3u : 4u;
-
     if (warp == W_KLOAD) {
-        // ===================== K producer (each CTA loads its 64 keys; 32 in a shared visit) =====================
+        // ===================== K producer (each CTA loads its 64 keys) =====================
         if (lane == 0) {
-            Ring rk(NK), ru(NK);
+            Ring rk(NK);
             for (int v = 0; v < plan.nv; ++v, rk.next()) {
                 const Visit x = plan.at(v, bifocal);
                 const int st = rk.s;
                 if (v >= NK) mbar_wait(&bars->k_empty[st], rk.ph ^ 1u);
-                if (SHARE && x.mode == 2) {
-                    mbar_arrive_expect_tx(&bars->peer_full[ru.s], nbox * 4096u);   // the other pair's rows will land here
-                    ru.next();
-                    mbar_arrive_expect_tx(&bars->k_full[st], KH_BYTES / 2);
-                    tma_load_3d(sK(st) + pr * 4096, &tmK32, &bars->k_full[st], 0, kvh, x.kt * BN + 64 * cta + 32 * pr);
-                    tma_load_3d(sK(st) + KBOX + pr * 4096, &tmK32, &bars->k_full[st], 64, kvh, x.kt * BN + 64 * cta + 32 * pr);
-                } else if (p.prerot && x.mode == 2) {
+                if (p.prerot && x.mode == 2) {
                     // pre-rotated variant: K' hi (fp16) and the e5m2 copies of K' and K' lo come from the workspace
                     mbar_arrive_expect_tx(&bars->k_full[st], KH_BYTES + (precise == 2 ? 2 * KBOX : precise == 3 ? KBOX : 0));
                     tma_load_3d(sK(st), &tmKh, &bars->k_full[st], 0, kvh, x.kt * BN + 64 * cta);
@@ -333,29 +299,6 @@ __device__ __forceinline__ void prefill_body(const CUtensorMap& tmK, const CUten
                 tma_load_3d(sV(rv.s), &tmV, &bars->v_full[rv.s], 64 * cta, kvh, x.kt * BN);
             }
         }
-    } else if (warp == W_XCHG) {
-        // ===================== SHARE: exchange of rotated rows between the two pairs of the cluster =====================
-        // per shared visit u: once our rotate warps have fenced their 32 rows and the other pair's K stage is free, send the
-        // rows to the CTA of the same parity in the other pair (bulk copies, async proxy, complete_tx on ITS peer_full);
-        // once the other pair's rows have landed here, arrive on our pair's kv_ready_sh.
-        if (SHARE && lane == 0) {
-            const int nsh = plan.nv - plan.n_local;                  // shared (remote) visits
-            const uint32_t peer_k = mapa_u32(smem_u32(kring), (uint32_t)(rank ^ 2));
-            const uint32_t peer_full0 = mapa_u32(smem_u32(&bars->peer_full[0]), (uint32_t)(rank ^ 2));
-            const uint32_t ready0 = mapa_u32(smem_u32(&bars->kv_ready_sh[0]), (uint32_t)(rank & ~1));
-            Ring rs(NK, plan.n_local), rp(NK, n_local_peer), ru(NK);
-            if (nsh > 0) mbar_wait(&bars->peer_go, 0);               // the other pair's local visits are over: its K stages are free
-            for (int u = 0; u < nsh; ++u, rs.next(), rp.next(), ru.next()) {
-                mbar_wait(&bars->rows_done[ru.s], ru.ph);
-                if (u >= NK) mbar_wait(&bars->peer_empty[rp.s], rp.ph ^ 1u);
-                const uint32_t src = smem_u32(kring) + (uint32_t)(rs.s * KST) + (uint32_t)pr * 4096u;
-                const uint32_t dst = peer_k + (uint32_t)(rp.s * KST) + (uint32_t)pr * 4096u;
-                const uint32_t mb = peer_full0 + 8u * (uint32_t)ru.s;
-                for (uint32_t b = 0; b < nbox; ++b) bulk_copy_to_peer(dst + b * KBOX, src + b * KBOX, 4096u, mb);
-                mbar_wait(&bars->peer_full[ru.s], ru.ph);
-                mbar_arrive_cluster_addr(ready0 + 8u * (uint32_t)ru.s);
-            }
-        }
     } else if (warp == W_MMA) {
         if (cta == 1) {
             // ===================== non-leader CTA: tell the leader when our V half has landed =====================
@@ -373,7 +316,7 @@ __device__ __forceinline__ void prefill_body(const CUtensorMap& tmK, const CUten
             const uint32_t tm = __shfl_sync(0xffffffffu, tmem, 0);
             const uint32_t kring0 = __shfl_sync(0xffffffffu, smem_u32(kring), 0);
             const uint32_t vring0 = __shfl_sync(0xffffffffu, smem_u32(smem), 0);
-            Ring rq(NK), ruq(NK), rvp(NV);                           // K stage / shared-visit slot of the next Q K^T, V stage of the next P V
+            Ring rq(NK), rvp(NV);                                    // K stage of the next Q K^T, V stage of the next P V
             auto issue_qk = [&](int v) {
                 const Visit x = plan.at(v, bifocal);
                 const uint32_t dS = tm + TM_S + (v & 1) * 128;
@@ -416,10 +359,6 @@ __device__ __forceinline__ void prefill_body(const CUtensorMap& tmK, const CUten
                     }
                     umma2_commit_mask(&bars->s_full[v & 1], own_mask);
                     umma2_commit_mask(&bars->k_empty[rq.s], own_mask);   // the K stage is free again
-                    if (SHARE) {                                     // ... and the other pair may write ITS rows of our next use of it
-                        umma2_commit_mask(&bars->peer_empty[rq.s], peer_mask);
-                        if (v == plan.n_local - 1) umma2_commit_mask(&bars->peer_go, peer_mask);
-                    }
                     if (plan.n_remote > 0 && v == plan.n_local - 1) umma2_commit_mask(&bars->q_local_done, own_mask);
                 }
                 __syncwarp();
@@ -440,17 +379,7 @@ __device__ __forceinline__ void prefill_body(const CUtensorMap& tmK, const CUten
                 __syncwarp();
                 rvp.next();
             };
-            // operands of visit v are in place: local visits (and every visit without SHARE) count the two rotate groups of
-            // the pair on k_ready (in a shared visit each CTA arrives once the other pair's rows have landed too)
-            auto wait_ready = [&](int v) {
-                if (SHARE && v >= plan.n_local) {                     // shared visit: one arrival per CTA of the pair
-                    mbar_wait(&bars->kv_ready_sh[ruq.s], ruq.ph);
-                    ruq.next();
-                } else {
-                    mbar_wait(&bars->k_ready[rq.s], rq.ph);
-                }
-            };
-            if (SHARE && plan.n_local == 0 && elect_one()) umma2_commit_mask(&bars->peer_go, peer_mask);   // no local visit: all stages free
+            auto wait_ready = [&](int) { mbar_wait(&bars->k_ready[rq.s], rq.ph); };   // both rotate groups are done with the stage
             __syncwarp();
             mbar_wait(&bars->q_ready, 0);
             if (plan.nv > 0) {
@@ -485,14 +414,13 @@ __device__ __forceinline__ void prefill_body(const CUtensorMap& tmK, const CUten
         tc_fence_before();
         __syncwarp();
         if (lane == 0) arrive_leader(&bars->q_ready);
-        constexpr int RR = SHARE ? 2 : 4;                             // key rows per rotate thread
+        constexpr int RR = 4;                                         // key rows per rotate thread
         KRot<RR> rot;
         if (plan.n_remote > 0 && !p.prerot) {
-            rot.init(p.lo, p.hi, t, p.G, SHARE ? 32 * pr : 0);
-            rot.selw = p.selinfo ? __ldg(p.selinfo + kvh * 16 + (t & 7)) : 0u;
+            rot.init(p.lo, p.hi, t, p.G, 0);
             rot.prefetch((unsigned)(plan.kt_hi * BN + 64 * cta));     // first remote visit
         }
-        Ring rk(NK), ru(NK);
+        Ring rk(NK);
         for (int v = 0; v < plan.nv; ++v, rk.next()) {
             const Visit x = plan.at(v, bifocal);
             const int st = rk.s;
@@ -505,22 +433,8 @@ __device__ __forceinline__ void prefill_body(const CUtensorMap& tmK, const CUten
                     tmem_st_wait();
                     tc_fence_before();
                 }
-                if (SHARE) {
-                    // shared visit: rotate our 32 rows, fence, tell the exchange thread (it sends them to the other pair and
-                    // hands the stage to the MMA warp once the other pair's rows have landed)
-                    rotate_k_rows<RR, KBOX>(smem_u32(sK(st)), smem_u32(sKl(st)), (unsigned)(x.kt * BN + 64 * cta), rot, precise == 3 ? 4 : precise);
-                    fence_proxy_async_smem();
-                    if (x.kt > 0) rot.prefetch((unsigned)((x.kt - 1) * BN + 64 * cta));
-                    __syncwarp();
-                    if (lane == 0) {
-                        mbar_arrive(&bars->rows_done[ru.s]);
-                        if (v == plan.n_local) arrive_leader(&bars->q_rot_done);
-                    }
-                    ru.next();
-                    continue;
-                }
                 if (!p.prerot) {
-                    rotate_k_rows<RR, KBOX>(smem_u32(sK(st)), smem_u32(sKl(st)), (unsigned)(x.kt * BN + 64 * cta), rot, precise == 3 ? 4 : precise);
+                    rotate_k_rows<RR, KBOX>(smem_u32(sK(st)), smem_u32(sKl(st)), (unsigned)(x.kt * BN + 64 * cta), rot, precise);
                     fence_proxy_async_smem();
                     if (x.kt > 0) rot.prefetch((unsigned)((x.kt - 1) * BN + 64 * cta));   // next remote visit's first row
                 }
@@ -668,7 +582,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1)
 prefill_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV,
                     const __grid_constant__ CUtensorMap tmKh, const __grid_constant__ CUtensorMap tmKe,
                     const __grid_constant__ CUtensorMap tmKl, const Params p) {
-    prefill_body<false>(tmK, tmV, tmKh, tmKe, tmKl, tmK, p);
+    prefill_body(tmK, tmV, tmKh, tmKe, tmKl, p);
 }
 
 // ---- 8(f)-1: rotate K once into a scratch (the workspace variant) -------------------------------------------

@@ -132,12 +132,6 @@ struct Plan {
         n_remote = kt_hi - kt_rlo + 1;
         nv = n_local + n_remote;
     }
-    __device__ Visit at(int v, bool bifocal) const {
-        Visit x;
-        if (v < n_local) { x.kt = qb - v; x.mode = bifocal ? 1 : 0; }
-        else { x.kt = kt_hi - (v - n_local); x.mode = 2; }
-        return x;
-    }
 };
 
 // The pair's merged visit list: the K tiles needed by ANY of its four query tiles.  UMMA "tile i" (i = 0, 1) is M = 256

@@ -135,7 +135,6 @@ template <int ROWS> struct KRot {
     const float2* lo; const float2* hi;
     int c, r0;
     unsigned G;
-    uint32_t selw;                  // mode 4: PRMT selector of the two compensated pairs of this thread's chunk
     __device__ __forceinline__ void init(const float2* lo_, const float2* hi_, int t, long long G_, int rbase = 0) {
         lo = lo_; hi = hi_; c = t & 7; r0 = rbase + ROWS * (t >> 3); G = (unsigned)G_;
         const float4* p1 = reinterpret_cast<const float4*>(lo + 64 + 8 * c);       // LO[1][8c..]
@@ -201,15 +200,9 @@ __device__ __forceinline__ void sts128(uint32_t a, uint32_t x, uint32_t y, uint3
     asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" ::"r"(a), "r"(x), "r"(y), "r"(z), "r"(w) : "memory");
 }
 
-// REMOTE: every store is repeated at rkh / rkl, shared::cluster addresses of the same stage in another CTA of the
-// cluster (the CTA pair working on the adjacent query block, which needs the same rotated rows).
-template <int ROWS, int KBOX, bool REMOTE = false>
-__device__ __forceinline__ void rotate_k_rows(uint32_t kh, uint32_t kl, unsigned pos0, KRot<ROWS>& R,
-                                              int precise, uint32_t rkh = 0, uint32_t rkl = 0,      // kh, kl: shared-space addresses
-                                              uint32_t c4 = 0x3210u) {   // mode 4: 16-byte chunk of lo1 | lo2 << 4 | hi1 << 8 | hi2 << 12
-    // precise: 4 = selective e5m2 compensation: one 128-byte row per key at kl = [lo1 | lo2 | hi1 | hi2] (16 B each: the two
-    //          pairs R.selw picks from each 8-pair chunk, as e5m2) | unused, SWIZZLE_128B;
-    //          0 = hi only; 1 = fp16 lo at kl (same layout as kh); 2 = e5m2 copies for the cross terms at kl:
+template <int ROWS, int KBOX>
+__device__ __forceinline__ void rotate_k_rows(uint32_t kh, uint32_t kl, unsigned pos0, KRot<ROWS>& R, int precise) {   // kh, kl: shared-space addresses
+    // precise: 0 = hi only; 1 = fp16 lo at kl (same layout as kh); 2 = e5m2 copies for the cross terms at kl:
     //          [box of KBOX bytes: K' as e5m2, rows x 128 channels][box: K' lo as e5m2], SWIZZLE_128B;
     //          3 = only K' lo as e5m2 at kl (one box)
     // first-row (cos, sin) from the prefetched table entries: HI * LO as complex numbers
@@ -250,17 +243,9 @@ __device__ __forceinline__ void rotate_k_rows(uint32_t kh, uint32_t kl, unsigned
         }
         sts128(kh + off, h1[0], h1[1], h1[2], h1[3]);
         sts128(kh + KBOX + off, h2[0], h2[1], h2[2], h2[3]);
-        if (REMOTE) {
-            ptx::sts128_cluster(rkh + off, h1[0], h1[1], h1[2], h1[3]);
-            ptx::sts128_cluster(rkh + KBOX + off, h2[0], h2[1], h2[2], h2[3]);
-        }
         if (precise == 1) {
             sts128(kl + off, l1[0], l1[1], l1[2], l1[3]);
             sts128(kl + KBOX + off, l2[0], l2[1], l2[2], l2[3]);
-            if (REMOTE) {
-                ptx::sts128_cluster(rkl + off, l1[0], l1[1], l1[2], l1[3]);
-                ptx::sts128_cluster(rkl + KBOX + off, l2[0], l2[1], l2[2], l2[3]);
-            }
         } else if (precise == 2) {
             // byte b of an e5m2 row is channel b: channels 8c.. sit in 16-byte chunk c/2, channels 64+8c.. in chunk 4+c/2
             const uint32_t o1 = r * 128 + ((((R.c >> 1)) ^ (r & 7)) << 4) + (R.c & 1) * 8;
@@ -271,18 +256,6 @@ __device__ __forceinline__ void rotate_k_rows(uint32_t kh, uint32_t kl, unsigned
             sts64(kl + o2, b0, b1);
             sts64(kl + KBOX + o1, c0, c1);
             sts64(kl + KBOX + o2, d0, d1);
-            if (REMOTE) {
-                ptx::sts64_cluster(rkl + o1, a0, a1);
-                ptx::sts64_cluster(rkl + o2, b0, b1);
-                ptx::sts64_cluster(rkl + KBOX + o1, c0, c1);
-                ptx::sts64_cluster(rkl + KBOX + o2, d0, d1);
-            }
-        } else if (precise == 4) {
-            const uint32_t rb = kl + r * 128 + 2 * R.c, x = (uint32_t)(r & 7);
-            sts16s(rb + (((c4 & 15u) ^ x) << 4), __byte_perm(e5m2x4(l1[0], l1[1]), e5m2x4(l1[2], l1[3]), R.selw));
-            sts16s(rb + ((((c4 >> 4) & 15u) ^ x) << 4), __byte_perm(e5m2x4(l2[0], l2[1]), e5m2x4(l2[2], l2[3]), R.selw));
-            sts16s(rb + ((((c4 >> 8) & 15u) ^ x) << 4), __byte_perm(e5m2x4(h1[0], h1[1]), e5m2x4(h1[2], h1[3]), R.selw));
-            sts16s(rb + ((((c4 >> 12) & 15u) ^ x) << 4), __byte_perm(e5m2x4(h2[0], h2[1]), e5m2x4(h2[2], h2[3]), R.selw));
         } else if (precise == 3) {
             const uint32_t o1 = r * 128 + ((((R.c >> 1)) ^ (r & 7)) << 4) + (R.c & 1) * 8;
             const uint32_t o2 = r * 128 + (((4 + (R.c >> 1)) ^ (r & 7)) << 4) + (R.c & 1) * 8;

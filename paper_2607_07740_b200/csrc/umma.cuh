@@ -289,29 +289,6 @@ __device__ __forceinline__ void umma2_commit_e(uint64_t* bar, uint32_t elect) {
         "@pe tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %2;\n\t}"
         ::"r"(smem_u32(bar)), "r"(elect), "h"((uint16_t)3) : "memory");
 }
-// ---- cluster of four (two CTA pairs sharing rotated K tiles): addresses in another CTA of the cluster ----------
-__device__ __forceinline__ uint32_t mapa_u32(uint32_t cta_addr, uint32_t rank) {
-    uint32_t r;
-    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(cta_addr), "r"(rank));
-    return r;
-}
-__device__ __forceinline__ void mbar_arrive_cluster_addr(uint32_t cluster_addr) {
-    asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
-}
-__device__ __forceinline__ void sts128_cluster(uint32_t a, uint32_t x, uint32_t y, uint32_t z, uint32_t w) {
-    asm volatile("st.shared::cluster.v4.u32 [%0], {%1,%2,%3,%4};" ::"r"(a), "r"(x), "r"(y), "r"(z), "r"(w) : "memory");
-}
-__device__ __forceinline__ void sts64_cluster(uint32_t a, uint32_t x, uint32_t y) {
-    asm volatile("st.shared::cluster.v2.u32 [%0], {%1,%2};" ::"r"(a), "r"(x), "r"(y) : "memory");
-}
-// bulk copy of `bytes` (multiple of 16) from this CTA's shared memory into another CTA of the cluster; the bytes are
-// counted (complete_tx) on an mbarrier of the DESTINATION CTA.  dst and mbar are shared::cluster addresses (mapa).
-__device__ __forceinline__ void bulk_copy_to_peer(uint32_t dst_cluster, uint32_t src_cta, uint32_t bytes, uint32_t mbar_cluster) {
-    asm volatile("cp.async.bulk.shared::cluster.shared::cta.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                 ::"r"(dst_cluster), "r"(src_cta), "r"(bytes), "r"(mbar_cluster) : "memory");
-}
-// generic-proxy writes (own and remote shared memory) -> visible to the async proxy
-__device__ __forceinline__ void fence_proxy_async_all() { asm volatile("fence.proxy.async;" ::: "memory"); }
 // commit with an explicit multicast mask (CTA ranks of the cluster that receive the arrival at the same offset)
 __device__ __forceinline__ void umma2_commit_mask(uint64_t* bar, uint32_t mask) {
     asm volatile(
