@@ -41,7 +41,9 @@ constexpr int RT = RW * 32;                          // rotate threads
 constexpr int RROWS = 1024 / RT;                     // key rows per rotate thread (8 chunks x 128 rows / RT)
 constexpr int NTHREADS = 96 + RT + 128;             // warps: 0 K producer, 1 MMA, 2 V producer, 3.. rotate, last 4 softmax
 constexpr float kLog2e = 1.4426950408889634f;
-constexpr uint32_t TM_S = 0, TM_O = 64;              // S0 | S1 (32 fp32 columns each: K'hi Q'hi | K'hi Q'lo) | O (16)
+constexpr uint32_t SCOLS = 4 * NH;                   // columns of one S buffer: [hi | lo | d/dn | d2/dn2] blocks of 16 heads
+constexpr uint32_t TM_S = 0, TM_O = 2 * SCOLS;       // S0 | S1 (64 fp32 columns each, see issue_s) | O (16)
+constexpr int TM_COLS = 256;
 
 struct Bars {
     uint64_t k_full[KS], k_ready[KS], k_empty[KS];
@@ -69,6 +71,7 @@ struct Params {
     double theta;                                    // for the table-header check (see the prologue)
     long long n_hi;                                  // rows of the HI table the host asked the table kernel for
     FreqMap fm;                                      // the remote map the tables must have been built for
+    int split;                                       // 1: the slow frequency pairs 32-63 are not rotated per key (see SPLIT below)
 };
 // batched / paged form: blockIdx.z = sequence b with its own length and group size; the cache is a pool of
 // 128-row pages (= the TMA tile) addressed through a page table.  A separate kernel argument: the per-sequence arrays are
@@ -119,7 +122,20 @@ constexpr uint32_t IDESC_S_BF16 = idesc_f16(1, 1, 0, 0, BN, NH);
 constexpr uint32_t IDESC_S_F16 = idesc_f16(0, 0, 0, 0, BN, NH);
 constexpr uint32_t IDESC_S_F16_N32 = idesc_f16(0, 0, 0, 0, BN, 2 * NH);
 constexpr uint32_t IDESC_S_E5M2 = idesc_f16(1, 1, 0, 0, BN, NH);  // kind::f8f6f4: format code 1 = e5m2
+constexpr uint32_t IDESC_S_BF16_N64 = idesc_f16(1, 1, 0, 0, BN, 4 * NH);
 constexpr uint32_t IDESC_PV = idesc_f16(1, 1, 1, 0, D, NH);      // A = V^T (smem, MN-major), B = P (smem, K-major)
+
+// SPLIT (slow pairs through the tensor core on the STORED keys).  The correction rotation of pair i at key row m of a tile
+// is Rot(alpha_ref + eps), alpha_ref the angle at the tile's reference row (n_ref = n(k0 + 64)) and
+// eps = (n_m - n_ref) a_i, a_i the table's unit-step angle (|a_i| = theta_i).  For i >= 32 and rope_theta >= 8.4e5,
+// |eps| <= 64 theta_32 <= 0.07, and  Rot(eps) = (1 - eps^2/2) I + eps J  holds to eps^3/6 <= 6e-5 (relative, per pair):
+//     q'^T Rot(alpha_ref + eps) k = qt^T k + dn (a J^T qt)^T k + dn^2 (-a^2/2 qt)^T k,   qt = Rot(alpha_ref)^T q',  dn = n_m - n_ref.
+// So those pairs need no per-key rotation at all: per tile the rotate group writes four 16-row blocks of a bf16 B operand
+// [qt hi | qt lo | a J^T qt | -a^2/2 qt] (16 heads x 32 pairs: 1/16 of the key tile's elements), the MMA warp multiplies the
+// stored bf16 K slices by them (N = 64), and the softmax thread of key m adds  S[.,0] + S[.,1] + dn (S[.,2] + dn S[.,3]).
+// The stored keys enter exactly (no fp16 re-rounding, no e5m2 residual), so these pairs are MORE accurate than the rotated
+// ones.  The operand lives in the unused bytes of the K stage's own e5m2 box (byte ranges 32-63 and 96-127 of each row belong
+// to the unrotated channels): rows 0-63 serve channels 32-47 / 48-63, rows 64-127 channels 96-111 / 112-127.
 
 struct DPlan {
     long long ks, ke, re, ls;
@@ -181,28 +197,51 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
     // overlaps its tail).
     if (!p.bifocal) griddep_wait();
     // the query loads go out before the TMA streams start: behind ~14 MB of in-flight cache tiles they take microseconds
-    const int rt = tid - 96;                                           // rotate-group thread index
-    __nv_bfloat16 qv1[NH * 64 / RT], qv2[NH * 64 / RT];
-    float2 tqh[NH * 64 / RT], tql[NH * 64 / RT];                       // HI / LO table entries of the query position
+    constexpr int NI = (NG * 64 + RT - 1) / RT;                        // (head, pair) items of the Q operands per rotate thread
+    // rotate-group thread index.  Group warp w' = 2 (w & 3) + (w >> 2) for the CTA's rotate warp w = warp - 3: the odd w' (which
+    // build the slow pairs' operand in SPLIT mode) and the even w' each land on all four sub-partitions
+    const int rt = ((((warp - 3) & 3) * 2 + (((warp - 3) >> 2) & 1)) << 5) | lane;
+    __nv_bfloat16 qv1[NI], qv2[NI];
+    float2 tqh[NI], tql[NI];                       // HI / LO table entries of the query position
     KRot<RROWS> rot;
     bool tab_early = false;
     unsigned tab_gen = 0;                                               // check word of the table header at the early read
     const long long nq = (p.L - 1) - (p.L - 1) / p.G;                  // -Delta(q) >= 0, Eq.(5)
+    // SPLIT: table entries of this thread's slow pair (rt & 63 >= 32): the unit step, the two possible steps of the reference
+    // row from one tile to the next (n_ref advances by D0 or D0 + 1, D0 = 128 - ceil(128 / G)), the first tile's reference row
+    float2 s_unit = make_float2(1.f, 0.f), s_e0 = s_unit, s_e1 = s_unit, s_rh = s_unit, s_rl = s_unit;
+    const unsigned sD0 = 128u - (unsigned)((128 + p.G - 1) / p.G);
     auto load_tables = [&]() {
+        if (p.split && (rt & 63) >= 32) {
+            const int si = rt & 63;
+            const unsigned pr = (unsigned)(plan.kt(0) * BN) + 64u, n = pr - pr / (unsigned)p.G;
+            s_unit = __ldg(&p.lo[64 + si]);
+            s_e0 = __ldg(&p.lo[(size_t)sD0 * 64 + si]);
+            s_e1 = __ldg(&p.lo[(size_t)(sD0 + 1) * 64 + si]);
+            s_rh = __ldg(&p.hi[(size_t)(n >> 8) * 64 + si]);
+            s_rl = __ldg(&p.lo[(size_t)(n & 255) * 64 + si]);
+        }
 #pragma unroll
-        for (int it = 0; it < NH * 64 / RT; ++it) {
+        for (int it = 0; it < NI; ++it) {
             const int idx = rt + it * RT;
             if (idx < p.g * 64) {
                 tqh[it] = __ldg(&p.hi[(nq >> 8) * 64 + (idx & 63)]);
                 tql[it] = __ldg(&p.lo[(nq & 255) * 64 + (idx & 63)]);
             }
         }
-        rot.init(p.lo, p.hi, rt, p.G);
+        // SPLIT: chunks 0-3 only.  The odd warps also build the slow pairs' operand every tile, so they rotate one row per
+        // thread (rows 96-127) and the even warps three (rows 0-95): both halves of the group finish a tile together
+        if (p.split) {
+            const int e = (rt >> 6) * 8 + ((rt & 31) >> 2);
+            
+            rot.init_at(p.lo, p.hi, rt & 3, (rt & 32) ? 96 + e : 3 * e, p.G);
+        }
+        else rot.init(p.lo, p.hi, rt, p.G);
         rot.prefetch((unsigned)(plan.kt(0) * BN));
     };
     if (warp >= 3 && warp < 3 + RW) {
 #pragma unroll
-        for (int it = 0; it < NH * 64 / RT; ++it) {
+        for (int it = 0; it < NI; ++it) {
             const int idx = rt + it * RT;
             if (idx < p.g * 64) {
                 const __nv_bfloat16* qh = p.q + (size_t)(kvh * p.g + (idx >> 6)) * D;
@@ -246,7 +285,7 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
         fence_barrier_init();
         prefetch_tmap(&tmK); prefetch_tmap(&tmV);
     }
-    if (warp == 1) tmem_alloc<128>(&bars->tmem_base);
+    if (warp == 1) tmem_alloc<TM_COLS>(&bars->tmem_base);
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
@@ -286,7 +325,7 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
         const uint32_t tm = __shfl_sync(0xffffffffu, tmem, 0);
         const uint32_t smem0 = __shfl_sync(0xffffffffu, smem_u32(smem), 0);
         auto issue_s = [&](int v) {
-            const uint32_t dS = tm + TM_S + (v & 1) * 2 * NH;
+            const uint32_t dS = tm + TM_S + (v & 1) * SCOLS;
             const uint32_t ka = smem0 + (v % KS) * KSTAGE, kla = ka + TILE;
             const uint32_t qa = smem0 + (uint32_t)OFF_Q;
             const bool rem = plan.remote(v);
@@ -296,6 +335,25 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
                     for (int ks = 0; ks < D / 16; ++ks)
                         umma_ss(dS, smem_desc_sw128(ka + (ks >> 2) * BOXB + (ks & 3) * 32, 16, 1024),
                                 smem_desc_sw128(qa + (ks >> 2) * (NH * 128) + (ks & 3) * 32, 16, 1024), IDESC_S_BF16, ks > 0);
+                } else if (p.split) {
+                    const uint32_t qc = qa + QBUF;
+                    // slow pairs first (they open all 64 columns): stored bf16 K slices 2, 3, 6, 7 times the per-tile operand
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) {
+                        const int ks = (j & 1) + 2 + (j >> 1) * 4;
+                        umma_ss(dS, smem_desc_sw128(ka + (ks >> 2) * BOXB + (ks & 3) * 32, 16, 1024),
+                                smem_desc_sw128(kla + (j >> 1) * 64 * 128 + 32 + (j & 1) * 64, 16, 1024), IDESC_S_BF16_N64, j > 0);
+                    }
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) {              // fast pairs: K'hi [Q'hi ; Q'lo] on slices 0, 1, 4, 5 (columns 0-31)
+                        const int ks = (j & 1) + (j >> 1) * 4;
+                        umma_ss(dS, smem_desc_sw128(ka + (ks >> 2) * BOXB + (ks & 3) * 32, 16, 1024),
+                                smem_desc_sw128(qc + (ks >> 2) * (2 * NH * 128) + (ks & 3) * 32, 16, 1024), IDESC_S_F16_N32, 1);
+                    }
+#pragma unroll
+                    for (int ks = 0; ks < D / 32; ks += 2)     // K'lo (e5m2) Q'hi (e5m2) of channels 0-31 and 64-95
+                        umma_ss_f8(dS, smem_desc_sw128(kla + ks * 32, 16, 1024),
+                                   smem_desc_sw128(qc + QCBUF + ks * 32, 16, 1024), IDESC_S_E5M2 | (1u << 13), 1);
                 } else {
                     const uint32_t qc = qa + QBUF;                  // rows 0-15 Q'hi, rows 16-31 Q'lo
 #pragma unroll
@@ -345,7 +403,7 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
         __syncwarp();
     } else if (warp >= 3 && warp < 3 + RW) {
         // ===================== rotate group (steps a4, a5) =====================
-        const int t = tid - 96;
+        const int t = rt;
         // Q operands [16 heads][128 ch]: raw bf16 for local tiles; Q' = R(Delta q) Q as fp16 hi / lo for remote tiles
         for (int i = t; i < (QBUF + QCBUF + QYBUF) / 4; i += RT) reinterpret_cast<uint32_t*>(sQ)[i] = 0u;
         for (int i = t; i < QBUF / 4; i += RT) reinterpret_cast<uint32_t*>(sP)[i] = 0u;
@@ -360,19 +418,25 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
                 load_tables();
             }
         }
+        float qy1[NI], qy2[NI];                 // Q' pairs of this thread in fp32 (SPLIT: the slow ones are re-based per tile)
 #pragma unroll
-        for (int it = 0; it < NH * 64 / RT; ++it) {
+        for (int it = 0; it < NI; ++it) { qy1[it] = 0.f; qy2[it] = 0.f; }
+#pragma unroll
+        for (int it = 0; it < NI; ++it) {                  // (no break: the register arrays keep static indices)
             const int idx = t + it * RT;
-            if (idx >= p.g * 64) break;
+            const bool mine = idx < p.g * 64;
             const int h = idx >> 6, i = idx & 63;
             const __nv_bfloat16 b1 = qv1[it], b2 = qv2[it];
-            *reinterpret_cast<__nv_bfloat16*>(sQ + bop_off(h, i)) = b1;
-            *reinterpret_cast<__nv_bfloat16*>(sQ + bop_off(h, i + 64)) = b2;
-            if (plan.nr > 0) {
+            if (mine) {
+                *reinterpret_cast<__nv_bfloat16*>(sQ + bop_off(h, i)) = b1;
+                *reinterpret_cast<__nv_bfloat16*>(sQ + bop_off(h, i + 64)) = b2;
+            }
+            if (mine && plan.nr > 0) {
                 const float2 ch = tqh[it], cl = tql[it];
                 const float c = ch.x * cl.x - ch.y * cl.y, s = ch.y * cl.x + ch.x * cl.y;
                 const float x1 = __bfloat162float(b1), x2 = __bfloat162float(b2);
                 const float y1 = x1 * c - x2 * s, y2 = x1 * s + x2 * c;
+                qy1[it] = y1; qy2[it] = y2;
                 const __half h1 = __float2half_rn(y1), h2 = __float2half_rn(y2);
                 *reinterpret_cast<__half*>(sQ + QBUF + bop_off<2 * NH>(h, i)) = h1;
                 *reinterpret_cast<__half*>(sQ + QBUF + bop_off<2 * NH>(h, i + 64)) = h2;
@@ -387,10 +451,56 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
         fence_proxy_async_smem();
         __syncwarp();
         if (lane == 0) mbar_arrive(&bars->q_ready);
+        // SPLIT: this thread's slow pair i = t & 63 (>= 32) of heads (t >> 6) + 4 it; table entries of the tile's reference row
+        const int si = t & 63;
+        const bool slow = p.split && plan.nr > 0 && si >= 32;
+        // sin of the unit step = its angle a_i to 2e-7 (|a_i| <= 1.1e-3); -a_i^2 / 2; cs(alpha_ref) of the current tile, carried
+        // from tile to tile by one complex multiplication (no table load inside the loop: an L2 hit behind the cache
+        // streams takes longer than a tile)
+        const float ua = s_unit.y, ub = -0.5f * ua * ua;
+        float rc = s_rh.x * s_rl.x - s_rh.y * s_rl.y, rs = s_rh.y * s_rl.x + s_rh.x * s_rl.y;
+        // n_ref advances by 128 - floor(128 / G) - [phase wraps], phase = (reference position) mod G: no division per tile
+        const unsigned gG = (unsigned)p.G, g_m = 128u % gG;
+        unsigned g_ph = ((unsigned)(plan.kt(0) * BN) + 64u) % gG;
+        const uint32_t sb0 = (uint32_t)((si < 48 ? 32 : 96) + (si & 15) * 2);     // byte of channel i in its operand row
         for (int v = 0; v < plan.nv; ++v) {
             const int s = v % KS;
             mbar_wait(&bars->k_full[s], (v / KS) & 1);
-            if (plan.remote(v)) {
+            if (plan.remote(v) && p.split) {
+                const uint32_t kl = smem_u32(sK(s)) + TILE;
+                if (t & 32) rotate_rows2<1, BOXB, 3, true>(smem_u32(sK(s)), kl, (unsigned)(plan.kt(v) * BN), rot, SelTree(), 0u, 0u);
+                else rotate_rows2<3, BOXB, 3, true>(smem_u32(sK(s)), kl, (unsigned)(plan.kt(v) * BN), rot, SelTree(), 0u, 0u);
+                if (slow) {
+                    const float c = rc, sn = rs;                                 // cs(alpha_ref) of pair i
+                    {
+                        g_ph += g_m;
+                        const bool wrap = g_ph >= gG;                            // one more multiple of G passed: n_ref advances by D0
+                        if (wrap) g_ph -= gG;
+                        const float2 e = (wrap || g_m == 0u) ? s_e0 : s_e1;
+                        rc = c * e.x - sn * e.y; rs = sn * e.x + c * e.y;
+                    }
+#pragma unroll
+                    for (int it = 0; it < NI; ++it) {
+                        const int h = (t >> 6) + 4 * it;
+                        if (h < p.g) {
+                            const float q1 = c * qy1[it] + sn * qy2[it], q2 = c * qy2[it] - sn * qy1[it];   // qt = Rot(alpha_ref)^T q'
+                            const uint16_t h1 = bf16_bits(q1), h2 = bf16_bits(q2);
+                            const float r1 = q1 - __uint_as_float((uint32_t)h1 << 16), r2 = q2 - __uint_as_float((uint32_t)h2 << 16);
+                            const uint16_t w1[4] = {h1, bf16_bits(r1), bf16_bits(ua * q2), bf16_bits(ub * q1)};     // channel i
+                            const uint16_t w2[4] = {h2, bf16_bits(r2), bf16_bits(-ua * q1), bf16_bits(ub * q2)};    // channel i + 64
+                            // row b 16 + h of the operand: the swizzle term depends on h only (16 rows = two swizzle periods)
+                            const uint32_t a = kl + (uint32_t)h * 128 + ((((sb0 >> 4) ^ ((uint32_t)h & 7u)) << 4) | (sb0 & 15u));
+#pragma unroll
+                            for (int b = 0; b < 4; ++b) {
+                                sts16(a + b * NH * 128, w1[b]);
+                                sts16(a + b * NH * 128 + 64 * 128, w2[b]);
+                            }
+                        }
+                    }
+                }
+                fence_proxy_async_smem();
+                if (plan.remote(v + 1)) rot.prefetch((unsigned)(plan.kt(v + 1) * BN));
+            } else if (plan.remote(v)) {
                 rotate_rows2<RROWS, BOXB, 3, true>(smem_u32(sK(s)), smem_u32(sK(s)) + TILE, (unsigned)(plan.kt(v) * BN), rot, SelTree(), 0u, 0u);
                 fence_proxy_async_smem();
                 if (plan.remote(v + 1)) rot.prefetch((unsigned)(plan.kt(v + 1) * BN));
@@ -415,14 +525,27 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
             mbar_wait(&bars->s_full[v & 1], (v >> 1) & 1);
             tc_fence_after();
             uint32_t sr[32];
-            tmem_ld32(tmem + lane_base + TM_S + (v & 1) * 2 * NH, sr);
-            tmem_ld_wait();
+            tmem_ld32(tmem + lane_base + TM_S + (v & 1) * SCOLS, sr);
             const bool rem = plan.remote(v);                          // remote: columns 16.. hold the K'hi Q'lo term
+            float tay[NG];                                            // SPLIT: dn (S[.,2] + dn S[.,3]) of the slow pairs
+#pragma unroll
+            for (int h = 0; h < NG; ++h) tay[h] = 0.f;
+            if (rem && p.split) {
+                uint32_t st[32];
+                tmem_ld32(tmem + lane_base + TM_S + (v & 1) * SCOLS + 2 * NH, st);
+                tmem_ld_wait();
+                const unsigned pk = (unsigned)key, pr = (unsigned)(plan.kt(v) * BN) + 64u, Gu = (unsigned)p.G;
+                const float dn = (float)((int)(pk - pk / Gu) - (int)(pr - pr / Gu));
+#pragma unroll
+                for (int h = 0; h < NG; ++h) tay[h] = dn * (__uint_as_float(st[h]) + dn * __uint_as_float(st[NH + h]));
+            } else {
+                tmem_ld_wait();
+            }
             float x[NG];
             bool jump = false;
 #pragma unroll
             for (int h = 0; h < NG; ++h) {
-                const float sc = __uint_as_float(sr[h]) + (rem ? __uint_as_float(sr[NH + h]) : 0.0f);
+                const float sc = __uint_as_float(sr[h]) + (rem ? __uint_as_float(sr[NH + h]) + tay[h] : 0.0f);
                 x[h] = (valid && h < g) ? sc * sl2 : -INFINITY;
                 jump |= x[h] > m_ref[h] + 8.0f;                      // lazy rescale: only on a jump of 2^8 (or from -inf)
             }
@@ -518,10 +641,16 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
     }
     tc_fence_before();
     __syncthreads();
-    if (warp == 1) tmem_dealloc<128>(tmem);
+    if (warp == 1) tmem_dealloc<TM_COLS>(tmem);
 }
 
 }  // namespace
+
+// SPLIT holds when the in-tile phase of pair 32 stays small: 64 theta_32 = 64 rope_theta^-1/2 <= 0.07 (third-order term
+// of the rotation <= 6e-5 per pair); the frequency-interpolation map keeps the per-key rotation
+static int split_ok(double theta, const FreqMap& fm) {
+    return (!fm.interp && 64.0 / sqrt(theta) <= 0.07) ? 1 : 0;
+}
 
 bool umma_decode_supported(int H_q, int H_kv, int d, int dtype) {
     if (dtype != JETLONG_BF16 || d != 128 || H_kv < 1 || H_q % H_kv) return false;
@@ -556,6 +685,7 @@ int launch_decode_umma(const void* q, const void* K, const void* V, float* part,
     p.lo = lo; p.hi = hi;
     p.theta = theta;
     p.n_hi = (L + 255) / 256 + 1; p.fm = fm;
+    p.split = bifocal ? split_ok(theta, fm) : 0;
     BatchInfo bi = {};                                                 // batch = 0: the single-sequence call
     auto kern = p.g <= 1 ? decode_umma_kernel<1, false> : p.g <= 2 ? decode_umma_kernel<2, false> : p.g <= 4 ? decode_umma_kernel<4, false>
               : p.g <= 8 ? decode_umma_kernel<8, false> : decode_umma_kernel<16, false>;
@@ -598,6 +728,7 @@ int launch_decode_umma_paged(const void* q, const void* Kpool, const void* Vpool
     p.lo = lo; p.hi = hi;
     p.theta = theta;
     p.n_hi = (Lmax + 255) / 256 + 1; p.fm = alias_map();
+    p.split = split_ok(theta, p.fm);
     BatchInfo bi = {};
     bi.batch = nb; bi.page_table = page_table; bi.max_pages = max_pages; bi.part_stride = part_stride;
     bool any_bifocal = false;

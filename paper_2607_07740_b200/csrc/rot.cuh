@@ -144,6 +144,11 @@ template <int ROWS> struct KRot {
             sc[j] = pack2(l.x, l.z); ss[j] = pack2(l.y, l.w);
         }
     }
+    // the same with the thread's chunk (8 frequency pairs) and first row given by the caller
+    __device__ __forceinline__ void init_at(const float2* lo_, const float2* hi_, int c_, int r0_, long long G_) {
+        init(lo_, hi_, c_, G_);
+        r0 = r0_;
+    }
     // pos0 = absolute position of this CTA's first key row of the tile
     __device__ __forceinline__ void prefetch(unsigned pos0) {
         const unsigned pos = pos0 + r0;
@@ -308,8 +313,8 @@ struct SelTree {
     }
 };
 
-template <int ROWS, int KBOX, int MODE, bool UNROLL = false>
-__device__ __forceinline__ void rotate_rows2(uint32_t kh, uint32_t kl, unsigned pos0, KRot<ROWS>& R, const SelTree& T,
+template <int ROWS, int KBOX, int MODE, bool UNROLL = false, int RR = ROWS>
+__device__ __forceinline__ void rotate_rows2(uint32_t kh, uint32_t kl, unsigned pos0, KRot<RR>& R, const SelTree& T,
                                              uint32_t b_lo, uint32_t b_hi) {
     uint64_t cc[4], cs[4], ncs[4], nss[4];
 #pragma unroll
