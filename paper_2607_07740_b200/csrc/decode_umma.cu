@@ -237,7 +237,8 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
             rot.init_at(p.lo, p.hi, rt & 3, (rt & 32) ? 96 + e : 3 * e, p.G);
         }
         else rot.init(p.lo, p.hi, rt, p.G);
-        rot.prefetch((unsigned)(plan.kt(0) * BN));
+        rot.seek((unsigned)(plan.kt(0) * BN));
+        rot.prefetch_carried();
     };
     if (warp >= 3 && warp < 3 + RW) {
 #pragma unroll
@@ -460,7 +461,7 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
         const float ua = s_unit.y, ub = -0.5f * ua * ua;
         float rc = s_rh.x * s_rl.x - s_rh.y * s_rl.y, rs = s_rh.y * s_rl.x + s_rh.x * s_rl.y;
         // n_ref advances by 128 - floor(128 / G) - [phase wraps], phase = (reference position) mod G: no division per tile
-        const unsigned gG = (unsigned)p.G, g_m = 128u % gG;
+        const unsigned gG = (unsigned)p.G, g_m = 128u % gG, g_d = 128u / gG;
         unsigned g_ph = ((unsigned)(plan.kt(0) * BN) + 64u) % gG;
         const uint32_t sb0 = (uint32_t)((si < 48 ? 32 : 96) + (si & 15) * 2);     // byte of channel i in its operand row
         for (int v = 0; v < plan.nv; ++v) {
@@ -468,8 +469,8 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
             mbar_wait(&bars->k_full[s], (v / KS) & 1);
             if (plan.remote(v) && p.split) {
                 const uint32_t kl = smem_u32(sK(s)) + TILE;
-                if (t & 32) rotate_rows2<1, BOXB, 3, true>(smem_u32(sK(s)), kl, (unsigned)(plan.kt(v) * BN), rot, SelTree(), 0u, 0u);
-                else rotate_rows2<3, BOXB, 3, true>(smem_u32(sK(s)), kl, (unsigned)(plan.kt(v) * BN), rot, SelTree(), 0u, 0u);
+                if (t & 32) rotate_rows2<1, BOXB, 3, true, true>(smem_u32(sK(s)), kl, (unsigned)(plan.kt(v) * BN), rot, SelTree(), 0u, 0u);
+                else rotate_rows2<3, BOXB, 3, true, true>(smem_u32(sK(s)), kl, (unsigned)(plan.kt(v) * BN), rot, SelTree(), 0u, 0u);
                 if (slow) {
                     const float c = rc, sn = rs;                                 // cs(alpha_ref) of pair i
                     {
@@ -499,11 +500,11 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
                     }
                 }
                 fence_proxy_async_smem();
-                if (plan.remote(v + 1)) rot.prefetch((unsigned)(plan.kt(v + 1) * BN));
+                if (plan.remote(v + 1)) { rot.step128(g_m, g_d); rot.prefetch_carried(); }
             } else if (plan.remote(v)) {
-                rotate_rows2<RROWS, BOXB, 3, true>(smem_u32(sK(s)), smem_u32(sK(s)) + TILE, (unsigned)(plan.kt(v) * BN), rot, SelTree(), 0u, 0u);
+                rotate_rows2<RROWS, BOXB, 3, true, true>(smem_u32(sK(s)), smem_u32(sK(s)) + TILE, (unsigned)(plan.kt(v) * BN), rot, SelTree(), 0u, 0u);
                 fence_proxy_async_smem();
-                if (plan.remote(v + 1)) rot.prefetch((unsigned)(plan.kt(v + 1) * BN));
+                if (plan.remote(v + 1)) { rot.step128(g_m, g_d); rot.prefetch_carried(); }
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(&bars->k_ready[s]);

@@ -135,6 +135,7 @@ template <int ROWS> struct KRot {
     const float2* lo; const float2* hi;
     int c, r0;
     unsigned G;
+    unsigned rem_, n_;              // decode (consecutive tiles): position mod G and n of this thread's first row, carried
     __device__ __forceinline__ void init(const float2* lo_, const float2* hi_, int t, long long G_, int rbase = 0) {
         lo = lo_; hi = hi_; c = t & 7; r0 = rbase + ROWS * (t >> 3); G = (unsigned)G_;
         const float4* p1 = reinterpret_cast<const float4*>(lo + 64 + 8 * c);       // LO[1][8c..]
@@ -148,6 +149,23 @@ template <int ROWS> struct KRot {
     __device__ __forceinline__ void init_at(const float2* lo_, const float2* hi_, int c_, int r0_, long long G_) {
         init(lo_, hi_, c_, G_);
         r0 = r0_;
+    }
+    // carried form for a run of consecutive 128-key tiles: seek() once (two divisions), then step128() per tile (none)
+    __device__ __forceinline__ void seek(unsigned pos0) {
+        const unsigned pos = pos0 + r0;
+        rem_ = pos % G; n_ = pos - pos / G;
+    }
+    __device__ __forceinline__ void step128(unsigned m128, unsigned d128) {        // m128 = 128 % G, d128 = 128 / G
+        rem_ += m128;
+        const unsigned wrap = rem_ >= G ? 1u : 0u;
+        rem_ -= wrap ? G : 0u;
+        n_ += 128u - d128 - wrap;
+    }
+    __device__ __forceinline__ void prefetch_carried() {
+        const float4* ph = reinterpret_cast<const float4*>(hi + (size_t)(n_ >> 8) * 64 + 8 * c);
+        const float4* pl = reinterpret_cast<const float4*>(lo + (size_t)(n_ & 255) * 64 + 8 * c);
+#pragma unroll
+        for (int j = 0; j < 4; ++j) { nh[j] = __ldg(ph + j); nl[j] = __ldg(pl + j); }
     }
     // pos0 = absolute position of this CTA's first key row of the tile
     __device__ __forceinline__ void prefetch(unsigned pos0) {
@@ -313,7 +331,7 @@ struct SelTree {
     }
 };
 
-template <int ROWS, int KBOX, int MODE, bool UNROLL = false, int RR = ROWS>
+template <int ROWS, int KBOX, int MODE, bool UNROLL = false, bool CARRIED = false, int RR = ROWS>
 __device__ __forceinline__ void rotate_rows2(uint32_t kh, uint32_t kl, unsigned pos0, KRot<RR>& R, const SelTree& T,
                                              uint32_t b_lo, uint32_t b_hi) {
     uint64_t cc[4], cs[4], ncs[4], nss[4];
@@ -325,7 +343,7 @@ __device__ __forceinline__ void rotate_rows2(uint32_t kh, uint32_t kl, unsigned 
         ncs[j] = neg2(cs[j]);
         nss[j] = neg2(R.ss[j]);
     }
-    unsigned rem = (pos0 + R.r0) % R.G;
+    unsigned rem = CARRIED ? R.rem_ : (pos0 + R.r0) % R.G;              // CARRIED: the caller keeps it (KRot::seek / step128)
     int off = R.r0 * 128 + ((R.c ^ (R.r0 & 7)) << 4);
     uint4 u1 = lds128(kh + off), u2 = lds128(kh + KBOX + off);
     // rolled on purpose: the SM's instruction caches are small (L0 ~6 KB, L1.5 32 KB) and four roles run different loops;
