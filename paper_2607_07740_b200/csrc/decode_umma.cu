@@ -122,7 +122,8 @@ constexpr uint32_t IDESC_S_BF16 = idesc_f16(1, 1, 0, 0, BN, NH);
 constexpr uint32_t IDESC_S_F16 = idesc_f16(0, 0, 0, 0, BN, NH);
 constexpr uint32_t IDESC_S_F16_N32 = idesc_f16(0, 0, 0, 0, BN, 2 * NH);
 constexpr uint32_t IDESC_S_E5M2 = idesc_f16(1, 1, 0, 0, BN, NH);  // kind::f8f6f4: format code 1 = e5m2
-constexpr uint32_t IDESC_S_BF16_N64 = idesc_f16(1, 1, 0, 0, BN, 4 * NH);
+constexpr int SB = 8;                                // rows (heads) per block of the slow pairs' operand: SPLIT serves g <= 8
+constexpr uint32_t IDESC_S_BF16_N48 = idesc_f16(1, 1, 0, 0, BN, 6 * SB);
 constexpr uint32_t IDESC_PV = idesc_f16(1, 1, 1, 0, D, NH);      // A = V^T (smem, MN-major), B = P (smem, K-major)
 
 // SPLIT (slow pairs through the tensor core on the STORED keys).  The correction rotation of pair i at key row m of a tile
@@ -130,12 +131,15 @@ constexpr uint32_t IDESC_PV = idesc_f16(1, 1, 1, 0, D, NH);      // A = V^T (sme
 // eps = (n_m - n_ref) a_i, a_i the table's unit-step angle (|a_i| = theta_i).  For i >= 32 and rope_theta >= 8.4e5,
 // |eps| <= 64 theta_32 <= 0.07, and  Rot(eps) = (1 - eps^2/2) I + eps J  holds to eps^3/6 <= 6e-5 (relative, per pair):
 //     q'^T Rot(alpha_ref + eps) k = qt^T k + dn (a J^T qt)^T k + dn^2 (-a^2/2 qt)^T k,   qt = Rot(alpha_ref)^T q',  dn = n_m - n_ref.
-// So those pairs need no per-key rotation at all: per tile the rotate group writes four 16-row blocks of a bf16 B operand
-// [qt hi | qt lo | a J^T qt | -a^2/2 qt] (16 heads x 32 pairs: 1/16 of the key tile's elements), the MMA warp multiplies the
-// stored bf16 K slices by them (N = 64), and the softmax thread of key m adds  S[.,0] + S[.,1] + dn (S[.,2] + dn S[.,3]).
-// The stored keys enter exactly (no fp16 re-rounding, no e5m2 residual), so these pairs are MORE accurate than the rotated
-// ones.  The operand lives in the unused bytes of the K stage's own e5m2 box (byte ranges 32-63 and 96-127 of each row belong
-// to the unrotated channels): rows 0-63 serve channels 32-47 / 48-63, rows 64-127 channels 96-111 / 112-127.
+// So those pairs need no per-key rotation at all: per tile the rotate group writes 8-row blocks of a bf16 B operand
+//     block 0: qt hi | 1: unused | 2: qt lo | 3: (a J^T qt) hi | 4: (a J^T qt) lo | 5: -a^2/2 qt      (8 heads x 32 pairs each;
+// hi / lo because one bf16 rounding of a full-size term is 2^-9, and of the first-order term still 64 theta_i 2^-9: with loud
+// channels on pair 32 that alone broke the lse tolerance, tests/test_gpu_robustness.py), the MMA warp multiplies the stored
+// bf16 K slices by them (N = 48), and the softmax thread of key m adds  S[h] + S[16 + h] + dn (S[24 + h] + S[32 + h] + dn S[40 + h])
+// (columns h and 16 + h also receive the fast pairs' K'hi Q'hi and K'hi Q'lo).  The stored keys enter exactly (no fp16
+// re-rounding, no e5m2 residual).  The operand lives in the unused bytes of the K stage's own e5m2 box (byte ranges 32-63 and
+// 96-127 of each row belong to the unrotated channels): rows 0-47 serve channels 32-47 / 48-63, rows 64-111 channels 96-111 /
+// 112-127.  More than 8 query heads per KV head do not fit that space: they keep the per-key rotation of all pairs.
 
 struct DPlan {
     long long ks, ke, re, ls;
@@ -338,12 +342,12 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
                                 smem_desc_sw128(qa + (ks >> 2) * (NH * 128) + (ks & 3) * 32, 16, 1024), IDESC_S_BF16, ks > 0);
                 } else if (p.split) {
                     const uint32_t qc = qa + QBUF;
-                    // slow pairs first (they open all 64 columns): stored bf16 K slices 2, 3, 6, 7 times the per-tile operand
+                    // slow pairs first (they open columns 0-47): stored bf16 K slices 2, 3, 6, 7 times the per-tile operand
 #pragma unroll
                     for (int j = 0; j < 4; ++j) {
                         const int ks = (j & 1) + 2 + (j >> 1) * 4;
                         umma_ss(dS, smem_desc_sw128(ka + (ks >> 2) * BOXB + (ks & 3) * 32, 16, 1024),
-                                smem_desc_sw128(kla + (j >> 1) * 64 * 128 + 32 + (j & 1) * 64, 16, 1024), IDESC_S_BF16_N64, j > 0);
+                                smem_desc_sw128(kla + (j >> 1) * 64 * 128 + 32 + (j & 1) * 64, 16, 1024), IDESC_S_BF16_N48, j > 0);
                     }
 #pragma unroll
                     for (int j = 0; j < 4; ++j) {              // fast pairs: K'hi [Q'hi ; Q'lo] on slices 0, 1, 4, 5 (columns 0-31)
@@ -487,14 +491,20 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
                             const float q1 = c * qy1[it] + sn * qy2[it], q2 = c * qy2[it] - sn * qy1[it];   // qt = Rot(alpha_ref)^T q'
                             const uint16_t h1 = bf16_bits(q1), h2 = bf16_bits(q2);
                             const float r1 = q1 - __uint_as_float((uint32_t)h1 << 16), r2 = q2 - __uint_as_float((uint32_t)h2 << 16);
-                            const uint16_t w1[4] = {h1, bf16_bits(r1), bf16_bits(ua * q2), bf16_bits(ub * q1)};     // channel i
-                            const uint16_t w2[4] = {h2, bf16_bits(r2), bf16_bits(-ua * q1), bf16_bits(ub * q2)};    // channel i + 64
-                            // row b 16 + h of the operand: the swizzle term depends on h only (16 rows = two swizzle periods)
+                            const float u1 = ua * q2, u2 = -ua * q1;                     // a J^T qt: hi and lo as well -- its bf16
+                            const uint16_t g1 = bf16_bits(u1), g2 = bf16_bits(u2);       // rounding alone is 64 theta_i 2^-9 of a full-size term
+                            const float v1 = u1 - __uint_as_float((uint32_t)g1 << 16), v2 = u2 - __uint_as_float((uint32_t)g2 << 16);
+                            // blocks 0, 2, 3, 4, 5: column 16 + h is where the fast pairs put their Q'lo term, which like qt lo
+                            // is not multiplied by dn; block 1 (columns 8-15) is never written and never read
+                            const uint16_t w1[5] = {h1, bf16_bits(r1), g1, bf16_bits(v1), bf16_bits(ub * q1)};     // channel i
+                            const uint16_t w2[5] = {h2, bf16_bits(r2), g2, bf16_bits(v2), bf16_bits(ub * q2)};     // channel i + 64
+                            // row 8 b + h of the operand: the swizzle term depends on h only (8 rows = one swizzle period)
                             const uint32_t a = kl + (uint32_t)h * 128 + ((((sb0 >> 4) ^ ((uint32_t)h & 7u)) << 4) | (sb0 & 15u));
 #pragma unroll
-                            for (int b = 0; b < 4; ++b) {
-                                sts16(a + b * NH * 128, w1[b]);
-                                sts16(a + b * NH * 128 + 64 * 128, w2[b]);
+                            for (int b = 0; b < 5; ++b) {
+                                const int blk = b == 0 ? 0 : b + 1;
+                                sts16(a + blk * SB * 128, w1[b]);
+                                sts16(a + blk * SB * 128 + 64 * 128, w2[b]);
                             }
                         }
                     }
@@ -532,13 +542,14 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
 #pragma unroll
             for (int h = 0; h < NG; ++h) tay[h] = 0.f;
             if (rem && p.split) {
-                uint32_t st[32];
-                tmem_ld32(tmem + lane_base + TM_S + (v & 1) * SCOLS + 2 * NH, st);
+                uint32_t st[16];                                       // columns 32-47: a J^T qt lo | -a^2/2 qt
+                tmem_ld16(tmem + lane_base + TM_S + (v & 1) * SCOLS + 2 * NH, st);
                 tmem_ld_wait();
                 const unsigned pk = (unsigned)key, pr = (unsigned)(plan.kt(v) * BN) + 64u, Gu = (unsigned)p.G;
                 const float dn = (float)((int)(pk - pk / Gu) - (int)(pr - pr / Gu));
 #pragma unroll
-                for (int h = 0; h < NG; ++h) tay[h] = dn * (__uint_as_float(st[h]) + dn * __uint_as_float(st[NH + h]));
+                for (int h = 0; h < NG && h < SB; ++h)
+                    tay[h] = dn * ((__uint_as_float(sr[3 * SB + h]) + __uint_as_float(st[h])) + dn * __uint_as_float(st[SB + h]));
             } else {
                 tmem_ld_wait();
             }
@@ -649,8 +660,8 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
 
 // SPLIT holds when the in-tile phase of pair 32 stays small: 64 theta_32 = 64 rope_theta^-1/2 <= 0.07 (third-order term
 // of the rotation <= 6e-5 per pair); the frequency-interpolation map keeps the per-key rotation
-static int split_ok(double theta, const FreqMap& fm) {
-    return (!fm.interp && 64.0 / sqrt(theta) <= 0.07) ? 1 : 0;
+static int split_ok(double theta, const FreqMap& fm, int g) {
+    return (!fm.interp && g <= SB && 64.0 / sqrt(theta) <= 0.07) ? 1 : 0;
 }
 
 bool umma_decode_supported(int H_q, int H_kv, int d, int dtype) {
@@ -686,7 +697,7 @@ int launch_decode_umma(const void* q, const void* K, const void* V, float* part,
     p.lo = lo; p.hi = hi;
     p.theta = theta;
     p.n_hi = (L + 255) / 256 + 1; p.fm = fm;
-    p.split = bifocal ? split_ok(theta, fm) : 0;
+    p.split = bifocal ? split_ok(theta, fm, p.g) : 0;
     BatchInfo bi = {};                                                 // batch = 0: the single-sequence call
     auto kern = p.g <= 1 ? decode_umma_kernel<1, false> : p.g <= 2 ? decode_umma_kernel<2, false> : p.g <= 4 ? decode_umma_kernel<4, false>
               : p.g <= 8 ? decode_umma_kernel<8, false> : decode_umma_kernel<16, false>;
@@ -729,7 +740,7 @@ int launch_decode_umma_paged(const void* q, const void* Kpool, const void* Vpool
     p.lo = lo; p.hi = hi;
     p.theta = theta;
     p.n_hi = (Lmax + 255) / 256 + 1; p.fm = alias_map();
-    p.split = split_ok(theta, p.fm);
+    p.split = split_ok(theta, p.fm, p.g);
     BatchInfo bi = {};
     bi.batch = nb; bi.page_table = page_table; bi.max_pages = max_pages; bi.part_stride = part_stride;
     bool any_bifocal = false;

@@ -81,6 +81,8 @@ def make_qkv(L, H_q, H_kv, d, rope_theta, dtype, seed, outliers=False, device="c
       "switch"     the outlier channels change halfway through the sequence (4 channels x8 on rows < L/2, 4 others on the rest)
       "q_outliers" the 4 loud channels are in the un-rotated x_q (per query head) instead of x_k
       "loud"       every channel of x_k x1.5 on top of the standard outlier channels
+      "slow_pairs" the loud channels are the frequency pairs 32 and 33 (channels d/4, d/4+1 and their partners), x8 in x_k and
+                   x4 in x_q: the stress input of the decode kernel's second-order treatment of the slow pairs
     """
     n_q = L if n_q is None else n_q
     dev = torch.device(device)
@@ -99,6 +101,10 @@ def make_qkv(L, H_q, H_kv, d, rope_theta, dtype, seed, outliers=False, device="c
         for h in range(H_q):
             idx = torch.randperm(d, generator=gen, device=dev)[:4]
             xq[:, h, idx] *= 8.0
+    elif profile == "slow_pairs":
+        idx = torch.tensor([d // 4, d // 4 + 1, d // 4 + d // 2, d // 4 + 1 + d // 2], device=dev)
+        xk[:, :, idx] *= 8.0
+        xq[:, :, idx] *= 4.0
     elif outliers or profile == "loud":
         for kv in range(H_kv):
             idx = torch.randperm(d, generator=gen, device=dev)[:4]

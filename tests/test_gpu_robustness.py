@@ -255,3 +255,28 @@ def test_prefill_host_pipeline(L, H_q, H_kv, d, dtype, w_pre, w0):
     ri, hi = torch.as_tensor(rows), torch.as_tensor(heads).long()
     check(out[ri, hi], lse[hi, ri], ro, rl, Q.dtype, "host pipeline L=%d" % L)
     assert torch.isfinite(out.float()).all() and torch.isfinite(lse).all()
+
+
+# ---- decode: the second-order treatment of the slow frequency pairs (DESIGN.md 5.3 SPLIT) ------------------------------
+@pytest.mark.parametrize("theta", [1e6, 8.4e5, 8.3e5], ids=["theta1e6", "theta_at_the_split_bound", "theta_below_the_bound"])
+@pytest.mark.parametrize("profile", [None, "slow_pairs"])
+def test_decode_slow_pair_expansion_margin(theta, profile):
+    """Decode rows against the oracle over seeds, lengths and group sizes (G = 2, 3, 5, 7: 128 % G == 0 and != 0, so both
+    steps of the per-tile reference row occur), with the standard inputs and with the loud channels put on pairs 32 / 33,
+    where the truncated third-order term is largest; rope_theta = 8.4e5 sits on the bound that admits the expansion,
+    8.3e5 just below it (per-key rotation of all pairs)."""
+    H_q, H_kv, d, w0 = 8, 2, 128, 256
+    worst_o = worst_l = 0.0
+    for L, w_pre in ((4000, 2048), (9000, 3072), (20000, 4096), (33333, 5000)):
+        assert J.jetlong_group_size(L, w_pre) in (2, 3, 5, 7)
+        for s in range(4):
+            Q, K, V = W.make_qkv(L, H_q, H_kv, d, theta, "bf16", 71000 + 31 * s + L, profile is None, DEV,
+                                 q_pos0=L - 1, n_q=1, profile=profile)
+            out, lse = J.jetlong_decode(Q[0].contiguous(), K, V, L, w_local=w0, w_pretrained=w_pre, rope_theta=theta)
+            torch.cuda.synchronize()
+            ro, rl = oracle_rows(Q, K, V, [L - 1] * H_q, list(range(H_q)), w_local=w0, w_pretrained=w_pre, rope_theta=theta,
+                                 q_pos_rows=[0] * H_q)
+            worst_o = max(worst_o, float(np.abs(out.double().cpu().numpy() - ro).max()))
+            worst_l = max(worst_l, float(np.abs(lse.double().cpu().numpy() - rl).max()))
+    print("decode, theta %.3g, profile %s: worst out %.3e, worst lse %.3e" % (theta, profile, worst_o, worst_l))
+    assert worst_l <= TOL[torch.bfloat16]["lse"] and worst_o <= TOL[torch.bfloat16]["out_abs"], (worst_o, worst_l)
