@@ -40,7 +40,8 @@ typedef enum {
     JETLONG_OK = 0,
     JETLONG_INVALID_ARG = 1,
     JETLONG_UNSUPPORTED = 2,
-    JETLONG_CUDA_ERROR = 3
+    JETLONG_CUDA_ERROR = 3,
+    JETLONG_SCRATCH_EXCEEDED = 4     /* jetlong_decode_static only: the call needs more than JETLONG_STATIC_SCRATCH_BYTES */
 } jetlong_status;
 
 enum { JETLONG_BF16 = 0, JETLONG_FP32 = 1 };
@@ -135,6 +136,31 @@ int jetlong_decode_paged(const void* q, const void* Kpool, const void* Vpool, co
                          void* out, float* lse, int H_q, int H_kv, int head_dim,
                          int64_t w_local, int64_t w_pretrained, double rope_theta,
                          int dtype, void* workspace, size_t workspace_bytes, void* stream);
+
+/* Allocation-free decode.  The same operation and kernels as jetlong_decode (default options), for callers that cannot
+ * allocate device memory: code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc.  There is no
+ * workspace argument: the rotation tables and the split partials live in ONE file-scope device array of
+ * JETLONG_STATIC_SCRATCH_BYTES bytes inside the library (every GPU that loads the library holds these 8 MiB until the process
+ * exits).  The entry point calls no cudaMalloc / cudaFree and no allocating library routine; the caller still passes q, the
+ * cache, out and lse (device pointers, as for jetlong_decode).
+ *   - Limit: jetlong_workspace_bytes(JETLONG_OP_DECODE, L, ...) <= JETLONG_STATIC_SCRATCH_BYTES, else
+ *     JETLONG_SCRATCH_EXCEEDED and nothing is launched.  8 MiB cover L up to 1.5 M rows at H_q / H_kv = 32 / 8, d = 128
+ *     (4.5 MB at L = 65536, 5.3 MB at 131072, 7.1 MB at 1 M: the partials of up to 2 x SMs splits, 520 B per
+ *     (split, query head), and the tables at 512 B per 256 rows).
+ *   - The array is shared by every call on the device and keeps the last call's contents.  Nothing in it has to start at
+ *     zero per call: the table header is re-validated (parameters and a hash of the table body) and rebuilt when it does
+ *     not fit the call, the partials are rewritten in full before they are read.
+ *   - Calls that overlap on the GPU (two streams, two host threads on one device) RACE on the array: serialise them, or use
+ *     jetlong_decode with one workspace per stream.
+ * jetlong_decode_static_init() resolves the array's device address for the CURRENT device (cudaGetSymbolAddress, once per
+ * device; JETLONG_CUDA_ERROR if that fails).  jetlong_decode_static does the same on its first call on a device; call the
+ * init yourself before a stream capture starts, because the first use of the library on a device loads its module. */
+#define JETLONG_STATIC_SCRATCH_BYTES (8u << 20)
+int jetlong_decode_static_init(void);
+int jetlong_decode_static(const void* q, const void* Kcache, const void* Vcache, void* out, float* lse,
+                          int64_t L, int H_q, int H_kv, int head_dim,
+                          int64_t w_local, int64_t w_pretrained, double rope_theta,
+                          int dtype, void* stream);
 
 /* Matched control ("without bifocal attention"): plain causal attention on the given
  * (already RoPE'd) Q, K with the same kernels, no classifier and no rotation. */

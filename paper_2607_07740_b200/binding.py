@@ -24,7 +24,8 @@ EXPORTS = ["jetlong_group_size", "jetlong_workspace_bytes", "jetlong_prefill", "
            "jetlong_launch_count", "jetlong_set_prefill_impl", "jetlong_prefill_uses_umma",
            "jetlong_set_prefill_precision", "jetlong_prefill_prerotated", "jetlong_prefill_unfused",
            "jetlong_prefill_opt", "jetlong_prefill_prerotated_opt", "jetlong_host_release", "jetlong_decode_opt",
-           "jetlong_decode_paged", "jetlong_decode_paged_workspace_bytes"]
+           "jetlong_decode_paged", "jetlong_decode_paged_workspace_bytes", "jetlong_decode_static",
+           "jetlong_decode_static_init"]
 DEFAULT = -2                                              # JETLONG_DEFAULT: take the calling thread's default
 
 
@@ -85,6 +86,10 @@ def lib():
         L.jetlong_decode_opt.argtypes = [vp] * 5 + tail + [vp]
         L.jetlong_decode.restype = i32
         L.jetlong_decode.argtypes = [vp] * 5 + tail
+        L.jetlong_decode_static.restype = i32
+        L.jetlong_decode_static.argtypes = [vp] * 5 + [i64, i32, i32, i32, i64, i64, dbl, i32, vp]
+        L.jetlong_decode_static_init.restype = i32
+        L.jetlong_decode_static_init.argtypes = []
         ctail = [i64, i32, i32, i32, i32, vp, sz, vp]
         L.jetlong_causal_prefill.restype = i32
         L.jetlong_causal_prefill.argtypes = [vp] * 5 + ctail
@@ -234,6 +239,24 @@ def jetlong_decode(q, Kcache, Vcache, L, *, w_local, w_pretrained, rope_theta, o
                                     int(L), H_q, H_kv, d, int(w_local), int(w_pretrained), float(rope_theta), dt,
                                     workspace.data_ptr(), workspace.numel(), _stream(),
                                     _options(remote_map=remote_map, yarn=yarn)))
+    return out, lse
+
+
+STATIC_SCRATCH_BYTES = 8 << 20
+
+
+def jetlong_decode_static_init():
+    """Resolve the device address of the library's static scratch for the current device (optional; see jetlong.h)."""
+    _check(lib().jetlong_decode_static_init())
+
+
+def jetlong_decode_static(q, Kcache, Vcache, L, *, w_local, w_pretrained, rope_theta, out, lse):
+    """jetlong_decode without any allocation: no workspace argument (the scratch is a static device array inside the
+    library, at most STATIC_SCRATCH_BYTES), and `out` / `lse` must be given.  Calls that overlap on the GPU race."""
+    H_q, H_kv, d, out, lse = _decode_args(q, Kcache, Vcache, L, out, lse)
+    _check(lib().jetlong_decode_static(q.data_ptr(), Kcache.data_ptr(), Vcache.data_ptr(), out.data_ptr(), lse.data_ptr(),
+                                       int(L), H_q, H_kv, d, int(w_local), int(w_pretrained), float(rope_theta), _dt(q),
+                                       _stream()))
     return out, lse
 
 

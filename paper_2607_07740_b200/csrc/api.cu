@@ -278,6 +278,57 @@ int jetlong_decode_paged(const void* q, const void* Kpool, const void* Vpool, co
                                lse, H_q, H_kv, w_local, rope_theta, workspace, (cudaStream_t)stream);
 }
 
+// ---- allocation-free decode (include/jetlong.h) --------------------------------------------------------------------
+// The scratch of jetlong_decode_static.  In host code this name is only a handle for the runtime, NOT a device address:
+// the address comes from cudaGetSymbolAddress, once per device, with that device current.
+static __device__ __align__(256) unsigned char g_static_scratch[JETLONG_STATIC_SCRATCH_BYTES];
+static void* g_static_ptr[64];
+static std::mutex g_static_mu;
+
+static int static_scratch(void** ws) {
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess && (dev < 0 || dev >= 64)) e = cudaErrorInvalidDevice;
+    if (e == cudaSuccess) {
+        std::lock_guard<std::mutex> lock(g_static_mu);
+        if (!g_static_ptr[dev]) {
+            void* ptr = nullptr;
+            e = cudaGetSymbolAddress(&ptr, g_static_scratch);
+            if (e == cudaSuccess && !ptr) e = cudaErrorInvalidSymbol;
+            if (e == cudaSuccess) g_static_ptr[dev] = ptr;
+        }
+        *ws = g_static_ptr[dev];
+    }
+    if (e != cudaSuccess) {
+        snprintf(g_err, sizeof(g_err), "jetlong_decode_static: address of the static scratch: %s", cudaGetErrorString(e));
+        cudaGetLastError();
+        return JETLONG_CUDA_ERROR;
+    }
+    return JETLONG_OK;
+}
+
+int jetlong_decode_static_init(void) {
+    int rc = device_ok();
+    if (rc != JETLONG_OK) return rc;
+    void* ws = nullptr;
+    return static_scratch(&ws);
+}
+
+int jetlong_decode_static(const void* q, const void* Kcache, const void* Vcache, void* out, float* lse, int64_t L, int H_q,
+                          int H_kv, int head_dim, int64_t w_local, int64_t w_pretrained, double rope_theta, int dtype,
+                          void* stream) {
+    int rc = validate(q, Kcache, Vcache, out, lse, L, H_q, H_kv, head_dim, w_local, w_pretrained, rope_theta, dtype);
+    if (rc != JETLONG_OK) return rc;
+    if (decode_workspace_bytes(L, H_q, H_kv, head_dim) > (size_t)JETLONG_STATIC_SCRATCH_BYTES) return JETLONG_SCRATCH_EXCEEDED;
+    rc = device_ok();
+    if (rc != JETLONG_OK) return rc;
+    void* ws = nullptr;
+    rc = static_scratch(&ws);
+    if (rc != JETLONG_OK) return rc;
+    return decode_common(q, Kcache, Vcache, out, lse, L, H_q, H_kv, head_dim, w_local, w_pretrained, rope_theta, dtype, ws,
+                         (size_t)JETLONG_STATIC_SCRATCH_BYTES, stream, true);
+}
+
 int jetlong_causal_decode(const void* q, const void* Kcache, const void* Vcache, void* out, float* lse, int64_t L,
                           int H_q, int H_kv, int head_dim, int dtype, void* workspace, size_t workspace_bytes,
                           void* stream) {
@@ -396,6 +447,9 @@ const char* jetlong_status_string(int status) {
         case JETLONG_INVALID_ARG: return "invalid argument";
         case JETLONG_UNSUPPORTED: return "unsupported device or configuration (needs compute capability 10.0, sm_100a)";
         case JETLONG_CUDA_ERROR: return g_err;
+        case JETLONG_SCRATCH_EXCEEDED:
+            return "the call needs more scratch than the library's static array holds (JETLONG_STATIC_SCRATCH_BYTES = 8 MiB): "
+                   "use jetlong_decode with a caller-provided workspace";
         default: return "unknown status";
     }
 }
