@@ -122,6 +122,14 @@ constexpr uint32_t IDESC_S_BF16 = idesc_f16(1, 1, 0, 0, BN, NH);
 constexpr uint32_t IDESC_S_F16 = idesc_f16(0, 0, 0, 0, BN, NH);
 constexpr uint32_t IDESC_S_F16_N32 = idesc_f16(0, 0, 0, 0, BN, 2 * NH);
 constexpr uint32_t IDESC_S_E5M2 = idesc_f16(1, 1, 0, 0, BN, NH);  // kind::f8f6f4: format code 1 = e5m2
+// Bifocal scan: when the producer issues the load of tile v it also asks the TMA unit to fetch tile v + 1 into L2
+// (cp.async.bulk.prefetch.tensor).  A K stage is busy from the issue of its load until the MMAs on the ROTATED tile have
+// completed; with three stages and ~3.5 us of load latency under full HBM load that life (latency + rotation) set the
+// period per tile.  The prefetched tile's load is an L2 hit, the stage turns over sooner.  Measured at 64K: 55.1 -> 51.6 us
+// (distance 1), 53.1 (2), 54.2 (3), 59.7 (4), 65.7 (5); K only 51.6, V only 53.9.  The control does not need it and loses
+// with it (45.1 -> 51.0 us at distance 3: more requests in flight than DRAM serves in order), so it is off there.
+constexpr int PFK = 1, PFV = 1;
+constexpr int RO = 1;                                // SPLIT: rows per thread on the odd rotate warps (the even ones take 4 - RO)
 constexpr int SB = 8;                                // rows (heads) per block of the slow pairs' operand: SPLIT serves g <= 8
 constexpr uint32_t IDESC_S_BF16_N48 = idesc_f16(1, 1, 0, 0, BN, 6 * SB);
 constexpr uint32_t IDESC_PV = idesc_f16(1, 1, 1, 0, D, NH);      // A = V^T (smem, MN-major), B = P (smem, K-major)
@@ -238,7 +246,7 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
         if (p.split) {
             const int e = (rt >> 6) * 8 + ((rt & 31) >> 2);
             
-            rot.init_at(p.lo, p.hi, rt & 3, (rt & 32) ? 96 + e : 3 * e, p.G);
+            rot.init_at(p.lo, p.hi, rt & 3, (rt & 32) ? 32 * (4 - RO) + RO * e : (4 - RO) * e, p.G);
         }
         else rot.init(p.lo, p.hi, rt, p.G);
         rot.seek((unsigned)(plan.kt(0) * BN));
@@ -308,6 +316,10 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
                 mbar_arrive_expect_tx(&bars->k_full[s], TILE);
                 tma_load_3d(sK(s), &tmK, &bars->k_full[s], 0, kvh, row0);
                 tma_load_3d(sK(s) + BOXB, &tmK, &bars->k_full[s], 64, kvh, row0);
+                if (PFK > 0 && p.bifocal && !pages && v + PFK < plan.nv) {      // tile v + PF into L2: its load will be an L2 hit
+                    tma_prefetch_3d(&tmK, 0, kvh, plan.kt(v + PFK) * BN);
+                    tma_prefetch_3d(&tmK, 64, kvh, plan.kt(v + PFK) * BN);
+                }
             }
         }
     } else if (warp == 2) {
@@ -323,6 +335,10 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
                 mbar_arrive_expect_tx(&bars->v_full[sv], TILE);
                 tma_load_3d(sV(sv), &tmV, &bars->v_full[sv], 0, kvh, row0);
                 tma_load_3d(sV(sv) + BOXB, &tmV, &bars->v_full[sv], 64, kvh, row0);
+                if (PFV > 0 && p.bifocal && !pages && v + PFV < plan.nv) {
+                    tma_prefetch_3d(&tmV, 0, kvh, plan.kt(v + PFV) * BN);
+                    tma_prefetch_3d(&tmV, 64, kvh, plan.kt(v + PFV) * BN);
+                }
             }
         }
     } else if (warp == 1) {
@@ -470,45 +486,50 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
         const uint32_t sb0 = (uint32_t)((si < 48 ? 32 : 96) + (si & 15) * 2);     // byte of channel i in its operand row
         for (int v = 0; v < plan.nv; ++v) {
             const int s = v % KS;
-            mbar_wait(&bars->k_full[s], (v / KS) & 1);
-            if (plan.remote(v) && p.split) {
+            if (slow && plan.remote(v)) {
+                // The slow pairs' operand of tile v does not depend on the tile: it is written while the tile is still in flight.
+                // Its bytes are free once the MMAs of the stage's previous tile have completed (k_empty, the barrier the K
+                // producer waited on before it issued this tile's load).
                 const uint32_t kl = smem_u32(sK(s)) + TILE;
-                if (t & 32) rotate_rows2<1, BOXB, 3, true, true>(smem_u32(sK(s)), kl, (unsigned)(plan.kt(v) * BN), rot, SelTree(), 0u, 0u);
-                else rotate_rows2<3, BOXB, 3, true, true>(smem_u32(sK(s)), kl, (unsigned)(plan.kt(v) * BN), rot, SelTree(), 0u, 0u);
-                if (slow) {
-                    const float c = rc, sn = rs;                                 // cs(alpha_ref) of pair i
-                    {
-                        g_ph += g_m;
-                        const bool wrap = g_ph >= gG;                            // one more multiple of G passed: n_ref advances by D0
-                        if (wrap) g_ph -= gG;
-                        const float2 e = (wrap || g_m == 0u) ? s_e0 : s_e1;
-                        rc = c * e.x - sn * e.y; rs = sn * e.x + c * e.y;
-                    }
+                if (v >= KS) mbar_wait(&bars->k_empty[s], ((v / KS) - 1) & 1);
+                const float c = rc, sn = rs;                                 // cs(alpha_ref) of pair i
+                {
+                    g_ph += g_m;
+                    const bool wrap = g_ph >= gG;                            // one more multiple of G passed: n_ref advances by D0
+                    if (wrap) g_ph -= gG;
+                    const float2 e = (wrap || g_m == 0u) ? s_e0 : s_e1;
+                    rc = c * e.x - sn * e.y; rs = sn * e.x + c * e.y;
+                }
 #pragma unroll
-                    for (int it = 0; it < NI; ++it) {
-                        const int h = (t >> 6) + 4 * it;
-                        if (h < p.g) {
-                            const float q1 = c * qy1[it] + sn * qy2[it], q2 = c * qy2[it] - sn * qy1[it];   // qt = Rot(alpha_ref)^T q'
-                            const uint16_t h1 = bf16_bits(q1), h2 = bf16_bits(q2);
-                            const float r1 = q1 - __uint_as_float((uint32_t)h1 << 16), r2 = q2 - __uint_as_float((uint32_t)h2 << 16);
-                            const float u1 = ua * q2, u2 = -ua * q1;                     // a J^T qt: hi and lo as well -- its bf16
-                            const uint16_t g1 = bf16_bits(u1), g2 = bf16_bits(u2);       // rounding alone is 64 theta_i 2^-9 of a full-size term
-                            const float v1 = u1 - __uint_as_float((uint32_t)g1 << 16), v2 = u2 - __uint_as_float((uint32_t)g2 << 16);
-                            // blocks 0, 2, 3, 4, 5: column 16 + h is where the fast pairs put their Q'lo term, which like qt lo
-                            // is not multiplied by dn; block 1 (columns 8-15) is never written and never read
-                            const uint16_t w1[5] = {h1, bf16_bits(r1), g1, bf16_bits(v1), bf16_bits(ub * q1)};     // channel i
-                            const uint16_t w2[5] = {h2, bf16_bits(r2), g2, bf16_bits(v2), bf16_bits(ub * q2)};     // channel i + 64
-                            // row 8 b + h of the operand: the swizzle term depends on h only (8 rows = one swizzle period)
-                            const uint32_t a = kl + (uint32_t)h * 128 + ((((sb0 >> 4) ^ ((uint32_t)h & 7u)) << 4) | (sb0 & 15u));
+                for (int it = 0; it < NI; ++it) {
+                    const int h = (t >> 6) + 4 * it;
+                    if (h < p.g) {
+                        const float q1 = c * qy1[it] + sn * qy2[it], q2 = c * qy2[it] - sn * qy1[it];   // qt = Rot(alpha_ref)^T q'
+                        const uint16_t h1 = bf16_bits(q1), h2 = bf16_bits(q2);
+                        const float r1 = q1 - __uint_as_float((uint32_t)h1 << 16), r2 = q2 - __uint_as_float((uint32_t)h2 << 16);
+                        const float u1 = ua * q2, u2 = -ua * q1;                     // a J^T qt: hi and lo as well -- its bf16
+                        const uint16_t g1 = bf16_bits(u1), g2 = bf16_bits(u2);       // rounding alone is 64 theta_i 2^-9 of a full-size term
+                        const float v1 = u1 - __uint_as_float((uint32_t)g1 << 16), v2 = u2 - __uint_as_float((uint32_t)g2 << 16);
+                        // blocks 0, 2, 3, 4, 5: column 16 + h is where the fast pairs put their Q'lo term, which like qt lo
+                        // is not multiplied by dn; block 1 (columns 8-15) is never written and never read
+                        const uint16_t w1[5] = {h1, bf16_bits(r1), g1, bf16_bits(v1), bf16_bits(ub * q1)};     // channel i
+                        const uint16_t w2[5] = {h2, bf16_bits(r2), g2, bf16_bits(v2), bf16_bits(ub * q2)};     // channel i + 64
+                        // row 8 b + h of the operand: the swizzle term depends on h only (8 rows = one swizzle period)
+                        const uint32_t a = kl + (uint32_t)h * 128 + ((((sb0 >> 4) ^ ((uint32_t)h & 7u)) << 4) | (sb0 & 15u));
 #pragma unroll
-                            for (int b = 0; b < 5; ++b) {
-                                const int blk = b == 0 ? 0 : b + 1;
-                                sts16(a + blk * SB * 128, w1[b]);
-                                sts16(a + blk * SB * 128 + 64 * 128, w2[b]);
-                            }
+                        for (int b = 0; b < 5; ++b) {
+                            const int blk = b == 0 ? 0 : b + 1;
+                            sts16(a + blk * SB * 128, w1[b]);
+                            sts16(a + blk * SB * 128 + 64 * 128, w2[b]);
                         }
                     }
                 }
+            }
+            mbar_wait(&bars->k_full[s], (v / KS) & 1);
+            if (plan.remote(v) && p.split) {
+                const uint32_t kl = smem_u32(sK(s)) + TILE;
+                if (t & 32) rotate_rows2<RO, BOXB, 3, true, true>(smem_u32(sK(s)), kl, (unsigned)(plan.kt(v) * BN), rot, SelTree(), 0u, 0u);
+                else rotate_rows2<4 - RO, BOXB, 3, true, true>(smem_u32(sK(s)), kl, (unsigned)(plan.kt(v) * BN), rot, SelTree(), 0u, 0u);
                 fence_proxy_async_smem();
                 if (plan.remote(v + 1)) { rot.step128(g_m, g_d); rot.prefetch_carried(); }
             } else if (plan.remote(v)) {
@@ -533,6 +554,11 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
         for (int v = 0; v < plan.nv; ++v) {
             const long long key = (long long)plan.kt(v) * BN + j;
             const bool valid = plan.remote(v) ? (key >= plan.ks && key < plan.re) : (key >= plan.ls && key < plan.ke);
+            float dn = 0.f;                                           // SPLIT: n(key) - n(reference row), ahead of the wait for S
+            if (p.split && plan.remote(v)) {
+                const unsigned pk = (unsigned)key, pr = (unsigned)(plan.kt(v) * BN) + 64u, Gu = (unsigned)p.G;
+                dn = (float)((int)(pk - pk / Gu) - (int)(pr - pr / Gu));
+            }
             mbar_wait(&bars->s_full[v & 1], (v >> 1) & 1);
             tc_fence_after();
             uint32_t sr[32];
@@ -545,8 +571,6 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
                 uint32_t st[16];                                       // columns 32-47: a J^T qt lo | -a^2/2 qt
                 tmem_ld16(tmem + lane_base + TM_S + (v & 1) * SCOLS + 2 * NH, st);
                 tmem_ld_wait();
-                const unsigned pk = (unsigned)key, pr = (unsigned)(plan.kt(v) * BN) + 64u, Gu = (unsigned)p.G;
-                const float dn = (float)((int)(pk - pk / Gu) - (int)(pr - pr / Gu));
 #pragma unroll
                 for (int h = 0; h < NG && h < SB; ++h)
                     tay[h] = dn * ((__uint_as_float(sr[3 * SB + h]) + __uint_as_float(st[h])) + dn * __uint_as_float(st[SB + h]));

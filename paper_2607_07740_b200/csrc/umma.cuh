@@ -79,6 +79,11 @@ __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* m, uin
         ::"r"(smem_u32(dst)), "l"(reinterpret_cast<uint64_t>(m)), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2)
         : "memory");
 }
+// the same box fetched into L2 only (no shared-memory destination, no barrier): a later tma_load_3d of it is an L2 hit
+__device__ __forceinline__ void tma_prefetch_3d(const CUtensorMap* m, int c0, int c1, int c2) {
+    asm volatile("cp.async.bulk.prefetch.tensor.3d.L2.global.tile [%0, {%1, %2, %3}];"
+                 ::"l"(reinterpret_cast<uint64_t>(m)), "r"(c0), "r"(c1), "r"(c2) : "memory");
+}
 
 // ---- TMEM ---------------------------------------------------------------------------------------------
 template <int COLS> __device__ __forceinline__ void tmem_alloc(uint32_t* dst_smem) {   // one full warp
