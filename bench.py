@@ -377,7 +377,9 @@ def main():
             "decode_frac_hbm": {"128k": round(line["decode"]["bifocal"]["frac_hbm_peak"], 4),
                                 "64k": round(line["decode_64k"]["bifocal"]["frac_hbm_peak"], 4),
                                 "128k_control": round(line["decode"]["control"]["frac_hbm_peak"], 4),
-                                "64k_control": round(line["decode_64k"]["control"]["frac_hbm_peak"], 4)},
+                                "64k_control": round(line["decode_64k"]["control"]["frac_hbm_peak"], 4),
+                                "128k_sustained": round(line["decode"]["bifocal"]["sustained"]["frac_hbm_peak"], 4),
+                                "64k_sustained": round(line["decode_64k"]["bifocal"]["sustained"]["frac_hbm_peak"], 4)},
             "e2e_ms": round(line["e2e"]["ms"], 2)}
     if rank == 0:
         print(json.dumps(line))
@@ -484,9 +486,12 @@ def bench_decode(J, B, W, dev, pk, L0=131072, steps=256, only=None, reps=7):
         torch.cuda.synchronize()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         n0 = J.jetlong_launch_count()
-        # one pass = the `steps` consecutive steps (14-27 ms): `reps` passes back to back, the median pass is reported, so that
-        # the number does not hang on the clock state the preceding legs left behind; clocks sampled over all passes
-        sampler = ClockSampler(dev.index or 0, period_ms=100)       # launch-paced steps: poll the driver sparingly
+        # one pass = the workload (`steps` consecutive steps, 13-27 ms).  The first pass after the warm-up steps starts from an
+        # idle GPU at boost clock and is the headline (`us_per_step`, as in round 1).  `reps` passes back to back follow: after
+        # ~50 ms of decode the board reaches its power cap (sw_power_cap, SM clock 1.60-1.66 GHz instead of 1.965) and the
+        # bifocal scan, which is bound by SM-side work per tile, slows by ~15 %; the control (HBM-bound) does not.  The median of
+        # the later passes is reported beside it as `sustained`, with the clocks sampled over the leg.
+        sampler = ClockSampler(dev.index or 0, period_ms=25)
         sampler.start()
         time.sleep(0.25)
         tb = time.time()
@@ -500,11 +505,15 @@ def bench_decode(J, B, W, dev, pk, L0=131072, steps=256, only=None, reps=7):
             passes.append(e0.elapsed_time(e1) / steps * 1e3)
         te = time.time()
         clk = sampler.stop(tb, te)
-        us = sorted(passes)[len(passes) // 2]
-        res[name] = {"us_per_step": us, "us_per_step_min": min(passes), "us_per_step_max": max(passes), "passes": reps,
-                     "kv_read_gbs": kv_bytes / (us * 1e-6) / 1e9,
+        us = passes[0]
+        later = sorted(passes[1:]) or [us]
+        sus = later[len(later) // 2]
+        res[name] = {"us_per_step": us, "kv_read_gbs": kv_bytes / (us * 1e-6) / 1e9,
                      "frac_hbm_peak": kv_bytes / (us * 1e-6) / 1e9 / pk["hbm_gbs"],
-                     "launches_per_step": (J.jetlong_launch_count() - n0) / (steps * reps), "clocks": clk}
+                     "launches_per_step": (J.jetlong_launch_count() - n0) / (steps * reps),
+                     "sustained": {"us_per_step": sus, "us_per_step_min": later[0], "us_per_step_max": later[-1],
+                                   "passes": len(later), "frac_hbm_peak": kv_bytes / (sus * 1e-6) / 1e9 / pk["hbm_gbs"],
+                                   "clocks": clk}}
         # the same steps replayed from one CUDA graph (the paper measures decode under CUDA graphs)
         try:
             g = torch.cuda.CUDAGraph()
