@@ -360,6 +360,7 @@ def main():
         line["decode"] = bench_decode(J, B, W, dev, pk, L0=131072, steps=256)
         line["decode"]["idle_before_s"] = 1.5
         line["decode_64k"] = bench_decode(J, B, W, dev, pk, L0=65536, steps=256)
+        line["decode_paged"] = bench_decode_paged(J, B, W, dev, pk)
         # ---- the CPU oracle on a bounded sample ---------------------------------------------------------
         cb = oracle_sample(cfg, 3072, Q, K, V)
         cb.pop("seconds")
@@ -379,7 +380,8 @@ def main():
                                 "128k_control": round(line["decode"]["control"]["frac_hbm_peak"], 4),
                                 "64k_control": round(line["decode_64k"]["control"]["frac_hbm_peak"], 4),
                                 "128k_sustained": round(line["decode"]["bifocal"]["sustained"]["frac_hbm_peak"], 4),
-                                "64k_sustained": round(line["decode_64k"]["bifocal"]["sustained"]["frac_hbm_peak"], 4)},
+                                "64k_sustained": round(line["decode_64k"]["bifocal"]["sustained"]["frac_hbm_peak"], 4),
+                                "paged_batch8": round(line["decode_paged"]["frac_hbm_peak"], 4)},
             "e2e_ms": round(line["e2e"]["ms"], 2)}
     if rank == 0:
         print(json.dumps(line))
@@ -459,6 +461,59 @@ def _umma_active(B, cfg):
         return bool(B.lib().jetlong_prefill_uses_umma(cfg.L, cfg.H_q, cfg.H_kv, cfg.d))
     except AttributeError:
         return False
+
+
+def bench_decode_paged(J, B, W, dev, pk, n_seq=8, L0=65536, steps=20, reps=5):
+    """one decode step of `n_seq` sequences of different lengths (L0 + 1111 b, G = 3 at the config-5 shape) over a
+    shuffled pool of 128-row pages, one call of jetlong_decode_paged per step.  Seeded N(0,1) cache rows (the timing does not
+    depend on the values); KV bytes = sum over sequences of 2 L_b H_kv d 2 B."""
+    c = W.C5
+    lens = [L0 + 1111 * b for b in range(n_seq)]
+    max_pages = (max(lens) + 127) // 128
+    n_pages = sum((x + 127) // 128 for x in lens) + 3
+    gen = torch.Generator(device="cpu")
+    gen.manual_seed(77400)
+    perm = torch.randperm(n_pages, generator=gen)
+    gd = torch.Generator(device=dev)
+    gd.manual_seed(77401)
+    Kpool = torch.randn((n_pages * 128, c.H_kv, c.d), device=dev, dtype=torch.float32, generator=gd).to(torch.bfloat16)
+    Vpool = torch.randn((n_pages * 128, c.H_kv, c.d), device=dev, dtype=torch.float32, generator=gd).to(torch.bfloat16)
+    q = torch.randn((n_seq, c.H_q, c.d), device=dev, dtype=torch.float32, generator=gd).to(torch.bfloat16)
+    pt = torch.zeros((n_seq, max_pages), dtype=torch.int32)
+    nxt = 0
+    for b, L in enumerate(lens):
+        npg = (L + 127) // 128
+        pt[b, :npg] = perm[nxt:nxt + npg].to(torch.int32)
+        nxt += npg
+    ptd = pt.to(dev)
+    n = int(B.lib().jetlong_decode_paged_workspace_bytes(max(lens), n_seq, c.H_q, c.H_kv, c.d))
+    ws = torch.zeros(max(n, 256), dtype=torch.uint8, device=dev)
+    out = torch.empty_like(q)
+    lse = torch.empty((n_seq, c.H_q), dtype=torch.float32, device=dev)
+
+    def run():
+        J.jetlong_decode_paged(q, Kpool, Vpool, ptd, lens, w_local=c.w_local, w_pretrained=c.w_pretrained,
+                               rope_theta=c.rope_theta, out=out, lse=lse, workspace=ws)
+    for _ in range(3):
+        run()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ts = []
+    for _ in range(reps):
+        e0.record()
+        for _ in range(steps):
+            run()
+        e1.record()
+        torch.cuda.synchronize()
+        ts.append(e0.elapsed_time(e1) / steps * 1e3)
+    kv = sum(2.0 * L * c.H_kv * c.d * 2 for L in lens)
+    us = ts[0]
+    med = sorted(ts)[len(ts) // 2]
+    return {"us_per_step": us, "kv_read_gbs": kv / (us * 1e-6) / 1e9, "frac_hbm_peak": kv / (us * 1e-6) / 1e9 / pk["hbm_gbs"],
+            "sustained": {"us_per_step": med, "frac_hbm_peak": kv / (med * 1e-6) / 1e9 / pk["hbm_gbs"], "passes": reps},
+            "workload": "%d sequences of %d..%d cached tokens (G = %d), config-5 head layout, shuffled pool of %d pages of 128 rows; "
+                        "%d steps per pass" % (n_seq, lens[0], lens[-1], J.jetlong_group_size(lens[0], c.w_pretrained), n_pages, steps),
+            "algorithmic_bytes_per_step": kv}
 
 
 def bench_decode(J, B, W, dev, pk, L0=131072, steps=256, only=None, reps=7):

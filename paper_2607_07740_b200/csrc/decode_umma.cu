@@ -129,6 +129,7 @@ constexpr uint32_t IDESC_S_E5M2 = idesc_f16(1, 1, 0, 0, BN, NH);  // kind::f8f6f
 // (distance 1), 53.1 (2), 54.2 (3), 59.7 (4), 65.7 (5); K only 51.6, V only 53.9.  The control does not need it and loses
 // with it (45.1 -> 51.0 us at distance 3: more requests in flight than DRAM serves in order), so it is off there.
 constexpr int PFK = 1, PFV = 1;
+static_assert(PFK <= 1 && PFV <= 1, "the paged producers know the page of tile v + 1 only");
 constexpr int RO = 1;                                // SPLIT: rows per thread on the odd rotate warps (the even ones take 4 - RO)
 constexpr int SB = 8;                                // rows (heads) per block of the slow pairs' operand: SPLIT serves g <= 8
 constexpr uint32_t IDESC_S_BF16_N48 = idesc_f16(1, 1, 0, 0, BN, 6 * SB);
@@ -316,9 +317,10 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
                 mbar_arrive_expect_tx(&bars->k_full[s], TILE);
                 tma_load_3d(sK(s), &tmK, &bars->k_full[s], 0, kvh, row0);
                 tma_load_3d(sK(s) + BOXB, &tmK, &bars->k_full[s], 64, kvh, row0);
-                if (PFK > 0 && p.bifocal && !pages && v + PFK < plan.nv) {      // tile v + PF into L2: its load will be an L2 hit
-                    tma_prefetch_3d(&tmK, 0, kvh, plan.kt(v + PFK) * BN);
-                    tma_prefetch_3d(&tmK, 64, kvh, plan.kt(v + PFK) * BN);
+                if (PFK > 0 && p.bifocal && v + PFK < plan.nv) {                // tile v + 1 into L2: its load will be an L2 hit
+                    const int row1 = (pages ? pg_next : plan.kt(v + PFK)) * BN;
+                    tma_prefetch_3d(&tmK, 0, kvh, row1);
+                    tma_prefetch_3d(&tmK, 64, kvh, row1);
                 }
             }
         }
@@ -335,9 +337,10 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
                 mbar_arrive_expect_tx(&bars->v_full[sv], TILE);
                 tma_load_3d(sV(sv), &tmV, &bars->v_full[sv], 0, kvh, row0);
                 tma_load_3d(sV(sv) + BOXB, &tmV, &bars->v_full[sv], 64, kvh, row0);
-                if (PFV > 0 && p.bifocal && !pages && v + PFV < plan.nv) {
-                    tma_prefetch_3d(&tmV, 0, kvh, plan.kt(v + PFV) * BN);
-                    tma_prefetch_3d(&tmV, 64, kvh, plan.kt(v + PFV) * BN);
+                if (PFV > 0 && p.bifocal && v + PFV < plan.nv) {
+                    const int row1 = (pages ? pg_next : plan.kt(v + PFV)) * BN;
+                    tma_prefetch_3d(&tmV, 0, kvh, row1);
+                    tma_prefetch_3d(&tmV, 64, kvh, row1);
                 }
             }
         }
