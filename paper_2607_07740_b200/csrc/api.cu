@@ -61,6 +61,7 @@ int launch_prefill_umma(const void* Q, const void* K, const void* V, void* out, 
 
 // decode.cu / decode_umma.cu
 bool umma_decode_supported(int H_q, int H_kv, int d, int dtype);
+bool umma_decode_paged_supported(int H_q, int H_kv, int d, int dtype);
 size_t decode_paged_workspace_bytes(long long Lmax, int batch, int H_q, int H_kv, int d);
 int launch_decode_paged(const void* q, const void* Kpool, const void* Vpool, const int* page_table, int max_pages,
                         long long pool_pages, const long long* Ls, const long long* Gs, int batch, void* out, float* lse,
@@ -269,7 +270,7 @@ int jetlong_decode_paged(const void* q, const void* Kpool, const void* Vpool, co
         Gs[b] = jetlong_group_size(seq_lens[b], w_pretrained);       // Eq.(2) per sequence, on the host
         if (Ls[b] > Lmax) Lmax = Ls[b];
     }
-    if (!umma_decode_supported(H_q, H_kv, head_dim, dtype)) return JETLONG_UNSUPPORTED;
+    if (!umma_decode_paged_supported(H_q, H_kv, head_dim, dtype)) return JETLONG_UNSUPPORTED;
     const size_t need = decode_paged_workspace_bytes(Lmax, batch, H_q, H_kv, head_dim);
     if (!workspace || workspace_bytes < need || !aligned16(workspace)) return JETLONG_INVALID_ARG;
     rc = device_ok();

@@ -65,7 +65,8 @@ struct Params {
     const __nv_bfloat16* q;
     float* part;                                     // [nsplit][H_q][D+2]
     long long L, w0, G, kps;                         // kps = keys per split, a multiple of BN
-    int H_q, H_kv, g, bifocal;
+    int H_q, H_kv, g, bifocal;                      // g = query heads per KV head served by THIS launch (<= 16)
+    int gq, h0;                                      // heads per KV head in q / the partials, first head of this launch in its group
     const float2* lo;
     const float2* hi;
     double theta;                                    // for the table-header check (see the prologue)
@@ -258,7 +259,7 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
         for (int it = 0; it < NI; ++it) {
             const int idx = rt + it * RT;
             if (idx < p.g * 64) {
-                const __nv_bfloat16* qh = p.q + (size_t)(kvh * p.g + (idx >> 6)) * D;
+                const __nv_bfloat16* qh = p.q + (size_t)(kvh * p.gq + p.h0 + (idx >> 6)) * D;
                 qv1[it] = qh[idx & 63];
                 qv2[it] = qh[(idx & 63) + 64];
             }
@@ -669,7 +670,7 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
 #pragma unroll
         for (int h = 0; h < NG; ++h) {
             if (h < g) {
-                float* dst = p.part + ((size_t)split * p.H_q + (size_t)kvh * g + h) * SS;
+                float* dst = p.part + ((size_t)split * p.H_q + (size_t)kvh * p.gq + p.h0 + h) * SS;
                 dst[j] = __uint_as_float(og[h]);
                 if (j == 0) {
                     dst[D] = m_ref[h];
@@ -692,8 +693,10 @@ static int split_ok(double theta, const FreqMap& fm, int g) {
 }
 
 bool umma_decode_supported(int H_q, int H_kv, int d, int dtype) {
-    if (dtype != JETLONG_BF16 || d != 128 || H_kv < 1 || H_q % H_kv) return false;
-    return H_q / H_kv <= NH;
+    return dtype == JETLONG_BF16 && d == 128 && H_kv >= 1 && H_q % H_kv == 0;     // any group size: 16 heads per launch
+}
+bool umma_decode_paged_supported(int H_q, int H_kv, int d, int dtype) {
+    return umma_decode_supported(H_q, H_kv, d, dtype) && H_q / H_kv <= NH;
 }
 
 // split plan: one CTA per SM (the kernel needs ~215 KB of shared memory), key ranges are multiples of the 128-key tile
@@ -719,29 +722,36 @@ int launch_decode_umma(const void* q, const void* K, const void* V, float* part,
     p.L = L; p.w0 = w0; p.G = G;
     int ns;
     umma_decode_plan(L, H_kv, &ns, &p.kps);
-    p.H_q = H_q; p.H_kv = H_kv; p.g = H_q / H_kv;
+    p.H_q = H_q; p.H_kv = H_kv; p.gq = H_q / H_kv;
     p.bifocal = bifocal ? 1 : 0;
     p.lo = lo; p.hi = hi;
     p.theta = theta;
     p.n_hi = (L + 255) / 256 + 1; p.fm = fm;
-    p.split = bifocal ? split_ok(theta, fm, p.g) : 0;
     BatchInfo bi = {};                                                 // batch = 0: the single-sequence call
-    auto kern = p.g <= 1 ? decode_umma_kernel<1, false> : p.g <= 2 ? decode_umma_kernel<2, false> : p.g <= 4 ? decode_umma_kernel<4, false>
-              : p.g <= 8 ? decode_umma_kernel<8, false> : decode_umma_kernel<16, false>;
-    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES) != cudaSuccess)
-        return check_launch("decode_umma attr");
-    cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(ns, H_kv);
-    cfg.blockDim = dim3(NTHREADS);
-    cfg.dynamicSmemBytes = SMEM_BYTES;
-    cfg.stream = st;
-    cudaLaunchAttribute at[1];
-    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    at[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = at;
-    cfg.numAttrs = 1;
-    cudaLaunchKernelEx(&cfg, kern, tmK, tmV, p, bi);
-    note_launch();
+    // More than 16 query heads per KV head: one launch per 16 heads of the group (the head operand is N = 16), each streaming
+    // the cache again; the launches write disjoint partials and chain by programmatic serialization (each waits for its
+    // predecessor before it writes, so the merge behind the last one sees them all).
+    for (int h0 = 0; h0 < p.gq; h0 += NH) {
+        p.h0 = h0;
+        p.g = p.gq - h0 < NH ? p.gq - h0 : NH;
+        p.split = bifocal ? split_ok(theta, fm, p.g) : 0;
+        auto kern = p.g <= 1 ? decode_umma_kernel<1, false> : p.g <= 2 ? decode_umma_kernel<2, false> : p.g <= 4 ? decode_umma_kernel<4, false>
+                  : p.g <= 8 ? decode_umma_kernel<8, false> : decode_umma_kernel<16, false>;
+        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES) != cudaSuccess)
+            return check_launch("decode_umma attr");
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(ns, H_kv);
+        cfg.blockDim = dim3(NTHREADS);
+        cfg.dynamicSmemBytes = SMEM_BYTES;
+        cfg.stream = st;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = at;
+        cfg.numAttrs = 1;
+        cudaLaunchKernelEx(&cfg, kern, tmK, tmV, p, bi);
+        note_launch();
+    }
     *nsplit_out = ns;
     return check_launch("decode_umma_kernel");
 }
@@ -762,7 +772,7 @@ int launch_decode_umma_paged(const void* q, const void* Kpool, const void* Vpool
     p.L = Lmax; p.w0 = w0; p.G = 1;
     int ns;
     umma_decode_plan(Lmax, H_kv * nb, &ns, &p.kps);                    // one CTA per SM over all (sequence, KV head) pairs
-    p.H_q = H_q; p.H_kv = H_kv; p.g = H_q / H_kv;
+    p.H_q = H_q; p.H_kv = H_kv; p.g = H_q / H_kv; p.gq = p.g; p.h0 = 0;
     p.bifocal = 0;
     p.lo = lo; p.hi = hi;
     p.theta = theta;

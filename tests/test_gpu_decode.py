@@ -34,6 +34,9 @@ def _decode_vs_oracle(L, H_q, H_kv, d, theta, w_pre, w0, dtype, seed, what):
     (64, 2, 1, 64, 1e4, 256, 3, "bf16"),           # G=1 -> control
     (1, 2, 1, 64, 1e4, 16, 3, "fp32"),
     (5, 8, 8, 128, 1e4, 2, 1, "bf16"),
+    (3000, 32, 1, 128, 1e6, 1024, 200, "bf16"),    # g=32: two launches of 16 heads on the tcgen05 kernel
+    (2049, 48, 2, 128, 1e6, 512, 100, "bf16"),     # g=24: 16 + 8 heads (the second launch takes the SPLIT form)
+    (700, 17, 1, 128, 1e6, 100, 10, "bf16"),       # g=17: 16 + 1
 ])
 def test_decode_small(L, H_q, H_kv, d, theta, w_pre, w0, dtype):
     _decode_vs_oracle(L, H_q, H_kv, d, theta, w_pre, w0, dtype, 4321 + L, "decode L=%d" % L)
