@@ -98,12 +98,13 @@ def test_config5_decode_steps(L0):
     print("C5 L0=%d errors over %d steps: %s" % (L0, steps, worst))
 
 
-def test_batched_paged_decode():
+@pytest.mark.parametrize("H_q,H_kv", [(8, 2), (16, 1)], ids=["g4_split_form", "g16_all_pairs_rotated"])
+def test_batched_paged_decode(H_q, H_kv):
     """batch > 1 over a paged cache.  Sequences of different lengths (G = 1, 2, 3, 5; one shorter than a
     page, one ragged, more than 16 in the batch so that two launches are needed) scattered over a shuffled page pool; each
     must equal the oracle's row L_b - 1 on ITS keys, gathered through the page table."""
     import oracle
-    H_q, H_kv, d, theta, w_pre, w0 = 8, 2, 128, 1e6, 1024, 256
+    d, theta, w_pre, w0 = 128, 1e6, 1024, 256
     lens = [100, 1024, 1025, 2048, 3000, 4097, 777, 2049, 5000, 128, 129, 4096, 3500, 1500, 2600, 900, 4999, 2047]
     Bn = len(lens)
     max_pages = (max(lens) + 127) // 128
