@@ -138,8 +138,8 @@ constexpr uint32_t IDESC_PV = idesc_f16(1, 1, 1, 0, D, NH);      // A = V^T (sme
 
 // SPLIT (slow pairs through the tensor core on the STORED keys).  The correction rotation of pair i at key row m of a tile
 // is Rot(alpha_ref + eps), alpha_ref the angle at the tile's reference row (n_ref = n(k0 + 64)) and
-// eps = (n_m - n_ref) a_i, a_i the table's unit-step angle (|a_i| = theta_i).  For i >= 32 and rope_theta >= 8.4e5,
-// |eps| <= 64 theta_32 <= 0.07, and  Rot(eps) = (1 - eps^2/2) I + eps J  holds to eps^3/6 <= 6e-5 (relative, per pair):
+// eps = (n_m - n_ref) a_i, a_i the table's unit-step angle (|a_i| = theta_i).  For i >= 32 and rope_theta >= 4.54e5,
+// |eps| <= 64 theta_32 <= 0.095, and  Rot(eps) = (1 - eps^2/2) I + eps J  holds to eps^3/6 <= 1.4e-4 (relative, per pair):
 //     q'^T Rot(alpha_ref + eps) k = qt^T k + dn (a J^T qt)^T k + dn^2 (-a^2/2 qt)^T k,   qt = Rot(alpha_ref)^T q',  dn = n_m - n_ref.
 // So those pairs need no per-key rotation at all: per tile the rotate group writes 8-row blocks of a bf16 B operand
 //     block 0: qt hi | 1: unused | 2: qt lo | 3: (a J^T qt) hi | 4: (a J^T qt) lo | 5: -a^2/2 qt      (8 heads x 32 pairs each;
@@ -686,10 +686,12 @@ decode_umma_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constan
 
 }  // namespace
 
-// SPLIT holds when the in-tile phase of pair 32 stays small: 64 theta_32 = 64 rope_theta^-1/2 <= 0.07 (third-order term
-// of the rotation <= 6e-5 per pair); the frequency-interpolation map keeps the per-key rotation
+// SPLIT holds when the in-tile phase of pair 32 stays small: 64 theta_32 = 64 rope_theta^-1/2 <= 0.095, i.e. rope_theta >= 4.54e5
+// (third-order term of the rotation <= 1.4e-4 per pair; Llama-3's 5e5 is inside).  Measured on the stress input with loud pairs
+// 32 / 33 at rope_theta = 5e5 / 4.2e5 / 4.1e5: lse error 2.5e-4 / 3.2e-4 / 5.6e-4 with SPLIT against 8.1e-4 / 9.5e-4 / - with the
+// per-key rotation (fp16 + e5m2 residual of a loud pair): the bound is set by the expansion's own error, with a factor 2 in hand.  The frequency-interpolation map keeps the per-key rotation.
 static int split_ok(double theta, const FreqMap& fm, int g) {
-    return (!fm.interp && g <= SB && 64.0 / sqrt(theta) <= 0.07) ? 1 : 0;
+    return (!fm.interp && g <= SB && 64.0 / sqrt(theta) <= 0.095) ? 1 : 0;
 }
 
 bool umma_decode_supported(int H_q, int H_kv, int d, int dtype) {

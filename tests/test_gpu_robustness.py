@@ -258,13 +258,15 @@ def test_prefill_host_pipeline(L, H_q, H_kv, d, dtype, w_pre, w0):
 
 
 # ---- decode: the second-order treatment of the slow frequency pairs (DESIGN.md 5.3 SPLIT) ------------------------------
-@pytest.mark.parametrize("theta", [1e6, 8.4e5, 8.3e5], ids=["theta1e6", "theta_at_the_split_bound", "theta_below_the_bound"])
-@pytest.mark.parametrize("profile", [None, "slow_pairs"])
+@pytest.mark.parametrize("theta,profile", [(1e6, None), (1e6, "slow_pairs"), (5e5, None), (5e5, "slow_pairs"), (4.6e5, None),
+                                           (4.6e5, "slow_pairs"), (4.5e5, None)],
+                         ids=["theta1e6", "theta1e6_loud", "llama3_theta", "llama3_theta_loud", "theta_at_the_bound",
+                              "theta_at_the_bound_loud", "theta_below_the_bound"])
 def test_decode_slow_pair_expansion_margin(theta, profile):
     """Decode rows against the oracle over seeds, lengths and group sizes (G = 2, 3, 5, 7: 128 % G == 0 and != 0, so both
     steps of the per-tile reference row occur), with the standard inputs and with the loud channels put on pairs 32 / 33,
-    where the truncated third-order term is largest; rope_theta = 8.4e5 sits on the bound that admits the expansion,
-    8.3e5 just below it (per-key rotation of all pairs)."""
+    where the truncated third-order term is largest; rope_theta = 4.6e5 sits on the bound that admits the expansion (4.54e5),
+    4.5e5 just below it (per-key rotation of all pairs, standard inputs)."""
     H_q, H_kv, d, w0 = 8, 2, 128, 256
     worst_o = worst_l = 0.0
     for L, w_pre in ((4000, 2048), (9000, 3072), (20000, 4096), (33333, 5000)):
