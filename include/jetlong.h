@@ -22,9 +22,10 @@
  *   - Value range (bf16 path): rotated remote operands are re-rounded to fp16 and e5m2 for the tensor core, so
  *     |Q|, |K| elements must stay below 2^15 (a rotated pair can grow by sqrt 2; fp16 overflows at 65504, e5m2 at
  *     61440).  Larger magnitudes give inf / NaN remote scores; activations of the models in scope are < 2^10.
- *     Precision of the default mode: its e5m2 cross terms meet the lse tolerance (1e-3) as long as no
- *     frequency pair is loud in Q AND in K with a product of the two factors above ~12 (loud = relative to the other
- *     channels' rms); beyond that choose JETLONG_PRECISION_COMPENSATED_F16 per call.
+ *     Precision of the default mode: a frequency pair that is loud in Q AND in K at once (product of the
+ *     two factors, relative to the other channels' rms, above ~12) is detected per KV head and its cross terms are kept
+ *     in fp16; the lse error then reaches the tolerance (measured up to 9.8e-4 against 1e-3).  For such data
+ *     JETLONG_PRECISION_COMPENSATED_F16 (4e-5, slower) can be chosen per call.
  *   - INVALID_ARG: null pointer, L < 1, H_q % H_kv != 0, head_dim not in {64, 128}, w_local < 0,
  *     w_pretrained < 1, rope_theta <= 0, unknown dtype, a pointer not 16-byte aligned, or a
  *     workspace smaller than jetlong_workspace_bytes() reports.

@@ -297,11 +297,15 @@ prefill_umma2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_const
     // whose other channels are too loud falls back from 3 to 2
     int precise = (bifocal && mp.n_rem > 0) ? p.precise : 0;
     if (precise == 3 && __ldg(p.selinfo + kvh * 16 + 8) != 0u) precise = 2;
+    // 4: the selected pairs' cross terms in fp16 instead of e5m2 -- asked for, or flagged by the selection kernel when a selected
+    // pair is loud in Q and in K at once; the workspace variant's scratch has no fp16 form of the compact rows
+    else if (precise == 3 && !p.prerot && __ldg(p.selinfo + kvh * 16 + 9) != 0u) precise = 4;
+    if (precise == 4 && p.prerot) precise = 3;
     // shared memory: Q tiles | cross-term Q' operands | K ring | V ring | barriers
-    const int QX_BYTES = precise == 3 ? QBOX : precise == 2 ? 4 * QBOX : 0;
-    const int KST = KH_BYTES + (precise == 3 ? KBOX : precise == 2 ? 2 * KBOX : 0);
-    const int NK = precise == 3 ? 4 : precise == 2 ? 2 : 5;
-    const int NV = precise == 3 ? 3 : precise == 2 ? 2 : 5;
+    const int QX_BYTES = precise == 3 ? QBOX : precise == 4 ? 2 * QBOX : precise == 2 ? 4 * QBOX : 0;
+    const int KST = KH_BYTES + ((precise == 3 || precise == 4) ? KBOX : precise == 2 ? 2 * KBOX : 0);
+    const int NK = (precise == 3 || precise == 4) ? 4 : precise == 2 ? 2 : 5;
+    const int NV = precise == 3 ? 3 : (precise == 2 || precise == 4) ? 2 : 5;
     unsigned char* sQ = smem;
     unsigned char* sQX = smem + Q_BYTES;
     unsigned char* kring = sQX + QX_BYTES;
@@ -406,6 +410,15 @@ prefill_umma2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_const
                     // compact operands: Q' row = [HI | LO] regions of 32 bytes (tile i at byte 64 i), K' row = [LO | HI]
                     umma2_ss_f8_e(dS, qx_lo0 + 4 * i, HI_K, klb, HI_K, id_hl, 1u, el);
                     umma2_ss_f8_e(dS, qx_lo0 + 4 * i + 2, HI_K, klb + 2, HI_K, id_lh, 1u, el);
+                } else if (mode == 2 && precise == 4) {
+                    // fp16 compact operands: Q' row of tile i (its own box) = [HI | LO] regions of 64 bytes, K' row = [LO | HI]
+                    const uint32_t q4 = qx_lo0 + (uint32_t)((i * QBOX) >> 4);
+#pragma unroll
+                    for (int ks = 0; ks < 2; ++ks)
+                        umma2_ss_e(dS, q4 + 2 * ks, HI_K, klb + 2 * ks, HI_K, IDESC_QK_F16 | IDESC_NEG_B, 1u, el);
+#pragma unroll
+                    for (int ks = 0; ks < 2; ++ks)
+                        umma2_ss_e(dS, q4 + 4 + 2 * ks, HI_K, klb + 4 + 2 * ks, HI_K, IDESC_QK_F16 | IDESC_NEG_A, 1u, el);
                 } else if (mode == 2 && precise == 2) {
                     const uint32_t qe = qx_lo0 + (uint32_t)(i * ((2 * QBOX) >> 4));   // [Q' e5m2 | Q' lo e5m2] of tile i
 #pragma unroll
@@ -508,7 +521,7 @@ prefill_umma2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_const
                 TR(3, m, 1);
                 if (x.mode == 2) {
                     if (rotating) {
-                        rotate_rows2<4, KBOX, KM>(smem_u32(sK(st)), smem_u32(sKl(st)), (unsigned)(x.kt * BN + 64 * cta), rot, sel, 0u, 32u);
+                        rotate_rows2<4, KBOX, KM>(smem_u32(sK(st)), smem_u32(sKl(st)), (unsigned)(x.kt * BN + 64 * cta), rot, sel, 0u, KM == 6 ? 64u : 32u);
                         fence_proxy_async_smem();
                         if (x.kt > 0) rot.prefetch((unsigned)((x.kt - 1) * BN + 64 * cta));   // next remote visit's first row
                     }
@@ -521,9 +534,10 @@ prefill_umma2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_const
                             KRot<4> qr;
                             qr.init(p.lo, p.hi, tid, p.G, 64 * half);
                             qr.prefetch((unsigned)((qb0 + i) * BM));
-                            const uint32_t qx = KM == 2 ? smem_u32(sQX) + (uint32_t)(i * 2 * QBOX) : smem_u32(sQX);
+                            const uint32_t qx = KM == 2 ? smem_u32(sQX) + (uint32_t)(i * 2 * QBOX)
+                                              : KM == 6 ? smem_u32(sQX) + (uint32_t)(i * QBOX) : smem_u32(sQX);
                             rotate_rows2<4, QBOX, KM>(smem_u32(sQ + i * QT_BYTES), qx, (unsigned)((qb0 + i) * BM), qr, sel,
-                                                      64u * i + 32u, 64u * i);
+                                                      KM == 6 ? 64u : 64u * i + 32u, KM == 6 ? 0u : 64u * i);
                         }
                         fence_proxy_async_smem();
                         __syncwarp();
@@ -536,6 +550,7 @@ prefill_umma2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_const
             }
         };
         if (precise == 3) visit_loop(std::integral_constant<int, 5>{});
+        else if (precise == 4) visit_loop(std::integral_constant<int, 6>{});
         else if (precise == 2) visit_loop(std::integral_constant<int, 2>{});
         else visit_loop(std::integral_constant<int, 0>{});
     } else {

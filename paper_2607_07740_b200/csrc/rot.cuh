@@ -300,7 +300,7 @@ __device__ __forceinline__ void rotate_k_rows(uint32_t kh, uint32_t kl, unsigned
 //     UMMA needs);
 //   * the next row's shared-memory loads are issued before the current row's arithmetic.
 // MODE 0: hi only.  MODE 2: full e5m2 copies at kl (as rotate_k_rows mode 2, lo negated).  MODE 3: only -lo as e5m2 at kl
-// (decode).  MODE 5 as above.
+// (decode).  MODE 5 as above.  MODE 6: as 5 with fp16 instead of e5m2 (regions of 64 bytes).
 __device__ __forceinline__ float fhsub_lo(uint32_t h, float y) {     // (low fp16 of h) - y
     float r;
     unsigned short hs;
@@ -392,6 +392,11 @@ __device__ __forceinline__ void rotate_rows2(uint32_t kh, uint32_t kl, unsigned 
             const uint32_t wh = __byte_perm(T.pick(h1) + 0x00800080u, T.pick(h2) + 0x00800080u, 0x7531);
             asm volatile("st.shared.u32 [%0], %1;" ::"r"(kl + r * 128 + ((((b_lo >> 4) + cw) ^ x) << 4) + cb), "r"(wl) : "memory");
             asm volatile("st.shared.u32 [%0], %1;" ::"r"(kl + r * 128 + ((((b_hi >> 4) + cw) ^ x) << 4) + cb), "r"(wh) : "memory");
+        } else if (MODE == 6) {
+            // MODE 5 with the selected pairs kept in fp16: regions of 64 bytes, chunk c = 8 bytes [x1(f0) x1(f1) | x2(f0) x2(f1)]
+            const uint32_t x = (uint32_t)(r & 7), cw = (uint32_t)(R.c >> 1), cb = (uint32_t)(R.c & 1) * 8u;
+            sts64(kl + r * 128 + ((((b_lo >> 4) + cw) ^ x) << 4) + cb, T.pick(l1), T.pick(l2));
+            sts64(kl + r * 128 + ((((b_hi >> 4) + cw) ^ x) << 4) + cb, T.pick(h1), T.pick(h2));
         }
         if (m + 1 < ROWS) {
             rem = (rem + 1 == R.G) ? 0u : rem + 1;

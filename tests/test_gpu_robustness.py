@@ -284,21 +284,26 @@ def test_decode_slow_pair_expansion_margin(theta, profile):
     assert worst_l <= TOL[torch.bfloat16]["lse"] and worst_o <= TOL[torch.bfloat16]["out_abs"], (worst_o, worst_l)
 
 
-def test_coincident_loud_pairs_need_fp16_cross_terms():
-    """DESIGN.md 5.2, known limit: the same frequency pairs loud in Q (x4) AND in K (x8).  The e5m2 cross terms of the default
-    precision leave the lse tolerance there (measured 3.4e-3); the fp16 cross terms (PRECISION_COMPENSATED_F16, per call) hold
-    it.  Pinned so that the limit stays documented and the escape route stays working."""
+def test_coincident_loud_pairs_switch_the_selected_cross_terms_to_fp16():
+    """the same frequency pairs loud in Q (x4) AND in K (x8).  With e5m2 cross terms the default precision
+    measured 3.4e-3 of lse here; the selection kernel now flags such heads and the two-tile kernel keeps the SELECTED pairs'
+    cross terms in fp16 (7e-4 .. 1e-3: what is left is the un-averaged noise of the pairs left out, the softmax of these rows
+    is peaked).  PRECISION_COMPENSATED_F16 (every pair in fp16, per call) stays the reference point at 4e-5."""
     L, w_pre, w0, theta = 8320, 2048, 256, 1e6
-    Q, K, V = W.make_qkv(L, 4, 2, 128, theta, "bf16", 61000 + L, False, DEV, profile="slow_pairs")
-    rows, heads = _pick(L, 4, 1024, 5)
-    ro, rl = oracle_rows(Q, K, V, rows, heads, w_local=w0, w_pretrained=w_pre, rope_theta=theta)
     errs = {}
-    for name, prec in (("default", J.PRECISION_COMPENSATED), ("fp16 cross terms", J.PRECISION_COMPENSATED_F16)):
-        out, lse = J.jetlong_prefill(Q, K, V, w_local=w0, w_pretrained=w_pre, rope_theta=theta, precision=prec)
-        torch.cuda.synchronize()
-        og, lg = gather(out, lse, rows, heads)
-        assert torch.isfinite(og.float()).all() and torch.isfinite(lg).all()
-        errs[name] = (float(np.abs(og.double().cpu().numpy() - ro).max()), float(np.abs(lg.double().cpu().numpy() - rl).max()))
+    for seed in (61000 + L, 61013 + L):
+        Q, K, V = W.make_qkv(L, 4, 2, 128, theta, "bf16", seed, False, DEV, profile="slow_pairs")
+        rows, heads = _pick(L, 4, 1024, 5)
+        ro, rl = oracle_rows(Q, K, V, rows, heads, w_local=w0, w_pretrained=w_pre, rope_theta=theta)
+        for name, prec in (("default", J.PRECISION_COMPENSATED), ("fp16 cross terms", J.PRECISION_COMPENSATED_F16)):
+            out, lse = J.jetlong_prefill(Q, K, V, w_local=w0, w_pretrained=w_pre, rope_theta=theta, precision=prec)
+            torch.cuda.synchronize()
+            og, lg = gather(out, lse, rows, heads)
+            assert torch.isfinite(og.float()).all() and torch.isfinite(lg).all()
+            eo = float(np.abs(og.double().cpu().numpy() - ro).max())
+            el = float(np.abs(lg.double().cpu().numpy() - rl).max())
+            errs[name] = (max(errs.get(name, (0, 0))[0], eo), max(errs.get(name, (0, 0))[1], el))
     print("coincident loud pairs (Q x4, K x8): %s" % errs)
     assert errs["fp16 cross terms"][1] <= TOL[torch.bfloat16]["lse"] and errs["fp16 cross terms"][0] <= TOL[torch.bfloat16]["out_abs"]
-    assert errs["default"][1] <= 5e-3 and errs["default"][0] <= TOL[torch.bfloat16]["out_abs"]
+    # the default: at the tolerance, not comfortably inside it (1e-3); 1.5e-3 would mean the flag or the fp16 path broke
+    assert errs["default"][1] <= 1.5e-3 and errs["default"][0] <= TOL[torch.bfloat16]["out_abs"]
